@@ -1,0 +1,283 @@
+"""bench.py — zone-updates/s of one full AGATE finite-volume MHD time step on B200 (BASELINE.json metric).
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--config C] [--impl reference]
+
+A "step" is one pass of the whole hot path over the resident state: Courant reduction (A7), then per Runge-Kutta
+stage ghost fill (A0) + the fused stage kernel (A1-A6).  Default workload: BASELINE.json config 5 (3D ideal MHD,
+512^3, PLM + eq.4 beta=1.3, HLLD, SSP-RK2, seeded synthetic state) on one GPU.  N > 1 runs N
+independent replicas of that problem, one per rank (the path is single-GPU by specification: "replicas only",
+weak scaling, no data-path collective); timing = barrier + device events, max over ranks.
+
+The JSON line carries: value (device-resident throughput), e2e (through the C-ABI with pinned HOST buffers, the
+full state copied in and out every step), roofline (dominant kernel = the fused stage kernel, bound = FP64 ALU
+pipe), cpu_baseline (the oracle, as it stands, on a bounded sample), clocks, gpu_launches.
+
+--impl reference times the CPU oracle (oracle/) on the box's host cores on a bounded sample of the same workload.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+METRIC = "zone-updates/sec per full step (fp64)"
+UNIT = "zone-updates/s"
+
+# Algorithmic flop per zone per full step (both stages + dt reduction), SURVEY §8(d) convention (add/sub/mul/
+# compare/min/max/div/sqrt = 1, FMA = 2): the lean hand count of SURVEY §8(d); the oracle's
+# own as-written count (oracle.count_ops) is higher (1774 / 2265 / 3350 / 2072 / 3292) because it evaluates both
+# sides' fluxes and divides where a shared reciprocal serves.  The smaller figure is used so the fraction is not
+# flattered.
+FLOP_PER_ZONE_STEP = {1: 1430.0, 2: 1890.0, 3: 2770.0, 4: 1760.0, 5: 2770.0}
+FLOP_DT_PER_ZONE = {1: 45.0, 2: 45.0, 3: 45.0, 4: 60.0, 5: 45.0}
+BYTES_PER_ZONE_STEP = 320.0            # 5 x 8 variables x 8 B
+FP64_NOMINAL_TFLOPS = 148 * 64 * 2 * 1.965e9 / 1e12     # 148 SMs x 64 DFMA lanes x 2 x max SM clock = 37.2
+
+# reduced size of the bounded CPU sample per config (same recipe and seed), and its step count
+CPU_SAMPLE = {1: (128, 10), 2: (512, 8), 3: (96, 4), 4: (512, 8), 5: (96, 4)}
+
+
+def parse():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=20)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--config", type=int, default=5, choices=[1, 2, 3, 4, 5])
+    ap.add_argument("--n", type=int, default=0, help="override the per-dimension resolution (debugging)")
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--no-cpu", action="store_true")
+    return ap.parse_args()
+
+
+def workload_name(wl):
+    return wl.name
+
+
+def measured_peaks():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        try:
+            return json.load(open(p)), "measured"
+        except Exception:
+            pass
+    return {"hbm_gbs": 6650.0}, "fallback"
+
+
+class ClockSampler:
+    """nvidia-smi clocks / throttle reasons sampled every 200 ms while the timed region runs."""
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+         "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index=0):
+        self.rows, self.proc, self.index = [], None, index
+
+    def __enter__(self):
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", "-i", str(self.index), f"--query-gpu={self.Q}",
+                                          "--format=csv,noheader,nounits", "-lms", "200"],
+                                         stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            self.th = threading.Thread(target=self._read, daemon=True)
+            self.th.start()
+        except Exception:
+            self.proc = None
+        return self
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.rows.append([x.strip() for x in line.split(",")])
+
+    def __exit__(self, *a):
+        if self.proc is not None:
+            time.sleep(0.25)
+            self.proc.terminate()
+            try:
+                self.proc.wait(timeout=2)
+            except Exception:
+                self.proc.kill()
+
+    def summary(self):
+        sm, mx, reasons = [], 0.0, set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for r in self.rows:
+            try:
+                sm.append(float(r[0])); mx = max(mx, float(r[1]))
+                for nm, v in zip(names, r[3:7]):
+                    if v.lower().startswith("active"):
+                        reasons.add(nm)
+            except Exception:
+                continue
+        sm.sort()
+        return {"sm_mhz": sm[len(sm) // 2] if sm else None, "sm_max_mhz": mx or None, "reasons": sorted(reasons),
+                "samples": len(sm)}
+
+
+def cpu_oracle_rate(config, steps=None, warmup=0):
+    """The oracle as it stands (single-threaded build default) on a bounded sample; returns dict for the JSON."""
+    import oracle
+    from workloads import make_workload
+    n, nst = CPU_SAMPLE[config]
+    if steps is not None:
+        nst = steps
+    wl = make_workload(config, n=n)
+    ref = oracle.RefSolver.from_workload(wl)
+    if warmup:
+        ref.advance(warmup)
+    t0 = time.perf_counter()
+    ref.advance(nst)
+    dt = time.perf_counter() - t0
+    ref.close()
+    return {"value": wl.zones * nst / dt, "unit": UNIT, "cores": oracle.get_threads(), "kind": "oracle",
+            "sample": f"config {config} recipe at {wl.shape[0]}^{wl.ndim}, {nst} full steps, "
+                      f"{os.cpu_count()} host cores present"}, dt / nst, wl
+
+
+def run_reference(args):
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    base, per_step, wl = cpu_oracle_rate(args.config, steps=args.steps, warmup=args.warmup)
+    line = {"metric": METRIC, "value": base["value"], "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
+            "warmup": args.warmup, "ms_per_step": per_step * 1e3, "higher_is_better": True, "scaling": "weak",
+            "vs_baseline": None, "dtype": "f64", "data": "synthetic", "impl": "reference",
+            "config": {"workload": f"BASELINE.json config {args.config} (bounded CPU sample: {base['sample']})"},
+            "cpu_baseline": base,
+            "e2e": {"value": base["value"], "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+            "gpu_launches": 0}
+    print(json.dumps(line))
+
+
+def run_ours(args):
+    import numpy as np
+    import torch
+    import torch.distributed as dist
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device — the CUDA path has no CPU fallback")
+    import paper_2503_20899_b200 as ag
+    from workloads import make_workload
+
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    torch.cuda.set_device(local)
+    dev = f"cuda:{local}"
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device(dev))
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    cfg = args.config
+    wl = make_workload(cfg, n=args.n or None)
+    zones = wl.zones
+    wl.W = None                                       # only U is needed; frees one state-sized host array
+    K, Wm = args.steps, args.warmup
+    sim = ag.Agate.from_workload(wl, device=dev, set_state=False)
+    Uh = torch.from_numpy(wl.U).pin_memory()
+    info = sim.launch_info()
+    fp64_peak = ag.measure_fp64_peak(10)
+
+    # ---- device-resident throughput: K steps, state already in HBM --------------------------------------
+    sim.set_state(Uh)
+    sim.advance(Wm)                                   # warm-up (also instantiates the CUDA graph)
+    sim.set_state(Uh)
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    barrier()
+    with ClockSampler(local) as clk:
+        e0.record(sim.stream)
+        sim.advance(K, sync=False)
+        e1.record(sim.stream)
+        barrier()
+    ms = e0.elapsed_time(e1)
+    sim.poll()
+    t_ms = torch.tensor([ms], dtype=torch.float64, device=dev)
+    if world > 1:
+        dist.all_reduce(t_ms, op=dist.ReduceOp.MAX)
+    ms_max = float(t_ms.item())
+    value = zones * world * K / (ms_max * 1e-3)
+
+    # ---- per-launch duration of the dominant kernel (fused stage), CUDA events on its own stream ---------
+    sim.set_state(Uh)
+    sim.set_timing(True)
+    sim.advance(K)
+    st_ms, st_n = sim.stage_time()
+    sim.set_timing(False)
+    stage_ms = st_ms / max(st_n, 1)
+    flop_stage = (FLOP_PER_ZONE_STEP[cfg] - FLOP_DT_PER_ZONE[cfg]) / 2.0 * zones
+    achieved = flop_stage / (stage_ms * 1e-3) / 1e12
+    peaks, peak_src = measured_peaks()
+    hbm_frac = (BYTES_PER_ZONE_STEP / 5.0 * 2.5 * zones / (stage_ms * 1e-3) / 1e9) / peaks["hbm_gbs"]
+    roofline = {"bound": "alu", "achieved": achieved, "peak": fp64_peak, "unit": "TFLOP/s",
+                "frac": achieved / fp64_peak, "traffic": None,
+                "kernel": "stage_kernel", "ms_per_launch": stage_ms, "launches_timed": st_n,
+                "stage_share_of_step": 2.0 * stage_ms * K / ms_max if st_n else None,
+                "peak_source": "FP64 DFMA micro-benchmark of this run (agate_measure_fp64_peak); nominal "
+                               f"{FP64_NOMINAL_TFLOPS:.1f} = 148 SM x 64 lanes x 2 x 1.965 GHz",
+                "hbm_frac_of_" + peak_src: hbm_frac,
+                "flop_per_zone_stage": flop_stage / zones}
+
+    # ---- end to end through the C-ABI with HOST buffers: every step copies the state in and out ---------
+    e2e = None
+    if not args.no_e2e:
+        Ke = min(K, 4)
+        out = torch.empty_like(Uh).pin_memory()
+        sim.set_state(Uh); sim.step(0.0); sim.get_state(out)            # warm-up
+        barrier()
+        t0 = time.perf_counter()
+        a, b = Uh, out
+        for _ in range(Ke):
+            sim.set_state(a)
+            sim.step(0.0, sync=False)
+            sim.get_state(b)
+            a, b = b, a
+        barrier()
+        te = time.perf_counter() - t0
+        t_e = torch.tensor([te], dtype=torch.float64, device=dev)
+        if world > 1:
+            dist.all_reduce(t_e, op=dist.ReduceOp.MAX)
+        nbytes = Uh.numel() * 8
+        e2e = {"value": zones * world * Ke / float(t_e.item()), "unit": UNIT, "h2d_bytes_per_step": nbytes,
+               "d2h_bytes_per_step": nbytes, "steps": Ke,
+               "note": "agate_set_state(host pinned) + agate_step + agate_get_state(host pinned) per step"}
+
+    if rank == 0:
+        line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": Wm,
+                "ms_per_step": ms_max / K, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+                "dtype": "f64", "data": "synthetic",
+                "config": {"workload": f"BASELINE.json config {cfg}: {wl.name}", "zones_per_gpu": zones,
+                           "parallelism": "replicas only" if world > 1 else "single GPU",
+                           "l2": "state (2 x %.2f GB) is larger than L2; no flush needed" % (zones * 64 / 1e9)
+                                 if zones * 64 > 2.5e8 else "state fits L2 (small config); numbers are L2-resident",
+                           "launch": info},
+                "roofline": roofline, "clocks": clk.summary(), "gpu_launches": info["launches_per_step"] * K,
+                "e2e": e2e}
+        if not args.no_cpu and world >= 1:
+            line["cpu_baseline"] = cpu_oracle_rate(cfg)[0]
+        print(json.dumps(line))
+    sim.close()
+    if world > 1:
+        dist.barrier()
+        dist.destroy_process_group()
+
+
+def main():
+    args = parse()
+    if args.impl == "reference":
+        run_reference(args)
+    else:
+        run_ours(args)
+
+
+if __name__ == "__main__":
+    main()

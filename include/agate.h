@@ -1,0 +1,131 @@
+/* agate.h — C-ABI boundary of the B200-native AGATE finite-volume MHD step.
+ *
+ * What the library computes (PAPER.md = /root/reference/PAPER.md, cited P:Lnnn; readings Rn are listed in
+ * DESIGN.md): one explicit Godunov-type finite-volume time step dU/dt = Delta(U,t) for the ideal
+ * and Hall MHD equations (Section 3.1, eqs.7-13) on a uniform periodic Cartesian grid:
+ *
+ *   A0 ghost fill (periodic, 2 layers)      A4 Riemann flux: HLL eq.5-6 or HLLD (R10)
+ *   A1 primitive recovery (R2)                     A5 flux difference, eq.1
+ *   A2 PLM reconstruction + eq.4 limiter       A6 Runge-Kutta stage combine (RK11 / SSP-RK22, R11)
+ *   A3 Davis signal speeds eq.6 + fast speed eq.12 (R3)    A7 global Courant reduction dt = C dx_min / v_max
+ *   A8 Hall terms: face current J, v_H = -d_i J / rho, whistler speed eq.13
+ *
+ * Every step of that path runs in hand-written CUDA kernels for sm_100a (fp64).  There is no CPU fallback:
+ * without a CUDA device every compute entry point returns AGATE_ERR_CUDA.
+ *
+ * Conventions
+ *   - Variable order, conserved U = (rho, mx, my, mz, E, Bx, By, Bz); all values IEEE float64.
+ *   - External state layout: interior-only SoA  U[8][nz][ny][nx], x fastest.  Ghost padding is internal.
+ *   - Every function returns an int status (AGATE_OK = 0); nothing throws or aborts; out-parameters are written
+ *     only on success.
+ *   - Ownership: all device memory belongs to the caller.  The library carves its two ghost-padded state
+ *     buffers, its scalars and its reduction scratch out of `workspace` and never allocates device memory.
+ *     Host arrays are borrowed for the duration of the call.
+ *   - All work is enqueued on the stream given to agate_init.  Calls that return a value to the host
+ *     (agate_compute_dt, agate_get_state to a host buffer, agate_advance with t_out != NULL, agate_step with
+ *     dt_used != NULL, agate_poll) synchronise that stream; the others do not.
+ *   - One context per stream; no global state; a context is not thread-safe.
+ */
+#ifndef AGATE_H
+#define AGATE_H
+#include <stddef.h>
+#include <stdint.h>
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct agate_ctx agate_ctx;   /* opaque; created by agate_init, freed by agate_destroy */
+
+typedef struct {
+  int32_t ndim;         /* 1, 2, 3: active dimensions are x[, y[, z]]  */
+  int32_t nx, ny, nz;   /* interior zones; inactive dimensions must be 1                             */
+  double  dx, dy, dz;   /* uniform spacings; inactive ones are ignored  */
+} agate_grid;
+
+typedef struct {
+  int32_t riemann;      /* 0 = HLL (eq.5), 1 = HLLD (R10; not in the paper)              */
+  int32_t limiter;      /* 0 = none (dU = 0), 1 = central (unlimited), 2 = eq.4   */
+  double  beta;         /* eq.4 beta in [1,2]: 1.0 = minmod, 1.3 = the paper's "MC" default */
+  int32_t rk;           /* 1 = RK11 (forward Euler), 2 = SSP-RK22 (R11)                       */
+  double  cfl;          /* Courant number C; <= 0 selects the paper default 0.8/0.45/0.325   */
+  double  d_i;          /* normalised ion inertial length (eqset AGATE_HALL only)            */
+} agate_solver;
+
+enum { AGATE_IDEAL = 0, AGATE_HALL = 1 };
+enum { AGATE_HLL = 0, AGATE_HLLD = 1 };
+enum {
+  AGATE_OK = 0,
+  AGATE_ERR_ARG = 1,          /* null pointer, bad size, unsupported combination (Hall + HLLD)       */
+  AGATE_ERR_STATE = 2,        /* call order: no state set yet                                        */
+  AGATE_ERR_UNPHYSICAL = 3,   /* rho <= 0, p <= 0 or a non-finite speed seen by the dt reduction (R14) */
+  AGATE_ERR_CUDA = 4,         /* CUDA runtime error, or no CUDA device                               */
+  AGATE_ERR_NOMEM = 5         /* workspace too small or misaligned                                   */
+};
+
+/* Bytes of device workspace agate_init needs for this problem (0 on invalid arguments). */
+size_t agate_workspace_bytes(const agate_grid* grid, int eqset, const agate_solver* solver);
+
+/* Create a context.  `workspace`: DEVICE pointer, caller-owned, >= agate_workspace_bytes(), 256-byte aligned,
+ * must outlive the context.  `stream`: a cudaStream_t (as void*), NULL = the legacy default stream.
+ * gamma > 1 is the adiabatic index.  Hall + HLLD is rejected with AGATE_ERR_ARG (the paper gives no
+ * such solver). */
+int agate_init(const agate_grid* grid, double gamma, int eqset, const agate_solver* solver,
+               void* workspace, size_t workspace_bytes, void* stream, agate_ctx** out);
+
+/* Copy an interior-only SoA state U[8][nz][ny][nx] into the context and set the time to t0.
+ * `U` is a HOST pointer when src_is_device == 0 (pinned memory makes the copy asynchronous), else a DEVICE
+ * pointer.  Fills the periodic ghost layers (A0).  Validates nothing physical (the dt reduction does). */
+int agate_set_state(agate_ctx*, const double* U, int src_is_device, double t0);
+
+/* A7: dt = C dx_min / max_cells(|v| + max(c_f, c_w)) of the current state -> *dt_out (HOST).
+ * Synchronises.  AGATE_ERR_UNPHYSICAL if any cell has rho <= 0, p <= 0 or a non-finite speed. */
+int agate_compute_dt(agate_ctx*, double* dt_out);
+
+/* One full time step (all RK stages: A0-A6 per stage).  dt > 0: use it; dt <= 0: run the dt reduction first and
+ * use its device-resident result (no host round trip).  dt_used (HOST, may be NULL): the step actually taken;
+ * non-NULL synchronises. */
+int agate_step(agate_ctx*, double dt, double* dt_used);
+
+/* n_steps self-timed steps: per step  dt = reduction(U^n); stage 1; stage 2; t += dt  — all enqueued without a
+ * host synchronisation (one CUDA graph launch per step).  t_out (HOST, may be NULL): time reached; non-NULL
+ * synchronises and reports AGATE_ERR_UNPHYSICAL if the reduction flagged any step. */
+int agate_advance(agate_ctx*, int32_t n_steps, double* t_out);
+
+/* Copy the current state out as interior-only SoA.  U_out is HOST (dst_is_device == 0; synchronises) or DEVICE.
+ * t_out (HOST, may be NULL) receives the current time (synchronises). */
+int agate_get_state(agate_ctx*, double* U_out, int dst_is_device, double* t_out);
+
+/* Synchronise the stream and report the sticky status (AGATE_ERR_UNPHYSICAL / AGATE_ERR_CUDA / AGATE_OK). */
+int agate_poll(agate_ctx*);
+
+/* The stage kernel's launch geometry for this context: out[0..2] = grid x,y,z, out[3] = threads per block,
+ * out[4] = dynamic shared memory bytes, out[5] = registers per thread, out[6] = resident blocks per SM,
+ * out[7] = kernels launched per step.  For bench.py's roofline bookkeeping; no device work. */
+int agate_launch_info(agate_ctx*, int64_t out[8]);
+
+/* Accumulated device time (ms, CUDA events on the context's stream) spent in stage-kernel launches since the
+ * last call with reset != 0, and the number of launches.  Only counts launches made while timing is enabled
+ * with agate_set_timing(ctx, 1) (timing forces per-launch events and bypasses the CUDA graph). */
+int agate_set_timing(agate_ctx*, int enabled);
+int agate_stage_time(agate_ctx*, double* ms_out, int64_t* launches_out, int reset);
+
+int agate_destroy(agate_ctx*);
+const char* agate_strerror(int status);
+
+/* ---- diagnostics (not on the hot path) -------------------------------------------------------------- */
+
+/* Evaluate the device Riemann flux (A3+A4[+A8]) on n independent face pairs.  All pointers are DEVICE.
+ * WL, WR: [8][n] primitive face states (rho,vx,vy,vz,p,Bx,By,Bz); J: [3][n] face current (Hall) or NULL;
+ * F: [8][n] output flux along `dir` (0,1,2).  Used by the GPU unit tests of the HLL/HLLD device functions. */
+int agate_test_face_flux(int eqset, int riemann, int dir, double gamma, double d_i, double dxmin,
+                         const double* WL, const double* WR, const double* J, double* F, int64_t n, void* stream);
+
+/* FP64 FMA throughput micro-benchmark (8 independent DFMA chains per thread on every SM): returns the sustained
+ * TFLOP/s (FMA = 2 flop) over `iters` launches in *tflops_out.  Gives the ALU roofline denominator, which
+ * MEASURED_PEAKS.json does not hold. */
+int agate_measure_fp64_peak(int iters, double* tflops_out, void* stream);
+
+#ifdef __cplusplus
+}
+#endif
+#endif

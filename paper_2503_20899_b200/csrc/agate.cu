@@ -1,0 +1,520 @@
+// agate.cu — C-ABI of the B200-native AGATE finite-volume MHD step (see include/agate.h).
+// Host side only: argument checks, workspace carving, kernel selection, launches, the per-step CUDA graph.
+// All arithmetic of the path is in agate_kernels.cuh / agate_physics.cuh.  No CPU fallback.
+#include "agate.h"
+
+#include <cuda_runtime.h>
+
+#include <cstdio>
+#include <cstdlib>
+#include <cstring>
+#include <new>
+#include <vector>
+
+#include "agate_kernels.cuh"
+
+using namespace agate;
+
+namespace {
+
+constexpr int TY3 = 12;   // 3-D: 32x12 tile, 14 warps, 1 CTA / SM, ring of 3 planes
+constexpr int TY2 = 6;    // 1-D / 2-D: 32x6 tile, 8 warps, 2 CTAs / SM
+constexpr int kDtBlocksMax = 148 * 8;
+
+inline size_t align_up(size_t x, size_t a) { return (x + a - 1) / a * a; }
+
+struct Layout {
+  int ghy, ghz, nxp, nyp, nzp;
+  long long sy, sz, sq;
+  size_t state_bytes;      // one padded copy of U (8 variables)
+  size_t off_A, off_B, off_scal, off_partial, total;
+};
+
+Layout make_layout(const agate_grid& g) {
+  Layout L;
+  L.ghy = (g.ndim >= 2) ? 2 : 0;
+  L.ghz = (g.ndim >= 3) ? 2 : 0;
+  L.nxp = g.nx + 4;
+  L.nyp = g.ny + 2 * L.ghy;
+  L.nzp = g.nz + 2 * L.ghz;
+  L.sy = L.nxp;
+  L.sz = (long long)L.nxp * L.nyp;
+  L.sq = L.sz * L.nzp;
+  L.sq = (long long)align_up((size_t)L.sq, 32);          // every variable starts 256-byte aligned
+  L.state_bytes = sizeof(double) * 8 * (size_t)L.sq;
+  L.off_A = 0;
+  L.off_B = align_up(L.off_A + L.state_bytes, 256);
+  L.off_scal = align_up(L.off_B + L.state_bytes, 256);
+  L.off_partial = L.off_scal + 256;                       // scal: 3 doubles + flag + ticket
+  L.total = L.off_partial + align_up(sizeof(double) * kDtBlocksMax, 256);
+  return L;
+}
+
+int check_args(const agate_grid* g, double gamma, int eqset, const agate_solver* s) {
+  if (!g || !s) return AGATE_ERR_ARG;
+  if (g->ndim < 1 || g->ndim > 3) return AGATE_ERR_ARG;
+  if (g->nx < 1 || g->ny < 1 || g->nz < 1) return AGATE_ERR_ARG;
+  if (g->ndim < 3 && g->nz != 1) return AGATE_ERR_ARG;
+  if (g->ndim < 2 && g->ny != 1) return AGATE_ERR_ARG;
+  if (!(g->dx > 0.0) || (g->ndim >= 2 && !(g->dy > 0.0)) || (g->ndim >= 3 && !(g->dz > 0.0))) return AGATE_ERR_ARG;
+  if (!(gamma > 1.0)) return AGATE_ERR_ARG;
+  if (eqset != AGATE_IDEAL && eqset != AGATE_HALL) return AGATE_ERR_ARG;
+  if (s->riemann < 0 || s->riemann > 1 || s->limiter < 0 || s->limiter > 2 || s->rk < 1 || s->rk > 2) return AGATE_ERR_ARG;
+  if (s->limiter == 2 && !(s->beta >= 1.0 && s->beta <= 2.0)) return AGATE_ERR_ARG;
+  if (eqset == AGATE_HALL && s->riemann == AGATE_HLLD) return AGATE_ERR_ARG;   // no Hall-HLLD in the paper
+  if (eqset == AGATE_HALL && !(s->d_i >= 0.0)) return AGATE_ERR_ARG;
+  if (eqset == AGATE_HALL && g->ndim == 3) return AGATE_ERR_ARG;               // 3-D Hall: not built yet
+  return AGATE_OK;
+}
+
+typedef void (*stage_fn_t)(const StageParams);
+
+struct StageKernel {
+  stage_fn_t fn;
+  int ty, np, threads;
+  size_t smem;
+};
+
+template <int TY, int NP, int R, bool H, int MINB>
+StageKernel make_stage() {
+  StageKernel k;
+  k.fn = stage_kernel<TY, NP, R, H, MINB>;
+  k.ty = TY; k.np = NP; k.threads = StageSmem<TY, NP>::NT; k.smem = StageSmem<TY, NP>::BYTES;
+  return k;
+}
+
+StageKernel pick_stage(int ndim, int eqset, int riemann) {
+  if (ndim == 3) {
+    if (riemann == AGATE_HLLD) return make_stage<TY3, 3, 1, false, 1>();
+    return make_stage<TY3, 3, 0, false, 1>();
+  }
+  if (eqset == AGATE_HALL) return make_stage<TY2, 1, 0, true, 2>();
+  if (riemann == AGATE_HLLD) return make_stage<TY2, 1, 1, false, 2>();
+  return make_stage<TY2, 1, 0, false, 2>();
+}
+
+}  // namespace
+
+struct agate_ctx {
+  agate_grid g;
+  agate_solver s;
+  double gamma;
+  int eqset;
+  Layout L;
+  Phys ph;
+  double dxmin, cfl;
+  cudaStream_t stream;
+  char* ws;
+  double *UA, *UB, *scal, *partial;
+  int* flag;
+  unsigned int* ticket;
+  bool have_state = false;
+  int sticky = AGATE_OK;
+  StageKernel sk;
+  dim3 sgrid;
+  int lz;
+  int dt_blocks, ghost_blocks;
+  GhostParams gpA, gpB;
+  cudaGraphExec_t graph = nullptr;
+  bool timing = false;
+  std::vector<cudaEvent_t> ev;     // pairs (start, stop) of timed stage launches
+  size_t ev_used = 0;
+  double stage_ms = 0.0;
+  int64_t stage_launches = 0;
+  int regs = 0, occ = 0;
+};
+
+namespace {
+
+#define CU_TRY(expr)                                   \
+  do {                                                 \
+    cudaError_t e__ = (expr);                          \
+    if (e__ != cudaSuccess) {                          \
+      c->sticky = AGATE_ERR_CUDA;                      \
+      return AGATE_ERR_CUDA;                           \
+    }                                                  \
+  } while (0)
+
+GhostParams make_ghost(const agate_ctx* c, double* U) {
+  GhostParams p;
+  const Layout& L = c->L;
+  p.U = U;
+  p.nx = c->g.nx; p.ny = c->g.ny; p.nz = c->g.nz;
+  p.ghy = L.ghy; p.ghz = L.ghz; p.nxp = L.nxp; p.nyp = L.nyp; p.nzp = L.nzp;
+  p.sy = L.sy; p.sz = L.sz; p.sq = L.sq;
+  p.nzs = (long long)2 * L.ghz * L.nyp * L.nxp;
+  p.nys = (long long)c->g.nz * 2 * L.ghy * L.nxp;
+  p.nxs = (long long)c->g.nz * c->g.ny * 4;
+  return p;
+}
+
+StageParams make_stage_params(const agate_ctx* c, const double* Uin, const double* U0, double* Uout, double a0,
+                              double a1) {
+  StageParams p;
+  const Layout& L = c->L;
+  p.Uin = Uin; p.U0 = U0; p.Uout = Uout; p.dt_ptr = c->scal;
+  p.a0 = a0; p.a1 = a1;
+  p.nx = c->g.nx; p.ny = c->g.ny; p.nz = c->g.nz; p.ndim = c->g.ndim;
+  p.ghy = L.ghy; p.ghz = L.ghz; p.nxp = L.nxp; p.nyp = L.nyp;
+  p.sy = L.sy; p.sz = L.sz; p.sq = L.sq;
+  p.idx = 1.0 / c->g.dx;
+  p.idy = (c->g.ndim >= 2) ? 1.0 / c->g.dy : 0.0;
+  p.idz = (c->g.ndim >= 3) ? 1.0 / c->g.dz : 0.0;
+  p.limiter = c->s.limiter; p.beta = c->s.beta;
+  p.lz = c->lz;
+  p.ph = c->ph;
+  return p;
+}
+
+int launch_ghost(agate_ctx* c, const GhostParams& gp) {
+  ghost_fill_kernel<<<c->ghost_blocks, 256, 0, c->stream>>>(gp);
+  CU_TRY(cudaGetLastError());
+  return AGATE_OK;
+}
+
+int launch_dt(agate_ctx* c, int add_t) {
+  DtParams p;
+  const Layout& L = c->L;
+  p.U = c->UA;
+  p.nx = c->g.nx; p.ny = c->g.ny; p.nz = c->g.nz; p.ghy = L.ghy; p.ghz = L.ghz;
+  p.sy = L.sy; p.sz = L.sz; p.sq = L.sq;
+  p.cfl_dx = c->cfl * c->dxmin;
+  p.ph = c->ph;
+  p.scal = c->scal; p.flag = c->flag; p.ticket = c->ticket; p.partial = c->partial;
+  p.add_t = add_t;
+  if (c->eqset == AGATE_HALL) dt_kernel<true><<<c->dt_blocks, 256, 0, c->stream>>>(p);
+  else dt_kernel<false><<<c->dt_blocks, 256, 0, c->stream>>>(p);
+  CU_TRY(cudaGetLastError());
+  return AGATE_OK;
+}
+
+int launch_stage(agate_ctx* c, const StageParams& sp) {
+  cudaEvent_t e0 = nullptr, e1 = nullptr;
+  if (c->timing) {
+    if (c->ev_used + 2 > c->ev.size()) {
+      for (int i = 0; i < 2; ++i) {
+        cudaEvent_t e;
+        CU_TRY(cudaEventCreate(&e));
+        c->ev.push_back(e);
+      }
+    }
+    e0 = c->ev[c->ev_used]; e1 = c->ev[c->ev_used + 1];
+    c->ev_used += 2;
+    CU_TRY(cudaEventRecord(e0, c->stream));
+  }
+  c->sk.fn<<<c->sgrid, c->sk.threads, c->sk.smem, c->stream>>>(sp);
+  CU_TRY(cudaGetLastError());
+  if (c->timing) CU_TRY(cudaEventRecord(e1, c->stream));
+  return AGATE_OK;
+}
+
+// One full time step enqueued on the stream; dt is already in scal[0].
+// SSP-RK22 (R11):  U1 = Un + dt L(Un);  Un+1 = Un/2 + (U1 + dt L(U1))/2.   RK11: Un+1 = Un + dt L(Un).
+int enqueue_stages(agate_ctx* c) {
+  int rc;
+  if ((rc = launch_ghost(c, c->gpA))) return rc;
+  if ((rc = launch_stage(c, make_stage_params(c, c->UA, nullptr, c->UB, 0.0, 1.0)))) return rc;
+  if (c->s.rk == 1) {
+    std::swap(c->UA, c->UB);
+    std::swap(c->gpA, c->gpB);
+    return AGATE_OK;
+  }
+  if ((rc = launch_ghost(c, c->gpB))) return rc;
+  return launch_stage(c, make_stage_params(c, c->UB, c->UA, c->UA, 0.5, 0.5));
+}
+
+int collect_status(agate_ctx* c) {
+  CU_TRY(cudaStreamSynchronize(c->stream));
+  int flag = 0;
+  CU_TRY(cudaMemcpy(&flag, c->flag, sizeof(int), cudaMemcpyDeviceToHost));
+  if (flag && c->sticky == AGATE_OK) c->sticky = AGATE_ERR_UNPHYSICAL;
+  return c->sticky;
+}
+
+int copy_state(agate_ctx* c, double* padded, double* ext, bool to_device, bool ext_is_device) {
+  const Layout& L = c->L;
+  for (int q = 0; q < 8; ++q) {
+    cudaMemcpy3DParms m;
+    memset(&m, 0, sizeof(m));
+    cudaPitchedPtr pp = make_cudaPitchedPtr(padded + (size_t)q * L.sq, sizeof(double) * L.nxp, L.nxp, L.nyp);
+    cudaPitchedPtr pe = make_cudaPitchedPtr(ext + (size_t)q * c->g.nx * c->g.ny * c->g.nz, sizeof(double) * c->g.nx,
+                                            c->g.nx, c->g.ny);
+    cudaPos ppos = make_cudaPos(sizeof(double) * 2, L.ghy, L.ghz);
+    cudaPos epos = make_cudaPos(0, 0, 0);
+    if (to_device) { m.srcPtr = pe; m.srcPos = epos; m.dstPtr = pp; m.dstPos = ppos; }
+    else { m.srcPtr = pp; m.srcPos = ppos; m.dstPtr = pe; m.dstPos = epos; }
+    m.extent = make_cudaExtent(sizeof(double) * c->g.nx, c->g.ny, c->g.nz);
+    m.kind = ext_is_device ? cudaMemcpyDeviceToDevice : (to_device ? cudaMemcpyHostToDevice : cudaMemcpyDeviceToHost);
+    CU_TRY(cudaMemcpy3DAsync(&m, c->stream));
+  }
+  return AGATE_OK;
+}
+
+}  // namespace
+
+extern "C" {
+
+size_t agate_workspace_bytes(const agate_grid* grid, int eqset, const agate_solver* solver) {
+  if (check_args(grid, 5.0 / 3.0, eqset, solver) != AGATE_OK) return 0;
+  return make_layout(*grid).total;
+}
+
+int agate_init(const agate_grid* grid, double gamma, int eqset, const agate_solver* solver, void* workspace,
+               size_t workspace_bytes, void* stream, agate_ctx** out) {
+  if (!out) return AGATE_ERR_ARG;
+  int rc = check_args(grid, gamma, eqset, solver);
+  if (rc) return rc;
+  if (!workspace) return AGATE_ERR_ARG;
+  Layout L = make_layout(*grid);
+  if (workspace_bytes < L.total || ((uintptr_t)workspace & 255u)) return AGATE_ERR_NOMEM;
+  int ndev = 0;
+  if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev < 1) return AGATE_ERR_CUDA;   // no CPU fallback
+
+  agate_ctx* c = new (std::nothrow) agate_ctx;
+  if (!c) return AGATE_ERR_NOMEM;
+  c->g = *grid; c->s = *solver; c->gamma = gamma; c->eqset = eqset; c->L = L;
+  c->dxmin = grid->dx;
+  if (grid->ndim >= 2) c->dxmin = fmin(c->dxmin, grid->dy);      // R5: min over ACTIVE dimensions
+  if (grid->ndim >= 3) c->dxmin = fmin(c->dxmin, grid->dz);
+  c->cfl = solver->cfl;
+  if (!(c->cfl > 0.0)) c->cfl = (grid->ndim == 1) ? 0.8 : (grid->ndim == 2 ? 0.45 : 0.325);
+  c->ph = make_phys(gamma, (eqset == AGATE_HALL) ? solver->d_i : 0.0, c->dxmin);
+  c->stream = (cudaStream_t)stream;
+  c->ws = (char*)workspace;
+  c->UA = (double*)(c->ws + L.off_A);
+  c->UB = (double*)(c->ws + L.off_B);
+  c->scal = (double*)(c->ws + L.off_scal);
+  c->flag = (int*)(c->ws + L.off_scal + 64);
+  c->ticket = (unsigned int*)(c->ws + L.off_scal + 128);
+  c->partial = (double*)(c->ws + L.off_partial);
+
+  c->sk = pick_stage(grid->ndim, eqset, solver->riemann);
+  cudaError_t e = cudaFuncSetAttribute((const void*)c->sk.fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)c->sk.smem);
+  cudaFuncAttributes fa;
+  if (e == cudaSuccess) e = cudaFuncGetAttributes(&fa, (const void*)c->sk.fn);
+  if (e == cudaSuccess) e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&c->occ, (const void*)c->sk.fn, c->sk.threads, c->sk.smem);
+  if (e != cudaSuccess) { delete c; return AGATE_ERR_CUDA; }
+  c->regs = fa.numRegs;
+
+  // z-chunk length: chunks of ~128 planes keep the chunk start-up (3 plane loads + 1 z-only pass) near 1 %
+  c->lz = grid->nz;
+  if (grid->ndim == 3) {
+    int want = 128;
+    if (const char* s = getenv("AGATE_LZ")) { int v = atoi(s); if (v > 0) want = v; }
+    int nchunk = (grid->nz + want - 1) / want;
+    c->lz = (grid->nz + nchunk - 1) / nchunk;
+  }
+  c->sgrid = dim3((grid->nx + TX - 1) / TX, (grid->ny + c->sk.ty - 1) / c->sk.ty,
+                  (grid->ndim == 3) ? (grid->nz + c->lz - 1) / c->lz : 1);
+  long long nrows = (long long)grid->ny * grid->nz;
+  c->dt_blocks = (int)(nrows < kDtBlocksMax ? nrows : kDtBlocksMax);
+  c->gpA = make_ghost(c, c->UA);
+  c->gpB = make_ghost(c, c->UB);
+  long long nghost = c->gpA.nzs + c->gpA.nys + c->gpA.nxs;
+  long long gb = (nghost + 255) / 256;
+  c->ghost_blocks = (int)(gb < 148 * 16 ? (gb < 1 ? 1 : gb) : 148 * 16);
+
+  if (cudaMemsetAsync(c->ws + L.off_scal, 0, L.total - L.off_scal, c->stream) != cudaSuccess) { delete c; return AGATE_ERR_CUDA; }
+  *out = c;
+  return AGATE_OK;
+}
+
+int agate_set_state(agate_ctx* c, const double* U, int src_is_device, double t0) {
+  if (!c || !U) return AGATE_ERR_ARG;
+  int rc = copy_state(c, c->UA, const_cast<double*>(U), true, src_is_device != 0);
+  if (rc) return rc;
+  const double sc[3] = {0.0, 0.0, t0};
+  CU_TRY(cudaMemcpyAsync(c->scal, sc, sizeof(sc), cudaMemcpyHostToDevice, c->stream));
+  CU_TRY(cudaMemsetAsync(c->flag, 0, sizeof(int), c->stream));
+  CU_TRY(cudaStreamSynchronize(c->stream));   // `sc` and the caller's U are borrowed only for this call
+  if ((rc = launch_ghost(c, c->gpA))) return rc;
+  c->have_state = true;
+  if (c->sticky == AGATE_ERR_UNPHYSICAL) c->sticky = AGATE_OK;
+  return AGATE_OK;
+}
+
+int agate_compute_dt(agate_ctx* c, double* dt_out) {
+  if (!c || !dt_out) return AGATE_ERR_ARG;
+  if (!c->have_state) return AGATE_ERR_STATE;
+  int rc = launch_dt(c, 0);
+  if (rc) return rc;
+  rc = collect_status(c);
+  if (rc) return rc;
+  double dt;
+  CU_TRY(cudaMemcpy(&dt, c->scal, sizeof(double), cudaMemcpyDeviceToHost));
+  *dt_out = dt;
+  return AGATE_OK;
+}
+
+int agate_step(agate_ctx* c, double dt, double* dt_used) {
+  if (!c) return AGATE_ERR_ARG;
+  if (!c->have_state) return AGATE_ERR_STATE;
+  int rc;
+  if (dt > 0.0) {
+    set_dt_kernel<<<1, 1, 0, c->stream>>>(c->scal, dt);
+    CU_TRY(cudaGetLastError());
+  } else if ((rc = launch_dt(c, 1))) {
+    return rc;
+  }
+  if ((rc = enqueue_stages(c))) return rc;
+  if (dt_used) {
+    if ((rc = collect_status(c))) return rc;
+    double v;
+    CU_TRY(cudaMemcpy(&v, c->scal, sizeof(double), cudaMemcpyDeviceToHost));
+    *dt_used = v;
+  }
+  return AGATE_OK;
+}
+
+int agate_advance(agate_ctx* c, int32_t n_steps, double* t_out) {
+  if (!c || n_steps < 0) return AGATE_ERR_ARG;
+  if (!c->have_state) return AGATE_ERR_STATE;
+  int rc;
+  // stream capture is not allowed on the legacy default stream
+  const bool use_graph = (c->s.rk == 2) && !c->timing && c->stream != nullptr && !getenv("AGATE_NO_GRAPH");
+  if (use_graph && !c->graph && n_steps > 0) {
+    cudaGraph_t g = nullptr;
+    CU_TRY(cudaStreamBeginCapture(c->stream, cudaStreamCaptureModeRelaxed));
+    rc = launch_dt(c, 1);
+    if (!rc) rc = enqueue_stages(c);
+    cudaError_t e = cudaStreamEndCapture(c->stream, &g);
+    if (rc || e != cudaSuccess) { if (g) cudaGraphDestroy(g); c->sticky = AGATE_ERR_CUDA; return AGATE_ERR_CUDA; }
+    e = cudaGraphInstantiate(&c->graph, g, 0);
+    cudaGraphDestroy(g);
+    if (e != cudaSuccess) { c->graph = nullptr; c->sticky = AGATE_ERR_CUDA; return AGATE_ERR_CUDA; }
+  }
+  for (int i = 0; i < n_steps; ++i) {
+    if (use_graph) {
+      CU_TRY(cudaGraphLaunch(c->graph, c->stream));
+    } else {
+      if ((rc = launch_dt(c, 1))) return rc;
+      if ((rc = enqueue_stages(c))) return rc;
+    }
+  }
+  if (t_out) {
+    if ((rc = collect_status(c))) return rc;
+    double sc[3];
+    CU_TRY(cudaMemcpy(sc, c->scal, sizeof(sc), cudaMemcpyDeviceToHost));
+    *t_out = sc[2];
+  }
+  return AGATE_OK;
+}
+
+int agate_get_state(agate_ctx* c, double* U_out, int dst_is_device, double* t_out) {
+  if (!c || !U_out) return AGATE_ERR_ARG;
+  if (!c->have_state) return AGATE_ERR_STATE;
+  int rc = copy_state(c, c->UA, U_out, false, dst_is_device != 0);
+  if (rc) return rc;
+  if (!dst_is_device || t_out) {
+    CU_TRY(cudaStreamSynchronize(c->stream));
+    if (t_out) {
+      double sc[3];
+      CU_TRY(cudaMemcpy(sc, c->scal, sizeof(sc), cudaMemcpyDeviceToHost));
+      *t_out = sc[2];
+    }
+  }
+  return AGATE_OK;
+}
+
+int agate_poll(agate_ctx* c) {
+  if (!c) return AGATE_ERR_ARG;
+  return collect_status(c);
+}
+
+int agate_launch_info(agate_ctx* c, int64_t out[8]) {
+  if (!c || !out) return AGATE_ERR_ARG;
+  out[0] = c->sgrid.x; out[1] = c->sgrid.y; out[2] = c->sgrid.z;
+  out[3] = c->sk.threads; out[4] = (int64_t)c->sk.smem; out[5] = c->regs; out[6] = c->occ;
+  out[7] = (c->s.rk == 2) ? 5 : 3;   // dt + (ghost + stage) per RK stage
+  return AGATE_OK;
+}
+
+int agate_set_timing(agate_ctx* c, int enabled) {
+  if (!c) return AGATE_ERR_ARG;
+  c->timing = enabled != 0;
+  return AGATE_OK;
+}
+
+int agate_stage_time(agate_ctx* c, double* ms_out, int64_t* launches_out, int reset) {
+  if (!c) return AGATE_ERR_ARG;
+  CU_TRY(cudaStreamSynchronize(c->stream));
+  for (size_t i = 0; i + 1 < c->ev_used; i += 2) {
+    float ms = 0.f;
+    CU_TRY(cudaEventElapsedTime(&ms, c->ev[i], c->ev[i + 1]));
+    c->stage_ms += ms;
+    c->stage_launches += 1;
+  }
+  c->ev_used = 0;
+  if (ms_out) *ms_out = c->stage_ms;
+  if (launches_out) *launches_out = c->stage_launches;
+  if (reset) { c->stage_ms = 0.0; c->stage_launches = 0; }
+  return AGATE_OK;
+}
+
+int agate_destroy(agate_ctx* c) {
+  if (!c) return AGATE_ERR_ARG;
+  cudaStreamSynchronize(c->stream);
+  if (c->graph) cudaGraphExecDestroy(c->graph);
+  for (cudaEvent_t e : c->ev) cudaEventDestroy(e);
+  delete c;
+  return AGATE_OK;
+}
+
+const char* agate_strerror(int status) {
+  switch (status) {
+    case AGATE_OK: return "ok";
+    case AGATE_ERR_ARG: return "invalid argument or unsupported combination";
+    case AGATE_ERR_STATE: return "call order: no state set";
+    case AGATE_ERR_UNPHYSICAL: return "unphysical state (rho <= 0, p <= 0 or non-finite speed)";
+    case AGATE_ERR_CUDA: return "CUDA error or no CUDA device";
+    case AGATE_ERR_NOMEM: return "workspace too small or misaligned";
+    default: return "unknown status";
+  }
+}
+
+int agate_test_face_flux(int eqset, int riemann, int dir, double gamma, double d_i, double dxmin, const double* WL,
+                         const double* WR, const double* J, double* F, int64_t n, void* stream) {
+  if (!WL || !WR || !F || n < 0 || dir < 0 || dir > 2 || !(gamma > 1.0)) return AGATE_ERR_ARG;
+  if (eqset == AGATE_HALL && riemann == AGATE_HLLD) return AGATE_ERR_ARG;
+  int ndev = 0;
+  if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev < 1) return AGATE_ERR_CUDA;
+  if (n == 0) return AGATE_OK;
+  Phys ph = make_phys(gamma, (eqset == AGATE_HALL) ? d_i : 0.0, dxmin);
+  const int nb = (int)((n + 127) / 128);
+  cudaStream_t st = (cudaStream_t)stream;
+  if (eqset == AGATE_HALL) face_flux_kernel<0, true><<<nb, 128, 0, st>>>(ph, dir, WL, WR, J, F, n);
+  else if (riemann == AGATE_HLLD) face_flux_kernel<1, false><<<nb, 128, 0, st>>>(ph, dir, WL, WR, J, F, n);
+  else face_flux_kernel<0, false><<<nb, 128, 0, st>>>(ph, dir, WL, WR, J, F, n);
+  if (cudaGetLastError() != cudaSuccess) return AGATE_ERR_CUDA;
+  if (cudaStreamSynchronize(st) != cudaSuccess) return AGATE_ERR_CUDA;
+  return AGATE_OK;
+}
+
+int agate_measure_fp64_peak(int iters, double* tflops_out, void* stream) {
+  if (!tflops_out || iters < 1) return AGATE_ERR_ARG;
+  int ndev = 0, dev = 0, sms = 0;
+  if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev < 1) return AGATE_ERR_CUDA;
+  cudaGetDevice(&dev);
+  cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
+  cudaStream_t st = (cudaStream_t)stream;
+  double* d = nullptr;
+  if (cudaMalloc(&d, 64) != cudaSuccess) return AGATE_ERR_CUDA;   // diagnostic only: 64 bytes, freed below
+  const int blocks = sms * 8, trips = 4096;
+  cudaEvent_t e0, e1;
+  cudaEventCreate(&e0); cudaEventCreate(&e1);
+  fp64_peak_kernel<<<blocks, 256, 0, st>>>(d, trips, 1.0000001, 1e-9);   // warm-up
+  cudaEventRecord(e0, st);
+  for (int i = 0; i < iters; ++i) fp64_peak_kernel<<<blocks, 256, 0, st>>>(d, trips, 1.0000001, 1e-9);
+  cudaEventRecord(e1, st);
+  cudaError_t e = cudaEventSynchronize(e1);
+  float ms = 0.f;
+  cudaEventElapsedTime(&ms, e0, e1);
+  cudaEventDestroy(e0); cudaEventDestroy(e1);
+  cudaFree(d);
+  if (e != cudaSuccess || !(ms > 0.f)) return AGATE_ERR_CUDA;
+  const double flops = 2.0 * 8 * 16 * (double)trips * 256.0 * blocks * iters;
+  *tflops_out = flops / (ms * 1e-3) / 1e12;
+  return AGATE_OK;
+}
+
+}  // extern "C"

@@ -1,0 +1,479 @@
+// agate_kernels.cuh — the three hot-path kernels (A0 ghost fill, A1-A6 fused stage, A7 dt reduction) plus the
+// two diagnostic kernels.  sm_100a, fp64, SoA, ghost-padded storage  U[8][nz+2gz][ny+2gy][nx+4].
+//
+// Fused stage kernel (one launch per Runge-Kutta stage; SURVEY §8(a) rows A1-A6[+A8]):
+//   * a CTA owns an x-y tile of TX=32 x TY cells and MARCHES along z over a chunk of planes (2.5-D streaming).
+//     Primitive variables W live only in shared memory: a ring of NP x-extended planes (TY rows of TX+4 cells)
+//     plus the four y-halo rows ("strips") of the current plane.  U is read from HBM/L2 once per stage per cell
+//     (plus the halo overlap of neighbouring tiles) and written once.
+//   * per plane, per direction: limited slopes are computed ONCE per cell (pool of cells incl. one halo ring)
+//     into the shared buffer S, every face flux is computed ONCE (pool of faces incl. the tile's low edge) into
+//     the shared buffer Fb, then each cell takes the difference of its two faces.  The CTA has TY+2 warps so
+//     that every pool fits one round; the two extra warps only work on the halo/edge tasks.
+//   * z direction: each thread owns its column; the left face state W(k)+dW(k)/2 and the flux F(k-1/2) of the
+//     previous plane are carried in per-thread shared-memory slots (WLz, Fzp), so every z slope and z flux is
+//     also computed once.
+//   * the Riemann solvers work in a rotated frame (agate_physics.cuh); the direction is a RUN-TIME value that
+//     only changes shared-memory indices, so there is ONE copy of the solver in the instruction stream.
+//   * epilogue = Runge-Kutta combine  Uout = a0*U0 + a1*(Uin + dt*L)  (A6), dt read from a device scalar.
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+#include "agate_physics.cuh"
+
+namespace agate {
+
+constexpr int TX = 32;        // tile width = warp width
+constexpr int RS = TX + 4;    // shared-memory row stride (2 halo cells each side)
+
+struct StageParams {
+  const double* Uin;     // stage input, ghosts filled
+  const double* U0;      // U^n for the combine (may alias Uout); unused when a0 == 0
+  double* Uout;
+  const double* dt_ptr;  // device scalar
+  double a0, a1;         // Uout = a0*U0 + a1*(Uin + dt*L)
+  int nx, ny, nz, ndim;
+  int ghy, ghz;          // ghost widths (2 if the dimension is active, else 0)
+  int nxp, nyp;          // padded extents
+  long long sy, sz, sq;  // element strides: row, plane, variable
+  double idx, idy, idz;  // 1/dx, 1/dy, 1/dz
+  int limiter;
+  double beta;
+  int lz;                // z-chunk length per CTA
+  Phys ph;
+};
+
+template <int TY, int NP>
+struct StageSmem {
+  static constexpr int NT = 32 * (TY + 2);
+  static constexpr int NCELL = 32 * TY;
+  static constexpr int PLANE = TY * RS;
+  static constexpr int STRIP0 = NP * PLANE;
+  static constexpr int NSLOT = STRIP0 + 4 * RS;
+  static constexpr int NS = 32 * (TY + 2);   // >= 34*TY slope cells (x) and 32*(TY+2) (y)
+  static constexpr int NF = 32 * (TY + 1);   // >= 33*TY faces (x) and 32*(TY+1) (y)
+  static constexpr int ZPRIV = (NP > 1) ? 2 * 8 * NCELL : 0;
+  static constexpr size_t BYTES = sizeof(double) * (size_t)(8 * NSLOT + 8 * NS + 8 * NF + ZPRIV);
+};
+
+template <int TY, int NP, int RIEMANN, bool HALL, int MINB>
+__global__ void __launch_bounds__(32 * (TY + 2), MINB) stage_kernel(const __grid_constant__ StageParams P) {
+  using SM = StageSmem<TY, NP>;
+  constexpr int NT = SM::NT, NCELL = SM::NCELL, PLANE = SM::PLANE, STRIP0 = SM::STRIP0, NSLOT = SM::NSLOT;
+  constexpr int NS = SM::NS, NF = SM::NF;
+  extern __shared__ __align__(16) double smem[];
+  double* const W = smem;              // [8][NSLOT]  primitives: ring planes + strips
+  double* const S = W + 8 * NSLOT;     // [8][NS]     limited slopes of the current direction
+  double* const Fb = S + 8 * NS;       // [8][NF]     face fluxes of the current direction (fixed frame)
+  double* const WLz = Fb + 8 * NF;     // [8][NCELL]  z: left state of the next face (per-thread slot)
+  double* const Fzp = WLz + 8 * NCELL; // [8][NCELL]  z: flux through the lower face (per-thread slot)
+
+  const int tid = threadIdx.x;
+  const int x0 = blockIdx.x * TX, y0 = blockIdx.y * TY;
+  const int tw = min(TX, P.nx - x0), th = min(TY, P.ny - y0);
+  const bool threeD = (NP > 1);
+  const int k0 = threeD ? blockIdx.z * P.lz : 0;
+  const int k1 = threeD ? min(P.nz, k0 + P.lz) : 1;
+  const double dt = *P.dt_ptr;
+  const int ci = tid & 31, cj = tid >> 5;
+  const bool cell_ok = (tid < NCELL) && (ci < tw) && (cj < th);
+  const int limiter = P.limiter;
+  const double beta = P.beta;
+
+  // ---- A1: load conserved cells of plane kk (interior index; may be a ghost plane) and store primitives ----
+  auto load_plane = [&](int kk, int ringbase, bool rows, bool strips) {
+    const int ntask = (rows ? PLANE : 0) + ((strips && P.ghy > 0) ? 4 * RS : 0);
+    const long long gz = (long long)(kk + P.ghz) * P.sz;
+    for (int t0 = tid; t0 < ntask; t0 += NT) {
+      int t = t0, slot, j;
+      if (rows && t < PLANE) {
+        j = t / RS;
+        slot = ringbase + t;
+      } else {
+        if (rows) t -= PLANE;
+        const int r = t / RS;
+        j = (r < 2) ? r - 2 : TY + r - 2;
+        slot = STRIP0 + t;
+      }
+      const int c = t % RS;
+      const int gx = x0 + c, gy = y0 + j + P.ghy;
+      if (gx < P.nxp && gy >= 0 && gy < P.nyp) {
+        const long long g = gz + (long long)gy * P.sy + gx;
+        double u[8], w[8];
+#pragma unroll
+        for (int q = 0; q < 8; ++q) u[q] = __ldg(P.Uin + q * P.sq + g);
+        cons_to_prim(P.ph, u, w);
+#pragma unroll
+        for (int q = 0; q < 8; ++q) W[q * NSLOT + slot] = w[q];
+      }
+    }
+  };
+  auto ring_of = [&](int kk) { return ((kk + 3) % 3) * PLANE; };   // kk >= -2
+
+  int kstart = 0;
+  if (threeD) {
+    // prologue: planes k0-2, k0-1, k0  ->  WLz = W(k0-1) + dW_z(k0-1)/2 for the own column
+    kstart = k0 - 1;
+    load_plane(k0 - 2, ring_of(k0 - 2), true, false);
+    load_plane(k0 - 1, ring_of(k0 - 1), true, false);
+    load_plane(k0, ring_of(k0), true, false);
+    __syncthreads();
+    if (cell_ok) {
+      const int off = cj * RS + ci + 2;
+      const int ca = ring_of(k0 - 2) + off, cb = ring_of(k0 - 1) + off, cc = ring_of(k0) + off;
+#pragma unroll
+      for (int q = 0; q < 8; ++q) {
+        const double a = W[q * NSLOT + ca], b = W[q * NSLOT + cb], c = W[q * NSLOT + cc];
+        WLz[q * NCELL + tid] = b + 0.5 * limited_slope(limiter, beta, c - b, b - a);
+      }
+    }
+  }
+
+  for (int k = kstart; k < k1; ++k) {
+    const bool zonly = threeD && (k < k0);        // first pass of a chunk only produces F_z(k0-1/2)
+    const int cur = threeD ? ring_of(k) : 0;
+    __syncthreads();                              // everyone is done with the ring slot about to be overwritten
+    if (threeD) load_plane(k + 2, ring_of(k + 2), true, false);
+    if (!zonly) load_plane(k, cur, !threeD, true);
+    __syncthreads();
+
+    auto rowoff = [&](int j) {
+      return (j >= 0 && j < TY) ? cur + j * RS : STRIP0 + ((j < 0) ? j + 2 : j - TY + 2) * RS;
+    };
+
+    double acc[8];
+#pragma unroll
+    for (int q = 0; q < 8; ++q) acc[q] = 0.0;
+
+#pragma unroll 1
+    for (int d = zonly ? 2 : 0; d < P.ndim; ++d) {
+      double L[8], R[8], Jr[3];
+      bool active = false;
+      int fidx = 0;
+      if (d == 0) {
+        // ---- A2 slopes along x: cells i = -1..tw of rows 0..th-1 ----
+        if (tid < 34 * TY) {
+          const int j = tid / 34, ii = tid - j * 34;
+          if (j < th && ii <= tw + 1) {
+            const int c = cur + j * RS + ii + 1;
+#pragma unroll
+            for (int q = 0; q < 8; ++q) {
+              const double a = W[q * NSLOT + c - 1], b = W[q * NSLOT + c], cc = W[q * NSLOT + c + 1];
+              S[q * NS + tid] = limited_slope(limiter, beta, cc - b, b - a);
+            }
+          }
+        }
+        __syncthreads();
+        // ---- face i-1/2 .. : faces fi = 0..tw of rows 0..th-1 ----
+        if (tid < 33 * TY) {
+          const int j = tid / 33, fi = tid - j * 33;
+          if (j < th && fi <= tw) {
+            active = true;
+            fidx = tid;
+            const int cL = cur + j * RS + fi + 1, sL = j * 34 + fi;
+#pragma unroll
+            for (int r = 0; r < 8; ++r) {
+              const int v = rot_var(r, 0);
+              L[r] = W[v * NSLOT + cL] + 0.5 * S[v * NS + sL];
+              R[r] = W[v * NSLOT + cL + 1] - 0.5 * S[v * NS + sL + 1];
+            }
+            if (HALL) {
+              // R15: J = curl B at the x-face from cell-centred B (vars 5,6,7) of the stage input
+              const double* Bx = W + 5 * NSLOT; const double* By = W + 6 * NSLOT; const double* Bz = W + 7 * NSLOT;
+              const int cR = cL + 1;
+              const double dxBy = (By[cR] - By[cL]) * P.idx, dxBz = (Bz[cR] - Bz[cL]) * P.idx;
+              double dyBx = 0.0, dyBz = 0.0;
+              if (P.ndim >= 2) {
+                const int up = rowoff(j + 1) - rowoff(j), dn = rowoff(j - 1) - rowoff(j);
+                const double h = 0.25 * P.idy;      // 0.5 * (...) / (2 dy)
+                dyBx = ((Bx[cL + up] - Bx[cL + dn]) + (Bx[cR + up] - Bx[cR + dn])) * h;
+                dyBz = ((Bz[cL + up] - Bz[cL + dn]) + (Bz[cR + up] - Bz[cR + dn])) * h;
+              }
+              // J = (dyBz - dzBy, dzBx - dxBz, dxBy - dyBx), dz == 0 here
+              Jr[0] = dyBz; Jr[1] = -dxBz; Jr[2] = dxBy - dyBx;     // rotated for n = 0: (Jx, Jy, Jz)
+            }
+          }
+        }
+      } else if (d == 1) {
+        // ---- A2 slopes along y: rows j = -1..th ----
+        {
+          const int jj = tid >> 5, i = tid & 31, j = jj - 1;
+          if (i < tw && j <= th) {
+            const int c = rowoff(j) + i + 2, cm = rowoff(j - 1) + i + 2, cp = rowoff(j + 1) + i + 2;
+#pragma unroll
+            for (int q = 0; q < 8; ++q) {
+              const double a = W[q * NSLOT + cm], b = W[q * NSLOT + c], cc = W[q * NSLOT + cp];
+              S[q * NS + tid] = limited_slope(limiter, beta, cc - b, b - a);
+            }
+          }
+        }
+        __syncthreads();
+        if (tid < 32 * (TY + 1)) {
+          const int fj = tid >> 5, i = tid & 31;
+          if (i < tw && fj <= th) {
+            active = true;
+            fidx = tid;
+            const int cL = rowoff(fj - 1) + i + 2, cR = rowoff(fj) + i + 2;
+#pragma unroll
+            for (int r = 0; r < 8; ++r) {
+              const int v = rot_var(r, 1);
+              L[r] = W[v * NSLOT + cL] + 0.5 * S[v * NS + tid];
+              R[r] = W[v * NSLOT + cR] - 0.5 * S[v * NS + tid + 32];
+            }
+            if (HALL) {
+              const double* Bx = W + 5 * NSLOT; const double* By = W + 6 * NSLOT; const double* Bz = W + 7 * NSLOT;
+              const double dyBx = (Bx[cR] - Bx[cL]) * P.idy, dyBz = (Bz[cR] - Bz[cL]) * P.idy;
+              const double h = 0.25 * P.idx;
+              const double dxBy = ((By[cL + 1] - By[cL - 1]) + (By[cR + 1] - By[cR - 1])) * h;
+              const double dxBz = ((Bz[cL + 1] - Bz[cL - 1]) + (Bz[cR + 1] - Bz[cR - 1])) * h;
+              const double Jx = dyBz, Jy = -dxBz, Jz = dxBy - dyBx;
+              Jr[0] = Jy; Jr[1] = Jz; Jr[2] = Jx;                    // rotated for n = 1: (Jy, Jz, Jx)
+            }
+          }
+        }
+      } else {
+        // ---- z: own column.  dW_z(k+1) from planes k, k+1, k+2; left state carried in WLz ----
+        if (cell_ok) {
+          active = true;
+          const int off = cj * RS + ci + 2;
+          const int ca = ring_of(k) + off, cb = ring_of(k + 1) + off, cc = ring_of(k + 2) + off;
+#pragma unroll
+          for (int r = 0; r < 8; ++r) {
+            const int v = rot_var(r, 2);
+            const double a = W[v * NSLOT + ca], b = W[v * NSLOT + cb], c = W[v * NSLOT + cc];
+            const double hs = 0.5 * limited_slope(limiter, beta, c - b, b - a);
+            L[r] = WLz[v * NCELL + tid];
+            R[r] = b - hs;
+            WLz[v * NCELL + tid] = b + hs;
+          }
+          if (HALL) { Jr[0] = 0.0; Jr[1] = 0.0; Jr[2] = 0.0; }      // 3-D Hall is rejected by agate_init
+        }
+      }
+
+      // ---- A3 + A4 (+A8): ONE call site of the Riemann solver for all directions ----
+      double Ff[8];
+      if (active) {
+        double Fr[8];
+        riemann_flux<RIEMANN, HALL>(P.ph, L, R, HALL ? Jr : nullptr, Fr);
+        unrotate(d, Fr, Ff);
+      }
+
+      // ---- A5: flux difference ----
+      if (d < 2) {
+        if (active) {
+#pragma unroll
+          for (int q = 0; q < 8; ++q) Fb[q * NF + fidx] = Ff[q];
+        }
+        __syncthreads();
+        if (cell_ok) {
+          const int lo = (d == 0) ? cj * 33 + ci : cj * 32 + ci;
+          const int hi = (d == 0) ? lo + 1 : lo + 32;
+          const double ih = (d == 0) ? P.idx : P.idy;
+#pragma unroll
+          for (int q = 0; q < 8; ++q) acc[q] -= (Fb[q * NF + hi] - Fb[q * NF + lo]) * ih;
+        }
+      } else if (cell_ok) {
+#pragma unroll
+        for (int q = 0; q < 8; ++q) {
+          if (!zonly) acc[q] -= (Ff[q] - Fzp[q * NCELL + tid]) * P.idz;
+          Fzp[q * NCELL + tid] = Ff[q];
+        }
+      }
+    }
+
+    // ---- A6: Runge-Kutta combine and store ----
+    if (cell_ok && !zonly) {
+      const long long g = (long long)(k + P.ghz) * P.sz + (long long)(y0 + cj + P.ghy) * P.sy + (x0 + ci + 2);
+#pragma unroll
+      for (int q = 0; q < 8; ++q) {
+        double val = __ldg(P.Uin + q * P.sq + g) + dt * acc[q];
+        if (P.a0 != 0.0) val = P.a0 * P.U0[q * P.sq + g] + P.a1 * val;
+        P.Uout[q * P.sq + g] = val;
+      }
+    }
+  }
+}
+
+// ------------------------------------------------------------------------------------------------------------
+// A0: periodic ghost fill.  One thread per ghost cell (faces, edges, corners): value of the interior cell at
+// the index wrapped mod n (R13).  Slab enumeration: z-ghost planes, then y-ghost rows, then x-ghost columns.
+// ------------------------------------------------------------------------------------------------------------
+struct GhostParams {
+  double* U;
+  int nx, ny, nz, ghy, ghz, nxp, nyp, nzp;
+  long long sy, sz, sq;
+  long long nzs, nys, nxs;   // cells in the z-, y-, x-slabs
+};
+
+__global__ void __launch_bounds__(256) ghost_fill_kernel(const __grid_constant__ GhostParams P) {
+  const long long total = P.nzs + P.nys + P.nxs;
+  for (long long t = (long long)blockIdx.x * blockDim.x + threadIdx.x; t < total;
+       t += (long long)gridDim.x * blockDim.x) {
+    int ip, jp, kp;   // padded coordinates of the ghost cell
+    if (t < P.nzs) {
+      const long long pl = (long long)P.nyp * P.nxp;
+      const int s = (int)(t / pl);
+      const long long r = t - (long long)s * pl;
+      kp = (s < P.ghz) ? s : P.nzp - 2 * P.ghz + s;
+      jp = (int)(r / P.nxp);
+      ip = (int)(r - (long long)jp * P.nxp);
+    } else if (t < P.nzs + P.nys) {
+      const long long u = t - P.nzs;
+      const long long per = (long long)2 * P.ghy * P.nxp;
+      const int kk = (int)(u / per);
+      const long long r = u - (long long)kk * per;
+      const int s = (int)(r / P.nxp);
+      kp = kk + P.ghz;
+      jp = (s < P.ghy) ? s : P.nyp - 2 * P.ghy + s;
+      ip = (int)(r - (long long)s * P.nxp);
+    } else {
+      const long long u = t - P.nzs - P.nys;
+      const long long row = u >> 2;
+      const int s = (int)(u & 3);
+      const int kk = (int)(row / P.ny);
+      kp = kk + P.ghz;
+      jp = (int)(row - (long long)kk * P.ny) + P.ghy;
+      ip = (s < 2) ? s : P.nxp - 4 + s;
+    }
+    int i = (ip - 2) % P.nx;          if (i < 0) i += P.nx;
+    int j = (jp - P.ghy) % P.ny;      if (j < 0) j += P.ny;
+    int k = (kp - P.ghz) % P.nz;      if (k < 0) k += P.nz;
+    const long long dst = (long long)kp * P.sz + (long long)jp * P.sy + ip;
+    const long long src = (long long)(k + P.ghz) * P.sz + (long long)(j + P.ghy) * P.sy + (i + 2);
+#pragma unroll
+    for (int q = 0; q < 8; ++q) P.U[q * P.sq + dst] = P.U[q * P.sq + src];
+  }
+}
+
+// ------------------------------------------------------------------------------------------------------------
+// A7: global Courant reduction.  Each thread scans cells of whole grid rows (coalesced), warp-shuffle max, one
+// shared-memory pass per block, block results to `partial`; the last block to finish (ticket counter) reduces
+// the partials, writes  scal[1] = v_max,  scal[0] = dt = C dx_min / v_max  and, if add_t, scal[2] += dt.
+// max is exact under any association, so the result is deterministic.
+// ------------------------------------------------------------------------------------------------------------
+struct DtParams {
+  const double* U;
+  int nx, ny, nz, ghy, ghz;
+  long long sy, sz, sq;
+  double cfl_dx;     // C * dx_min
+  Phys ph;
+  double* scal;      // [0] dt, [1] vmax, [2] t
+  int* flag;         // sticky: 1 = unphysical cell seen
+  unsigned int* ticket;
+  double* partial;   // [gridDim.x]
+  int add_t;
+};
+
+__device__ __forceinline__ double warp_max(double v) {
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) v = fmax(v, __shfl_xor_sync(0xffffffffu, v, o));
+  return v;
+}
+
+template <bool HALL>
+__global__ void __launch_bounds__(256) dt_kernel(const __grid_constant__ DtParams P) {
+  __shared__ double wmax[8];
+  __shared__ int wbad[8];
+  __shared__ bool last;
+  double vm = 0.0;
+  int bad = 0;
+  const long long nrows = (long long)P.ny * P.nz;
+  for (long long r = blockIdx.x; r < nrows; r += gridDim.x) {
+    const int kk = (int)(r / P.ny), jj = (int)(r - (long long)kk * P.ny);
+    const long long base = (long long)(kk + P.ghz) * P.sz + (long long)(jj + P.ghy) * P.sy + 2;
+    for (int i = threadIdx.x; i < P.nx; i += blockDim.x) {
+      double u[8];
+#pragma unroll
+      for (int q = 0; q < 8; ++q) u[q] = __ldg(P.U + q * P.sq + base + i);
+      const double sp = cell_speed<HALL>(P.ph, u);
+      if (sp < 0.0) bad = 1; else vm = fmax(vm, sp);
+    }
+  }
+  vm = warp_max(vm);
+  bad = __any_sync(0xffffffffu, bad);
+  const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
+  if (lane == 0) { wmax[wid] = vm; wbad[wid] = bad; }
+  __syncthreads();
+  if (wid == 0) {
+    vm = (lane < (int)(blockDim.x >> 5)) ? wmax[lane] : 0.0;
+    bad = (lane < (int)(blockDim.x >> 5)) ? wbad[lane] : 0;
+    vm = warp_max(vm);
+    bad = __any_sync(0xffffffffu, bad);
+    if (lane == 0) {
+      P.partial[blockIdx.x] = vm;
+      if (bad) atomicOr(P.flag, 1);
+      __threadfence();
+      const unsigned int tk = atomicAdd(P.ticket, 1u);
+      last = (tk == gridDim.x - 1);
+    }
+  }
+  __syncthreads();
+  if (last) {
+    __threadfence();
+    double v = 0.0;
+    for (int b = threadIdx.x; b < (int)gridDim.x; b += blockDim.x) v = fmax(v, P.partial[b]);
+    v = warp_max(v);
+    if (lane == 0) wmax[wid] = v;
+    __syncthreads();
+    if (wid == 0) {
+      v = (lane < (int)(blockDim.x >> 5)) ? wmax[lane] : 0.0;
+      v = warp_max(v);
+      if (lane == 0) {
+        const double dt = P.cfl_dx / v;
+        P.scal[1] = v;
+        P.scal[0] = dt;
+        if (P.add_t) P.scal[2] += dt;
+        *P.ticket = 0u;
+      }
+    }
+  }
+}
+
+// host-chosen dt (agate_step with dt > 0): scal[0] = dt, t += dt
+__global__ void set_dt_kernel(double* scal, double dt) {
+  scal[0] = dt;
+  scal[2] += dt;
+}
+
+// ------------------------------------------------------------------------------------------------------------
+// Diagnostics
+// ------------------------------------------------------------------------------------------------------------
+template <int RIEMANN, bool HALL>
+__global__ void face_flux_kernel(Phys ph, int dir, const double* WL, const double* WR, const double* J, double* F,
+                                 long long n) {
+  const long long t = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  if (t >= n) return;
+  double L[8], R[8], Jr[3] = {0.0, 0.0, 0.0}, Fr[8], Ff[8];
+#pragma unroll
+  for (int r = 0; r < 8; ++r) {
+    const int v = rot_var(r, dir);
+    L[r] = WL[v * n + t];
+    R[r] = WR[v * n + t];
+  }
+  if (HALL && J) {
+#pragma unroll
+    for (int c = 0; c < 3; ++c) Jr[c] = J[((dir + c) % 3) * n + t];
+  }
+  riemann_flux<RIEMANN, HALL>(ph, L, R, HALL ? Jr : nullptr, Fr);
+  unrotate(dir, Fr, Ff);
+#pragma unroll
+  for (int q = 0; q < 8; ++q) F[q * n + t] = Ff[q];
+}
+
+// 8 independent DFMA chains per thread; 2 * 8 * inner flops per thread per outer trip
+__global__ void __launch_bounds__(256) fp64_peak_kernel(double* out, int trips, double a, double b) {
+  double x0 = threadIdx.x * 1e-3, x1 = x0 + 1, x2 = x0 + 2, x3 = x0 + 3, x4 = x0 + 4, x5 = x0 + 5, x6 = x0 + 6,
+         x7 = x0 + 7;
+  for (int t = 0; t < trips; ++t) {
+#pragma unroll
+    for (int u = 0; u < 16; ++u) {
+      x0 = fma(x0, a, b); x1 = fma(x1, a, b); x2 = fma(x2, a, b); x3 = fma(x3, a, b);
+      x4 = fma(x4, a, b); x5 = fma(x5, a, b); x6 = fma(x6, a, b); x7 = fma(x7, a, b);
+    }
+  }
+  const double s = ((x0 + x1) + (x2 + x3)) + ((x4 + x5) + (x6 + x7));
+  if (s == 12345.678) out[0] = s;   // keeps the chains alive; practically never true
+}
+
+}  // namespace agate

@@ -1,0 +1,321 @@
+// agate_physics.cuh — point functions of the AGATE finite-volume step (CUDA path).
+//
+// Everything here works in the ROTATED frame of one face: a state is
+//     w[0]=rho  w[1]=u (normal velocity)  w[2]=v  w[3]=w (transverse, cyclic order)
+//     w[4]=p    w[5]=Bn                   w[6]=Bt1 w[7]=Bt2
+// and a flux F[8] is ordered the same way (F[1] = normal momentum flux, F[5] = flux of Bn).
+// The callers (stage kernel, unit-test kernel) permute variables when they read/write shared or global memory,
+// so ONE body of each Riemann solver serves the x, y and z sweeps.
+//
+// Citations: PAPER.md (P:Lnnn) and the readings Rn of DESIGN.md.
+//   cons<->prim            P:L140 (R2: p/(gamma-1))
+//   eq.4 limiter           P:L97-102 (R7)
+//   fast speed eq.12       P:L148-151 (R3), whistler speed eq.13
+//   physical flux eqs.7-10 P:L128-140 with psi == 0 (R12)
+//   HLL eq.5 + Davis eq.6  P:L104-116 (R8, R9)
+//   HLLD                   R10 (Miyoshi-Kusano five-wave solver; outer speeds from eq.6; Bn = mean; F[Bn] = 0)
+//   Hall v_T = v + v_H     P:L140 (R15)
+//
+// Functions are __host__ __device__ so that the host-only unit test (tests/test_physics_host.py) can compile
+// this header with g++ and compare it against the oracle without a GPU.  The file shares nothing with oracle/.
+#pragma once
+#include <math.h>
+
+#if defined(__CUDACC__)
+#define AG_HD __host__ __device__ __forceinline__
+#else
+#define AG_HD inline
+#endif
+
+namespace agate {
+
+constexpr double kHlldEps = 1e-12;  // R10 guards
+
+struct Phys {
+  double gamma;   // adiabatic index
+  double gm1;     // gamma - 1
+  double igm1;    // 1 / (gamma - 1)
+  double gogm1;   // gamma / (gamma - 1)
+  double d_i;     // Hall: normalised ion inertial length
+  double cwk;     // Hall: d_i * pi / (2 dx_min)   (eq.13 with k_max = pi / dx_min, R15)
+};
+
+AG_HD Phys make_phys(double gamma, double d_i, double dxmin) {
+  Phys ph;
+  ph.gamma = gamma;
+  ph.gm1 = gamma - 1.0;
+  ph.igm1 = 1.0 / (gamma - 1.0);
+  ph.gogm1 = gamma / (gamma - 1.0);
+  ph.d_i = d_i;
+  ph.cwk = d_i * 3.14159265358979323846264338327950288 / (2.0 * dxmin);
+  return ph;
+}
+
+// rotated slot r (rho,u,v,w,p,Bn,Bt1,Bt2) -> fixed variable index for face normal n
+AG_HD int rot_var(int r, int n) {
+  const int base = (r >= 5) ? 5 : 1;
+  const int c = (r >= 5) ? r - 5 : r - 1;
+  if (r == 0) return 0;
+  if (r == 4) return 4;
+  int d = n + c;
+  d = (d >= 3) ? d - 3 : d;
+  return base + d;
+}
+
+// rotated flux -> fixed (x,y,z) component order, by selects (no dynamic register indexing)
+AG_HD void unrotate(int n, const double r[8], double f[8]) {
+  f[0] = r[0];
+  f[4] = r[4];
+  f[1] = (n == 0) ? r[1] : ((n == 1) ? r[3] : r[2]);
+  f[2] = (n == 0) ? r[2] : ((n == 1) ? r[1] : r[3]);
+  f[3] = (n == 0) ? r[3] : ((n == 1) ? r[2] : r[1]);
+  f[5] = (n == 0) ? r[5] : ((n == 1) ? r[7] : r[6]);
+  f[6] = (n == 0) ? r[6] : ((n == 1) ? r[5] : r[7]);
+  f[7] = (n == 0) ? r[7] : ((n == 1) ? r[6] : r[5]);
+}
+
+// Reciprocal / reciprocal square root.  One place to change the precision policy; both are IEEE-correct
+// division / sqrt today (parity budget 1e-12 would also admit 1-2 ulp versions).
+AG_HD double rcp(double x) { return 1.0 / x; }
+AG_HD double rsq(double x) { return 1.0 / sqrt(x); }
+
+// A1 (R2): fixed-frame conserved (rho, m, E, B) -> primitive (rho, v, p, B).  Frame-agnostic.
+AG_HD void cons_to_prim(const Phys& ph, const double U[8], double W[8]) {
+  const double ir = rcp(U[0]);
+  const double vx = U[1] * ir, vy = U[2] * ir, vz = U[3] * ir;
+  const double v2 = vx * vx + vy * vy + vz * vz;
+  const double b2 = U[5] * U[5] + U[6] * U[6] + U[7] * U[7];
+  W[0] = U[0]; W[1] = vx; W[2] = vy; W[3] = vz;
+  W[4] = ph.gm1 * (U[4] - 0.5 * U[0] * v2 - 0.5 * b2);
+  W[5] = U[5]; W[6] = U[6]; W[7] = U[7];
+}
+
+// eq.4 (R7).  dp = W(i+1)-W(i), dm = W(i)-W(i-1).
+AG_HD double limited_slope(int limiter, double beta, double dp, double dm) {
+  if (limiter == 2) {
+    const double a = beta * fabs(dp);
+    const double b = beta * fabs(dm);
+    const double c = 0.5 * fabs(dp + dm);
+    const double m = copysign(fmin(fmin(a, b), c), dp);
+    return (dp * dm > 0.0) ? m : 0.0;
+  }
+  if (limiter == 1) return 0.5 * (dp + dm);
+  return 0.0;
+}
+
+// Per-side quantities every solver needs.
+struct Side {
+  double ir;    // 1/rho
+  double B2;    // |B|^2
+  double pt;    // p + |B|^2/2
+  double cf;    // fast speed along the normal, eq.12 (R3)
+};
+
+AG_HD Side side_of(const Phys& ph, const double w[8]) {
+  Side s;
+  s.ir = rcp(w[0]);
+  s.B2 = w[5] * w[5] + w[6] * w[6] + w[7] * w[7];
+  s.pt = w[4] + 0.5 * s.B2;
+  const double a2 = ph.gamma * w[4] * s.ir;          // v_s^2 = gamma p / rho
+  const double b2 = s.B2 * s.ir;                     // v_A^2 = B^2 / rho
+  const double sm = a2 + b2;
+  const double rad = fmax(sm * sm - 4.0 * a2 * (w[5] * w[5] * s.ir), 0.0);
+  s.cf = sqrt(0.5 * (sm + sqrt(rad)));
+  return s;
+}
+
+// eq.13:  c_w = aw + sqrt(aw^2 + v_A^2),  aw = d_i pi |B| / (2 rho dx_min)
+AG_HD double whistler_speed(const Phys& ph, const double w[8], const Side& s) {
+  const double aw = ph.cwk * sqrt(s.B2) * s.ir;
+  return aw + sqrt(aw * aw + s.B2 * s.ir);
+}
+
+// Total energy density (R2).
+AG_HD double energy_of(const Phys& ph, const double w[8], const Side& s) {
+  return 0.5 * w[0] * (w[1] * w[1] + w[2] * w[2] + w[3] * w[3]) + 0.5 * s.B2 + w[4] * ph.igm1;
+}
+
+// eqs.7-10 with psi == 0 in the rotated frame; vH = Hall velocity (rotated) or nullptr (ideal: v_T = v).
+AG_HD void phys_flux(const Phys& ph, const double w[8], const Side& s, const double* vH, double f[8]) {
+  const double ru = w[0] * w[1];
+  double tn = w[1], t1 = w[2], t2 = w[3];
+  if (vH) { tn += vH[0]; t1 += vH[1]; t2 += vH[2]; }
+  const double v2 = w[1] * w[1] + w[2] * w[2] + w[3] * w[3];
+  const double tB = tn * w[5] + t1 * w[6] + t2 * w[7];
+  f[0] = ru;                                                                    // eq.7
+  f[1] = ru * w[1] - w[5] * w[5] + s.pt;                                        // eq.8
+  f[2] = ru * w[2] - w[5] * w[6];
+  f[3] = ru * w[3] - w[5] * w[7];
+  f[4] = (0.5 * w[0] * v2 + ph.gogm1 * w[4]) * w[1] + s.B2 * tn - tB * w[5];     // eq.9
+  f[5] = 0.0;                                                                   // eq.10, c == n
+  f[6] = tn * w[6] - w[5] * t1;
+  f[7] = tn * w[7] - w[5] * t2;
+}
+
+// HLL, eq.5 with the Davis speeds eq.6; all 8 components through eq.5 (R9).
+// Hall (R15): c = max(c_f, c_w) per side, v_H^a = -d_i J / rho^a in phi.  J in the rotated frame.
+template <bool HALL>
+AG_HD void flux_hll(const Phys& ph, const double L[8], const double R[8], const double* J, double F[8]) {
+  const Side sl = side_of(ph, L), sr = side_of(ph, R);
+  double cl = sl.cf, cr = sr.cf;
+  double vhl[3], vhr[3];
+  if (HALL) {
+    cl = fmax(cl, whistler_speed(ph, L, sl));
+    cr = fmax(cr, whistler_speed(ph, R, sr));
+    for (int c = 0; c < 3; ++c) {
+      vhl[c] = -(ph.d_i * J[c]) * sl.ir;
+      vhr[c] = -(ph.d_i * J[c]) * sr.ir;
+    }
+  }
+  const double sL = fmin(fmin(L[1] - cl, R[1] - cr), 0.0);       // s'_L = min(s_L, 0)
+  const double sR = fmax(fmax(L[1] + cl, R[1] + cr), 0.0);       // s'_R = max(s_R, 0)
+  double fl[8], fr[8];
+  phys_flux(ph, L, sl, HALL ? vhl : nullptr, fl);
+  phys_flux(ph, R, sr, HALL ? vhr : nullptr, fr);
+  const double ul[8] = {L[0], L[0] * L[1], L[0] * L[2], L[0] * L[3], energy_of(ph, L, sl), L[5], L[6], L[7]};
+  const double ur[8] = {R[0], R[0] * R[1], R[0] * R[2], R[0] * R[3], energy_of(ph, R, sr), R[5], R[6], R[7]};
+  const double iw = rcp(sR - sL);
+  const double ss = sL * sR;
+#pragma unroll
+  for (int q = 0; q < 8; ++q) F[q] = (sR * fl[q] - sL * fr[q] + ss * (ur[q] - ul[q])) * iw;
+}
+
+// Star-state transverse components behind one outer wave (R10):  S = outer speed, m = rho (S - u).
+struct Star {
+  double rs;          // rho*
+  double idS;         // 1 / (S - SM)
+  double v, w, b1, b2;
+};
+
+AG_HD Star star_of(const double a[8], double S, double m, double SM, double bn, double bn2, double pts) {
+  Star st;
+  const double dS = S - SM;
+  const double den = m * dS - bn2;
+  const bool degenerate = fabs(den) < kHlldEps * pts;       // B_t = 0 and c_f = |Bn|/sqrt(rho)
+  const double dsafe = degenerate ? 1.0 : den;
+  const double r1 = rcp(dS * dsafe);                         // one reciprocal serves 1/dS and 1/den
+  st.idS = dsafe * r1;
+  const double iden = dS * r1;
+  st.rs = m * st.idS;
+  const double t = degenerate ? 0.0 : bn * (SM - a[1]) * iden;
+  const double f = degenerate ? 1.0 : (m * (S - a[1]) - bn2) * iden;
+  st.v = a[2] - a[6] * t;
+  st.w = a[3] - a[7] * t;
+  st.b1 = a[6] * f;
+  st.b2 = a[7] * f;
+  return st;
+}
+
+// HLLD (R10).  The Riemann fan is mirrored (x -> -x: swap sides, negate u and Bn) when the contact moves left,
+// so that a single "upwind side = A" code path serves both halves of the fan and lanes of a warp only diverge
+// on single-star vs double-star.  Mirror symmetry of the solver is oracle pin P6(v).
+AG_HD void flux_hlld(const Phys& ph, const double Lin[8], const double Rin[8], double F[8]) {
+  const double bn0 = 0.5 * (Lin[5] + Rin[5]);                // single-valued Bn: arithmetic mean
+  double L[8], R[8];
+#pragma unroll
+  for (int q = 0; q < 8; ++q) { L[q] = Lin[q]; R[q] = Rin[q]; }
+  L[5] = bn0; R[5] = bn0;
+  const Side sl = side_of(ph, L), sr = side_of(ph, R);
+  const double SL = fmin(L[1] - sl.cf, R[1] - sr.cf);        // eq.6
+  const double SR = fmax(L[1] + sl.cf, R[1] + sr.cf);
+  const double mL = L[0] * (SL - L[1]), mR = R[0] * (SR - R[1]);     // mL < 0 < mR
+  const double idm = rcp(mR - mL);
+  const double SM0 = (mR * R[1] - mL * L[1] - sr.pt + sl.pt) * idm;
+  const double pts = (mR * sl.pt - mL * sr.pt + mL * mR * (R[1] - L[1])) * idm;
+  const bool supL = SL >= 0.0;
+  const bool supR = !supL && (SR <= 0.0);
+  const bool flip = supL ? false : (supR ? true : (SM0 < 0.0));
+
+  // mirrored frame: A = upwind side, B = the other side
+  double A[8], B[8];
+#pragma unroll
+  for (int q = 0; q < 8; ++q) { A[q] = flip ? R[q] : L[q]; B[q] = flip ? L[q] : R[q]; }
+  const double bn = flip ? -bn0 : bn0;
+  A[1] = flip ? -A[1] : A[1]; B[1] = flip ? -B[1] : B[1];
+  A[5] = bn; B[5] = bn;
+  Side sa; sa.ir = flip ? sr.ir : sl.ir; sa.B2 = flip ? sr.B2 : sl.B2; sa.pt = flip ? sr.pt : sl.pt; sa.cf = 0.0;
+  const double SA = flip ? -SR : SL, SB = flip ? -SL : SR;
+  const double mA = flip ? -mR : mL, mB = flip ? -mL : mR;
+  const double SM = flip ? -SM0 : SM0;                       // >= 0 unless supersonic
+  const double bn2 = bn0 * bn0;
+
+  double fa[8];
+  phys_flux(ph, A, sa, nullptr, fa);
+  const double EA = energy_of(ph, A, sa);
+
+  const Star a = star_of(A, SA, mA, SM, bn, bn2, pts);
+  const double vBA = A[1] * bn + A[2] * A[6] + A[3] * A[7];
+  const double vBsA = SM * bn + a.v * a.b1 + a.w * a.b2;
+  const double EsA = ((SA - A[1]) * EA - sa.pt * A[1] + pts * SM + bn * (vBA - vBsA)) * a.idS;
+
+  double Fm[8];
+  Fm[0] = fa[0] + SA * (a.rs - A[0]);
+  Fm[1] = fa[1] + SA * (a.rs * SM - A[0] * A[1]);
+  Fm[2] = fa[2] + SA * (a.rs * a.v - A[0] * A[2]);
+  Fm[3] = fa[3] + SA * (a.rs * a.w - A[0] * A[3]);
+  Fm[4] = fa[4] + SA * (EsA - EA);
+  Fm[6] = fa[6] + SA * (a.b1 - A[6]);
+  Fm[7] = fa[7] + SA * (a.b2 - A[7]);
+
+  const double irsA = rsq(a.rs);
+  const double SsA = SM - fabs(bn) * irsA;                   // S*_A
+  const bool twostar = (SsA < 0.0) && !(0.5 * bn2 < kHlldEps * pts);
+  if (twostar) {
+    const Star b = star_of(B, SB, mB, SM, bn, bn2, pts);
+    const double qA = a.rs * irsA, qB = sqrt(b.rs);
+    const double I = rcp(qA + qB);
+    const double sg = (bn > 0.0) ? 1.0 : -1.0;
+    const double vss = (qA * a.v + qB * b.v + (b.b1 - a.b1) * sg) * I;
+    const double wss = (qA * a.w + qB * b.w + (b.b2 - a.b2) * sg) * I;
+    const double b1ss = (qA * b.b1 + qB * a.b1 + qA * qB * (b.v - a.v) * sg) * I;
+    const double b2ss = (qA * b.b2 + qB * a.b2 + qA * qB * (b.w - a.w) * sg) * I;
+    const double vBss = SM * bn + vss * b1ss + wss * b2ss;
+    Fm[2] += SsA * (a.rs * (vss - a.v));
+    Fm[3] += SsA * (a.rs * (wss - a.w));
+    Fm[4] += SsA * (-(qA * (vBsA - vBss) * sg));
+    Fm[6] += SsA * (b1ss - a.b1);
+    Fm[7] += SsA * (b2ss - a.b2);
+  }
+  if (supL || supR) {
+#pragma unroll
+    for (int q = 0; q < 8; ++q) Fm[q] = fa[q];
+  }
+  F[0] = flip ? -Fm[0] : Fm[0];
+  F[1] = Fm[1];
+  F[2] = flip ? -Fm[2] : Fm[2];
+  F[3] = flip ? -Fm[3] : Fm[3];
+  F[4] = flip ? -Fm[4] : Fm[4];
+  F[5] = 0.0;                                                // F[Bn] = 0 in every branch (R10)
+  F[6] = flip ? -Fm[6] : Fm[6];
+  F[7] = flip ? -Fm[7] : Fm[7];
+}
+
+template <int RIEMANN, bool HALL>
+AG_HD void riemann_flux(const Phys& ph, const double L[8], const double R[8], const double* J, double F[8]) {
+  if (RIEMANN == 1) flux_hlld(ph, L, R, F);
+  else flux_hll<HALL>(ph, L, R, J, F);
+}
+
+// A7 per cell (R3, R4): |v|_2 + max(max_d c_f,d , c_w).  Returns a negative value for an unphysical
+// cell (rho <= 0, p <= 0 or a non-finite speed) so that the caller can raise the flag (R14).
+template <bool HALL>
+AG_HD double cell_speed(const Phys& ph, const double U[8]) {
+  double W[8];
+  cons_to_prim(ph, U, W);
+  if (!(W[0] > 0.0) || !(W[4] > 0.0)) return -1.0;
+  const double ir = rcp(W[0]);
+  const double B2 = W[5] * W[5] + W[6] * W[6] + W[7] * W[7];
+  const double a2 = ph.gamma * W[4] * ir, b2 = B2 * ir, sm = a2 + b2;
+  // max over d of c_f,d  ==  c_f at the smallest B_d^2 (R4)
+  const double bmin2 = fmin(fmin(W[5] * W[5], W[6] * W[6]), W[7] * W[7]);
+  const double rad = fmax(sm * sm - 4.0 * a2 * (bmin2 * ir), 0.0);
+  double c = sqrt(0.5 * (sm + sqrt(rad)));
+  if (HALL) {
+    const double aw = ph.cwk * sqrt(B2) * ir;
+    c = fmax(c, aw + sqrt(aw * aw + b2));
+  }
+  const double sp = sqrt(W[1] * W[1] + W[2] * W[2] + W[3] * W[3]) + c;
+  return (sp - sp == 0.0) ? sp : -1.0;     // finite test that survives fast-math-free builds
+}
+
+}  // namespace agate

@@ -1,0 +1,33 @@
+// physics_shim.cpp — HOST build of the CUDA path's point functions (paper_2503_20899_b200/csrc/agate_physics.cuh)
+// so that `-m "not gpu"` tests can compare them with the oracle without a GPU.  Test infrastructure only:
+// compiled by tests/test_physics_host.py with g++; it is not part of the product library.
+#include "agate_physics.cuh"
+
+using namespace agate;
+
+extern "C" {
+
+void shim_face_flux(int eqset, int riemann, int dir, double gamma, double d_i, double dxmin, const double* WL,
+                    const double* WR, const double* J, double* F) {
+  Phys ph = make_phys(gamma, eqset == 1 ? d_i : 0.0, dxmin);
+  double L[8], R[8], Jr[3] = {0, 0, 0}, Fr[8];
+  for (int r = 0; r < 8; ++r) { L[r] = WL[rot_var(r, dir)]; R[r] = WR[rot_var(r, dir)]; }
+  if (J) for (int c = 0; c < 3; ++c) Jr[c] = J[(dir + c) % 3];
+  if (eqset == 1) riemann_flux<0, true>(ph, L, R, Jr, Fr);
+  else if (riemann == 1) riemann_flux<1, false>(ph, L, R, nullptr, Fr);
+  else riemann_flux<0, false>(ph, L, R, nullptr, Fr);
+  unrotate(dir, Fr, F);
+}
+
+void shim_cons_to_prim(double gamma, const double* U, double* W) {
+  Phys ph = make_phys(gamma, 0.0, 1.0);
+  cons_to_prim(ph, U, W);
+}
+
+double shim_slope(int limiter, double beta, double dp, double dm) { return limited_slope(limiter, beta, dp, dm); }
+
+double shim_cell_speed(int eqset, double gamma, double d_i, double dxmin, const double* U) {
+  Phys ph = make_phys(gamma, eqset == 1 ? d_i : 0.0, dxmin);
+  return eqset == 1 ? cell_speed<true>(ph, U) : cell_speed<false>(ph, U);
+}
+}
