@@ -57,9 +57,11 @@ def lib():
     """Load (building if stale) libagate.so.  Raises if it cannot be built or loaded — never falls back."""
     global _lib
     if _lib is None:
-        path = _build.LIB
-        if _build.is_stale():
-            path = _build.build()
+        path = os.environ.get("AGATE_LIB")          # explicit override (kernel-variant experiments)
+        if not path:
+            path = _build.LIB
+            if _build.is_stale():
+                path = _build.build()
         L = C.CDLL(path)
         L.agate_workspace_bytes.argtypes = [C.POINTER(Grid), C.c_int, C.POINTER(SolverCfg)]
         L.agate_workspace_bytes.restype = C.c_size_t

@@ -15,9 +15,16 @@
 
 using namespace agate;
 
+#ifndef AGATE_TY3
+#define AGATE_TY3 6
+#endif
+#ifndef AGATE_MINB3
+#define AGATE_MINB3 2
+#endif
+
 namespace {
 
-constexpr int TY3 = 12;   // 3-D: 32x12 tile, 14 warps, 1 CTA / SM, ring of 3 planes
+constexpr int TY3 = AGATE_TY3;   // 3-D tile height (rows); CTA = 32 x (TY3+2) threads
 constexpr int TY2 = 6;    // 1-D / 2-D: 32x6 tile, 8 warps, 2 CTAs / SM
 constexpr int kDtBlocksMax = 148 * 8;
 
@@ -85,8 +92,8 @@ StageKernel make_stage() {
 
 StageKernel pick_stage(int ndim, int eqset, int riemann) {
   if (ndim == 3) {
-    if (riemann == AGATE_HLLD) return make_stage<TY3, 3, 1, false, 1>();
-    return make_stage<TY3, 3, 0, false, 1>();
+    if (riemann == AGATE_HLLD) return make_stage<TY3, 3, 1, false, AGATE_MINB3>();
+    return make_stage<TY3, 3, 0, false, AGATE_MINB3>();
   }
   if (eqset == AGATE_HALL) return make_stage<TY2, 1, 0, true, 2>();
   if (riemann == AGATE_HLLD) return make_stage<TY2, 1, 1, false, 2>();
