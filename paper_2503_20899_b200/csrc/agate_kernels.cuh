@@ -32,7 +32,7 @@ struct StageParams {
   const double* U0;      // U^n for the combine (may alias Uout); unused when a0 == 0
   double* Uout;
   const double* dt_ptr;  // device scalar
-  double a0, a1;         // Uout = a0*U0 + a1*(Uin + dt*L)
+  double a0, a1;         // a0 == 0: Uout = Uin + dt*L;  a0 == a1: Uout = a1*(U0 + Uin + dt*L)  (SSP-RK22: 1/2)
   int nx, ny, nz, ndim;
   int ghy, ghz;          // ghost widths (2 if the dimension is active, else 0)
   int nxp, nyp;          // padded extents
@@ -142,9 +142,21 @@ __global__ void __launch_bounds__(32 * (TY + 2), MINB) stage_kernel(const __grid
       return (j >= 0 && j < TY) ? cur + j * RS : STRIP0 + ((j < 0) ? j + 2 : j - TY + 2) * RS;
     };
 
+    // A6 folded into the accumulator: acc starts as Uin (+ U0 in the second SSP stage) so that the global loads
+    // are in flight while the x sweep runs; the stage result is  c0 * (acc - dt * sum_d dF_d / dx_d).
     double acc[8];
+    const long long gcell = (long long)(k + P.ghz) * P.sz + (long long)(y0 + cj + P.ghy) * P.sy + (x0 + ci + 2);
+    if (cell_ok && !zonly) {
 #pragma unroll
-    for (int q = 0; q < 8; ++q) acc[q] = 0.0;
+      for (int q = 0; q < 8; ++q) acc[q] = __ldg(P.Uin + q * P.sq + gcell);
+      if (P.a0 != 0.0) {
+#pragma unroll
+        for (int q = 0; q < 8; ++q) acc[q] += P.U0[q * P.sq + gcell];
+      }
+    } else {
+#pragma unroll
+      for (int q = 0; q < 8; ++q) acc[q] = 0.0;
+    }
 
 #pragma unroll 1
     for (int d = zonly ? 2 : 0; d < P.ndim; ++d) {
@@ -269,14 +281,14 @@ __global__ void __launch_bounds__(32 * (TY + 2), MINB) stage_kernel(const __grid
         if (cell_ok) {
           const int lo = (d == 0) ? cj * 33 + ci : cj * 32 + ci;
           const int hi = (d == 0) ? lo + 1 : lo + 32;
-          const double ih = (d == 0) ? P.idx : P.idy;
+          const double ih = dt * ((d == 0) ? P.idx : P.idy);
 #pragma unroll
           for (int q = 0; q < 8; ++q) acc[q] -= (Fb[q * NF + hi] - Fb[q * NF + lo]) * ih;
         }
       } else if (cell_ok) {
 #pragma unroll
         for (int q = 0; q < 8; ++q) {
-          if (!zonly) acc[q] -= (Ff[q] - Fzp[q * NCELL + tid]) * P.idz;
+          if (!zonly) acc[q] -= (Ff[q] - Fzp[q * NCELL + tid]) * (dt * P.idz);
           Fzp[q * NCELL + tid] = Ff[q];
         }
       }
@@ -284,13 +296,10 @@ __global__ void __launch_bounds__(32 * (TY + 2), MINB) stage_kernel(const __grid
 
     // ---- A6: Runge-Kutta combine and store ----
     if (cell_ok && !zonly) {
-      const long long g = (long long)(k + P.ghz) * P.sz + (long long)(y0 + cj + P.ghy) * P.sy + (x0 + ci + 2);
+      // stage 1 (a0 == 0): Uout = acc;  stage 2 (a0 == a1 == 1/2): Uout = (U0 + Uin - dt sum dF/dx) / 2
+      const double c0 = (P.a0 != 0.0) ? P.a1 : 1.0;
 #pragma unroll
-      for (int q = 0; q < 8; ++q) {
-        double val = __ldg(P.Uin + q * P.sq + g) + dt * acc[q];
-        if (P.a0 != 0.0) val = P.a0 * P.U0[q * P.sq + g] + P.a1 * val;
-        P.Uout[q * P.sq + g] = val;
-      }
+      for (int q = 0; q < 8; ++q) P.Uout[q * P.sq + gcell] = c0 * acc[q];
     }
   }
 }
