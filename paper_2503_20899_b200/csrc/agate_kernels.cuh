@@ -264,18 +264,22 @@ __global__ void __launch_bounds__(32 * (TY + 2), MINB) stage_kernel(const __grid
       }
 
       // ---- A3 + A4 (+A8): ONE call site of the Riemann solver for all directions ----
-      double Ff[8];
-      if (active) {
-        double Fr[8];
-        riemann_flux<RIEMANN, HALL>(P.ph, L, R, HALL ? Jr : nullptr, Fr);
-        unrotate(d, Fr, Ff);
-      }
+      double Fr[8];
+      if (active) riemann_flux<RIEMANN, HALL>(P.ph, L, R, HALL ? Jr : nullptr, Fr);
 
-      // ---- A5: flux difference ----
+      // ---- A5: flux difference.  The rotated flux goes back to the fixed frame through its shared-memory index
+      //      (x, y) or a uniform three-way branch (z): no per-component selects. ----
       if (d < 2) {
         if (active) {
-#pragma unroll
-          for (int q = 0; q < 8; ++q) Fb[q * NF + fidx] = Ff[q];
+          const int m1 = (d == 0) ? 1 : 2, m2 = (d == 0) ? 2 : 3, m3 = (d == 0) ? 3 : 1;   // rot_var(r, d), r = 1..3
+          Fb[0 * NF + fidx] = Fr[0];
+          Fb[m1 * NF + fidx] = Fr[1];
+          Fb[m2 * NF + fidx] = Fr[2];
+          Fb[m3 * NF + fidx] = Fr[3];
+          Fb[4 * NF + fidx] = Fr[4];
+          Fb[(4 + m1) * NF + fidx] = Fr[5];
+          Fb[(4 + m2) * NF + fidx] = Fr[6];
+          Fb[(4 + m3) * NF + fidx] = Fr[7];
         }
         __syncthreads();
         if (cell_ok) {
@@ -286,6 +290,8 @@ __global__ void __launch_bounds__(32 * (TY + 2), MINB) stage_kernel(const __grid
           for (int q = 0; q < 8; ++q) acc[q] -= (Fb[q * NF + hi] - Fb[q * NF + lo]) * ih;
         }
       } else if (cell_ok) {
+        // z (n = 2): rotated (u,v,w) = (vz,vx,vy)  ->  fixed slots 3,1,2 and 7,5,6
+        const double Ff[8] = {Fr[0], Fr[2], Fr[3], Fr[1], Fr[4], Fr[6], Fr[7], Fr[5]};
 #pragma unroll
         for (int q = 0; q < 8; ++q) {
           if (!zonly) acc[q] -= (Ff[q] - Fzp[q * NCELL + tid]) * (dt * P.idz);
