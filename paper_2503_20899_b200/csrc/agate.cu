@@ -12,19 +12,20 @@
 #include <vector>
 
 #include "agate_kernels.cuh"
+#include "agate_stage3d.cuh"
 
 using namespace agate;
 
 #ifndef AGATE_TY3
-#define AGATE_TY3 6
+#define AGATE_TY3 11    // 3-D tile height: 11 owner warps + 1 helper = 12 warps (3 per scheduler, 168 registers), 186 KB
 #endif
 #ifndef AGATE_MINB3
-#define AGATE_MINB3 2
+#define AGATE_MINB3 1
 #endif
 
 namespace {
 
-constexpr int TY3 = AGATE_TY3;   // 3-D tile height (rows); CTA = 32 x (TY3+2) threads
+constexpr int TY3 = AGATE_TY3;   // 3-D tile height (rows); CTA = 32 x (TY3+1) threads (agate_stage3d.cuh)
 constexpr int TY2 = 6;    // 1-D / 2-D: 32x6 tile, 8 warps, 2 CTAs / SM
 constexpr int kDtBlocksMax = 148 * 8;
 
@@ -90,10 +91,22 @@ StageKernel make_stage() {
   return k;
 }
 
+template <int TY, int R, int MINB>
+StageKernel make_stage3d() {
+  StageKernel k;
+  k.fn = stage3d_kernel<TY, R, MINB>;
+  k.ty = TY; k.np = 3; k.threads = Stage3dSmem<TY>::NT; k.smem = Stage3dSmem<TY>::BYTES;
+  return k;
+}
+
 StageKernel pick_stage(int ndim, int eqset, int riemann) {
   if (ndim == 3) {
-    if (riemann == AGATE_HLLD) return make_stage<TY3, 3, 1, false, AGATE_MINB3>();
-    return make_stage<TY3, 3, 0, false, AGATE_MINB3>();
+    if (getenv("AGATE_STAGE_V1")) {      // the pooled kernel of agate_kernels.cuh, kept for A/B measurements
+      if (riemann == AGATE_HLLD) return make_stage<6, 3, 1, false, 2>();
+      return make_stage<6, 3, 0, false, 2>();
+    }
+    if (riemann == AGATE_HLLD) return make_stage3d<TY3, 1, AGATE_MINB3>();
+    return make_stage3d<TY3, 0, AGATE_MINB3>();
   }
   if (eqset == AGATE_HALL) return make_stage<TY2, 1, 0, true, 2>();
   if (riemann == AGATE_HLLD) return make_stage<TY2, 1, 1, false, 2>();
@@ -304,12 +317,28 @@ int agate_init(const agate_grid* grid, double gamma, int eqset, const agate_solv
   c->regs = fa.numRegs;
 
   // z-chunk length: chunks of ~128 planes keep the chunk start-up (3 plane loads + 1 z-only pass) near 1 %
+  // z-chunk length: the grid is (x-y tiles) x (z chunks).  Pick the chunk count that minimises
+  //   waves x (planes per chunk + start-up),  waves = ceil(CTAs / resident CTAs):  whole waves, short start-up
+  //   (a chunk costs about four extra planes: three loads and the step that closes its last plane).
   c->lz = grid->nz;
   if (grid->ndim == 3) {
-    int want = 128;
-    if (const char* s = getenv("AGATE_LZ")) { int v = atoi(s); if (v > 0) want = v; }
-    int nchunk = (grid->nz + want - 1) / want;
-    c->lz = (grid->nz + nchunk - 1) / nchunk;
+    int dev = 0, sms = 148;
+    cudaGetDevice(&dev);
+    cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
+    const long long slots = (long long)sms * (c->occ > 0 ? c->occ : 1);
+    const long long tiles = (long long)((grid->nx + TX - 1) / TX) * ((grid->ny + c->sk.ty - 1) / c->sk.ty);
+    int best_n = 1;
+    double best_t = 1e300;
+    for (int n = 1; n <= grid->nz && n <= 64; ++n) {
+      const int lz = (grid->nz + n - 1) / n;
+      if (lz < 8 && n > 1) break;
+      const int nn = (grid->nz + lz - 1) / lz;
+      const long long waves = (tiles * nn + slots - 1) / slots;
+      const double t = (double)waves * (lz + 4.0);
+      if (t < best_t * 0.999) { best_t = t; best_n = nn; }
+    }
+    c->lz = (grid->nz + best_n - 1) / best_n;
+    if (const char* s = getenv("AGATE_LZ")) { int v = atoi(s); if (v > 0 && v <= grid->nz) c->lz = v; }
   }
   c->sgrid = dim3((grid->nx + TX - 1) / TX, (grid->ny + c->sk.ty - 1) / c->sk.ty,
                   (grid->ndim == 3) ? (grid->nz + c->lz - 1) / c->lz : 1);

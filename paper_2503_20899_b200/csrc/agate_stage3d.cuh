@@ -1,25 +1,27 @@
-// agate_stage3d.cuh — warp-specialised fused stage kernel for 3-D grids, sm_100a.
+// agate_stage3d.cuh — row-owner fused stage kernel for 3-D grids, sm_100a.
 //
 // Same arithmetic as stage_kernel (agate_kernels.cuh); what differs is how the CTA is organised:
-//   * CTA = TY "owner" warps + 2 helper warps.  Owner warp j owns row j of a 32 x TY x-y tile and marches along z;
-//     lane i owns cell (i, j).  The owner of a cell computes its limited slopes, both face states, the Riemann flux
-//     through its HIGH face in x, y and z, and the flux difference (A2-A5), so slopes and fluxes are computed once.
-//   * x: neighbours are lanes of the same warp -> right state and low-face flux travel by warp shuffles.  The two
-//     cells outside the row (x = -1 and x = 32) belong to helper warp H0, which hands  R(32)  and  F(-1/2)  over
-//     through tiny shared buffers.
-//   * y: neighbours are adjacent warps -> right state and flux travel through the shared buffers YR / YF, guarded
-//     by per-row mbarriers (producer = one warp, consumer = the neighbouring warp).  Row -1 belongs to H0, row TY
-//     (slopes only) to helper warp H1.  There is no CTA-wide barrier in the steady state.
-//   * z: private column; the left state W(k)+dW(k)/2 and the flux F(k-1/2) are carried in per-thread shared slots.
-//   * H1 is also the PRODUCER: when every warp is done with plane k-1 it issues TMA bulk copies
-//     (cp.async.bulk ... mbarrier::complete_tx) of the conserved rows of plane k+2 straight into the freed ring
-//     slot and of the y-halo rows ("strips") of plane k+1 into the idle strip buffer.  Owners turn their own cell of
-//     the raw plane into primitives in place (A1) when the z sweep first needs it; H1 converts the strips and the
-//     x-halo columns.  Global-load latency is therefore never on the owners' critical path.
-//   * A6: the accumulator starts as Uin (+U0 in the second SSP stage), loaded at the top of the plane.
+//   * CTA = TY "owner" warps + 1 helper warp H.  Owner warp j owns row j of a 32 x TY x-y tile and marches along z;
+//     lane i owns cell (i, j).  The owner of a cell computes its limited slopes and the Riemann flux through its
+//     HIGH face in x and y and its LOW face in z, so every slope and every flux is computed once.
+//   * x: neighbours are lanes of the same warp -> the right state and the low-face flux travel by warp shuffles.
+//     The cells outside the row (x = -1, 32) belong to H, which hands  R(32)  and  F(-1/2)  over in XR / XF.
+//   * y: neighbours are adjacent warps -> the right state travels through YR, the flux through YF.  Row -1 (its
+//     flux through face -1/2) and row TY (its right state) belong to H.
+//   * z: private column, one plane behind: step k computes F(k-1/2) from planes k-1, k, k+1 and completes plane
+//     k-1.  The left state W(k-1)+dW(k-1)/2 is carried in a per-thread shared slot, the accumulator in registers.
+//   * TWO CTA-wide barriers per plane.  Phase A: y-difference of the previous plane, z slope + flux, store of
+//     plane k-1, y slope -> YR.  Phase B: y flux -> YF, x slope + flux + difference.  H mirrors the owners with the
+//     tile-edge tasks (one Riemann call per phase), so no warp idles while the others solve.
+//   * no global-load latency on the critical path: conserved cells are brought in by cp.async (LDGSTS) one phase
+//     ahead, straight into their final shared-memory slot, and turned into primitives IN PLACE (A1) by the thread
+//     that issued the copy: owners their own cell of plane k+2, H the x-halo columns and the y-halo rows.
+//   * ONE call site of the Riemann solver: the three tasks of a warp per plane run through one loop.
+//   * A6: the accumulator of plane k gets Uin (+U0 in the second SSP stage) right after
+//     barrier 1 (the loads are issued just before it), then the x and y differences; plane k leaves in step k+1.
 //
-// Shared memory per CTA (TY = 6): ring 3 planes x 8 x 6 x 36, strips 2 x 8 x 4 x 36, YR 8 x 8 x 32, YF 8 x 6 x 32,
-// z carries 2 x 8 x 192, x hand-over buffers, 25 mbarriers  =  115 KB  ->  2 CTAs per SM.
+// Shared memory per CTA: ring 3 planes x 8 x TY x 36, y-halo rows 2 x 8 x 4 x 36, YR/YF 8 x (TY+1) x 32 each,
+// z carries 2 x 8 x TY x 32, XR/XF 8 x TY each:  TY = 6 -> 111 KB (2 CTAs/SM, 14 warps),  TY = 14 -> 227 KB (1 CTA, 15).
 #pragma once
 #include <cuda_runtime.h>
 #include <stdint.h>
@@ -28,63 +30,326 @@
 
 namespace agate {
 
-// ---- mbarrier / TMA bulk-copy wrappers (PTX ISA: mbarrier, cp.async.bulk) ----
-__device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
-__device__ __forceinline__ void mbar_init(uint32_t bar, uint32_t count) {
-  asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(bar), "r"(count) : "memory");
-}
-__device__ __forceinline__ void mbar_arrive(uint32_t bar) {
-  asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(bar) : "memory");
-}
-__device__ __forceinline__ void mbar_expect_tx(uint32_t bar, uint32_t bytes) {
-  asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar), "r"(bytes) : "memory");
-}
-__device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity) {
-  asm volatile(
-      "{\n"
-      ".reg .pred p;\n"
-      "LAB_WAIT:\n"
-      "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n"
-      "@p bra DONE;\n"
-      "bra LAB_WAIT;\n"
-      "DONE:\n"
-      "}\n" ::"r"(bar),
-      "r"(parity)
-      : "memory");
-}
-// one warp announces "my writes are published": all lanes' writes ordered before lane 0's release-arrive
-__device__ __forceinline__ void warp_arrive(uint32_t bar, int lane) {
-  __syncwarp();
-  if (lane == 0) mbar_arrive(bar);
-}
-__device__ __forceinline__ void bulk_g2s(uint32_t dst, const void* src, uint32_t bytes, uint32_t bar) {
-  asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(dst),
-               "l"(src), "r"(bytes), "r"(bar)
+__device__ __forceinline__ void cp_async8(double* sdst, const double* gsrc) {
+  asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" ::"r"((uint32_t)__cvta_generic_to_shared(sdst)), "l"(gsrc)
                : "memory");
 }
+__device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wait_all;" ::: "memory"); }
+__device__ __forceinline__ void prefetch_l2(const void* p) { asm volatile("prefetch.global.L2 [%0];" ::"l"(p)); }
 
 template <int TY>
 struct Stage3dSmem {
-  static constexpr int NW = TY + 2;                 // warps: TY owners + H0 + H1
+  static_assert(TY >= 2 && TY <= 16, "the x-edge task packs two cells per row into one warp");
+  static constexpr int NW = TY + 1;                 // warps: TY owners + H
   static constexpr int NT = 32 * NW;
   static constexpr int PL = TY * RS;                // one ring plane of one variable
-  static constexpr int NRING = 3 * PL;
-  static constexpr int SB = 4 * RS;                 // one strip buffer of one variable (rows -2,-1,TY,TY+1)
-  static constexpr int QS = NRING + 2 * SB;         // per-variable stride of W
-  static constexpr int YQS = (TY + 2) * 32;         // YR: rows 0..TY-1 owners, rows TY, TY+1 = H1's two buffers
-  static constexpr int FQS = TY * 32;               // YF: row j = flux through face j+1/2 (written by owner j)
-  static constexpr int ZQ = TY * 32;                // z carries
-  static constexpr int XQ = TY;                     // x hand-over: [buf][q][row]
-  static constexpr int OFF_W = 0;
-  static constexpr int OFF_YR = OFF_W + 8 * QS;
-  static constexpr int OFF_YF = OFF_YR + 8 * YQS;
-  static constexpr int OFF_WLZ = OFF_YF + 8 * FQS;
-  static constexpr int OFF_FZP = OFF_WLZ + 8 * ZQ;
-  static constexpr int OFF_XR = OFF_FZP + 8 * ZQ;   // [2][8][TY]
-  static constexpr int OFF_XF = OFF_XR + 2 * 8 * XQ;
-  static constexpr int OFF_XO = OFF_XF + 2 * 8 * XQ;   // [8][TY] lane 0's own x flux
-  static constexpr int OFF_BAR = OFF_XO + 8 * XQ;      // mbarriers (8 bytes each)
-  static constexpr int NBAR = 13 + 2 * TY;
-  static constexpr size_t BYTES = sizeof(double) * (size_t)(OFF_BAR + NBAR);
+  static constexpr int SB = 4 * RS;                 // one y-halo buffer of one variable (rows -2,-1,TY,TY+1)
+  static constexpr int QS = 3 * PL + 2 * SB;        // per-variable stride of W
+  static constexpr int YS = (TY + 1) * 32;          // YR rows 0..TY;  YF rows -1..TY-1 (stored at j+1)
+  static constexpr int ZS = TY * 32;                // z carry
+  static constexpr int XS = TY;                     // x hand-over, one entry per row
+  static constexpr int OFF_YR = 8 * QS;
+  static constexpr int OFF_YF = OFF_YR + 8 * YS;
+  static constexpr int OFF_WLZ = OFF_YF + 8 * YS;
+  static constexpr int OFF_FZL = OFF_WLZ + 8 * ZS;
+  static constexpr int OFF_XR = OFF_FZL + 8 * ZS;
+  static constexpr int OFF_XF = OFF_XR + 8 * XS;
+  static constexpr int TOTAL = OFF_XF + 8 * XS;
+  static constexpr size_t BYTES = sizeof(double) * (size_t)TOTAL;
 };
 
+template <int TY, int RIEMANN, int MINB>
+__global__ void __launch_bounds__(32 * (TY + 1), MINB) stage3d_kernel(const __grid_constant__ StageParams P) {
+  using SM = Stage3dSmem<TY>;
+  constexpr int NT = SM::NT, PL = SM::PL, SB = SM::SB, QS = SM::QS, YS = SM::YS, ZS = SM::ZS, XS = SM::XS;
+  extern __shared__ __align__(16) double smem[];
+  double* const W = smem;                    // [8][QS]  primitives: ring planes + two y-halo buffers
+  double* const YR = smem + SM::OFF_YR;      // [8][YS]  right state  W(j) - dW_y(j)/2  of rows 0..TY   (fixed order)
+  double* const YF = smem + SM::OFF_YF;      // [8][YS]  y flux through face j+1/2, rows -1..TY-1       (rotated, n=1)
+  double* const WLz = smem + SM::OFF_WLZ;    // [8][ZS]  z: left state of the next face                (fixed order)
+  double* const FzL = smem + SM::OFF_FZL;    // [8][ZS]  z: flux through the low face of plane k-1     (fixed order)
+  double* const XR = smem + SM::OFF_XR;      // [8][XS]  right state of cell x = 32, per row
+  double* const XF = smem + SM::OFF_XF;      // [8][XS]  x flux through face -1/2, per row
+
+  const int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5;
+  const bool owner = wid < TY;
+  const int x0 = blockIdx.x * TX, y0 = blockIdx.y * TY;
+  const int tw = min(TX, P.nx - x0), th = min(TY, P.ny - y0);
+  const int k0 = blockIdx.z * P.lz, k1 = min(P.nz, k0 + P.lz);
+  const double dt = *P.dt_ptr;
+  const double cx = dt * P.idx, cy = dt * P.idy, cz = dt * P.idz;
+  const bool two = (P.a0 != 0.0);                       // second SSP stage: Uout = a1 (U0 + Uin + dt L)
+  const double c0 = two ? P.a1 : 1.0;
+  const int limiter = P.limiter;
+  const double beta = P.beta;
+  const bool cell_ok = owner && lane < tw && wid < th;
+  // padded-array bounds of what this thread copies (ragged tiles only)
+  const bool own_in = owner && (x0 + lane + 2 < P.nxp) && (y0 + wid + 2 < P.nyp);
+  const int own_off = wid * RS + lane + 2;              // own cell inside a ring plane (owners)
+  const long long own_g = (long long)(y0 + wid + 2) * P.sy + (x0 + lane + 2);   // + (p+2) * sz
+
+  auto slot_of = [](int p) { return ((p + 3) % 3) * PL; };     // p >= -2
+  auto conv_in_place = [&](int off) {
+    double u[8], w[8];
+#pragma unroll
+    for (int q = 0; q < 8; ++q) u[q] = W[q * QS + off];
+    cons_to_prim(P.ph, u, w);
+#pragma unroll
+    for (int q = 0; q < 8; ++q) W[q * QS + off] = w[q];
+  };
+  auto copy_cell = [&](int off, long long g) {
+#pragma unroll
+    for (int q = 0; q < 8; ++q) cp_async8(W + q * QS + off, P.Uin + q * P.sq + g);
+  };
+  // H's copy tasks for plane p: t < 4 TY -> x-halo columns of the ring rows;  else -> the four y-halo rows
+  constexpr int NHT = 4 * TY + 4 * RS;
+  auto htask = [&](int t, int p, int& off, long long& g) -> bool {
+    int j, c;
+    if (t < 4 * TY) {
+      j = t >> 2;
+      c = t & 3;
+      c = (c < 2) ? c : 32 + c;
+      off = slot_of(p) + j * RS + c;
+    } else {
+      const int u = t - 4 * TY, r = u / RS;
+      c = u - r * RS;
+      j = (r < 2) ? r - 2 : TY + r - 2;
+      off = 3 * PL + (p & 1) * SB + u;
+    }
+    g = (long long)(p + 2) * P.sz + (long long)(y0 + j + 2) * P.sy + (x0 + c);
+    return (x0 + c < P.nxp) && (y0 + j + 2 < P.nyp);
+  };
+  auto h_copy = [&](int p) {
+    for (int t = lane; t < NHT; t += 32) {
+      int off; long long g;
+      if (htask(t, p, off, g)) copy_cell(off, g);
+    }
+  };
+  auto h_conv = [&](int p) {
+    for (int t = lane; t < NHT; t += 32) {
+      int off; long long g;
+      if (htask(t, p, off, g)) conv_in_place(off);
+    }
+  };
+
+  // ---- prologue: everything step k0 needs that the steady state would have produced earlier ----
+  for (int i = tid; i < 8 * QS; i += NT) W[i] = 1.0;           // cells outside the padded array (ragged tiles)
+  __syncthreads();
+  if (owner) {
+    if (own_in) {
+      copy_cell(slot_of(k0 - 2) + own_off, own_g + (long long)k0 * P.sz);
+      copy_cell(slot_of(k0 - 1) + own_off, own_g + (long long)(k0 + 1) * P.sz);
+      copy_cell(slot_of(k0) + own_off, own_g + (long long)(k0 + 2) * P.sz);
+    }
+    cp_async_wait_all();
+    if (own_in) {
+      conv_in_place(slot_of(k0 - 2) + own_off);
+      conv_in_place(slot_of(k0 - 1) + own_off);
+      conv_in_place(slot_of(k0) + own_off);
+    }
+    const int ca = slot_of(k0 - 2) + own_off, cb = slot_of(k0 - 1) + own_off, cc = slot_of(k0) + own_off;
+#pragma unroll
+    for (int q = 0; q < 8; ++q) {
+      const double a = W[q * QS + ca], b = W[q * QS + cb], c = W[q * QS + cc];
+      WLz[q * ZS + tid] = b + 0.5 * limited_slope(limiter, beta, c - b, b - a);
+    }
+    // plane k0+1 goes into the slot plane k0-2 just left (own cell only: no other thread touches it)
+    if (own_in) copy_cell(slot_of(k0 + 1) + own_off, own_g + (long long)(k0 + 3) * P.sz);
+  } else {
+    h_copy(k0);
+    cp_async_wait_all();
+    h_conv(k0);
+    if (k0 + 1 < k1) h_copy(k0 + 1);
+  }
+  __syncthreads();
+
+  double acc[8];
+#pragma unroll
+  for (int q = 0; q < 8; ++q) acc[q] = 0.0;
+
+  for (int k = k0; k <= k1; ++k) {
+    const bool full = k < k1;       // plane k gets its x and y sweeps (step k1 only closes plane k1-1)
+    const bool emit = k > k0;       // plane k-1 is completed in this step
+    const int sm = slot_of(k - 1), sc = slot_of(k), sp = slot_of(k + 1);
+    const int hb = 3 * PL + (k & 1) * SB;                 // y-halo rows of plane k
+    double Ly[8], ua[8], ub[8];
+
+#pragma unroll 1
+    for (int s = 0; s < 3; ++s) {
+      double L[8], R[8], F[8];
+      bool flux = false;
+      // ------------------------------------------------------------------ prepare the face states of task s
+      if (owner) {
+        if (s == 0) {
+          if (emit) {
+            // A5 (y) of plane k-1: YF holds the rotated (n = 1) fluxes of the previous phase B
+#pragma unroll
+            for (int r = 0; r < 8; ++r)
+              acc[rot_var(r, 1)] -= cy * (YF[r * YS + (wid + 1) * 32 + lane] - YF[r * YS + wid * 32 + lane]);
+          }
+          cp_async_wait_all();
+          if (own_in) conv_in_place(sp + own_off);          // A1 of the own cell of plane k+1
+          // A2 (z): slope of plane k;  face k-1/2:  L carried,  R = W(k) - dW/2
+#pragma unroll
+          for (int r = 0; r < 8; ++r) {
+            const int v = rot_var(r, 2);
+            const double a = W[v * QS + sm + own_off], b = W[v * QS + sc + own_off], c = W[v * QS + sp + own_off];
+            const double hs = 0.5 * limited_slope(limiter, beta, c - b, b - a);
+            L[r] = WLz[v * ZS + tid];
+            R[r] = b - hs;
+            WLz[v * ZS + tid] = b + hs;
+          }
+          flux = true;
+        } else if (full) {
+          if (s == 1) {
+#pragma unroll
+            for (int q = 0; q < 8; ++q) acc[q] += two ? (ua[q] + ub[q]) : ua[q];      // A6: Uin (+ U0)
+#pragma unroll
+            for (int r = 0; r < 8; ++r) {
+              L[r] = Ly[r];
+              R[r] = YR[rot_var(r, 1) * YS + (wid + 1) * 32 + lane];
+            }
+          } else {
+            // A2 (x): own slope; the right state of face i+1/2 comes from lane i+1 (lane 31: from H)
+            const int c = sc + own_off;
+#pragma unroll
+            for (int r = 0; r < 8; ++r) {
+              const double a = W[r * QS + c - 1], b = W[r * QS + c], cc = W[r * QS + c + 1];
+              const double hs = 0.5 * limited_slope(limiter, beta, cc - b, b - a);
+              L[r] = b + hs;
+              const double rn = __shfl_down_sync(0xffffffffu, b - hs, 1);
+              R[r] = (lane == 31) ? XR[r * XS + wid] : rn;
+            }
+          }
+          flux = true;
+        }
+      } else if (full) {
+        if (s == 0) {
+          // row TY: right state for the owners of row TY-1
+          {
+            const int cm = sc + (TY - 1) * RS + lane + 2, c0r = hb + 2 * RS + lane + 2, cp = hb + 3 * RS + lane + 2;
+#pragma unroll
+            for (int q = 0; q < 8; ++q) {
+              const double a = W[q * QS + cm], b = W[q * QS + c0r], c = W[q * QS + cp];
+              YR[q * YS + TY * 32 + lane] = b - 0.5 * limited_slope(limiter, beta, c - b, b - a);
+            }
+          }
+          // column x = 32: right state for lane 31 of every row
+          if (lane < TY) {
+            const int c = sc + lane * RS + 34;
+#pragma unroll
+            for (int q = 0; q < 8; ++q) {
+              const double a = W[q * QS + c - 1], b = W[q * QS + c], cc = W[q * QS + c + 1];
+              XR[q * XS + lane] = b - 0.5 * limited_slope(limiter, beta, cc - b, b - a);
+            }
+          }
+          // face x = -1/2 of every row: lanes 0..15 hold cell -1 (left state), lanes 16..31 cell 0 (right state)
+          {
+            const int row = min(lane & 15, TY - 1), half = lane >> 4;
+            const int c = sc + row * RS + 1 + half;
+#pragma unroll
+            for (int r = 0; r < 8; ++r) {
+              const double a = W[r * QS + c - 1], b = W[r * QS + c], cc = W[r * QS + c + 1];
+              const double hs = 0.5 * limited_slope(limiter, beta, cc - b, b - a);
+              L[r] = b + hs;
+              R[r] = __shfl_down_sync(0xffffffffu, b - hs, 16);
+            }
+          }
+          flux = true;
+        } else if (s == 1) {
+          // row -1: flux through face y = -1/2
+          const int cm = hb + lane + 2, c0r = hb + RS + lane + 2, cp = sc + lane + 2;
+#pragma unroll
+          for (int r = 0; r < 8; ++r) {
+            const int v = rot_var(r, 1);
+            const double a = W[v * QS + cm], b = W[v * QS + c0r], c = W[v * QS + cp];
+            L[r] = b + 0.5 * limited_slope(limiter, beta, c - b, b - a);
+            R[r] = YR[v * YS + lane];
+          }
+          flux = true;
+        }
+      }
+
+      // ------------------------------------------------------------------ A3 + A4: the one Riemann call site
+      if (flux) riemann_flux<RIEMANN, false>(P.ph, L, R, nullptr, F);
+
+      // ------------------------------------------------------------------ consume the flux of task s
+      if (owner) {
+        if (s == 0) {
+          // A5 (z) + A6: plane k-1 is complete;  the accumulator of plane k starts with its low z face
+          const long long g = own_g + (long long)(k + 1) * P.sz;          // own cell of plane k-1
+#pragma unroll
+          for (int r = 0; r < 8; ++r) {
+            const int v = rot_var(r, 2);
+            // the difference is formed before it meets U, so that a uniform state stays bitwise fixed (pin P1)
+            if (emit && cell_ok) P.Uout[v * P.sq + g] = c0 * (acc[v] - cz * (F[r] - FzL[v * ZS + tid]));
+            FzL[v * ZS + tid] = F[r];
+            acc[v] = 0.0;
+          }
+          if (full) {
+            // A2 (y): own slope -> right state for the row below, left state kept for phase B
+            const int c = sc + own_off;
+            const int cm = (wid == 0) ? hb + RS + lane + 2 : c - RS;
+            const int cp = (wid == TY - 1) ? hb + 2 * RS + lane + 2 : c + RS;
+#pragma unroll
+            for (int r = 0; r < 8; ++r) {
+              const int v = rot_var(r, 1);
+              const double a = W[v * QS + cm], b = W[v * QS + c], cc = W[v * QS + cp];
+              const double hs = 0.5 * limited_slope(limiter, beta, cc - b, b - a);
+              YR[v * YS + wid * 32 + lane] = b - hs;
+              Ly[r] = b + hs;
+            }
+            // Uin (+U0) of the own cell of plane k: in flight across barrier 1
+            const long long gk = g + P.sz;
+#pragma unroll
+            for (int q = 0; q < 8; ++q) {
+              ua[q] = cell_ok ? __ldg(P.Uin + q * P.sq + gk) : 0.0;
+              ub[q] = (cell_ok && two) ? P.U0[q * P.sq + gk] : 0.0;
+            }
+          }
+        } else if (full) {
+          if (s == 1) {
+#pragma unroll
+            for (int r = 0; r < 8; ++r) YF[r * YS + (wid + 1) * 32 + lane] = F[r];
+          } else {
+            // A5 (x): low-face flux from lane i-1 (lane 0: from H)
+#pragma unroll
+            for (int r = 0; r < 8; ++r) {
+              const double fl = __shfl_up_sync(0xffffffffu, F[r], 1);
+              acc[r] -= cx * (F[r] - ((lane == 0) ? XF[r * XS + wid] : fl));
+            }
+            // own cell of plane k+2 -> the slot plane k-1 left in phase A
+            if (own_in && k + 2 <= k1 + 1) copy_cell(sm + own_off, own_g + (long long)(k + 4) * P.sz);
+            // second SSP stage: U0 of plane k+1 is first touched one step from now; pull its lines into L2 (one
+            // lane per 64 bytes)
+            if (two && cell_ok && (lane & 7) == 0 && k + 1 < k1) {
+#pragma unroll
+              for (int q = 0; q < 8; ++q) prefetch_l2(P.U0 + q * P.sq + own_g + (long long)(k + 3) * P.sz);
+            }
+          }
+        }
+      } else {
+        if (s == 0) {
+          if (full && lane < 16 && lane < TY) {
+#pragma unroll
+            for (int r = 0; r < 8; ++r) XF[r * XS + lane] = F[r];
+          }
+        } else if (s == 1) {
+          if (full) {
+#pragma unroll
+            for (int r = 0; r < 8; ++r) YF[r * YS + lane] = F[r];
+          }
+        } else {
+          // A1 for the halo cells of plane k+1 (copies issued one phase B ago), then the copies for plane k+2
+          cp_async_wait_all();
+          if (k + 1 < k1) h_conv(k + 1);
+          if (k + 2 < k1) h_copy(k + 2);
+        }
+      }
+      if (s != 1) __syncthreads();        // barrier 1 after phase A, barrier 2 after phase B
+    }
+  }
+  cp_async_wait_all();
+}
+
+}  // namespace agate
