@@ -266,115 +266,86 @@ AG_HD Star star_of(const double a[8], double S, double m, double SM, double bn, 
   return st;
 }
 
-// HLLD (R10).  The Riemann fan is mirrored (x -> -x: swap sides, negate u and Bn) when the contact moves left,
-// so that a single "upwind side = A" code path serves both halves of the fan and lanes of a warp only diverge
-// on single-star vs double-star.  Mirror symmetry of the solver is oracle pin P6(v).
+// HLLD (R10), straight-line.  The star-state formulas are the same for both sides with the side's own outer speed,
+// so nothing is mirrored: both star states are computed (a warp needs both as soon as one lane is in a double-star
+// region), the double-star state is symmetric in L and R, and the upwind side alpha (L if S_M >= 0, else R) enters
+// through selects of its state and one sign  sigma = +1 (L) / -1 (R).  The double-star and supersonic cases switch
+// their terms on and off through the wave speed that multiplies them, so there is no branch and no divergence.
+AG_HD double sel(bool c, double a, double b) { return c ? a : b; }
+
 AG_HD void flux_hlld(const Phys& ph, const double L[8], const double R[8], double F[8]) {
-  const double bn0 = 0.5 * (L[5] + R[5]);                    // single-valued Bn: arithmetic mean
-  const double bn2 = bn0 * bn0;
-  // per-side speeds with Bn := bn0 (the caller's L[5], R[5] are not used below)
-  Side sl, sr;
-  {
-    sl.ir = rcp(L[0]); sr.ir = rcp(R[0]);
-    sl.B2 = bn2 + L[6] * L[6] + L[7] * L[7];
-    sr.B2 = bn2 + R[6] * R[6] + R[7] * R[7];
-    sl.pt = L[4] + 0.5 * sl.B2; sr.pt = R[4] + 0.5 * sr.B2;
-    const double a2l = ph.gamma * L[4] * sl.ir, sml = a2l + sl.B2 * sl.ir;
-    const double a2r = ph.gamma * R[4] * sr.ir, smr = a2r + sr.B2 * sr.ir;
-    const double radl = dmax(sml * sml - 4.0 * a2l * (bn2 * sl.ir), kTiny);
-    const double radr = dmax(smr * smr - 4.0 * a2r * (bn2 * sr.ir), kTiny);
-    sl.cf = sqrt_pos(0.5 * (sml + sqrt_pos(radl)));
-    sr.cf = sqrt_pos(0.5 * (smr + sqrt_pos(radr)));
-  }
-  const double SL = dmin(L[1] - sl.cf, R[1] - sr.cf);        // eq.6
-  const double SR = dmax(L[1] + sl.cf, R[1] + sr.cf);
+  const double bn = 0.5 * (L[5] + R[5]);                     // single-valued Bn: arithmetic mean
+  const double bn2 = bn * bn;
+  // per-side speeds with Bn := bn (the caller's L[5], R[5] are not used below)
+  const double irl = rcp(L[0]), irr = rcp(R[0]);
+  const double B2l = bn2 + L[6] * L[6] + L[7] * L[7], B2r = bn2 + R[6] * R[6] + R[7] * R[7];
+  const double ptl = L[4] + 0.5 * B2l, ptr = R[4] + 0.5 * B2r;
+  const double a2l = ph.gamma * L[4] * irl, sml = a2l + B2l * irl;
+  const double a2r = ph.gamma * R[4] * irr, smr = a2r + B2r * irr;
+  const double radl = dmax(sml * sml - 4.0 * a2l * (bn2 * irl), kTiny);
+  const double radr = dmax(smr * smr - 4.0 * a2r * (bn2 * irr), kTiny);
+  const double cfl = sqrt_pos(0.5 * (sml + sqrt_pos(radl)));
+  const double cfr = sqrt_pos(0.5 * (smr + sqrt_pos(radr)));
+  const double SL = dmin(L[1] - cfl, R[1] - cfr);            // eq.6
+  const double SR = dmax(L[1] + cfl, R[1] + cfr);
   const double mL = L[0] * (SL - L[1]), mR = R[0] * (SR - R[1]);     // mL < 0 < mR
   const double idm = rcp(mR - mL);
-  const double SM0 = (mR * R[1] - mL * L[1] - sr.pt + sl.pt) * idm;
-  const double pts = (mR * sl.pt - mL * sr.pt + mL * mR * (R[1] - L[1])) * idm;
+  const double SM = (mR * R[1] - mL * L[1] - ptr + ptl) * idm;
+  const double pts = (mR * ptl - mL * ptr + mL * mR * (R[1] - L[1])) * idm;
+
+  const Star l = star_of(L, SL, mL, SM, bn, bn2, pts);
+  const Star r = star_of(R, SR, mR, SM, bn, bn2, pts);
+  // double-star state (symmetric in L, R)
+  const double irsl = rsq(l.rs), irsr = rsq(r.rs);
+  const double ql = l.rs * irsl, qr = r.rs * irsr;           // sqrt(rho*)
+  const double I = rcp(ql + qr);
+  const double sgn = (bn > 0.0) ? 1.0 : -1.0;
+  const double qq = ql * qr * sgn;
+  const double vss = (ql * l.v + qr * r.v + (r.b1 - l.b1) * sgn) * I;
+  const double wss = (ql * l.w + qr * r.w + (r.b2 - l.b2) * sgn) * I;
+  const double b1ss = (ql * r.b1 + qr * l.b1 + qq * (r.v - l.v)) * I;
+  const double b2ss = (ql * r.b2 + qr * l.b2 + qq * (r.w - l.w)) * I;
+
+  // upwind side
   const bool supL = SL >= 0.0;
   const bool supR = !supL && (SR <= 0.0);
-  const bool flip = supL ? false : (supR ? true : (SM0 < 0.0));
-  const unsigned long long sg = flip ? 0x8000000000000000ull : 0ull;
-
-  // mirrored frame: A = upwind side
+  const bool rt = supL ? false : (supR ? true : (SM < 0.0));
   double A[8];
-  A[0] = flip ? R[0] : L[0];
-  A[1] = xorsign(flip ? R[1] : L[1], sg);
-  A[2] = flip ? R[2] : L[2];
-  A[3] = flip ? R[3] : L[3];
-  A[4] = flip ? R[4] : L[4];
-  A[6] = flip ? R[6] : L[6];
-  A[7] = flip ? R[7] : L[7];
-  const double bn = xorsign(bn0, sg);
-  A[5] = bn;
+  A[0] = sel(rt, R[0], L[0]); A[1] = sel(rt, R[1], L[1]); A[2] = sel(rt, R[2], L[2]); A[3] = sel(rt, R[3], L[3]);
+  A[4] = sel(rt, R[4], L[4]); A[5] = bn;                  A[6] = sel(rt, R[6], L[6]); A[7] = sel(rt, R[7], L[7]);
   Side sa;
   sa.ir = 0.0; sa.cf = 0.0;
-  sa.B2 = flip ? sr.B2 : sl.B2;
-  sa.pt = flip ? sr.pt : sl.pt;
-  const double SA = xorsign(flip ? SR : SL, sg);
-  const double mA = xorsign(flip ? mR : mL, sg);
-  const double SM = xorsign(SM0, sg);                        // >= 0 unless supersonic
+  sa.B2 = sel(rt, B2r, B2l);
+  sa.pt = sel(rt, ptr, ptl);
+  const double SA = sel(rt, SR, SL);
+  Star a;
+  a.rs = sel(rt, r.rs, l.rs); a.idS = sel(rt, r.idS, l.idS);
+  a.v = sel(rt, r.v, l.v);    a.w = sel(rt, r.w, l.w);
+  a.b1 = sel(rt, r.b1, l.b1); a.b2 = sel(rt, r.b2, l.b2);
+  const double qa = sel(rt, qr, ql), irsa = sel(rt, irsr, irsl);
+  const double sig = rt ? -1.0 : 1.0;
 
   double fa[8];
   phys_flux(ph, A, sa, nullptr, fa);
   const double EA = energy_of(ph, A, sa);
-
-  const Star a = star_of(A, SA, mA, SM, bn, bn2, pts);
   const double vBA = A[1] * bn + A[2] * A[6] + A[3] * A[7];
   const double vBsA = SM * bn + a.v * a.b1 + a.w * a.b2;
+  const double vBss = SM * bn + vss * b1ss + wss * b2ss;
   const double EsA = ((SA - A[1]) * EA - sa.pt * A[1] + pts * SM + bn * (vBA - vBsA)) * a.idS;
 
-  double Fm[8];
-  Fm[0] = fa[0] + SA * (a.rs - A[0]);
-  Fm[1] = fa[1] + SA * (a.rs * SM - A[0] * A[1]);
-  Fm[2] = fa[2] + SA * (a.rs * a.v - A[0] * A[2]);
-  Fm[3] = fa[3] + SA * (a.rs * a.w - A[0] * A[3]);
-  Fm[4] = fa[4] + SA * (EsA - EA);
-  Fm[6] = fa[6] + SA * (a.b1 - A[6]);
-  Fm[7] = fa[7] + SA * (a.b2 - A[7]);
-
-  // S*_A = SM - |Bn|/sqrt(rho*_A) < 0  <=>  SM^2 rho*_A < Bn^2   (SM >= 0): no square root for the decision
-  const bool twostar = (SM * SM * a.rs < bn2) && !(0.5 * bn2 < kHlldEps * pts) && !(supL || supR);
-  if (twostar) {
-    double B[8];
-    B[0] = flip ? L[0] : R[0];
-    B[1] = xorsign(flip ? L[1] : R[1], sg);
-    B[2] = flip ? L[2] : R[2];
-    B[3] = flip ? L[3] : R[3];
-    B[6] = flip ? L[6] : R[6];
-    B[7] = flip ? L[7] : R[7];
-    const double SB = xorsign(flip ? SL : SR, sg);
-    const double mB = xorsign(flip ? mL : mR, sg);
-    const Star b = star_of(B, SB, mB, SM, bn, bn2, pts);
-    const double irsA = rsq(a.rs);
-    const double SsA = SM - fabs(bn) * irsA;                 // S*_A
-    const double qA = a.rs * irsA, qB = sqrt_pos(b.rs);
-    const double I = rcp(qA + qB);
-    const double sgn = (bn > 0.0) ? 1.0 : -1.0;
-    const double vss = (qA * a.v + qB * b.v + (b.b1 - a.b1) * sgn) * I;
-    const double wss = (qA * a.w + qB * b.w + (b.b2 - a.b2) * sgn) * I;
-    const double b1ss = (qA * b.b1 + qB * a.b1 + qA * qB * (b.v - a.v) * sgn) * I;
-    const double b2ss = (qA * b.b2 + qB * a.b2 + qA * qB * (b.w - a.w) * sgn) * I;
-    const double vBss = SM * bn + vss * b1ss + wss * b2ss;
-    Fm[2] += SsA * (a.rs * (vss - a.v));
-    Fm[3] += SsA * (a.rs * (wss - a.w));
-    Fm[4] -= SsA * (qA * (vBsA - vBss) * sgn);
-    Fm[6] += SsA * (b1ss - a.b1);
-    Fm[7] += SsA * (b2ss - a.b2);
-  }
-  if (supL || supR) {
-#pragma unroll
-    for (int q = 0; q < 8; ++q) Fm[q] = fa[q];
-  }
-  F[0] = xorsign(Fm[0], sg);
-  F[1] = Fm[1];
-  F[2] = xorsign(Fm[2], sg);
-  F[3] = xorsign(Fm[3], sg);
-  F[4] = xorsign(Fm[4], sg);
+  // S*_alpha = SM - sigma |Bn| / sqrt(rho*_alpha) lies on the far side of zero  <=>  SM^2 rho*_alpha < Bn^2
+  const bool sup = supL || supR;
+  const bool twostar = (SM * SM * a.rs < bn2) && !(0.5 * bn2 < kHlldEps * pts) && !sup;
+  const double SAe = sup ? 0.0 : SA;                          // supersonic: F = F_alpha
+  const double Sse = twostar ? (SM - sig * (fabs(bn) * irsa)) : 0.0;   // single-star: no double-star jump
+  F[0] = fa[0] + SAe * (a.rs - A[0]);
+  F[1] = fa[1] + SAe * (a.rs * SM - A[0] * A[1]);
+  F[2] = fa[2] + SAe * (a.rs * a.v - A[0] * A[2]) + Sse * (a.rs * (vss - a.v));
+  F[3] = fa[3] + SAe * (a.rs * a.w - A[0] * A[3]) + Sse * (a.rs * (wss - a.w));
+  F[4] = fa[4] + SAe * (EsA - EA) - Sse * (qa * (vBsA - vBss) * (sgn * sig));
   F[5] = 0.0;                                                // F[Bn] = 0 in every branch (R10)
-  F[6] = xorsign(Fm[6], sg);
-  F[7] = xorsign(Fm[7], sg);
+  F[6] = fa[6] + SAe * (a.b1 - A[6]) + Sse * (b1ss - a.b1);
+  F[7] = fa[7] + SAe * (a.b2 - A[7]) + Sse * (b2ss - a.b2);
 }
 
 template <int RIEMANN, bool HALL>
