@@ -99,17 +99,19 @@ __global__ void __launch_bounds__(32 * (TY + 1), MINB) stage3d_kernel(const __gr
   };
   auto copy_cell = [&](int off, long long g) {
 #pragma unroll
-    for (int q = 0; q < 8; ++q) cp_async8(W + q * QS + off, P.Uin + q * P.sq + g);
+    const double* src = P.Uin + g;           // running pointer: one 64-bit add per variable
+#pragma unroll
+    for (int q = 0; q < 8; ++q, src += P.sq) cp_async8(W + q * QS + off, src);
   };
   // H's copy tasks for plane p: t < 4 TY -> x-halo columns of the ring rows;  else -> the four y-halo rows
   constexpr int NHT = 4 * TY + 4 * RS;
-  auto htask = [&](int t, int p, int& off, long long& g) -> bool {
+  auto htask = [&](int t, int p, int slot, int& off, long long& g) -> bool {
     int j, c;
     if (t < 4 * TY) {
       j = t >> 2;
       c = t & 3;
       c = (c < 2) ? c : 32 + c;
-      off = slot_of(p) + j * RS + c;
+      off = slot + j * RS + c;
     } else {
       const int u = t - 4 * TY, r = u / RS;
       c = u - r * RS;
@@ -119,16 +121,16 @@ __global__ void __launch_bounds__(32 * (TY + 1), MINB) stage3d_kernel(const __gr
     g = (long long)(p + 2) * P.sz + (long long)(y0 + j + 2) * P.sy + (x0 + c);
     return (x0 + c < P.nxp) && (y0 + j + 2 < P.nyp);
   };
-  auto h_copy = [&](int p) {
+  auto h_copy = [&](int p, int slot) {
     for (int t = lane; t < NHT; t += 32) {
       int off; long long g;
-      if (htask(t, p, off, g)) copy_cell(off, g);
+      if (htask(t, p, slot, off, g)) copy_cell(off, g);
     }
   };
-  auto h_conv = [&](int p) {
+  auto h_conv = [&](int p, int slot) {
     for (int t = lane; t < NHT; t += 32) {
       int off; long long g;
-      if (htask(t, p, off, g)) conv_in_place(off);
+      if (htask(t, p, slot, off, g)) conv_in_place(off);
     }
   };
 
@@ -156,10 +158,10 @@ __global__ void __launch_bounds__(32 * (TY + 1), MINB) stage3d_kernel(const __gr
     // plane k0+1 goes into the slot plane k0-2 just left (own cell only: no other thread touches it)
     if (own_in) copy_cell(slot_of(k0 + 1) + own_off, own_g + (long long)(k0 + 3) * P.sz);
   } else {
-    h_copy(k0);
+    h_copy(k0, slot_of(k0));
     cp_async_wait_all();
-    h_conv(k0);
-    if (k0 + 1 < k1) h_copy(k0 + 1);
+    h_conv(k0, slot_of(k0));
+    if (k0 + 1 < k1) h_copy(k0 + 1, slot_of(k0 + 1));
   }
   __syncthreads();
 
@@ -167,10 +169,12 @@ __global__ void __launch_bounds__(32 * (TY + 1), MINB) stage3d_kernel(const __gr
 #pragma unroll
   for (int q = 0; q < 8; ++q) acc[q] = 0.0;
 
-  for (int k = k0; k <= k1; ++k) {
+  // ring slots of planes k-1, k, k+1 (rotated at the end of a step) and the own cell's offset in plane k-1
+  int sm = slot_of(k0 - 1), sc = slot_of(k0), sp = slot_of(k0 + 1);
+  long long gm = own_g + (long long)(k0 + 1) * P.sz;
+  for (int k = k0; k <= k1; ++k, gm += P.sz) {
     const bool full = k < k1;       // plane k gets its x and y sweeps (step k1 only closes plane k1-1)
     const bool emit = k > k0;       // plane k-1 is completed in this step
-    const int sm = slot_of(k - 1), sc = slot_of(k), sp = slot_of(k + 1);
     const int hb = 3 * PL + (k & 1) * SB;                 // y-halo rows of plane k
     double Ly[8], ua[8], ub[8];
 
@@ -277,12 +281,13 @@ __global__ void __launch_bounds__(32 * (TY + 1), MINB) stage3d_kernel(const __gr
       if (owner) {
         if (s == 0) {
           // A5 (z) + A6: plane k-1 is complete;  the accumulator of plane k starts with its low z face
-          const long long g = own_g + (long long)(k + 1) * P.sz;          // own cell of plane k-1
+          double* po = P.Uout + gm;                                       // own cell of plane k-1
 #pragma unroll
-          for (int r = 0; r < 8; ++r) {
-            const int v = rot_var(r, 2);
+          for (int v = 0; v < 8; ++v, po += P.sq) {
+            constexpr int inv2[8] = {0, 2, 3, 1, 4, 6, 7, 5};             // rot_var(inv2[v], 2) == v
+            const int r = inv2[v];
             // the difference is formed before it meets U, so that a uniform state stays bitwise fixed (pin P1)
-            if (emit && cell_ok) P.Uout[v * P.sq + g] = c0 * (acc[v] - cz * (F[r] - FzL[v * ZS + tid]));
+            if (emit && cell_ok) *po = c0 * (acc[v] - cz * (F[r] - FzL[v * ZS + tid]));
             FzL[v * ZS + tid] = F[r];
             acc[v] = 0.0;
           }
@@ -300,11 +305,12 @@ __global__ void __launch_bounds__(32 * (TY + 1), MINB) stage3d_kernel(const __gr
               Ly[r] = b + hs;
             }
             // Uin (+U0) of the own cell of plane k: in flight across barrier 1
-            const long long gk = g + P.sz;
+            const double* pa = P.Uin + gm + P.sz;
+            const double* pb = P.U0 + gm + P.sz;
 #pragma unroll
-            for (int q = 0; q < 8; ++q) {
-              ua[q] = cell_ok ? __ldg(P.Uin + q * P.sq + gk) : 0.0;
-              ub[q] = (cell_ok && two) ? P.U0[q * P.sq + gk] : 0.0;
+            for (int q = 0; q < 8; ++q, pa += P.sq, pb += P.sq) {
+              ua[q] = cell_ok ? __ldg(pa) : 0.0;
+              ub[q] = (cell_ok && two) ? *pb : 0.0;
             }
           }
         } else if (full) {
@@ -319,12 +325,12 @@ __global__ void __launch_bounds__(32 * (TY + 1), MINB) stage3d_kernel(const __gr
               acc[r] -= cx * (F[r] - ((lane == 0) ? XF[r * XS + wid] : fl));
             }
             // own cell of plane k+2 -> the slot plane k-1 left in phase A
-            if (own_in && k + 2 <= k1 + 1) copy_cell(sm + own_off, own_g + (long long)(k + 4) * P.sz);
+            if (own_in && k + 2 <= k1 + 1) copy_cell(sm + own_off, gm + 3 * P.sz);
             // second SSP stage: U0 of plane k+1 is first touched one step from now; pull its lines into L2 (one
             // lane per 64 bytes)
             if (two && cell_ok && (lane & 7) == 0 && k + 1 < k1) {
 #pragma unroll
-              for (int q = 0; q < 8; ++q) prefetch_l2(P.U0 + q * P.sq + own_g + (long long)(k + 3) * P.sz);
+              for (int q = 0; q < 8; ++q) prefetch_l2(P.U0 + q * P.sq + gm + 2 * P.sz);
             }
           }
         }
@@ -342,12 +348,13 @@ __global__ void __launch_bounds__(32 * (TY + 1), MINB) stage3d_kernel(const __gr
         } else {
           // A1 for the halo cells of plane k+1 (copies issued one phase B ago), then the copies for plane k+2
           cp_async_wait_all();
-          if (k + 1 < k1) h_conv(k + 1);
-          if (k + 2 < k1) h_copy(k + 2);
+          if (k + 1 < k1) h_conv(k + 1, sp);
+          if (k + 2 < k1) h_copy(k + 2, sm);
         }
       }
       if (s != 1) __syncthreads();        // barrier 1 after phase A, barrier 2 after phase B
     }
+    { const int t = sm; sm = sc; sc = sp; sp = t; }
   }
   cp_async_wait_all();
 }
