@@ -91,22 +91,26 @@ StageKernel make_stage() {
   return k;
 }
 
-template <int TY, int R, int MINB>
+template <int TY, int R, int LIM, int MINB>
 StageKernel make_stage3d() {
   StageKernel k;
-  k.fn = stage3d_kernel<TY, R, MINB>;
+  k.fn = stage3d_kernel<TY, R, LIM, MINB>;
   k.ty = TY; k.np = 3; k.threads = Stage3dSmem<TY>::NT; k.smem = Stage3dSmem<TY>::BYTES;
   return k;
 }
 
-StageKernel pick_stage(int ndim, int eqset, int riemann) {
+StageKernel pick_stage(int ndim, int eqset, int riemann, int limiter) {
   if (ndim == 3) {
     if (getenv("AGATE_STAGE_V1")) {      // the pooled kernel of agate_kernels.cuh, kept for A/B measurements
       if (riemann == AGATE_HLLD) return make_stage<6, 3, 1, false, 2>();
       return make_stage<6, 3, 0, false, 2>();
     }
-    if (riemann == AGATE_HLLD) return make_stage3d<TY3, 1, AGATE_MINB3>();
-    return make_stage3d<TY3, 0, AGATE_MINB3>();
+    if (limiter == 2) {                  // eq.4 (every BASELINE config): limiter fixed at compile time
+      if (riemann == AGATE_HLLD) return make_stage3d<TY3, 1, 2, AGATE_MINB3>();
+      return make_stage3d<TY3, 0, 2, AGATE_MINB3>();
+    }
+    if (riemann == AGATE_HLLD) return make_stage3d<TY3, 1, -1, AGATE_MINB3>();
+    return make_stage3d<TY3, 0, -1, AGATE_MINB3>();
   }
   if (eqset == AGATE_HALL) return make_stage<TY2, 1, 0, true, 2>();
   if (riemann == AGATE_HLLD) return make_stage<TY2, 1, 1, false, 2>();
@@ -308,7 +312,7 @@ int agate_init(const agate_grid* grid, double gamma, int eqset, const agate_solv
   c->ticket = (unsigned int*)(c->ws + L.off_scal + 128);
   c->partial = (double*)(c->ws + L.off_partial);
 
-  c->sk = pick_stage(grid->ndim, eqset, solver->riemann);
+  c->sk = pick_stage(grid->ndim, eqset, solver->riemann, solver->limiter);
   cudaError_t e = cudaFuncSetAttribute((const void*)c->sk.fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)c->sk.smem);
   cudaFuncAttributes fa;
   if (e == cudaSuccess) e = cudaFuncGetAttributes(&fa, (const void*)c->sk.fn);

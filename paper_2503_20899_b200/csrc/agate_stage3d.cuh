@@ -58,7 +58,9 @@ struct Stage3dSmem {
   static constexpr size_t BYTES = sizeof(double) * (size_t)TOTAL;
 };
 
-template <int TY, int RIEMANN, int MINB>
+// LIM >= 0 fixes the limiter at compile time (no branch per slope, one basic block for all eight variables);
+// LIM < 0 reads it from the parameters.
+template <int TY, int RIEMANN, int LIM, int MINB>
 __global__ void __launch_bounds__(32 * (TY + 1), MINB) stage3d_kernel(const __grid_constant__ StageParams P) {
   using SM = Stage3dSmem<TY>;
   constexpr int NT = SM::NT, PL = SM::PL, SB = SM::SB, QS = SM::QS, YS = SM::YS, ZS = SM::ZS, XS = SM::XS;
@@ -80,7 +82,7 @@ __global__ void __launch_bounds__(32 * (TY + 1), MINB) stage3d_kernel(const __gr
   const double cx = dt * P.idx, cy = dt * P.idy, cz = dt * P.idz;
   const bool two = (P.a0 != 0.0);                       // second SSP stage: Uout = a1 (U0 + Uin + dt L)
   const double c0 = two ? P.a1 : 1.0;
-  const int limiter = P.limiter;
+  const int limiter = (LIM >= 0) ? LIM : P.limiter;
   const double beta = P.beta;
   const bool cell_ok = owner && lane < tw && wid < th;
   // padded-array bounds of what this thread copies (ragged tiles only)
