@@ -83,7 +83,7 @@ __global__ void __launch_bounds__(32 * (TY + 1), MINB) stage3d_kernel(const __gr
   const bool two = (P.a0 != 0.0);                       // second SSP stage: Uout = a1 (U0 + Uin + dt L)
   const double c0 = two ? P.a1 : 1.0;
   const int limiter = (LIM >= 0) ? LIM : P.limiter;
-  const double beta = P.beta;
+  const double hbeta = 0.5 * P.beta;
   const bool cell_ok = owner && lane < tw && wid < th;
   // padded-array bounds of what this thread copies (ragged tiles only)
   const bool own_in = owner && (x0 + lane + 2 < P.nxp) && (y0 + wid + 2 < P.nyp);
@@ -155,7 +155,7 @@ __global__ void __launch_bounds__(32 * (TY + 1), MINB) stage3d_kernel(const __gr
 #pragma unroll
     for (int q = 0; q < 8; ++q) {
       const double a = W[q * QS + ca], b = W[q * QS + cb], c = W[q * QS + cc];
-      WLz[q * ZS + tid] = b + 0.5 * limited_slope(limiter, beta, c - b, b - a);
+      WLz[q * ZS + tid] = b + half_slope(limiter, hbeta, c - b, b - a);
     }
     // plane k0+1 goes into the slot plane k0-2 just left (own cell only: no other thread touches it)
     if (own_in) copy_cell(slot_of(k0 + 1) + own_off, own_g + (long long)(k0 + 3) * P.sz);
@@ -200,7 +200,7 @@ __global__ void __launch_bounds__(32 * (TY + 1), MINB) stage3d_kernel(const __gr
           for (int r = 0; r < 8; ++r) {
             const int v = rot_var(r, 2);
             const double a = W[v * QS + sm + own_off], b = W[v * QS + sc + own_off], c = W[v * QS + sp + own_off];
-            const double hs = 0.5 * limited_slope(limiter, beta, c - b, b - a);
+            const double hs = half_slope(limiter, hbeta, c - b, b - a);
             L[r] = WLz[v * ZS + tid];
             R[r] = b - hs;
             WLz[v * ZS + tid] = b + hs;
@@ -221,7 +221,7 @@ __global__ void __launch_bounds__(32 * (TY + 1), MINB) stage3d_kernel(const __gr
 #pragma unroll
             for (int r = 0; r < 8; ++r) {
               const double a = W[r * QS + c - 1], b = W[r * QS + c], cc = W[r * QS + c + 1];
-              const double hs = 0.5 * limited_slope(limiter, beta, cc - b, b - a);
+              const double hs = half_slope(limiter, hbeta, cc - b, b - a);
               L[r] = b + hs;
               const double rn = __shfl_down_sync(0xffffffffu, b - hs, 1);
               R[r] = (lane == 31) ? XR[r * XS + wid] : rn;
@@ -237,7 +237,7 @@ __global__ void __launch_bounds__(32 * (TY + 1), MINB) stage3d_kernel(const __gr
 #pragma unroll
             for (int q = 0; q < 8; ++q) {
               const double a = W[q * QS + cm], b = W[q * QS + c0r], c = W[q * QS + cp];
-              YR[q * YS + TY * 32 + lane] = b - 0.5 * limited_slope(limiter, beta, c - b, b - a);
+              YR[q * YS + TY * 32 + lane] = b - half_slope(limiter, hbeta, c - b, b - a);
             }
           }
           // column x = 32: right state for lane 31 of every row
@@ -246,7 +246,7 @@ __global__ void __launch_bounds__(32 * (TY + 1), MINB) stage3d_kernel(const __gr
 #pragma unroll
             for (int q = 0; q < 8; ++q) {
               const double a = W[q * QS + c - 1], b = W[q * QS + c], cc = W[q * QS + c + 1];
-              XR[q * XS + lane] = b - 0.5 * limited_slope(limiter, beta, cc - b, b - a);
+              XR[q * XS + lane] = b - half_slope(limiter, hbeta, cc - b, b - a);
             }
           }
           // face x = -1/2 of every row: lanes 0..15 hold cell -1 (left state), lanes 16..31 cell 0 (right state)
@@ -256,7 +256,7 @@ __global__ void __launch_bounds__(32 * (TY + 1), MINB) stage3d_kernel(const __gr
 #pragma unroll
             for (int r = 0; r < 8; ++r) {
               const double a = W[r * QS + c - 1], b = W[r * QS + c], cc = W[r * QS + c + 1];
-              const double hs = 0.5 * limited_slope(limiter, beta, cc - b, b - a);
+              const double hs = half_slope(limiter, hbeta, cc - b, b - a);
               L[r] = b + hs;
               R[r] = __shfl_down_sync(0xffffffffu, b - hs, 16);
             }
@@ -269,7 +269,7 @@ __global__ void __launch_bounds__(32 * (TY + 1), MINB) stage3d_kernel(const __gr
           for (int r = 0; r < 8; ++r) {
             const int v = rot_var(r, 1);
             const double a = W[v * QS + cm], b = W[v * QS + c0r], c = W[v * QS + cp];
-            L[r] = b + 0.5 * limited_slope(limiter, beta, c - b, b - a);
+            L[r] = b + half_slope(limiter, hbeta, c - b, b - a);
             R[r] = YR[v * YS + lane];
           }
           flux = true;
@@ -302,7 +302,7 @@ __global__ void __launch_bounds__(32 * (TY + 1), MINB) stage3d_kernel(const __gr
             for (int r = 0; r < 8; ++r) {
               const int v = rot_var(r, 1);
               const double a = W[v * QS + cm], b = W[v * QS + c], cc = W[v * QS + cp];
-              const double hs = 0.5 * limited_slope(limiter, beta, cc - b, b - a);
+              const double hs = half_slope(limiter, hbeta, cc - b, b - a);
               YR[v * YS + wid * 32 + lane] = b - hs;
               Ly[r] = b + hs;
             }
