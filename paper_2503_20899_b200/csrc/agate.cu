@@ -81,6 +81,7 @@ struct StageKernel {
   stage_fn_t fn;
   int ty, np, threads;
   size_t smem;
+  bool even_split = false;   // stage3d_kernel: one-wave grid, work split evenly (see agate_stage3d.cuh)
 };
 
 template <int TY, int NP, int R, bool H, int MINB>
@@ -96,6 +97,7 @@ StageKernel make_stage3d() {
   StageKernel k;
   k.fn = stage3d_kernel<TY, R, LIM, MINB>;
   k.ty = TY; k.np = 3; k.threads = Stage3dSmem<TY>::NT; k.smem = Stage3dSmem<TY>::BYTES;
+  k.even_split = true;
   return k;
 }
 
@@ -186,6 +188,8 @@ StageParams make_stage_params(const agate_ctx* c, const double* Uin, const doubl
   p.idz = (c->g.ndim >= 3) ? 1.0 / c->g.dz : 0.0;
   p.limiter = c->s.limiter; p.beta = c->s.beta;
   p.lz = c->lz;
+  p.ntx = (c->g.nx + TX - 1) / TX;
+  p.nty = (c->g.ny + c->sk.ty - 1) / c->sk.ty;
   p.ph = c->ph;
   return p;
 }
@@ -320,12 +324,11 @@ int agate_init(const agate_grid* grid, double gamma, int eqset, const agate_solv
   if (e != cudaSuccess) { delete c; return AGATE_ERR_CUDA; }
   c->regs = fa.numRegs;
 
-  // z-chunk length: chunks of ~128 planes keep the chunk start-up (3 plane loads + 1 z-only pass) near 1 %
   // z-chunk length: the grid is (x-y tiles) x (z chunks).  Pick the chunk count that minimises
   //   waves x (planes per chunk + start-up),  waves = ceil(CTAs / resident CTAs):  whole waves, short start-up
   //   (a chunk costs about four extra planes: three loads and the step that closes its last plane).
   c->lz = grid->nz;
-  if (grid->ndim == 3) {
+  if (grid->ndim == 3 && !c->sk.even_split) {
     int dev = 0, sms = 148;
     cudaGetDevice(&dev);
     cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
@@ -346,6 +349,20 @@ int agate_init(const agate_grid* grid, double gamma, int eqset, const agate_solv
   }
   c->sgrid = dim3((grid->nx + TX - 1) / TX, (grid->ny + c->sk.ty - 1) / c->sk.ty,
                   (grid->ndim == 3) ? (grid->nz + c->lz - 1) / c->lz : 1);
+  if (c->sk.even_split) {
+    // one resident wave; a CTA gets at least ~16 tile-planes so that a segment's start-up (three plane loads and
+    // the step that closes its last plane) stays small on tiny grids
+    int dev = 0, sms = 148;
+    cudaGetDevice(&dev);
+    cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
+    const long long slots = (long long)sms * (c->occ > 0 ? c->occ : 1);
+    const long long work = (long long)c->sgrid.x * c->sgrid.y * grid->nz;
+    long long g = (work + 15) / 16;
+    if (g > slots) g = slots;
+    if (g < 1) g = 1;
+    if (const char* s = getenv("AGATE_GRID")) { int v = atoi(s); if (v > 0) g = v; }
+    c->sgrid = dim3((unsigned)g, 1, 1);
+  }
   long long nrows = (long long)grid->ny * grid->nz;
   c->dt_blocks = (int)(nrows < kDtBlocksMax ? nrows : kDtBlocksMax);
   c->gpA = make_ghost(c, c->UA);

@@ -40,7 +40,8 @@ struct StageParams {
   double idx, idy, idz;  // 1/dx, 1/dy, 1/dz
   int limiter;
   double beta;
-  int lz;                // z-chunk length per CTA
+  int lz;                // z-chunk length per CTA (stage_kernel)
+  int ntx, nty;          // x-y tiles (stage3d_kernel: work = ntx * nty * nz tile-planes, split evenly over the grid)
   Phys ph;
 };
 

@@ -75,15 +75,25 @@ __global__ void __launch_bounds__(32 * (TY + 1), MINB) stage3d_kernel(const __gr
 
   const int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5;
   const bool owner = wid < TY;
-  const int x0 = blockIdx.x * TX, y0 = blockIdx.y * TY;
-  const int tw = min(TX, P.nx - x0), th = min(TY, P.ny - y0);
-  const int k0 = blockIdx.z * P.lz, k1 = min(P.nz, k0 + P.lz);
   const double dt = *P.dt_ptr;
   const double cx = dt * P.idx, cy = dt * P.idy, cz = dt * P.idz;
   const bool two = (P.a0 != 0.0);                       // second SSP stage: Uout = a1 (U0 + Uin + dt L)
   const double c0 = two ? P.a1 : 1.0;
   const int limiter = (LIM >= 0) ? LIM : P.limiter;
   const double hbeta = 0.5 * P.beta;
+
+  // Work = (x-y tile, plane) pairs in tile-major order, split EVENLY over the CTAs of a one-wave grid: a CTA walks
+  // its range as segments [k0, k1) of consecutive planes of one tile.  No tail wave, whatever the grid size.
+  const long long wtot = (long long)P.ntx * P.nty * P.nz;
+  long long wpos = wtot * blockIdx.x / gridDim.x;
+  const long long wend = wtot * (blockIdx.x + 1) / gridDim.x;
+  while (wpos < wend) {
+  const int tile = (int)(wpos / P.nz);
+  const int k0 = (int)(wpos - (long long)tile * P.nz);
+  const int k1 = (int)min((long long)P.nz, k0 + (wend - wpos));
+  wpos += k1 - k0;
+  const int x0 = (tile % P.ntx) * TX, y0 = (tile / P.ntx) * TY;
+  const int tw = min(TX, P.nx - x0), th = min(TY, P.ny - y0);
   const bool cell_ok = owner && lane < tw && wid < th;
   // padded-array bounds of what this thread copies (ragged tiles only)
   const bool own_in = owner && (x0 + lane + 2 < P.nxp) && (y0 + wid + 2 < P.nyp);
@@ -359,6 +369,8 @@ __global__ void __launch_bounds__(32 * (TY + 1), MINB) stage3d_kernel(const __gr
     { const int t = sm; sm = sc; sc = sp; sp = t; }
   }
   cp_async_wait_all();
+  __syncthreads();                 // the next segment reuses the shared buffers
+  }
 }
 
 }  // namespace agate
