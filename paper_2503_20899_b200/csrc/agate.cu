@@ -82,6 +82,7 @@ struct StageKernel {
   int ty, np, threads;
   size_t smem;
   bool even_split = false;   // stage3d_kernel: one-wave grid, work split evenly (see agate_stage3d.cuh)
+  bool fused_dt = false;     // stage3d_kernel: A7 of the next step inside the last stage of this one
 };
 
 template <int TY, int NP, int R, bool H, int MINB>
@@ -98,6 +99,7 @@ StageKernel make_stage3d() {
   k.fn = stage3d_kernel<TY, R, LIM, MINB>;
   k.ty = TY; k.np = 3; k.threads = Stage3dSmem<TY>::NT; k.smem = Stage3dSmem<TY>::BYTES;
   k.even_split = true;
+  k.fused_dt = true;
   return k;
 }
 
@@ -134,6 +136,8 @@ struct agate_ctx {
   double *UA, *UB, *scal, *partial;
   int* flag;
   unsigned int* ticket;
+  unsigned long long* vnext;       // fused A7: bit pattern of v_max of the current state (valid iff vmax_valid)
+  bool vmax_valid = false;
   bool have_state = false;
   int sticky = AGATE_OK;
   StageKernel sk;
@@ -175,7 +179,7 @@ GhostParams make_ghost(const agate_ctx* c, double* U) {
 }
 
 StageParams make_stage_params(const agate_ctx* c, const double* Uin, const double* U0, double* Uout, double a0,
-                              double a1) {
+                              double a1, bool last_stage) {
   StageParams p;
   const Layout& L = c->L;
   p.Uin = Uin; p.U0 = U0; p.Uout = Uout; p.dt_ptr = c->scal;
@@ -187,6 +191,8 @@ StageParams make_stage_params(const agate_ctx* c, const double* Uin, const doubl
   p.idy = (c->g.ndim >= 2) ? 1.0 / c->g.dy : 0.0;
   p.idz = (c->g.ndim >= 3) ? 1.0 / c->g.dz : 0.0;
   p.limiter = c->s.limiter; p.beta = c->s.beta;
+  p.vnext = (last_stage && c->sk.fused_dt) ? c->vnext : nullptr;
+  p.flag = c->flag;
   p.lz = c->lz;
   p.ntx = (c->g.nx + TX - 1) / TX;
   p.nty = (c->g.ny + c->sk.ty - 1) / c->sk.ty;
@@ -241,14 +247,34 @@ int launch_stage(agate_ctx* c, const StageParams& sp) {
 int enqueue_stages(agate_ctx* c) {
   int rc;
   if ((rc = launch_ghost(c, c->gpA))) return rc;
-  if ((rc = launch_stage(c, make_stage_params(c, c->UA, nullptr, c->UB, 0.0, 1.0)))) return rc;
+  if ((rc = launch_stage(c, make_stage_params(c, c->UA, nullptr, c->UB, 0.0, 1.0, c->s.rk == 1)))) return rc;
   if (c->s.rk == 1) {
     std::swap(c->UA, c->UB);
     std::swap(c->gpA, c->gpB);
     return AGATE_OK;
   }
   if ((rc = launch_ghost(c, c->gpB))) return rc;
-  return launch_stage(c, make_stage_params(c, c->UB, c->UA, c->UA, 0.5, 0.5));
+  return launch_stage(c, make_stage_params(c, c->UB, c->UA, c->UA, 0.5, 0.5, true));
+}
+
+// Head of a self-timed step: dt = C dx_min / v_max(U^n), t += dt  (R11).  Separate reduction pass, or -- when the
+// previous step's last stage already reduced v_max of what it stored -- one thread that turns it into dt.
+int launch_step_head(agate_ctx* c) {
+  if (!c->sk.fused_dt) return launch_dt(c, 1);
+  begin_step_kernel<<<1, 1, 0, c->stream>>>(c->scal, c->vnext, c->cfl * c->dxmin);
+  CU_TRY(cudaGetLastError());
+  return AGATE_OK;
+}
+
+// the fused path needs v_max of the current state once after agate_set_state
+int ensure_vmax(agate_ctx* c) {
+  if (!c->sk.fused_dt || c->vmax_valid) return AGATE_OK;
+  int rc = launch_dt(c, 0);
+  if (rc) return rc;
+  seed_vnext_kernel<<<1, 1, 0, c->stream>>>(c->scal, c->vnext);
+  CU_TRY(cudaGetLastError());
+  c->vmax_valid = true;
+  return AGATE_OK;
 }
 
 int collect_status(agate_ctx* c) {
@@ -314,6 +340,7 @@ int agate_init(const agate_grid* grid, double gamma, int eqset, const agate_solv
   c->scal = (double*)(c->ws + L.off_scal);
   c->flag = (int*)(c->ws + L.off_scal + 64);
   c->ticket = (unsigned int*)(c->ws + L.off_scal + 128);
+  c->vnext = (unsigned long long*)(c->ws + L.off_scal + 192);
   c->partial = (double*)(c->ws + L.off_partial);
 
   c->sk = pick_stage(grid->ndim, eqset, solver->riemann, solver->limiter);
@@ -386,6 +413,7 @@ int agate_set_state(agate_ctx* c, const double* U, int src_is_device, double t0)
   CU_TRY(cudaStreamSynchronize(c->stream));   // `sc` and the caller's U are borrowed only for this call
   if ((rc = launch_ghost(c, c->gpA))) return rc;
   c->have_state = true;
+  c->vmax_valid = false;
   if (c->sticky == AGATE_ERR_UNPHYSICAL) c->sticky = AGATE_OK;
   return AGATE_OK;
 }
@@ -408,12 +436,14 @@ int agate_step(agate_ctx* c, double dt, double* dt_used) {
   if (!c->have_state) return AGATE_ERR_STATE;
   int rc;
   if (dt > 0.0) {
-    set_dt_kernel<<<1, 1, 0, c->stream>>>(c->scal, dt);
+    set_dt_kernel<<<1, 1, 0, c->stream>>>(c->scal, dt, c->sk.fused_dt ? c->vnext : nullptr);
     CU_TRY(cudaGetLastError());
-  } else if ((rc = launch_dt(c, 1))) {
-    return rc;
+  } else {
+    if ((rc = ensure_vmax(c))) return rc;
+    if ((rc = launch_step_head(c))) return rc;
   }
   if ((rc = enqueue_stages(c))) return rc;
+  c->vmax_valid = c->sk.fused_dt;
   if (dt_used) {
     if ((rc = collect_status(c))) return rc;
     double v;
@@ -429,10 +459,11 @@ int agate_advance(agate_ctx* c, int32_t n_steps, double* t_out) {
   int rc;
   // stream capture is not allowed on the legacy default stream
   const bool use_graph = (c->s.rk == 2) && !c->timing && c->stream != nullptr && !getenv("AGATE_NO_GRAPH");
+  if (n_steps > 0 && (rc = ensure_vmax(c))) return rc;
   if (use_graph && !c->graph && n_steps > 0) {
     cudaGraph_t g = nullptr;
     CU_TRY(cudaStreamBeginCapture(c->stream, cudaStreamCaptureModeRelaxed));
-    rc = launch_dt(c, 1);
+    rc = launch_step_head(c);
     if (!rc) rc = enqueue_stages(c);
     cudaError_t e = cudaStreamEndCapture(c->stream, &g);
     if (rc || e != cudaSuccess) { if (g) cudaGraphDestroy(g); c->sticky = AGATE_ERR_CUDA; return AGATE_ERR_CUDA; }
@@ -444,7 +475,7 @@ int agate_advance(agate_ctx* c, int32_t n_steps, double* t_out) {
     if (use_graph) {
       CU_TRY(cudaGraphLaunch(c->graph, c->stream));
     } else {
-      if ((rc = launch_dt(c, 1))) return rc;
+      if ((rc = launch_step_head(c))) return rc;
       if ((rc = enqueue_stages(c))) return rc;
     }
   }

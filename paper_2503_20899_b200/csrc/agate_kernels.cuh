@@ -40,6 +40,11 @@ struct StageParams {
   double idx, idy, idz;  // 1/dx, 1/dy, 1/dz
   int limiter;
   double beta;
+  // A7 fused into the last stage of a step (stage3d_kernel): running max of the cell speeds of the values stored,
+  // as the bit pattern of a positive double (atomicMax on integers is exact and order-independent), and the sticky
+  // unphysical-state flag.  nullptr: not this stage.
+  unsigned long long* vnext;
+  int* flag;
   int lz;                // z-chunk length per CTA (stage_kernel)
   int ntx, nty;          // x-y tiles (stage3d_kernel: work = ntx * nty * nz tile-planes, split evenly over the grid)
   Phys ph;
@@ -402,7 +407,9 @@ __global__ void __launch_bounds__(256) dt_kernel(const __grid_constant__ DtParam
       double u[8];
 #pragma unroll
       for (int q = 0; q < 8; ++q) u[q] = __ldg(P.U + q * P.sq + base + i);
-      const double sp = cell_speed<HALL>(P.ph, u);
+      // ideal MHD: the same straight-line function the fused stage epilogue uses, so that a stand-alone
+      // reduction and the fused one give the same dt bit for bit
+      const double sp = HALL ? cell_speed<HALL>(P.ph, u) : cell_speed_inline(P.ph, u);
       if (sp < 0.0) bad = 1; else vm = fmax(vm, sp);
     }
   }
@@ -446,10 +453,27 @@ __global__ void __launch_bounds__(256) dt_kernel(const __grid_constant__ DtParam
   }
 }
 
-// host-chosen dt (agate_step with dt > 0): scal[0] = dt, t += dt
-__global__ void set_dt_kernel(double* scal, double dt) {
+// host-chosen dt (agate_step with dt > 0): scal[0] = dt, t += dt; the fused reduction starts from zero
+__global__ void set_dt_kernel(double* scal, double dt, unsigned long long* vnext) {
   scal[0] = dt;
   scal[2] += dt;
+  if (vnext) *vnext = 0ull;
+}
+
+// Head of a step when A7 is fused into the previous step's last stage: v_max of the current state is already in
+// *vnext.  dt = C dx_min / v_max, t += dt, and the reduction of this step starts from zero.
+__global__ void begin_step_kernel(double* scal, unsigned long long* vnext, double cfl_dx) {
+  const double v = __longlong_as_double((long long)*vnext);
+  const double dt = cfl_dx / v;
+  scal[1] = v;
+  scal[0] = dt;
+  scal[2] += dt;
+  *vnext = 0ull;
+}
+
+// after a stand-alone dt_kernel: hand its v_max to the fused path
+__global__ void seed_vnext_kernel(const double* scal, unsigned long long* vnext) {
+  *vnext = (unsigned long long)__double_as_longlong(scal[1]);
 }
 
 // ------------------------------------------------------------------------------------------------------------

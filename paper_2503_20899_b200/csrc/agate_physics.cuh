@@ -395,4 +395,19 @@ AG_HD double cell_speed(const Phys& ph, const double U[8]) {
   return (sp - sp == 0.0) ? sp : -1.0;     // finite test that survives fast-math-free builds
 }
 
+// A7 inside the stage epilogue (ideal MHD): the same quantity as cell_speed<false> with the straight-line roots of
+// this file, evaluated on the conserved values the stage is about to store.
+AG_HD double cell_speed_inline(const Phys& ph, const double U[8]) {
+  const double ir = rcp(U[0]);
+  const double v2 = (U[1] * U[1] + U[2] * U[2] + U[3] * U[3]) * (ir * ir);
+  const double bx2 = U[5] * U[5], by2 = U[6] * U[6], bz2 = U[7] * U[7];
+  const double B2 = bx2 + by2 + bz2;
+  const double p = ph.gm1 * (U[4] - 0.5 * U[0] * v2 - 0.5 * B2);
+  if (!(U[0] > 0.0) || !(p > 0.0)) return -1.0;
+  const double a2 = ph.gamma * p * ir, sm = a2 + B2 * ir;
+  const double rad = dmax(sm * sm - 4.0 * a2 * (dmin(dmin(bx2, by2), bz2) * ir), kTiny);
+  const double sp = sqrt_pos(dmax(v2, kTiny)) + sqrt_pos(0.5 * (sm + sqrt_pos(rad)));
+  return (sp - sp == 0.0) ? sp : -1.0;
+}
+
 }  // namespace agate

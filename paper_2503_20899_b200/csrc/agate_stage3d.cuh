@@ -84,6 +84,8 @@ __global__ void __launch_bounds__(32 * (TY + 1), MINB) stage3d_kernel(const __gr
 
   // Work = (x-y tile, plane) pairs in tile-major order, split EVENLY over the CTAs of a one-wave grid: a CTA walks
   // its range as segments [k0, k1) of consecutive planes of one tile.  No tail wave, whatever the grid size.
+  double vmx = 0.0;
+  int bad = 0;
   const long long wtot = (long long)P.ntx * P.nty * P.nz;
   long long wpos = wtot * blockIdx.x / gridDim.x;
   const long long wend = wtot * (blockIdx.x + 1) / gridDim.x;
@@ -294,14 +296,20 @@ __global__ void __launch_bounds__(32 * (TY + 1), MINB) stage3d_kernel(const __gr
         if (s == 0) {
           // A5 (z) + A6: plane k-1 is complete;  the accumulator of plane k starts with its low z face
           double* po = P.Uout + gm;                                       // own cell of plane k-1
+          double o[8];
 #pragma unroll
           for (int v = 0; v < 8; ++v, po += P.sq) {
             constexpr int inv2[8] = {0, 2, 3, 1, 4, 6, 7, 5};             // rot_var(inv2[v], 2) == v
             const int r = inv2[v];
             // the difference is formed before it meets U, so that a uniform state stays bitwise fixed (pin P1)
-            if (emit && cell_ok) *po = c0 * (acc[v] - cz * (F[r] - FzL[v * ZS + tid]));
+            o[v] = c0 * (acc[v] - cz * (F[r] - FzL[v * ZS + tid]));
+            if (emit && cell_ok) *po = o[v];
             FzL[v * ZS + tid] = F[r];
             acc[v] = 0.0;
+          }
+          if (P.vnext != nullptr && emit && cell_ok) {                    // A7 on the values just stored
+            const double sp = cell_speed_inline(P.ph, o);
+            if (sp < 0.0) bad = 1; else vmx = dmax(vmx, sp);
           }
           if (full) {
             // A2 (y): own slope -> right state for the row below, left state kept for phase B
@@ -370,6 +378,14 @@ __global__ void __launch_bounds__(32 * (TY + 1), MINB) stage3d_kernel(const __gr
   }
   cp_async_wait_all();
   __syncthreads();                 // the next segment reuses the shared buffers
+  }
+  if (P.vnext != nullptr) {
+    vmx = warp_max(vmx);
+    bad = __any_sync(0xffffffffu, bad);
+    if (lane == 0) {
+      if (vmx > 0.0) atomicMax(P.vnext, (unsigned long long)__double_as_longlong(vmx));
+      if (bad) atomicOr(P.flag, 1);
+    }
   }
 }
 

@@ -125,14 +125,27 @@ def test_config2_reduced(ag, n, steps):
     assert_parity(*run_pair(ag, wl, steps))
 
 
-@pytest.mark.parametrize("n,lz", [(40, 0), (40, 16), (72, 0)])
-def test_config3_reduced(ag, n, lz, monkeypatch):
-    """Config 3 recipe (3D HLLD).  n=40: ragged in x (32+8) and y (3*12+4); lz=16 forces 3 z-chunks per column
-    (chunk prologue path), lz=0 the default chunking."""
-    if lz:
-        monkeypatch.setenv("AGATE_LZ", str(lz))
+@pytest.mark.parametrize("n,grid", [(40, 0), (40, 1), (40, 7), (40, 37), (40, 160), (72, 0)])
+def test_config3_reduced(ag, n, grid, monkeypatch):
+    """Config 3 recipe (3D HLLD) through the row-owner kernel.  n=40: ragged in x (32+8) and y (3*11+7).  The work
+    (tile-planes) is split evenly over `grid` CTAs: 1 = every tile a whole segment of one CTA, 7 / 37 = segments that
+    start and end in the middle of a tile column, 160 = one or two planes per segment (every plane through the segment
+    prologue and the closing step), 0 = the library's own choice."""
+    if grid:
+        monkeypatch.setenv("AGATE_GRID", str(grid))
     wl = make_workload(3, n=n)
     assert_parity(*run_pair(ag, wl, 5 if n == 40 else 2))
+
+
+@pytest.mark.parametrize("lz", [0, 16])
+def test_config3_reduced_pooled_kernel(ag, lz, monkeypatch):
+    """Same recipe through the pooled 3-D kernel of agate_kernels.cuh (kept for A/B measurements); lz=16 forces three
+    z-chunks per column."""
+    monkeypatch.setenv("AGATE_STAGE_V1", "1")
+    if lz:
+        monkeypatch.setenv("AGATE_LZ", str(lz))
+    wl = make_workload(3, n=40)
+    assert_parity(*run_pair(ag, wl, 3))
 
 
 @pytest.mark.parametrize("n", [64, 100])
@@ -157,6 +170,53 @@ def test_advance_matches_oracle_advance(ag):
     assert abs(tg - tr) <= 1e-13 * tr
     assert np.all(rel_linf(gpu.get_state(), ref.get_state()) <= TOL_N)
     assert abs(gpu.t - tr) <= 1e-13 * tr
+
+
+@pytest.mark.parametrize("rk", [1, 2])
+def test_fused_dt_sequences_3d(ag, rk):
+    """3-D path: the Courant reduction of step n+1 runs inside the last stage of step n (A7 fused).  Every way into a
+    step must see the right v_max: after set_state (stand-alone reduction), after a self-timed step (fused), after a
+    step with a host-chosen dt (fused, restarted from zero), inside agate_advance (graph replay), after a second
+    set_state (stale value dropped).  dt and t against the oracle at every point."""
+    wl = make_workload(3, n=40)
+    ref = oracle.RefSolver.from_workload(wl, rk=rk)
+    gpu = ag.Agate.from_workload(wl, rk=rk)
+
+    def same_dt():
+        dr, dg = ref.compute_dt(), gpu.compute_dt()
+        assert abs(dg - dr) <= TOL_DT * dr
+        return dr
+
+    d = same_dt()
+    ref.step(d); assert abs(gpu.step(0.0) - d) <= TOL_DT * d              # stand-alone reduction feeds step 1
+    d = same_dt()
+    ref.step(d); assert abs(gpu.step(0.0) - d) <= TOL_DT * d              # fused reduction of step 1 feeds step 2
+    ref.step(0.4 * d); assert gpu.step(0.4 * d) == 0.4 * d                # host-chosen dt
+    d = same_dt()
+    ref.step(d); assert abs(gpu.step(0.0) - d) <= TOL_DT * d              # fused reduction after a host-chosen dt
+    tr = ref.advance(3); tg = gpu.advance(3)
+    assert abs(tg - tr) <= 1e-13 * tr
+    assert np.all(rel_linf(gpu.get_state(), ref.get_state()) <= TOL_N)
+    U0 = wl.U.copy()
+    ref.set_state(U0, 0.0); gpu.set_state(U0, 0.0)                        # v_max of the old state must not leak
+    tr = ref.advance(2); tg = gpu.advance(2)
+    assert abs(tg - tr) <= 1e-13 * tr
+    assert np.all(rel_linf(gpu.get_state(), ref.get_state()) <= TOL_N)
+    ref.close(); gpu.close()
+
+
+def test_fused_dt_flags_unphysical_3d(ag):
+    """R14 through the fused reduction: a step that drives a cell to negative pressure must be reported by the next
+    synchronising call (the stage that stores the value also evaluates its speed)."""
+    wl = make_workload(3, n=24)
+    gpu = ag.Agate.from_workload(wl)
+    d = gpu.compute_dt()
+    gpu.step(400.0 * d, sync=False)            # far beyond the Courant limit
+    with pytest.raises(ag.AgateError) as ei:
+        gpu.poll()
+        gpu.step(0.0)
+    assert ei.value.code == ag.ERR_UNPHYSICAL
+    gpu.close()
 
 
 # ---- solver options and edge cases --------------------------------------------------------------------------
