@@ -82,18 +82,31 @@ __global__ void __launch_bounds__(32 * (TY + 1), MINB) stage3d_kernel(const __gr
   const int limiter = (LIM >= 0) ? LIM : P.limiter;
   const double hbeta = 0.5 * P.beta;
 
-  // Work = (x-y tile, plane) pairs in tile-major order, split EVENLY over the CTAs of a one-wave grid: a CTA walks
-  // its range as segments [k0, k1) of consecutive planes of one tile.  No tail wave, whatever the grid size.
+  // Work = (x-y tile, plane) pairs, split EVENLY over the CTAs of a one-wave grid (no tail wave, whatever the grid
+  // size).  First the rounds: in round r CTA b takes the whole column of tile r * grid + b, so the CTAs resident at
+  // one time march side by side through neighbouring tiles and the halo cells they share are served by L2, not by
+  // DRAM.  Then the tiles that do not fill a round: their planes, in tile-major order, are cut into equal ranges,
+  // and a CTA walks its range as segments [k0, k1) of consecutive planes of one tile.
   double vmx = 0.0;
   int bad = 0;
-  const long long wtot = (long long)P.ntx * P.nty * P.nz;
+  const int ntile = P.ntx * P.nty;
+  const int nround = ntile / (int)gridDim.x;
+  const long long wtot = (long long)(ntile - nround * (int)gridDim.x) * P.nz;
   long long wpos = wtot * blockIdx.x / gridDim.x;
   const long long wend = wtot * (blockIdx.x + 1) / gridDim.x;
-  while (wpos < wend) {
-  const int tile = (int)(wpos / P.nz);
-  const int k0 = (int)(wpos - (long long)tile * P.nz);
-  const int k1 = (int)min((long long)P.nz, k0 + (wend - wpos));
-  wpos += k1 - k0;
+  for (int round = 0; round < nround || wpos < wend; ++round) {
+  int tile, k0, k1;
+  if (round < nround) {
+    tile = round * (int)gridDim.x + (int)blockIdx.x;
+    k0 = 0;
+    k1 = P.nz;
+  } else {
+    const int rt = (int)(wpos / P.nz);
+    tile = nround * (int)gridDim.x + rt;
+    k0 = (int)(wpos - (long long)rt * P.nz);
+    k1 = (int)min((long long)P.nz, k0 + (wend - wpos));
+    wpos += k1 - k0;
+  }
   const int x0 = (tile % P.ntx) * TX, y0 = (tile / P.ntx) * TY;
   const int tw = min(TX, P.nx - x0), th = min(TY, P.ny - y0);
   const bool cell_ok = owner && lane < tw && wid < th;
