@@ -3,7 +3,8 @@
     python bench.py [--gpus N] [--steps K] [--warmup W] [--config C] [--impl reference]
 
 A "step" is one pass of the whole hot path over the resident state: Courant reduction (A7), then per Runge-Kutta
-stage ghost fill (A0) + the fused stage kernel (A1-A6).  Default workload: BASELINE.json config 5 (3D ideal MHD,
+stage ghost fill (A0) + the fused stage kernel (A1-A6).  On 3-D grids A7 of step n+1 runs inside the last stage of
+step n and the step starts with a one-thread kernel that turns that v_max into dt.  Default workload: BASELINE.json config 5 (3D ideal MHD,
 512^3, PLM + eq.4 beta=1.3, HLLD, SSP-RK2, seeded synthetic state) on one GPU.  N > 1 runs N
 independent replicas of that problem, one per rank (the path is single-GPU by specification: "replicas only",
 weak scaling, no data-path collective); timing = barrier + device events, max over ranks.
@@ -39,6 +40,9 @@ UNIT = "zone-updates/s"
 FLOP_PER_ZONE_STEP = {1: 1430.0, 2: 1890.0, 3: 2770.0, 4: 1760.0, 5: 2770.0}
 FLOP_DT_PER_ZONE = {1: 45.0, 2: 45.0, 3: 45.0, 4: 60.0, 5: 45.0}
 BYTES_PER_ZONE_STEP = 320.0            # 5 x 8 variables x 8 B
+# DRAM bytes per launch of the dominant kernel (dram__bytes_read.sum + dram__bytes_write.sum, mean of the two stage
+# launches of one step) from the committed `ncu` capture of the same command: profiles/r1_stage3d.md
+NCU_TRAFFIC_BYTES = {5: 0.5 * (9372441088 + 8649890048 + 17961833984 + 8646440704)}
 FP64_NOMINAL_TFLOPS = 148 * 64 * 2 * 1.965e9 / 1e12     # 148 SMs x 64 DFMA lanes x 2 x max SM clock = 37.2
 
 # reduced size of the bounded CPU sample per config (same recipe and seed), and its step count
@@ -219,8 +223,9 @@ def run_ours(args):
     peaks, peak_src = measured_peaks()
     hbm_frac = (BYTES_PER_ZONE_STEP / 5.0 * 2.5 * zones / (stage_ms * 1e-3) / 1e9) / peaks["hbm_gbs"]
     roofline = {"bound": "alu", "achieved": achieved, "peak": fp64_peak, "unit": "TFLOP/s",
-                "frac": achieved / fp64_peak, "traffic": None,
-                "kernel": "stage_kernel", "ms_per_launch": stage_ms, "launches_timed": st_n,
+                "frac": achieved / fp64_peak, "traffic": NCU_TRAFFIC_BYTES.get(cfg) if not args.n else None,
+                "algorithmic_bytes": BYTES_PER_ZONE_STEP / 2.0 * zones,
+                "kernel": "stage3d_kernel" if wl.ndim == 3 else "stage_kernel", "ms_per_launch": stage_ms, "launches_timed": st_n,
                 "stage_share_of_step": 2.0 * stage_ms * K / ms_max if st_n else None,
                 "peak_source": "FP64 DFMA micro-benchmark of this run (agate_measure_fp64_peak); nominal "
                                f"{FP64_NOMINAL_TFLOPS:.1f} = 148 SM x 64 lanes x 2 x 1.965 GHz",
