@@ -16,7 +16,9 @@
 //   * no global-load latency on the critical path: conserved cells are brought in by cp.async (LDGSTS) one phase
 //     ahead, straight into their final shared-memory slot, and turned into primitives IN PLACE (A1) by the thread
 //     that issued the copy: owners their own cell of plane k+2, H the x-halo columns and the y-halo rows.
-//   * ONE call site of the Riemann solver: the three tasks of a warp per plane run through one loop.
+//   * the three tasks of a warp per plane run through one loop that is unrolled: three inlined copies of the solver,
+//     each with its direction's variable permutation resolved at compile time (3 % faster than one call site with
+//     the states marshalled into common registers; 91 KB of SASS, no instruction-fetch stalls measured).
 //   * A6: the accumulator of plane k gets Uin (+U0 in the second SSP stage) right after
 //     barrier 1 (the loads are issued just before it), then the x and y differences; plane k leaves in step k+1.
 //
@@ -205,7 +207,7 @@ __global__ void __launch_bounds__(32 * (TY + 1), MINB) stage3d_kernel(const __gr
     const int hb = 3 * PL + (k & 1) * SB;                 // y-halo rows of plane k
     double Ly[8], ua[8], ub[8];
 
-#pragma unroll 1
+#pragma unroll
     for (int s = 0; s < 3; ++s) {
       double L[8], R[8], F[8];
       bool flux = false;
