@@ -281,7 +281,8 @@ int collect_status(agate_ctx* c) {
   CU_TRY(cudaStreamSynchronize(c->stream));
   int flag = 0;
   CU_TRY(cudaMemcpy(&flag, c->flag, sizeof(int), cudaMemcpyDeviceToHost));
-  if (flag && c->sticky == AGATE_OK) c->sticky = AGATE_ERR_UNPHYSICAL;
+  if ((flag & 2) && c->sticky == AGATE_OK) c->sticky = AGATE_ERR_CUDA;          // a hand-over wait ran out (stage3d)
+  if ((flag & 1) && c->sticky == AGATE_OK) c->sticky = AGATE_ERR_UNPHYSICAL;
   return c->sticky;
 }
 

@@ -10,7 +10,9 @@
 //     flux through face -1/2) and row TY (its right state) belong to H.
 //   * z: private column, one plane behind: step k computes F(k-1/2) from planes k-1, k, k+1 and completes plane
 //     k-1.  The left state W(k-1)+dW(k-1)/2 is carried in a per-thread shared slot, the accumulator in registers.
-//   * TWO CTA-wide barriers per plane.  Phase A: y-difference of the previous plane, z slope + flux, store of
+//   * NO CTA-wide barrier in the steady state: two phases per plane, and at each phase boundary a warp publishes a
+//     phase counter (st.release) and waits (ld.acquire) only for the warps whose data it reads or overwrites -- its
+//     two neighbours and H; H waits for all owners once per plane.  Phase A: y-difference of the previous plane, z slope + flux, store of
 //     plane k-1, y slope -> YR.  Phase B: y flux -> YF, x slope + flux + difference.  H mirrors the owners with the
 //     tile-edge tasks (one Riemann call per phase), so no warp idles while the others solve.
 //   * no global-load latency on the critical path: conserved cells are brought in by cp.async (LDGSTS) one phase
@@ -37,6 +39,24 @@ __device__ __forceinline__ void cp_async8(double* sdst, const double* gsrc) {
                : "memory");
 }
 __device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wait_all;" ::: "memory"); }
+// Pairwise hand-over between the warps of a CTA: prog[w] = number of phases warp w has completed and published.
+__device__ __forceinline__ void publish(int* prog_w, int value, int lane) {
+  __syncwarp();                                   // every lane's shared-memory writes are ordered before lane 0's release
+  if (lane == 0) asm volatile("st.release.cta.shared.s32 [%0], %1;" ::"r"((uint32_t)__cvta_generic_to_shared(prog_w)), "r"(value) : "memory");
+}
+__device__ __forceinline__ int peek(const int* prog_w) {
+  int v;
+  asm volatile("ld.acquire.cta.shared.s32 %0, [%1];" : "=r"(v) : "r"((uint32_t)__cvta_generic_to_shared(prog_w)) : "memory");
+  return v;
+}
+// spin until prog[w] >= value; a bounded spin (a lost hand-over would otherwise hang the GPU): on overflow the
+// caller's sticky flag gets bit 1 and the kernel runs on
+__device__ __forceinline__ void await(const int* prog_w, int value, int* flag) {
+  int spins = 0;
+  while (peek(prog_w) < value) {
+    if (++spins > (1 << 24)) { atomicOr(flag, 2); break; }
+  }
+}
 __device__ __forceinline__ void prefetch_l2(const void* p) { asm volatile("prefetch.global.L2 [%0];" ::"l"(p)); }
 
 template <int TY>
@@ -56,7 +76,8 @@ struct Stage3dSmem {
   static constexpr int OFF_FZL = OFF_WLZ + 8 * ZS;
   static constexpr int OFF_XR = OFF_FZL + 8 * ZS;
   static constexpr int OFF_XF = OFF_XR + 8 * XS;
-  static constexpr int TOTAL = OFF_XF + 8 * XS;
+  static constexpr int OFF_PROG = OFF_XF + 8 * XS;  // 16 ints: per-warp phase counters
+  static constexpr int TOTAL = OFF_PROG + 8;
   static constexpr size_t BYTES = sizeof(double) * (size_t)TOTAL;
 };
 
@@ -74,6 +95,7 @@ __global__ void __launch_bounds__(32 * (TY + 1), MINB) stage3d_kernel(const __gr
   double* const FzL = smem + SM::OFF_FZL;    // [8][ZS]  z: flux through the low face of plane k-1     (fixed order)
   double* const XR = smem + SM::OFF_XR;      // [8][XS]  right state of cell x = 32, per row
   double* const XF = smem + SM::OFF_XF;      // [8][XS]  x flux through face -1/2, per row
+  int* const prog = reinterpret_cast<int*>(smem + SM::OFF_PROG);   // [TY+1] phases completed, per warp
 
   const int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5;
   const bool owner = wid < TY;
@@ -91,6 +113,9 @@ __global__ void __launch_bounds__(32 * (TY + 1), MINB) stage3d_kernel(const __gr
   // and a CTA walks its range as segments [k0, k1) of consecutive planes of one tile.
   double vmx = 0.0;
   int bad = 0;
+  int ph = 0;                                     // phases this warp has completed (the same count in every warp)
+  if (tid < 16) prog[tid] = 0;
+  __syncthreads();
   const int ntile = P.ntx * P.nty;
   const int nround = ntile / (int)gridDim.x;
   const long long wtot = (long long)(ntile - nround * (int)gridDim.x) * P.nz;
@@ -211,6 +236,29 @@ __global__ void __launch_bounds__(32 * (TY + 1), MINB) stage3d_kernel(const __gr
     for (int s = 0; s < 3; ++s) {
       double L[8], R[8], F[8];
       bool flux = false;
+      // ---- hand-over: what this phase reads must be published, what it overwrites must have been read.  Every
+      //      wait is on a phase EARLIER than the one about to start, so the waits cannot form a cycle.
+      if (s == 0) {
+        // phase A.  owner j: YF / YR row pair with the warp below (H for row 0), ring rows j+-1 of plane k, and the
+        // y-halo rows (H) for the top row.  H: every owner is done with XR / XF / YR[TY] and the halo columns.
+        if (owner) {
+          await(prog + (wid == 0 ? TY : wid - 1), ph, P.flag);
+          await(prog + (wid == TY - 1 ? TY : wid + 1), wid == TY - 1 ? ph : ph - 1, P.flag);
+        } else {
+          await(prog + min(lane, TY - 1), ph, P.flag);
+          __syncwarp();
+        }
+      } else if (s == 1) {
+        // phase B.  owner j: YR of the row above (H for the top row), XR / XF and the halo columns (H).
+        // H: YR[0] (owner 0), and both edge owners are done with the y-halo rows H is about to refill.
+        if (owner) {
+          await(prog + (wid == TY - 1 ? TY : wid + 1), ph, P.flag);
+          await(prog + TY, ph, P.flag);
+        } else {
+          await(prog + 0, ph, P.flag);
+          await(prog + TY - 1, ph, P.flag);
+        }
+      }
       // ------------------------------------------------------------------ prepare the face states of task s
       if (owner) {
         if (s == 0) {
@@ -387,7 +435,7 @@ __global__ void __launch_bounds__(32 * (TY + 1), MINB) stage3d_kernel(const __gr
           if (k + 2 < k1) h_copy(k + 2, sm);
         }
       }
-      if (s != 1) __syncthreads();        // barrier 1 after phase A, barrier 2 after phase B
+      if (s != 1) publish(prog + wid, ++ph, lane);   // end of phase A (s = 0) and of phase B (s = 2)
     }
     { const int t = sm; sm = sc; sc = sp; sp = t; }
   }
