@@ -54,7 +54,8 @@ __device__ __forceinline__ int peek(const int* prog_w) {
 __device__ __forceinline__ void await(const int* prog_w, int value, int* flag) {
   int spins = 0;
   while (peek(prog_w) < value) {
-    if (++spins > (1 << 24)) { atomicOr(flag, 2); break; }
+    __nanosleep(40);                              // the wait is for ~a phase of another warp; keep the issue slots free
+    if (++spins > (1 << 22)) { atomicOr(flag, 2); break; }
   }
 }
 __device__ __forceinline__ void prefetch_l2(const void* p) { asm volatile("prefetch.global.L2 [%0];" ::"l"(p)); }

@@ -219,6 +219,22 @@ def test_fused_dt_flags_unphysical_3d(ag):
     gpu.close()
 
 
+def test_3d_run_to_run_bitwise(ag):
+    """The 3-D kernel hands data between warps through phase counters instead of CTA barriers; a lost ordering would
+    show up as run-to-run differences.  Same input, same launch configuration, 8 steps, three runs: bitwise equal
+    (dt included), on a grid with ragged tiles and several segments per CTA."""
+    wl = make_workload(5, n=72)
+    outs = []
+    for _ in range(3):
+        gpu = ag.Agate.from_workload(wl)
+        t = gpu.advance(8)
+        outs.append((t, gpu.get_state()))
+        gpu.close()
+    for t, U in outs[1:]:
+        assert t == outs[0][0]
+        assert np.array_equal(U, outs[0][1])
+
+
 # ---- solver options and edge cases --------------------------------------------------------------------------
 @pytest.mark.parametrize("riemann", [HLL, HLLD])
 @pytest.mark.parametrize("limiter,beta", [(0, 1.0), (1, 1.0), (2, 1.0), (2, 2.0)])
