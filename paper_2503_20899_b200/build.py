@@ -17,7 +17,7 @@ INCLUDE = os.path.join(_ROOT, "include")
 LIB = os.path.join(_HERE, "libagate.so")
 SOURCES = [os.path.join(CSRC, "agate.cu")]
 DEPS = SOURCES + [os.path.join(CSRC, "agate_kernels.cuh"), os.path.join(CSRC, "agate_physics.cuh"),
-                  os.path.join(CSRC, "agate_stage3d.cuh"),
+                  os.path.join(CSRC, "agate_stage3d.cuh"), os.path.join(CSRC, "agate_stage2d.cuh"),
                   os.path.join(INCLUDE, "agate.h")]
 
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",

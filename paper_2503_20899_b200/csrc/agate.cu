@@ -12,6 +12,7 @@
 #include <vector>
 
 #include "agate_kernels.cuh"
+#include "agate_stage2d.cuh"
 #include "agate_stage3d.cuh"
 
 using namespace agate;
@@ -82,7 +83,8 @@ struct StageKernel {
   int ty, np, threads;
   size_t smem;
   bool even_split = false;   // stage3d_kernel: one-wave grid, work split evenly (see agate_stage3d.cuh)
-  bool fused_dt = false;     // stage3d_kernel: A7 of the next step inside the last stage of this one
+  bool fused_dt = false;     // stage3d / stage2d kernels: A7 of the next step inside the last stage of this one
+  bool strips2d = false;     // stage2d_kernel: one-wave grid of autonomous warps (see agate_stage2d.cuh)
 };
 
 template <int TY, int NP, int R, bool H, int MINB>
@@ -103,6 +105,16 @@ StageKernel make_stage3d() {
   return k;
 }
 
+template <int R, int LIM>
+StageKernel make_stage2d() {
+  StageKernel k;
+  k.fn = stage2d_kernel<R, LIM>;
+  k.ty = 1; k.np = 1; k.threads = 32 * NW2; k.smem = Stage2dSmem::BYTES;
+  k.strips2d = true;
+  k.fused_dt = true;
+  return k;
+}
+
 StageKernel pick_stage(int ndim, int eqset, int riemann, int limiter) {
   if (ndim == 3) {
     if (getenv("AGATE_STAGE_V1")) {      // the pooled kernel of agate_kernels.cuh, kept for A/B measurements
@@ -115,6 +127,14 @@ StageKernel pick_stage(int ndim, int eqset, int riemann, int limiter) {
     }
     if (riemann == AGATE_HLLD) return make_stage3d<TY3, 1, -1, AGATE_MINB3>();
     return make_stage3d<TY3, 0, -1, AGATE_MINB3>();
+  }
+  if (ndim == 2 && eqset == AGATE_IDEAL && !getenv("AGATE_STAGE_V1")) {   // warp-autonomous strips
+    if (limiter == 2) {
+      if (riemann == AGATE_HLLD) return make_stage2d<1, 2>();
+      return make_stage2d<0, 2>();
+    }
+    if (riemann == AGATE_HLLD) return make_stage2d<1, -1>();
+    return make_stage2d<0, -1>();
   }
   if (eqset == AGATE_HALL) return make_stage<TY2, 1, 0, true, 2>();
   if (riemann == AGATE_HLLD) return make_stage<TY2, 1, 1, false, 2>();
@@ -377,6 +397,19 @@ int agate_init(const agate_grid* grid, double gamma, int eqset, const agate_solv
   }
   c->sgrid = dim3((grid->nx + TX - 1) / TX, (grid->ny + c->sk.ty - 1) / c->sk.ty,
                   (grid->ndim == 3) ? (grid->nz + c->lz - 1) / c->lz : 1);
+  if (c->sk.strips2d) {
+    // one resident wave of 6-warp CTAs; a warp gets at least ~16 rows of its 30-column strip
+    int dev = 0, sms = 148;
+    cudaGetDevice(&dev);
+    cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
+    const long long slots = (long long)sms * (c->occ > 0 ? c->occ : 1);
+    const long long work = (long long)((grid->nx + SW2 - 1) / SW2) * grid->ny;
+    long long g = (work + 16 * NW2 - 1) / (16 * NW2);
+    if (g > slots) g = slots;
+    if (g < 1) g = 1;
+    if (const char* s = getenv("AGATE_GRID")) { int v = atoi(s); if (v > 0) g = v; }
+    c->sgrid = dim3((unsigned)g, 1, 1);
+  }
   if (c->sk.even_split) {
     // one resident wave; a CTA gets at least ~16 tile-planes so that a segment's start-up (three plane loads and
     // the step that closes its last plane) stays small on tiny grids

@@ -1,0 +1,227 @@
+// agate_stage2d.cuh — warp-autonomous fused stage kernel for 2-D ideal-MHD grids, sm_100a.
+//
+// Same arithmetic as the other two stage kernels; what differs is that a WARP, not a CTA, is the unit of work:
+//   * a warp owns a strip of 30 columns and marches along y.  Lanes 1..30 own the strip's cells of the current row,
+//     lanes 0 and 31 hold the strip's x-halo cells (x = -1, 30): they compute slopes and face states like the others
+//     but store nothing.  30 of 32 lanes do useful updates; in exchange there is NO synchronisation between warps at
+//     all (no barrier, no flag) and no helper warp.
+//   * x: the right state of face i+1/2 and the flux of face i-1/2 travel by warp shuffles.
+//   * y: private column, one row behind (like z in stage3d_kernel): step j computes F(j-1/2) from rows j-1, j, j+1 and
+//     completes row j-1.  The left state W(j-1)+dW/2 and the low-face flux are carried in per-lane shared slots,
+//     the accumulator in registers.
+//   * conserved rows arrive by cp.async one step ahead in a private ring of 4 rows x 34 cells and are turned into
+//     primitives in place (A1); the raw Uin (+U0, copied straight into the same slot) of the own cell is kept for A6.
+//   * work = (strip, row) pairs in strip-major order, cut into equal ranges over all warps of a one-wave grid.
+//   * A7 of the next step rides in the last stage, as in stage3d_kernel.
+//
+// Shared memory per warp: ring 4 x 8 x 34, two y carries 8 x 32, raw U 2 x 8 x 32  =  16.5 KB;  6 warps per CTA,
+// 2 CTAs per SM (12 warps, <= 168 registers).
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+#include "agate_stage3d.cuh"
+
+namespace agate {
+
+constexpr int SW2 = 30;        // cells a warp updates per row
+constexpr int RW2 = 34;        // cells per ring row: x = xs-2 .. xs+31
+constexpr int NW2 = 6;         // warps per CTA
+
+struct Stage2dSmem {
+  static constexpr int RING = 4 * 8 * RW2;          // [slot][q][c]
+  static constexpr int OFF_WLY = RING;              // [q][lane]
+  static constexpr int OFF_FYL = OFF_WLY + 8 * 32;
+  static constexpr int OFF_URAW = OFF_FYL + 8 * 32; // [2][q][lane]
+  static constexpr int PER_WARP = OFF_URAW + 2 * 8 * 32;
+  static constexpr size_t BYTES = sizeof(double) * (size_t)PER_WARP * NW2;
+};
+
+template <int RIEMANN, int LIM>
+__global__ void __launch_bounds__(32 * NW2, 2) stage2d_kernel(const __grid_constant__ StageParams P) {
+  using SM = Stage2dSmem;
+  extern __shared__ __align__(16) double smem[];
+  const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
+  double* const ring = smem + (size_t)wid * SM::PER_WARP;      // this warp's private buffers
+  double* const WLy = ring + SM::OFF_WLY;
+  double* const FyL = ring + SM::OFF_FYL;
+  double* const Uraw = ring + SM::OFF_URAW;
+
+  const double dt = *P.dt_ptr;
+  const double cx = dt * P.idx, cy = dt * P.idy;
+  const bool two = (P.a0 != 0.0);
+  const double c0 = two ? P.a1 : 1.0;
+  const int limiter = (LIM >= 0) ? LIM : P.limiter;
+  const double hbeta = 0.5 * P.beta;
+  double vmx = 0.0;
+  int bad = 0;
+
+  const int nstrip = (P.nx + SW2 - 1) / SW2;
+  const long long wtot = (long long)nstrip * P.ny;
+  const long long nwarp = (long long)gridDim.x * NW2, gw = (long long)blockIdx.x * NW2 + wid;
+  long long wpos = wtot * gw / nwarp;
+  const long long wend = wtot * (gw + 1) / nwarp;
+
+  auto slot_of = [](int r) { return ((r + 4) & 3) * (8 * RW2); };      // r >= -4
+  auto conv = [&](int off) {                                            // A1 in place; returns nothing
+    double u[8], w[8];
+#pragma unroll
+    for (int q = 0; q < 8; ++q) u[q] = ring[off + q * RW2];
+    cons_to_prim(P.ph, u, w);
+#pragma unroll
+    for (int q = 0; q < 8; ++q) ring[off + q * RW2] = w[q];
+  };
+
+  while (wpos < wend) {
+    const int strip = (int)(wpos / P.ny);
+    const int j0 = (int)(wpos - (long long)strip * P.ny);
+    const int j1 = (int)min((long long)P.ny, j0 + (wend - wpos));
+    wpos += j1 - j0;
+    const int xs = strip * SW2;
+    const int x = xs - 1 + lane;                                 // the lane's own column
+    const bool cell_ok = lane >= 1 && lane <= SW2 && x < P.nx;
+    const bool own_in = xs + lane + 1 < P.nxp;                   // own cell c = lane + 1 inside the padded row
+    // extra halo cell of lanes 0 (c = 0) and 1 (c = 33)
+    const int cex = (lane == 0) ? 0 : RW2 - 1;
+    const bool ex_in = lane < 2 && xs + cex < P.nxp;
+    const long long g_own = (long long)xs + lane + 1, g_ex = (long long)xs + cex;     // + (row + 2) * sy
+
+    // copies of row r: the own cell (and U0 of it straight into the raw-U slot), the extra cell
+    auto copy_row = [&](int r, bool with_u0) {
+      const long long gr = (long long)(r + 2) * P.sy;
+      const int so = slot_of(r);
+      if (own_in) {
+        const double* src = P.Uin + gr + g_own;
+#pragma unroll
+        for (int q = 0; q < 8; ++q, src += P.sq) cp_async8(ring + so + q * RW2 + lane + 1, src);
+        if (two && with_u0) {
+          const double* s0 = P.U0 + gr + g_own;
+#pragma unroll
+          for (int q = 0; q < 8; ++q, s0 += P.sq) cp_async8(Uraw + ((r & 1) * 8 + q) * 32 + lane, s0);
+        }
+      }
+      if (ex_in) {
+        const double* src = P.Uin + gr + g_ex;
+#pragma unroll
+        for (int q = 0; q < 8; ++q, src += P.sq) cp_async8(ring + so + q * RW2 + cex, src);
+      }
+    };
+    // A1 for row r, and the raw Uin (+U0) of the own cell for A6
+    auto conv_row = [&](int r, bool keep_raw) {
+      const int so = slot_of(r);
+      if (own_in) {
+        if (keep_raw) {
+#pragma unroll
+          for (int q = 0; q < 8; ++q) {
+            const int a = ((r & 1) * 8 + q) * 32 + lane;
+            const double u = ring[so + q * RW2 + lane + 1];
+            Uraw[a] = two ? (u + Uraw[a]) : u;
+          }
+        }
+        conv(so + lane + 1);
+      }
+      if (ex_in) conv(so + cex);
+    };
+
+    // ---- prologue: rows j0-2, j0-1, j0 and the carried left state of face j0-1/2 ----
+#pragma unroll
+    for (int i = 0; i < 4 * 8 * RW2 / 32; ++i) ring[i * 32 + lane] = 1.0;      // cells outside the padded array
+    __syncwarp();
+    copy_row(j0 - 2, false); copy_row(j0 - 1, false); copy_row(j0, true);
+    cp_async_wait_all();
+    __syncwarp();
+    conv_row(j0 - 2, false); conv_row(j0 - 1, false); conv_row(j0, true);
+    __syncwarp();
+    {
+      const int c = lane + 1;
+#pragma unroll
+      for (int q = 0; q < 8; ++q) {
+        const double a = ring[slot_of(j0 - 2) + q * RW2 + c], b = ring[slot_of(j0 - 1) + q * RW2 + c];
+        const double cc = ring[slot_of(j0) + q * RW2 + c];
+        WLy[q * 32 + lane] = b + half_slope(limiter, hbeta, cc - b, b - a);
+      }
+    }
+    copy_row(j0 + 1, true);
+
+    double acc[8];
+#pragma unroll
+    for (int q = 0; q < 8; ++q) acc[q] = 0.0;
+
+    for (int j = j0; j <= j1; ++j) {
+      const bool full = j < j1;       // row j gets its x sweep (step j1 only closes row j1-1)
+      const bool emit = j > j0;       // row j-1 is completed in this step
+      const int sm = slot_of(j - 1), sc = slot_of(j), sp = slot_of(j + 1);
+      const int c = lane + 1;
+      double L[8], R[8], F[8];
+
+      // row j+1 has had a whole step to arrive
+      cp_async_wait_all();
+      __syncwarp();
+      conv_row(j + 1, true);
+      __syncwarp();
+
+      // ---- y task: A2 slope of row j, face j-1/2 (L carried, R = W(j) - dW/2), A3 + A4 ----
+#pragma unroll
+      for (int r = 0; r < 8; ++r) {
+        const int v = rot_var(r, 1);
+        const double a = ring[sm + v * RW2 + c], b = ring[sc + v * RW2 + c], cc = ring[sp + v * RW2 + c];
+        const double hs = half_slope(limiter, hbeta, cc - b, b - a);
+        L[r] = WLy[v * 32 + lane];
+        R[r] = b - hs;
+        WLy[v * 32 + lane] = b + hs;
+      }
+      riemann_flux<RIEMANN, false>(P.ph, L, R, nullptr, F);
+      {
+        // A5 (y) + A6: row j-1 is complete; the accumulator of row j starts from the raw Uin (+U0)
+        double* po = P.Uout + (long long)(j + 1) * P.sy + g_own;          // own cell of row j-1
+        double o[8];
+#pragma unroll
+        for (int v = 0; v < 8; ++v, po += P.sq) {
+          constexpr int inv1[8] = {0, 3, 1, 2, 4, 7, 5, 6};               // rot_var(inv1[v], 1) == v
+          const int r = inv1[v];
+          // the difference is formed before it meets U, so that a uniform state stays bitwise fixed (pin P1)
+          o[v] = c0 * (acc[v] - cy * (F[r] - FyL[v * 32 + lane]));
+          if (emit && cell_ok) *po = o[v];
+          FyL[v * 32 + lane] = F[r];
+          acc[v] = Uraw[((j & 1) * 8 + v) * 32 + lane];
+        }
+        if (P.vnext != nullptr && emit && cell_ok) {                      // A7 on the values just stored
+          const double sp2 = cell_speed_inline(P.ph, o);
+          if (sp2 < 0.0) bad = 1; else vmx = dmax(vmx, sp2);
+        }
+      }
+      __syncwarp();
+      // row j+2 into the slot row j-2 left; its U0 into the raw slot row j just left
+      if (j + 2 <= j1 + 1) copy_row(j + 2, true);
+
+      // ---- x task: A2 own slope, right state from lane i+1, A3 + A4, low-face flux from lane i-1 ----
+      if (full) {
+#pragma unroll
+        for (int r = 0; r < 8; ++r) {
+          const double a = ring[sc + r * RW2 + c - 1], b = ring[sc + r * RW2 + c], cc = ring[sc + r * RW2 + c + 1];
+          const double hs = half_slope(limiter, hbeta, cc - b, b - a);
+          L[r] = b + hs;
+          R[r] = __shfl_down_sync(0xffffffffu, b - hs, 1);
+        }
+        riemann_flux<RIEMANN, false>(P.ph, L, R, nullptr, F);
+#pragma unroll
+        for (int r = 0; r < 8; ++r) {
+          const double fl = __shfl_up_sync(0xffffffffu, F[r], 1);
+          acc[r] -= cx * (F[r] - fl);
+        }
+      }
+    }
+    cp_async_wait_all();
+    __syncwarp();
+  }
+  if (P.vnext != nullptr) {
+    vmx = warp_max(vmx);
+    bad = __any_sync(0xffffffffu, bad);
+    if (lane == 0) {
+      if (vmx > 0.0) atomicMax(P.vnext, (unsigned long long)__double_as_longlong(vmx));
+      if (bad) atomicOr(P.flag, 1);
+    }
+  }
+}
+
+}  // namespace agate

@@ -153,7 +153,6 @@ __global__ void __launch_bounds__(32 * (TY + 1), MINB) stage3d_kernel(const __gr
     for (int q = 0; q < 8; ++q) W[q * QS + off] = w[q];
   };
   auto copy_cell = [&](int off, long long g) {
-#pragma unroll
     const double* src = P.Uin + g;           // running pointer: one 64-bit add per variable
 #pragma unroll
     for (int q = 0; q < 8; ++q, src += P.sq) cp_async8(W + q * QS + off, src);
