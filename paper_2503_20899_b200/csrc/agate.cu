@@ -105,13 +105,13 @@ StageKernel make_stage3d() {
   return k;
 }
 
-template <int R, int LIM>
+template <int R, int LIM, bool H>
 StageKernel make_stage2d() {
   StageKernel k;
-  k.fn = stage2d_kernel<R, LIM>;
+  k.fn = stage2d_kernel<R, LIM, H>;
   k.ty = 1; k.np = 1; k.threads = 32 * NW2; k.smem = Stage2dSmem::BYTES;
   k.strips2d = true;
-  k.fused_dt = true;
+  k.fused_dt = !H;           // the fused reduction evaluates the ideal-MHD speed; Hall keeps the dt_kernel pass
   return k;
 }
 
@@ -128,13 +128,14 @@ StageKernel pick_stage(int ndim, int eqset, int riemann, int limiter) {
     if (riemann == AGATE_HLLD) return make_stage3d<TY3, 1, -1, AGATE_MINB3>();
     return make_stage3d<TY3, 0, -1, AGATE_MINB3>();
   }
-  if (ndim == 2 && eqset == AGATE_IDEAL && !getenv("AGATE_STAGE_V1")) {   // warp-autonomous strips
+  if (ndim == 2 && !getenv("AGATE_STAGE_V1")) {   // warp-autonomous strips
+    if (eqset == AGATE_HALL) return (limiter == 2) ? make_stage2d<0, 2, true>() : make_stage2d<0, -1, true>();
     if (limiter == 2) {
-      if (riemann == AGATE_HLLD) return make_stage2d<1, 2>();
-      return make_stage2d<0, 2>();
+      if (riemann == AGATE_HLLD) return make_stage2d<1, 2, false>();
+      return make_stage2d<0, 2, false>();
     }
-    if (riemann == AGATE_HLLD) return make_stage2d<1, -1>();
-    return make_stage2d<0, -1>();
+    if (riemann == AGATE_HLLD) return make_stage2d<1, -1, false>();
+    return make_stage2d<0, -1, false>();
   }
   if (eqset == AGATE_HALL) return make_stage<TY2, 1, 0, true, 2>();
   if (riemann == AGATE_HLLD) return make_stage<TY2, 1, 1, false, 2>();

@@ -1,4 +1,5 @@
-// agate_stage2d.cuh — warp-autonomous fused stage kernel for 2-D ideal-MHD grids, sm_100a.
+// agate_stage2d.cuh — warp-autonomous fused stage kernel for 2-D grids, ideal and Hall MHD,
+// sm_100a.
 //
 // Same arithmetic as the other two stage kernels; what differs is that a WARP, not a CTA, is the unit of work:
 //   * a warp owns a strip of 30 columns and marches along y.  Lanes 1..30 own the strip's cells of the current row,
@@ -12,7 +13,8 @@
 //   * conserved rows arrive by cp.async one step ahead in a private ring of 4 rows x 34 cells and are turned into
 //     primitives in place (A1); the raw Uin (+U0, copied straight into the same slot) of the own cell is kept for A6.
 //   * work = (strip, row) pairs in strip-major order, cut into equal ranges over all warps of a one-wave grid.
-//   * A7 of the next step rides in the last stage, as in stage3d_kernel.
+//   * A7 of the next step rides in the last stage, as in stage3d_kernel (ideal MHD; Hall keeps the dt_kernel pass).
+//   * Hall (A8): the face current comes from the cell-centred B of the three ring rows around the face.
 //
 // Shared memory per warp: ring 4 x 8 x 34, two y carries 8 x 32, raw U 2 x 8 x 32  =  16.5 KB;  6 warps per CTA,
 // 2 CTAs per SM (12 warps, <= 168 registers).
@@ -37,7 +39,7 @@ struct Stage2dSmem {
   static constexpr size_t BYTES = sizeof(double) * (size_t)PER_WARP * NW2;
 };
 
-template <int RIEMANN, int LIM>
+template <int RIEMANN, int LIM, bool HALL>
 __global__ void __launch_bounds__(32 * NW2, 2) stage2d_kernel(const __grid_constant__ StageParams P) {
   using SM = Stage2dSmem;
   extern __shared__ __align__(16) double smem[];
@@ -170,7 +172,18 @@ __global__ void __launch_bounds__(32 * NW2, 2) stage2d_kernel(const __grid_const
         R[r] = b - hs;
         WLy[v * 32 + lane] = b + hs;
       }
-      riemann_flux<RIEMANN, false>(P.ph, L, R, nullptr, F);
+      double Jr[3];
+      if (HALL) {
+        // A8 (R15): J = curl B at the y-face j-1/2 of column c from the cell-centred B of rows j-1 (sm) and j (sc)
+        const double* Bx = ring + 5 * RW2; const double* By = ring + 6 * RW2; const double* Bz = ring + 7 * RW2;
+        const int cL = sm + c, cR = sc + c;
+        const double dyBx = (Bx[cR] - Bx[cL]) * P.idy, dyBz = (Bz[cR] - Bz[cL]) * P.idy;
+        const double h = 0.25 * P.idx;
+        const double dxBy = ((By[cL + 1] - By[cL - 1]) + (By[cR + 1] - By[cR - 1])) * h;
+        const double dxBz = ((Bz[cL + 1] - Bz[cL - 1]) + (Bz[cR + 1] - Bz[cR - 1])) * h;
+        Jr[0] = -dxBz; Jr[1] = dxBy - dyBx; Jr[2] = dyBz;              // rotated for n = 1: (Jy, Jz, Jx)
+      }
+      riemann_flux<RIEMANN, HALL>(P.ph, L, R, HALL ? Jr : nullptr, F);
       {
         // A5 (y) + A6: row j-1 is complete; the accumulator of row j starts from the raw Uin (+U0)
         double* po = P.Uout + (long long)(j + 1) * P.sy + g_own;          // own cell of row j-1
@@ -203,7 +216,17 @@ __global__ void __launch_bounds__(32 * NW2, 2) stage2d_kernel(const __grid_const
           L[r] = b + hs;
           R[r] = __shfl_down_sync(0xffffffffu, b - hs, 1);
         }
-        riemann_flux<RIEMANN, false>(P.ph, L, R, nullptr, F);
+        if (HALL) {
+          // A8: J at the x-face between columns c and c+1 of row j; transverse differences from rows j-1, j+1
+          const double* Bx = ring + 5 * RW2; const double* By = ring + 6 * RW2; const double* Bz = ring + 7 * RW2;
+          const int cc1 = min(c + 1, RW2 - 1);                           // lane 31 has no right neighbour (its face is unused)
+          const double dxBy = (By[sc + cc1] - By[sc + c]) * P.idx, dxBz = (Bz[sc + cc1] - Bz[sc + c]) * P.idx;
+          const double h = 0.25 * P.idy;
+          const double dyBx = ((Bx[sp + c] - Bx[sm + c]) + (Bx[sp + cc1] - Bx[sm + cc1])) * h;
+          const double dyBz = ((Bz[sp + c] - Bz[sm + c]) + (Bz[sp + cc1] - Bz[sm + cc1])) * h;
+          Jr[0] = dyBz; Jr[1] = -dxBz; Jr[2] = dxBy - dyBx;              // rotated for n = 0: (Jx, Jy, Jz)
+        }
+        riemann_flux<RIEMANN, HALL>(P.ph, L, R, HALL ? Jr : nullptr, F);
 #pragma unroll
         for (int r = 0; r < 8; ++r) {
           const double fl = __shfl_up_sync(0xffffffffu, F[r], 1);
