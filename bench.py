@@ -225,7 +225,7 @@ def run_ours(args):
     roofline = {"bound": "alu", "achieved": achieved, "peak": fp64_peak, "unit": "TFLOP/s",
                 "frac": achieved / fp64_peak, "traffic": NCU_TRAFFIC_BYTES.get(cfg) if not args.n else None,
                 "algorithmic_bytes": BYTES_PER_ZONE_STEP / 2.0 * zones,
-                "kernel": "stage3d_kernel" if wl.ndim == 3 else "stage_kernel", "ms_per_launch": stage_ms, "launches_timed": st_n,
+                "kernel": {3: "stage3d_kernel", 2: "stage2d_kernel"}.get(wl.ndim, "stage_kernel"), "ms_per_launch": stage_ms, "launches_timed": st_n,
                 "stage_share_of_step": 2.0 * stage_ms * K / ms_max if st_n else None,
                 "peak_source": "FP64 DFMA micro-benchmark of this run (agate_measure_fp64_peak); nominal "
                                f"{FP64_NOMINAL_TFLOPS:.1f} = 148 SM x 64 lanes x 2 x 1.965 GHz",

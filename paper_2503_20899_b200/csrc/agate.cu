@@ -399,13 +399,13 @@ int agate_init(const agate_grid* grid, double gamma, int eqset, const agate_solv
   c->sgrid = dim3((grid->nx + TX - 1) / TX, (grid->ny + c->sk.ty - 1) / c->sk.ty,
                   (grid->ndim == 3) ? (grid->nz + c->lz - 1) / c->lz : 1);
   if (c->sk.strips2d) {
-    // one resident wave of 6-warp CTAs; a warp gets at least ~16 rows of its 30-column strip
+    // one resident wave of 6-warp CTAs; a warp gets at least ~4 rows of its 30-column strip
     int dev = 0, sms = 148;
     cudaGetDevice(&dev);
     cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
     const long long slots = (long long)sms * (c->occ > 0 ? c->occ : 1);
     const long long work = (long long)((grid->nx + SW2 - 1) / SW2) * grid->ny;
-    long long g = (work + 16 * NW2 - 1) / (16 * NW2);
+    long long g = (work + 4 * NW2 - 1) / (4 * NW2);
     if (g > slots) g = slots;
     if (g < 1) g = 1;
     if (const char* s = getenv("AGATE_GRID")) { int v = atoi(s); if (v > 0) g = v; }

@@ -12,7 +12,8 @@
 //     the accumulator in registers.
 //   * conserved rows arrive by cp.async one step ahead in a private ring of 4 rows x 34 cells and are turned into
 //     primitives in place (A1); the raw Uin (+U0, copied straight into the same slot) of the own cell is kept for A6.
-//   * work = (strip, row) pairs in strip-major order, cut into equal ranges over all warps of a one-wave grid.
+//   * work = (strip, row) pairs over the warps of a one-wave grid: every strip cut into the same row ranges,
+//     consecutive warps on consecutive strips (L2 serves the shared halo columns).
 //   * A7 of the next step rides in the last stage, as in stage3d_kernel (ideal MHD; Hall keeps the dt_kernel pass).
 //   * Hall (A8): the face current comes from the cell-centred B of the three ring rows around the face.
 //
@@ -61,8 +62,24 @@ __global__ void __launch_bounds__(32 * NW2, 2) stage2d_kernel(const __grid_const
   const int nstrip = (P.nx + SW2 - 1) / SW2;
   const long long wtot = (long long)nstrip * P.ny;
   const long long nwarp = (long long)gridDim.x * NW2, gw = (long long)blockIdx.x * NW2 + wid;
-  long long wpos = wtot * gw / nwarp;
-  const long long wend = wtot * (gw + 1) / nwarp;
+  // Work = (strip, row) pairs, strip-major.  With at least one warp per strip, every strip is cut into the SAME
+  // nchunk row ranges and consecutive warps take consecutive strips of one range: neighbouring strips advance side
+  // by side and the halo columns they share are served by L2 (a few warps of the wave stay idle: nwarp mod nstrip).
+  // Otherwise (more strips than warps) the pairs are cut into equal ranges and a warp walks its range as segments.
+  long long wpos, wend;
+  if (nwarp >= nstrip) {
+    const int nchunk = (int)min(nwarp / nstrip, (long long)P.ny);
+    const int chunk = (int)(gw / nstrip), strip = (int)(gw - (long long)chunk * nstrip);
+    if (chunk < nchunk) {
+      wpos = (long long)strip * P.ny + (long long)P.ny * chunk / nchunk;
+      wend = (long long)strip * P.ny + (long long)P.ny * (chunk + 1) / nchunk;
+    } else {
+      wpos = wend = 0;
+    }
+  } else {
+    wpos = wtot * gw / nwarp;
+    wend = wtot * (gw + 1) / nwarp;
+  }
 
   auto slot_of = [](int r) { return ((r + 4) & 3) * (8 * RW2); };      // r >= -4
   auto conv = [&](int off) {                                            // A1 in place; returns nothing

@@ -117,12 +117,24 @@ def test_config1_full(ag):
     assert_parity(*run_pair(ag, wl, wl.n_steps))
 
 
-@pytest.mark.parametrize("n,steps", [(100, 12), (256, 4)])
-def test_config2_reduced(ag, n, steps):
-    """Config 2 recipe (2D HLLD, beta=1.3, shear layer).  n=100: 3 full x-tiles + a 4-wide ragged one, 16 full
-    y-tiles of 6 + ragged 4."""
+@pytest.mark.parametrize("n,steps,grid", [(100, 12, 0), (256, 4, 0), (100, 4, 1), (100, 4, 5), (100, 4, 40)])
+def test_config2_reduced(ag, n, steps, grid, monkeypatch):
+    """Config 2 recipe (2D HLLD, beta=1.3, shear layer) through the strip kernel.  n=100: 3 full 30-column strips + a
+    ragged one of 10.  `grid` CTAs of 6 warps share the (strip, row) pairs evenly: 1 = 16-17 rows per warp, segments
+    that cross from one strip into the next; 5 / 40 = ever shorter segments (40: one or two rows each, every row
+    through the segment prologue and the closing step); 0 = the library's own choice."""
+    if grid:
+        monkeypatch.setenv("AGATE_GRID", str(grid))
     wl = make_workload(2, n=n)
     assert_parity(*run_pair(ag, wl, steps))
+
+
+@pytest.mark.parametrize("cfg", [2, 4])
+def test_config2_4_reduced_pooled_kernel(ag, cfg, monkeypatch):
+    """The pooled kernel of agate_kernels.cuh (1-D grids; 2-D kept for A/B measurements) on the 2-D recipes."""
+    monkeypatch.setenv("AGATE_STAGE_V1", "1")
+    wl = make_workload(cfg, n=100)
+    assert_parity(*run_pair(ag, wl, 4))
 
 
 @pytest.mark.parametrize("n,grid", [(40, 0), (40, 1), (40, 7), (40, 37), (40, 160), (72, 0)])
