@@ -42,7 +42,8 @@ FLOP_DT_PER_ZONE = {1: 45.0, 2: 45.0, 3: 45.0, 4: 60.0, 5: 45.0}
 BYTES_PER_ZONE_STEP = 320.0            # 5 x 8 variables x 8 B
 # DRAM bytes per launch of the dominant kernel (dram__bytes_read.sum + dram__bytes_write.sum, mean of the two stage
 # launches of one step) from the committed `ncu` capture of the same command: profiles/r1_stage3d.md
-NCU_TRAFFIC_BYTES = {5: 0.5 * (9372441088 + 8649890048 + 17961833984 + 8646440704)}
+NCU_TRAFFIC_BYTES = {5: 0.5 * (9617129216 + 8682435584 + 18299382528 + 8663042304),
+                     2: 0.5 * (285912064 + 227066880 + 561840896 + 226612736)}
 FP64_NOMINAL_TFLOPS = 148 * 64 * 2 * 1.965e9 / 1e12     # 148 SMs x 64 DFMA lanes x 2 x max SM clock = 37.2
 
 # reduced size of the bounded CPU sample per config (same recipe and seed), and its step count
