@@ -89,9 +89,8 @@ AG_HD double rcp(double x) {
 #if defined(__CUDA_ARCH__)
   double y;
   asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(y) : "d"(x));
-  const double e = fma(-x, y, 1.0);               // 1 - x y          (~2^-22)
-  const double y1 = fma(y, e, y);                 // 1 - x y1 = e^2 exactly, so the second step needs no new residual
-  return fma(y1, e * e, y1);
+  const double e = fma(-x, y, 1.0);               // 1 - x y          (~2^-21)
+  return fma(y, fma(e, e, e), y);                 // third-order step  y (1 + e + e^2);  the e^3 term is below 2^-60
 #else
   return 1.0 / x;
 #endif
