@@ -21,6 +21,7 @@ _HDR = os.path.join(_HERE, "agate_ref.h")
 _LIB = os.path.join(_HERE, "libagate_ref.so")
 
 IDEAL, HALL = 0, 1
+IDEAL_GLM = 3        # ideal MHD + GLM divergence cleaning: 9 variables per cell, psi last (eqs.10-11; R22)
 HLL, HLLD = 0, 1
 
 
@@ -65,6 +66,11 @@ def lib():
         L.agate_ref_get_state.argtypes = [vp, _dp, _dp]
         L.agate_ref_rhs.argtypes = [vp, _dp]
         L.agate_ref_destroy.argtypes = [vp]
+        L.agate_ref_nvar.argtypes = [vp]
+        L.agate_ref_nvar.restype = C.c_int
+        L.agate_ref_glm_ch.argtypes = [vp, _dp]
+        L.agate_ref_glm_face.argtypes = [C.c_double] * 5 + [_dp, _dp]
+        L.agate_ref_glm_face.restype = None
         L.agate_ref_set_threads.argtypes = [C.c_int]
         L.agate_ref_get_threads.restype = C.c_int
         L.agate_ref_cons_to_prim.argtypes = [C.c_double, _dp, _dp]
@@ -145,6 +151,13 @@ def face_flux(riemann, d, gamma, WL, WR, eqset=IDEAL, d_i=0.0, dxmin=1.0, J=None
     return F
 
 
+def glm_face(ch, bnL, bnR, psL, psR):
+    """(B_n*, psi*) of the 2x2 linear GLM Riemann problem at one face."""
+    a, b = C.c_double(), C.c_double()
+    lib().agate_ref_glm_face(float(ch), float(bnL), float(bnR), float(psL), float(psR), C.byref(a), C.byref(b))
+    return a.value, b.value
+
+
 def hlld_branch(d, gamma, WL, WR):
     wl, pl = _vec(WL); wr, pr = _vec(WR)
     return int(lib().agate_ref_hlld_branch(int(d), float(gamma), pl, pr))
@@ -171,6 +184,7 @@ class RefSolver:
         rc = lib().agate_ref_create(C.byref(self.grid), self.gamma, self.eqset, C.byref(self.cfg), C.byref(self._h))
         if rc:
             raise RefError(rc, "create")
+        self.nvar = int(lib().agate_ref_nvar(self._h))
 
     @classmethod
     def from_workload(cls, wl, **over):
@@ -188,13 +202,18 @@ class RefSolver:
     def set_state(self, U, t0=0.0):
         nx, ny, nz = self.shape
         U = np.ascontiguousarray(U, dtype=np.float64)
-        assert U.size == 8 * nx * ny * nz
+        assert U.size == self.nvar * nx * ny * nz
         self._chk(lib().agate_ref_set_state(self._h, U.ctypes.data_as(_dp), float(t0)), "set_state")
 
     def compute_dt(self):
         dt = C.c_double()
         self._chk(lib().agate_ref_compute_dt(self._h, C.byref(dt)), "compute_dt")
         return dt.value
+
+    def glm_ch(self):
+        v = C.c_double()
+        self._chk(lib().agate_ref_glm_ch(self._h, C.byref(v)), "glm_ch")
+        return v.value
 
     def vmax(self):
         v = C.c_double()
@@ -213,7 +232,7 @@ class RefSolver:
 
     def get_state(self):
         nx, ny, nz = self.shape
-        U = np.empty((8, nz, ny, nx))
+        U = np.empty((self.nvar, nz, ny, nx))
         t = C.c_double()
         self._chk(lib().agate_ref_get_state(self._h, U.ctypes.data_as(_dp), C.byref(t)), "get_state")
         self.t = t.value
@@ -221,7 +240,7 @@ class RefSolver:
 
     def rhs(self):
         nx, ny, nz = self.shape
-        Lo = np.empty((8, nz, ny, nx))
+        Lo = np.empty((self.nvar, nz, ny, nx))
         self._chk(lib().agate_ref_rhs(self._h, Lo.ctypes.data_as(_dp)), "rhs")
         return Lo
 

@@ -271,6 +271,16 @@ int flux_hlld(int n, double gamma, const T WLin[8], const T WRin[8], T F[8]) {
   return 3 + degenerate;
 }
 
+// GLM (eqs.10-11; R22).  Along the face normal, (B_n, psi) obey  dB_n/dt + dpsi/dx = 0,
+// dpsi/dt + c_h^2 dB_n/dx = 0: characteristic variables B_n -+ psi/c_h move at -+c_h, and the state
+// on the face (x/t = 0) is
+//   B_n* = (B_nL + B_nR)/2 - (psi_R - psi_L)/(2 c_h),   psi* = (psi_L + psi_R)/2 - c_h (B_nR - B_nL)/2.
+template <class T>
+void glm_face(double ch, T bnL, T bnR, T psL, T psR, T* bns, T* pss) {
+  *bns = T(0.5) * (bnL + bnR) - T(0.5) * (psR - psL) / T(ch);
+  *pss = T(0.5) * (psL + psR) - T(0.5) * T(ch) * (bnR - bnL);
+}
+
 template <class T>
 void face_flux(int eqset, int riemann, int n, double gamma, double d_i, double dxmin,
                const T WL[8], const T WR[8], const T* J, T F[8]) {
@@ -293,6 +303,9 @@ template <class T> struct Solver {
   size_t ntot, nint;    // padded / interior cell counts
   double h[3];          // spacings
   double dxmin, cfl;
+  int nv;               // variables per cell: 8, or 9 with the GLM scalar psi (index 8) behind the MHD ones
+  bool glm;
+  double ch = 0.0;      // GLM: c_h of the step being taken (R22: 0.95 v_max(U^n))
   std::vector<T> Un, U1, W, L;
   double t = 0.0;
   bool have_state = false;
@@ -309,8 +322,10 @@ template <class T> struct Solver {
     for (int d = 1; d < g.ndim; ++d) dxmin = std::fmin(dxmin, h[d]);
     cfl = s.cfl;
     if (!(cfl > 0.0)) cfl = (g.ndim == 1) ? 0.8 : (g.ndim == 2 ? 0.45 : 0.325);
-    Un.assign(8 * ntot, T(0.0)); U1.assign(8 * ntot, T(0.0)); W.assign(8 * ntot, T(0.0));
-    L.assign(8 * nint, T(0.0));
+    glm = (eqset == AGATE_REF_IDEAL_GLM);
+    nv = glm ? 9 : 8;
+    Un.assign(nv * ntot, T(0.0)); U1.assign(nv * ntot, T(0.0)); W.assign(nv * ntot, T(0.0));
+    L.assign(nv * nint, T(0.0));
   }
   inline ptrdiff_t pidx(int i, int j, int k) const {
     return (ptrdiff_t)(i + gh[0]) + st[1] * (j + gh[1]) + st[2] * (k + gh[2]);
@@ -319,7 +334,7 @@ template <class T> struct Solver {
 
   // A0 (R13): every ghost cell (faces, edges, corners) = interior cell at the index wrapped mod n.
   void fill_ghosts(std::vector<T>& U) const {
-    for (int q = 0; q < 8; ++q)
+    for (int q = 0; q < nv; ++q)
 #pragma omp parallel for num_threads(g_threads) if (g_threads > 1)
       for (int k = -gh[2]; k < nd[2] + gh[2]; ++k)
         for (int j = -gh[1]; j < nd[1] + gh[1]; ++j)
@@ -337,6 +352,7 @@ template <class T> struct Solver {
       for (int q = 0; q < 8; ++q) u[q] = U[q * ntot + c];
       cons_to_prim(gamma, u, w);
       for (int q = 0; q < 8; ++q) W[q * ntot + c] = w[q];
+      if (glm) W[8 * ntot + c] = U[8 * ntot + c];                 // psi is its own primitive
     }
   }
 
@@ -367,29 +383,41 @@ template <class T> struct Solver {
       for (int a1 = 0; a1 < nd[d1]; ++a1) {
         int ijk[3]; ijk[d] = 0; ijk[d1] = a1; ijk[d2] = a2;
         const ptrdiff_t base = pidx(ijk[0], ijk[1], ijk[2]);           // cell 0 of this line
-        std::vector<T> dW(8 * (n + 2)), F(8 * (n + 1));
+        std::vector<T> dW(nv * (n + 2)), F(nv * (n + 1));
         for (int c = -1; c <= n; ++c)                                    // A2: slopes of cells -1..n
-          for (int q = 0; q < 8; ++q) {
+          for (int q = 0; q < nv; ++q) {
             const T* Wq = &W[q * ntot + base];
             T dp = Wq[(c + 1) * sd] - Wq[c * sd];
             T dm = Wq[c * sd] - Wq[(c - 1) * sd];
             dW[q * (n + 2) + (c + 1)] = slope<T>(s.limiter, s.beta, dp, dm);
           }
         for (int c = -1; c < n; ++c) {                                   // face c+1/2, between cells c and c+1
-          T WL[8], WR[8], Ff[8], J[3];
-          for (int q = 0; q < 8; ++q) {
+          T WL[9], WR[9], Ff[9], J[3];
+          for (int q = 0; q < nv; ++q) {
             const T* Wq = &W[q * ntot + base];
             WL[q] = Wq[c * sd] + T(0.5) * dW[q * (n + 2) + (c + 1)];             // eq.2
             WR[q] = Wq[(c + 1) * sd] - T(0.5) * dW[q * (n + 2) + (c + 2)];       // eq.3
           }
           if (hall) face_current(d, base + c * sd, J);
-          face_flux<T>(eqset, s.riemann, d, gamma, s.d_i, dxmin, WL, WR, hall ? J : nullptr, Ff);
-          for (int q = 0; q < 8; ++q) F[q * (n + 1) + (c + 1)] = Ff[q];
+          if (glm) {
+            // eqs.10-11 (R22): (B_n, psi) decouple into a 2x2 linear system with speeds -+c_h; its Riemann
+            // solution gives the single-valued face values, the MHD solver sees B_n* on both sides, and the two
+            // GLM fluxes are  F[B_n] = psi*,  F[psi] = c_h^2 B_n*.
+            T bns, pss;
+            glm_face<T>(ch, WL[5 + d], WR[5 + d], WL[8], WR[8], &bns, &pss);
+            WL[5 + d] = bns; WR[5 + d] = bns;
+            face_flux<T>(AGATE_REF_IDEAL, s.riemann, d, gamma, s.d_i, dxmin, WL, WR, nullptr, Ff);
+            Ff[5 + d] = pss;
+            Ff[8] = T(ch) * T(ch) * bns;
+          } else {
+            face_flux<T>(eqset, s.riemann, d, gamma, s.d_i, dxmin, WL, WR, hall ? J : nullptr, Ff);
+          }
+          for (int q = 0; q < nv; ++q) F[q * (n + 1) + (c + 1)] = Ff[q];
         }
         for (int c = 0; c < n; ++c) {                                    // A5
           ijk[d] = c;
           const size_t ii = iidx(ijk[0], ijk[1], ijk[2]);
-          for (int q = 0; q < 8; ++q)
+          for (int q = 0; q < nv; ++q)
             L[q * nint + ii] -= (F[q * (n + 1) + (c + 1)] - F[q * (n + 1) + c]) / T(h[d]);
         }
       }
@@ -432,37 +460,49 @@ template <class T> struct Solver {
   }
 
   // R11: SSP-RK2 (Heun / Shu-Osher form), dt fixed for both stages; RK11 = forward Euler.
+  // GLM (R22): c_h = 0.95 v_max(U^n) for the whole step, whoever chose dt; after the Runge-Kutta update
+  // psi <- psi exp(-dt c_h^2 / c_p^2) with c_p^2 = 0.18 c_h, the exact solution of eq.11's source.
+  void glm_source(double dt) {
+    const T decay = T(std::exp(-dt * ch / 0.18));
+    for (int k = 0; k < nd[2]; ++k) for (int j = 0; j < nd[1]; ++j) for (int i = 0; i < nd[0]; ++i) {
+      const size_t p = 8 * ntot + pidx(i, j, k);
+      Un[p] = Un[p] * decay;
+    }
+  }
   void step(double dt) {
+    if (glm) { double vm = 0.0; vmax(&vm); ch = 0.95 * vm; }
     fill_ghosts(Un);
     rhs(Un);
     if (s.rk == 1) {
-      for (int q = 0; q < 8; ++q) for (int k = 0; k < nd[2]; ++k) for (int j = 0; j < nd[1]; ++j) for (int i = 0; i < nd[0]; ++i) {
+      for (int q = 0; q < nv; ++q) for (int k = 0; k < nd[2]; ++k) for (int j = 0; j < nd[1]; ++j) for (int i = 0; i < nd[0]; ++i) {
         const size_t p = q * ntot + pidx(i, j, k);
         Un[p] = Un[p] + T(dt) * L[q * nint + iidx(i, j, k)];
       }
+      if (glm) glm_source(dt);
       t += dt;
       return;
     }
-    for (int q = 0; q < 8; ++q) for (int k = 0; k < nd[2]; ++k) for (int j = 0; j < nd[1]; ++j) for (int i = 0; i < nd[0]; ++i) {
+    for (int q = 0; q < nv; ++q) for (int k = 0; k < nd[2]; ++k) for (int j = 0; j < nd[1]; ++j) for (int i = 0; i < nd[0]; ++i) {
       const size_t p = q * ntot + pidx(i, j, k);
       U1[p] = Un[p] + T(dt) * L[q * nint + iidx(i, j, k)];                         // stage 1
     }
     fill_ghosts(U1);
     rhs(U1);
-    for (int q = 0; q < 8; ++q) for (int k = 0; k < nd[2]; ++k) for (int j = 0; j < nd[1]; ++j) for (int i = 0; i < nd[0]; ++i) {
+    for (int q = 0; q < nv; ++q) for (int k = 0; k < nd[2]; ++k) for (int j = 0; j < nd[1]; ++j) for (int i = 0; i < nd[0]; ++i) {
       const size_t p = q * ntot + pidx(i, j, k);
       Un[p] = T(0.5) * Un[p] + T(0.5) * (U1[p] + T(dt) * L[q * nint + iidx(i, j, k)]);   // stage 2
     }
+    if (glm) glm_source(dt);
     t += dt;
   }
 
   void set_state(const double* U, double t0) {
-    for (int q = 0; q < 8; ++q) for (int k = 0; k < nd[2]; ++k) for (int j = 0; j < nd[1]; ++j) for (int i = 0; i < nd[0]; ++i)
+    for (int q = 0; q < nv; ++q) for (int k = 0; k < nd[2]; ++k) for (int j = 0; j < nd[1]; ++j) for (int i = 0; i < nd[0]; ++i)
       Un[q * ntot + pidx(i, j, k)] = T(U[q * nint + iidx(i, j, k)]);
     t = t0; have_state = true;
   }
   void get_state(double* U) const {
-    for (int q = 0; q < 8; ++q) for (int k = 0; k < nd[2]; ++k) for (int j = 0; j < nd[1]; ++j) for (int i = 0; i < nd[0]; ++i)
+    for (int q = 0; q < nv; ++q) for (int k = 0; k < nd[2]; ++k) for (int j = 0; j < nd[1]; ++j) for (int i = 0; i < nd[0]; ++i)
       U[q * nint + iidx(i, j, k)] = val(Un[q * ntot + pidx(i, j, k)]);
   }
 };
@@ -475,7 +515,7 @@ int check_args(const agate_ref_grid* g, double gamma, int eqset, const agate_ref
   if (g->ndim < 2 && g->ny != 1) return 1;
   if (!(g->dx > 0.0) || (g->ndim >= 2 && !(g->dy > 0.0)) || (g->ndim >= 3 && !(g->dz > 0.0))) return 1;
   if (!(gamma > 1.0)) return 1;
-  if (eqset != AGATE_REF_IDEAL && eqset != AGATE_REF_HALL) return 1;
+  if (eqset != AGATE_REF_IDEAL && eqset != AGATE_REF_HALL && eqset != AGATE_REF_IDEAL_GLM) return 1;
   if (s->riemann < 0 || s->riemann > 1 || s->limiter < 0 || s->limiter > 2 || s->rk < 1 || s->rk > 2) return 1;
   if (s->limiter == 2 && !(s->beta >= 1.0 && s->beta <= 2.0)) return 1;
   if (eqset == AGATE_REF_HALL && s->riemann == 1) return 1;        // no Hall-HLLD in the paper
@@ -557,10 +597,20 @@ int agate_ref_get_state(agate_ref_ctx* c, double* U, double* t_out) {
 int agate_ref_rhs(agate_ref_ctx* c, double* Lout) {
   if (!c || !Lout) return 1;
   if (!c->s->have_state) return 2;
+  if (c->s->glm) { double vm = 0.0; c->s->vmax(&vm); c->s->ch = 0.95 * vm; }
   c->s->fill_ghosts(c->s->Un);
   c->s->rhs(c->s->Un);
-  std::memcpy(Lout, c->s->L.data(), sizeof(double) * 8 * c->s->nint);
+  std::memcpy(Lout, c->s->L.data(), sizeof(double) * c->s->nv * c->s->nint);
   return 0;
+}
+int agate_ref_nvar(agate_ref_ctx* c) { return c ? c->s->nv : 0; }
+int agate_ref_glm_ch(agate_ref_ctx* c, double* ch_out) {
+  if (!c || !ch_out) return 1;
+  *ch_out = c->s->ch;
+  return 0;
+}
+void agate_ref_glm_face(double ch, double bnL, double bnR, double psL, double psR, double* bns, double* pss) {
+  glm_face<double>(ch, bnL, bnR, psL, psR, bns, pss);
 }
 int agate_ref_destroy(agate_ref_ctx* c) {
   if (!c) return 1;

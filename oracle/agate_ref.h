@@ -36,7 +36,10 @@ typedef struct {
   double  d_i;           /* normalised ion inertial length (Hall) */
 } agate_ref_solver;
 
-enum { AGATE_REF_IDEAL = 0, AGATE_REF_HALL = 1 };
+enum { AGATE_REF_IDEAL = 0, AGATE_REF_HALL = 1, AGATE_REF_IDEAL_GLM = 3 };
+/* AGATE_REF_IDEAL_GLM (eqs.10-11; R22): 9 variables per cell, the GLM scalar psi
+ * last: U[9][nz][ny][nx].  c_h = 0.95 v_max(U^n) per step, c_p^2 = 0.18 c_h; face (B_n, psi) from the 2x2
+ * linear Riemann problem; psi <- psi exp(-dt c_h^2/c_p^2) after the Runge-Kutta update. */
 
 /* ---- the stepping interface (mirrors the product's C-ABI on host memory) ---- */
 int agate_ref_create(const agate_ref_grid*, double gamma, int eqset, const agate_ref_solver*, agate_ref_ctx** out);
@@ -47,6 +50,9 @@ int agate_ref_advance(agate_ref_ctx*, int32_t n_steps, double* t_out);    /* n s
 int agate_ref_get_state(agate_ref_ctx*, double* U_out, double* t_out);
 int agate_ref_rhs(agate_ref_ctx*, double* L_out);                         /* L(U) of eq.1, interior SoA */
 int agate_ref_vmax(agate_ref_ctx*, double* vmax_out);                     /* max_i(|v_i|+c_i) (L156)    */
+int agate_ref_nvar(agate_ref_ctx*);                                       /* 8, or 9 with GLM          */
+int agate_ref_glm_ch(agate_ref_ctx*, double* ch_out);                     /* c_h of the last step / rhs */
+void agate_ref_glm_face(double ch, double bnL, double bnR, double psL, double psR, double* bn_star, double* psi_star);
 int agate_ref_destroy(agate_ref_ctx*);
 void agate_ref_set_threads(int n);      /* OpenMP build only: 0/1 = serial; results are bitwise identical */
 int  agate_ref_get_threads(void);
