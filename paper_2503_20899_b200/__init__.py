@@ -22,6 +22,7 @@ import numpy as np
 from . import build as _build
 
 IDEAL, HALL = 0, 1
+IDEAL_GLM = 3        # 9 variables per cell (psi last); see include/agate.h
 HLL, HLLD = 0, 1
 OK, ERR_ARG, ERR_STATE, ERR_UNPHYSICAL, ERR_CUDA, ERR_NOMEM = range(6)
 
@@ -102,6 +103,7 @@ class Agate:
         nx, ny, nz = (int(s) for s in shape)
         self.shape = (nx, ny, nz)
         self.zones = nx * ny * nz
+        self.nvar = 9 if int(eqset) == IDEAL_GLM else 8
         self.grid = Grid(ndim, nx, ny, nz, dx[0], dx[1], dx[2])
         self.cfg = SolverCfg(riemann, limiter, beta, rk, cfl, d_i)
         self.device = torch.device(device)
@@ -138,7 +140,7 @@ class Agate:
     def set_state(self, U, t0=0.0):
         """U: numpy array / CPU torch tensor (host path) or CUDA torch tensor (device path), [8,nz,ny,nx] f64."""
         torch = _torch_cuda()
-        n = 8 * self.zones
+        n = self.nvar * self.zones
         if isinstance(U, torch.Tensor):
             assert U.dtype == torch.float64 and U.numel() == n and U.is_contiguous()
             self._keep = U
@@ -156,13 +158,13 @@ class Agate:
         torch = _torch_cuda()
         nx, ny, nz = self.shape
         if out is None:
-            out = np.empty((8, nz, ny, nx))
+            out = np.empty((self.nvar, nz, ny, nx))
         t = C.c_double()
         if isinstance(out, torch.Tensor):
-            assert out.dtype == torch.float64 and out.numel() == 8 * self.zones and out.is_contiguous()
+            assert out.dtype == torch.float64 and out.numel() == self.nvar * self.zones and out.is_contiguous()
             ptr, on_dev = out.data_ptr(), out.is_cuda
         else:
-            assert out.dtype == np.float64 and out.size == 8 * self.zones and out.flags.c_contiguous
+            assert out.dtype == np.float64 and out.size == self.nvar * self.zones and out.flags.c_contiguous
             ptr, on_dev = out.ctypes.data, False
         with torch.cuda.device(self.device):
             self._chk(lib().agate_get_state(self._h, _vp(ptr), int(on_dev), C.byref(t)), "agate_get_state")

@@ -39,7 +39,7 @@ struct Layout {
   size_t off_A, off_B, off_scal, off_partial, total;
 };
 
-Layout make_layout(const agate_grid& g) {
+Layout make_layout(const agate_grid& g, int nv) {
   Layout L;
   L.ghy = (g.ndim >= 2) ? 2 : 0;
   L.ghz = (g.ndim >= 3) ? 2 : 0;
@@ -50,7 +50,7 @@ Layout make_layout(const agate_grid& g) {
   L.sz = (long long)L.nxp * L.nyp;
   L.sq = L.sz * L.nzp;
   L.sq = (long long)align_up((size_t)L.sq, 32);          // every variable starts 256-byte aligned
-  L.state_bytes = sizeof(double) * 8 * (size_t)L.sq;
+  L.state_bytes = sizeof(double) * (size_t)nv * (size_t)L.sq;
   L.off_A = 0;
   L.off_B = align_up(L.off_A + L.state_bytes, 256);
   L.off_scal = align_up(L.off_B + L.state_bytes, 256);
@@ -67,7 +67,8 @@ int check_args(const agate_grid* g, double gamma, int eqset, const agate_solver*
   if (g->ndim < 2 && g->ny != 1) return AGATE_ERR_ARG;
   if (!(g->dx > 0.0) || (g->ndim >= 2 && !(g->dy > 0.0)) || (g->ndim >= 3 && !(g->dz > 0.0))) return AGATE_ERR_ARG;
   if (!(gamma > 1.0)) return AGATE_ERR_ARG;
-  if (eqset != AGATE_IDEAL && eqset != AGATE_HALL) return AGATE_ERR_ARG;
+  if (eqset != AGATE_IDEAL && eqset != AGATE_HALL && eqset != AGATE_IDEAL_GLM) return AGATE_ERR_ARG;
+  if (eqset == AGATE_IDEAL_GLM && g->ndim != 2) return AGATE_ERR_ARG;            // GLM: 2-D strip kernel only so far
   if (s->riemann < 0 || s->riemann > 1 || s->limiter < 0 || s->limiter > 2 || s->rk < 1 || s->rk > 2) return AGATE_ERR_ARG;
   if (s->limiter == 2 && !(s->beta >= 1.0 && s->beta <= 2.0)) return AGATE_ERR_ARG;
   if (eqset == AGATE_HALL && s->riemann == AGATE_HLLD) return AGATE_ERR_ARG;   // no Hall-HLLD in the paper
@@ -85,6 +86,7 @@ struct StageKernel {
   bool even_split = false;   // stage3d_kernel: one-wave grid, work split evenly (see agate_stage3d.cuh)
   bool fused_dt = false;     // stage3d / stage2d kernels: A7 of the next step inside the last stage of this one
   bool strips2d = false;     // stage2d_kernel: one-wave grid of autonomous warps (see agate_stage2d.cuh)
+  int warps2d = 0;           // ... warps per CTA
 };
 
 template <int TY, int NP, int R, bool H, int MINB>
@@ -105,11 +107,12 @@ StageKernel make_stage3d() {
   return k;
 }
 
-template <int R, int LIM, bool H>
+template <int R, int LIM, bool H, bool GLM = false>
 StageKernel make_stage2d() {
   StageKernel k;
-  k.fn = stage2d_kernel<R, LIM, H>;
-  k.ty = 1; k.np = 1; k.threads = 32 * NW2; k.smem = Stage2dSmem::BYTES;
+  k.fn = stage2d_kernel<R, LIM, H, GLM>;
+  k.ty = 1; k.np = 1; k.threads = 32 * Stage2dSmem<GLM>::NW; k.smem = Stage2dSmem<GLM>::BYTES;
+  k.warps2d = Stage2dSmem<GLM>::NW;
   k.strips2d = true;
   k.fused_dt = !H;           // the fused reduction evaluates the ideal-MHD speed; Hall keeps the dt_kernel pass
   return k;
@@ -130,6 +133,10 @@ StageKernel pick_stage(int ndim, int eqset, int riemann, int limiter) {
   }
   if (ndim == 2 && !getenv("AGATE_STAGE_V1")) {   // warp-autonomous strips
     if (eqset == AGATE_HALL) return (limiter == 2) ? make_stage2d<0, 2, true>() : make_stage2d<0, -1, true>();
+    if (eqset == AGATE_IDEAL_GLM) {
+      if (riemann == AGATE_HLLD) return (limiter == 2) ? make_stage2d<1, 2, false, true>() : make_stage2d<1, -1, false, true>();
+      return (limiter == 2) ? make_stage2d<0, 2, false, true>() : make_stage2d<0, -1, false, true>();
+    }
     if (limiter == 2) {
       if (riemann == AGATE_HLLD) return make_stage2d<1, 2, false>();
       return make_stage2d<0, 2, false>();
@@ -149,6 +156,7 @@ struct agate_ctx {
   agate_solver s;
   double gamma;
   int eqset;
+  int nv;                          // variables per cell: 8, or 9 with the GLM scalar
   Layout L;
   Phys ph;
   double dxmin, cfl;
@@ -190,6 +198,7 @@ GhostParams make_ghost(const agate_ctx* c, double* U) {
   GhostParams p;
   const Layout& L = c->L;
   p.U = U;
+  p.nv = c->nv;
   p.nx = c->g.nx; p.ny = c->g.ny; p.nz = c->g.nz;
   p.ghy = L.ghy; p.ghz = L.ghz; p.nxp = L.nxp; p.nyp = L.nyp; p.nzp = L.nzp;
   p.sy = L.sy; p.sz = L.sz; p.sq = L.sq;
@@ -214,6 +223,8 @@ StageParams make_stage_params(const agate_ctx* c, const double* Uin, const doubl
   p.limiter = c->s.limiter; p.beta = c->s.beta;
   p.vnext = (last_stage && c->sk.fused_dt) ? c->vnext : nullptr;
   p.flag = c->flag;
+  p.ch_ptr = c->scal + 3;
+  p.last_stage = last_stage ? 1 : 0;
   p.lz = c->lz;
   p.ntx = (c->g.nx + TX - 1) / TX;
   p.nty = (c->g.ny + c->sk.ty - 1) / c->sk.ty;
@@ -309,7 +320,7 @@ int collect_status(agate_ctx* c) {
 
 int copy_state(agate_ctx* c, double* padded, double* ext, bool to_device, bool ext_is_device) {
   const Layout& L = c->L;
-  for (int q = 0; q < 8; ++q) {
+  for (int q = 0; q < c->nv; ++q) {
     cudaMemcpy3DParms m;
     memset(&m, 0, sizeof(m));
     cudaPitchedPtr pp = make_cudaPitchedPtr(padded + (size_t)q * L.sq, sizeof(double) * L.nxp, L.nxp, L.nyp);
@@ -332,7 +343,7 @@ extern "C" {
 
 size_t agate_workspace_bytes(const agate_grid* grid, int eqset, const agate_solver* solver) {
   if (check_args(grid, 5.0 / 3.0, eqset, solver) != AGATE_OK) return 0;
-  return make_layout(*grid).total;
+  return make_layout(*grid, eqset == AGATE_IDEAL_GLM ? 9 : 8).total;
 }
 
 int agate_init(const agate_grid* grid, double gamma, int eqset, const agate_solver* solver, void* workspace,
@@ -341,14 +352,15 @@ int agate_init(const agate_grid* grid, double gamma, int eqset, const agate_solv
   int rc = check_args(grid, gamma, eqset, solver);
   if (rc) return rc;
   if (!workspace) return AGATE_ERR_ARG;
-  Layout L = make_layout(*grid);
+  const int nv = (eqset == AGATE_IDEAL_GLM) ? 9 : 8;
+  Layout L = make_layout(*grid, nv);
   if (workspace_bytes < L.total || ((uintptr_t)workspace & 255u)) return AGATE_ERR_NOMEM;
   int ndev = 0;
   if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev < 1) return AGATE_ERR_CUDA;   // no CPU fallback
 
   agate_ctx* c = new (std::nothrow) agate_ctx;
   if (!c) return AGATE_ERR_NOMEM;
-  c->g = *grid; c->s = *solver; c->gamma = gamma; c->eqset = eqset; c->L = L;
+  c->g = *grid; c->s = *solver; c->gamma = gamma; c->eqset = eqset; c->L = L; c->nv = nv;
   c->dxmin = grid->dx;
   if (grid->ndim >= 2) c->dxmin = fmin(c->dxmin, grid->dy);      // R5: min over ACTIVE dimensions
   if (grid->ndim >= 3) c->dxmin = fmin(c->dxmin, grid->dz);
@@ -405,7 +417,7 @@ int agate_init(const agate_grid* grid, double gamma, int eqset, const agate_solv
     cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
     const long long slots = (long long)sms * (c->occ > 0 ? c->occ : 1);
     const long long work = (long long)((grid->nx + SW2 - 1) / SW2) * grid->ny;
-    long long g = (work + 4 * NW2 - 1) / (4 * NW2);
+    long long g = (work + 4 * c->sk.warps2d - 1) / (4 * c->sk.warps2d);
     if (g > slots) g = slots;
     if (g < 1) g = 1;
     if (const char* s = getenv("AGATE_GRID")) { int v = atoi(s); if (v > 0) g = v; }
@@ -471,6 +483,7 @@ int agate_step(agate_ctx* c, double dt, double* dt_used) {
   if (!c->have_state) return AGATE_ERR_STATE;
   int rc;
   if (dt > 0.0) {
+    if (c->eqset == AGATE_IDEAL_GLM && (rc = ensure_vmax(c))) return rc;      // c_h = 0.95 v_max(U^n) whoever chose dt
     set_dt_kernel<<<1, 1, 0, c->stream>>>(c->scal, dt, c->sk.fused_dt ? c->vnext : nullptr);
     CU_TRY(cudaGetLastError());
   } else {

@@ -45,6 +45,8 @@ struct StageParams {
   // unphysical-state flag.  nullptr: not this stage.
   unsigned long long* vnext;
   int* flag;
+  const double* ch_ptr;  // GLM: c_h of this step (device scalar, scal[3])
+  int last_stage;        // GLM: the source term multiplies psi in the stage that completes the step
   int lz;                // z-chunk length per CTA (stage_kernel)
   int ntx, nty;          // x-y tiles (stage3d_kernel: work = ntx * nty * nz tile-planes, split evenly over the grid)
   Phys ph;
@@ -322,6 +324,7 @@ __global__ void __launch_bounds__(32 * (TY + 2), MINB) stage_kernel(const __grid
 // ------------------------------------------------------------------------------------------------------------
 struct GhostParams {
   double* U;
+  int nv;
   int nx, ny, nz, ghy, ghz, nxp, nyp, nzp;
   long long sy, sz, sq;
   long long nzs, nys, nxs;   // cells in the z-, y-, x-slabs
@@ -362,8 +365,7 @@ __global__ void __launch_bounds__(256) ghost_fill_kernel(const __grid_constant__
     int k = (kp - P.ghz) % P.nz;      if (k < 0) k += P.nz;
     const long long dst = (long long)kp * P.sz + (long long)jp * P.sy + ip;
     const long long src = (long long)(k + P.ghz) * P.sz + (long long)(j + P.ghy) * P.sy + (i + 2);
-#pragma unroll
-    for (int q = 0; q < 8; ++q) P.U[q * P.sq + dst] = P.U[q * P.sq + src];
+    for (int q = 0; q < P.nv; ++q) P.U[q * P.sq + dst] = P.U[q * P.sq + src];
   }
 }
 
@@ -446,6 +448,7 @@ __global__ void __launch_bounds__(256) dt_kernel(const __grid_constant__ DtParam
         const double dt = P.cfl_dx / v;
         P.scal[1] = v;
         P.scal[0] = dt;
+        P.scal[3] = 0.95 * v;          // GLM (R22): c_h
         if (P.add_t) P.scal[2] += dt;
         *P.ticket = 0u;
       }
@@ -457,7 +460,10 @@ __global__ void __launch_bounds__(256) dt_kernel(const __grid_constant__ DtParam
 __global__ void set_dt_kernel(double* scal, double dt, unsigned long long* vnext) {
   scal[0] = dt;
   scal[2] += dt;
-  if (vnext) *vnext = 0ull;
+  if (vnext) {
+    scal[3] = 0.95 * __longlong_as_double((long long)*vnext);      // GLM (R22): c_h = 0.95 v_max(U^n)
+    *vnext = 0ull;
+  }
 }
 
 // Head of a step when A7 is fused into the previous step's last stage: v_max of the current state is already in
@@ -468,6 +474,7 @@ __global__ void begin_step_kernel(double* scal, unsigned long long* vnext, doubl
   scal[1] = v;
   scal[0] = dt;
   scal[2] += dt;
+  scal[3] = 0.95 * v;                                              // GLM (R22): c_h
   *vnext = 0ull;
 }
 

@@ -29,20 +29,26 @@ namespace agate {
 
 constexpr int SW2 = 30;        // cells a warp updates per row
 constexpr int RW2 = 34;        // cells per ring row: x = xs-2 .. xs+31
-constexpr int NW2 = 6;         // warps per CTA
+constexpr int NW2 = 6;         // warps per CTA of the 8-variable kernels
 
+// GLM = true: nine variables per cell, the scalar psi (index 8) behind the MHD ones (NEXT-1; eqs.10-11; R22)
+template <bool GLM>
 struct Stage2dSmem {
-  static constexpr int RING = 4 * 8 * RW2;          // [slot][q][c]
+  static constexpr int NV = GLM ? 9 : 8;
+  static constexpr int NW = GLM ? 5 : 6;            // warps per CTA (two CTAs per SM must fit 227 KB)
+  static constexpr int RING = 4 * NV * RW2;         // [slot][q][c]
   static constexpr int OFF_WLY = RING;              // [q][lane]
-  static constexpr int OFF_FYL = OFF_WLY + 8 * 32;
-  static constexpr int OFF_URAW = OFF_FYL + 8 * 32; // [2][q][lane]
-  static constexpr int PER_WARP = OFF_URAW + 2 * 8 * 32;
-  static constexpr size_t BYTES = sizeof(double) * (size_t)PER_WARP * NW2;
+  static constexpr int OFF_FYL = OFF_WLY + NV * 32;
+  static constexpr int OFF_URAW = OFF_FYL + NV * 32; // [2][q][lane]
+  static constexpr int PER_WARP = OFF_URAW + 2 * NV * 32;
+  static constexpr size_t BYTES = sizeof(double) * (size_t)PER_WARP * NW;
 };
 
-template <int RIEMANN, int LIM, bool HALL>
-__global__ void __launch_bounds__(32 * NW2, 2) stage2d_kernel(const __grid_constant__ StageParams P) {
-  using SM = Stage2dSmem;
+template <int RIEMANN, int LIM, bool HALL, bool GLM>
+__global__ void __launch_bounds__(32 * Stage2dSmem<GLM>::NW, 2) stage2d_kernel(const __grid_constant__ StageParams P) {
+  static_assert(!(HALL && GLM), "Hall + GLM is not built");
+  using SM = Stage2dSmem<GLM>;
+  constexpr int NV = SM::NV, NW2 = SM::NW;
   extern __shared__ __align__(16) double smem[];
   const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
   double* const ring = smem + (size_t)wid * SM::PER_WARP;      // this warp's private buffers
@@ -58,6 +64,11 @@ __global__ void __launch_bounds__(32 * NW2, 2) stage2d_kernel(const __grid_const
   const double hbeta = 0.5 * P.beta;
   double vmx = 0.0;
   int bad = 0;
+  // GLM (R22): c_h of this step from the device scalar; the source term multiplies psi by exp(-dt c_h / 0.18)
+  // (c_h^2 / c_p^2 with c_p^2 = 0.18 c_h) in the stage that completes the step
+  const double ch = GLM ? *P.ch_ptr : 0.0;
+  const double ich = GLM ? 1.0 / ch : 0.0;
+  const double decay = (GLM && P.last_stage) ? exp(-dt * ch / 0.18) : 1.0;
 
   const int nstrip = (P.nx + SW2 - 1) / SW2;
   const long long wtot = (long long)nstrip * P.ny;
@@ -81,7 +92,7 @@ __global__ void __launch_bounds__(32 * NW2, 2) stage2d_kernel(const __grid_const
     wend = wtot * (gw + 1) / nwarp;
   }
 
-  auto slot_of = [](int r) { return ((r + 4) & 3) * (8 * RW2); };      // r >= -4
+  auto slot_of = [](int r) { return ((r + 4) & 3) * (NV * RW2); };     // r >= -4
   auto conv = [&](int off) {                                            // A1 in place; returns nothing
     double u[8], w[8];
 #pragma unroll
@@ -112,17 +123,17 @@ __global__ void __launch_bounds__(32 * NW2, 2) stage2d_kernel(const __grid_const
       if (own_in) {
         const double* src = P.Uin + gr + g_own;
 #pragma unroll
-        for (int q = 0; q < 8; ++q, src += P.sq) cp_async8(ring + so + q * RW2 + lane + 1, src);
+        for (int q = 0; q < NV; ++q, src += P.sq) cp_async8(ring + so + q * RW2 + lane + 1, src);
         if (two && with_u0) {
           const double* s0 = P.U0 + gr + g_own;
 #pragma unroll
-          for (int q = 0; q < 8; ++q, s0 += P.sq) cp_async8(Uraw + ((r & 1) * 8 + q) * 32 + lane, s0);
+          for (int q = 0; q < NV; ++q, s0 += P.sq) cp_async8(Uraw + ((r & 1) * NV + q) * 32 + lane, s0);
         }
       }
       if (ex_in) {
         const double* src = P.Uin + gr + g_ex;
 #pragma unroll
-        for (int q = 0; q < 8; ++q, src += P.sq) cp_async8(ring + so + q * RW2 + cex, src);
+        for (int q = 0; q < NV; ++q, src += P.sq) cp_async8(ring + so + q * RW2 + cex, src);
       }
     };
     // A1 for row r, and the raw Uin (+U0) of the own cell for A6
@@ -131,8 +142,8 @@ __global__ void __launch_bounds__(32 * NW2, 2) stage2d_kernel(const __grid_const
       if (own_in) {
         if (keep_raw) {
 #pragma unroll
-          for (int q = 0; q < 8; ++q) {
-            const int a = ((r & 1) * 8 + q) * 32 + lane;
+          for (int q = 0; q < NV; ++q) {
+            const int a = ((r & 1) * NV + q) * 32 + lane;
             const double u = ring[so + q * RW2 + lane + 1];
             Uraw[a] = two ? (u + Uraw[a]) : u;
           }
@@ -144,7 +155,7 @@ __global__ void __launch_bounds__(32 * NW2, 2) stage2d_kernel(const __grid_const
 
     // ---- prologue: rows j0-2, j0-1, j0 and the carried left state of face j0-1/2 ----
 #pragma unroll
-    for (int i = 0; i < 4 * 8 * RW2 / 32; ++i) ring[i * 32 + lane] = 1.0;      // cells outside the padded array
+    for (int i = 0; i < 4 * NV * RW2 / 32; ++i) ring[i * 32 + lane] = 1.0;     // cells outside the padded array
     __syncwarp();
     copy_row(j0 - 2, false); copy_row(j0 - 1, false); copy_row(j0, true);
     cp_async_wait_all();
@@ -154,7 +165,7 @@ __global__ void __launch_bounds__(32 * NW2, 2) stage2d_kernel(const __grid_const
     {
       const int c = lane + 1;
 #pragma unroll
-      for (int q = 0; q < 8; ++q) {
+      for (int q = 0; q < NV; ++q) {
         const double a = ring[slot_of(j0 - 2) + q * RW2 + c], b = ring[slot_of(j0 - 1) + q * RW2 + c];
         const double cc = ring[slot_of(j0) + q * RW2 + c];
         WLy[q * 32 + lane] = b + half_slope(limiter, hbeta, cc - b, b - a);
@@ -162,16 +173,16 @@ __global__ void __launch_bounds__(32 * NW2, 2) stage2d_kernel(const __grid_const
     }
     copy_row(j0 + 1, true);
 
-    double acc[8];
+    double acc[NV];
 #pragma unroll
-    for (int q = 0; q < 8; ++q) acc[q] = 0.0;
+    for (int q = 0; q < NV; ++q) acc[q] = 0.0;
 
     for (int j = j0; j <= j1; ++j) {
       const bool full = j < j1;       // row j gets its x sweep (step j1 only closes row j1-1)
       const bool emit = j > j0;       // row j-1 is completed in this step
       const int sm = slot_of(j - 1), sc = slot_of(j), sp = slot_of(j + 1);
       const int c = lane + 1;
-      double L[8], R[8], F[8];
+      double L[NV], R[NV], F[NV];
 
       // row j+1 has had a whole step to arrive
       cp_async_wait_all();
@@ -181,8 +192,8 @@ __global__ void __launch_bounds__(32 * NW2, 2) stage2d_kernel(const __grid_const
 
       // ---- y task: A2 slope of row j, face j-1/2 (L carried, R = W(j) - dW/2), A3 + A4 ----
 #pragma unroll
-      for (int r = 0; r < 8; ++r) {
-        const int v = rot_var(r, 1);
+      for (int r = 0; r < NV; ++r) {
+        const int v = (r < 8) ? rot_var(r, 1) : r;
         const double a = ring[sm + v * RW2 + c], b = ring[sc + v * RW2 + c], cc = ring[sp + v * RW2 + c];
         const double hs = half_slope(limiter, hbeta, cc - b, b - a);
         L[r] = WLy[v * 32 + lane];
@@ -200,20 +211,30 @@ __global__ void __launch_bounds__(32 * NW2, 2) stage2d_kernel(const __grid_const
         const double dxBz = ((Bz[cL + 1] - Bz[cL - 1]) + (Bz[cR + 1] - Bz[cR - 1])) * h;
         Jr[0] = -dxBz; Jr[1] = dxBy - dyBx; Jr[2] = dyBz;              // rotated for n = 1: (Jy, Jz, Jx)
       }
+      double bns = 0.0, pss = 0.0;
+      if (GLM) {
+        // (B_n, psi) at the face from the 2x2 linear Riemann problem (speeds -+c_h); the MHD solver sees B_n* on
+        // both sides, and  F[B_n] = psi*,  F[psi] = c_h^2 B_n*
+        bns = 0.5 * (L[5] + R[5]) - 0.5 * (R[NV - 1] - L[NV - 1]) * ich;
+        pss = 0.5 * (L[NV - 1] + R[NV - 1]) - 0.5 * ch * (R[5] - L[5]);
+        L[5] = bns; R[5] = bns;
+      }
       riemann_flux<RIEMANN, HALL>(P.ph, L, R, HALL ? Jr : nullptr, F);
+      if (GLM) { F[5] = pss; F[NV - 1] = ch * ch * bns; }
       {
         // A5 (y) + A6: row j-1 is complete; the accumulator of row j starts from the raw Uin (+U0)
         double* po = P.Uout + (long long)(j + 1) * P.sy + g_own;          // own cell of row j-1
-        double o[8];
+        double o[NV];
 #pragma unroll
-        for (int v = 0; v < 8; ++v, po += P.sq) {
-          constexpr int inv1[8] = {0, 3, 1, 2, 4, 7, 5, 6};               // rot_var(inv1[v], 1) == v
+        for (int v = 0; v < NV; ++v, po += P.sq) {
+          constexpr int inv1[9] = {0, 3, 1, 2, 4, 7, 5, 6, 8};            // rot_var(inv1[v], 1) == v
           const int r = inv1[v];
           // the difference is formed before it meets U, so that a uniform state stays bitwise fixed (pin P1)
           o[v] = c0 * (acc[v] - cy * (F[r] - FyL[v * 32 + lane]));
+          if (GLM && v == NV - 1) o[v] *= decay;                          // eq.11's source, integrated exactly
           if (emit && cell_ok) *po = o[v];
           FyL[v * 32 + lane] = F[r];
-          acc[v] = Uraw[((j & 1) * 8 + v) * 32 + lane];
+          acc[v] = Uraw[((j & 1) * NV + v) * 32 + lane];
         }
         if (P.vnext != nullptr && emit && cell_ok) {                      // A7 on the values just stored
           const double sp2 = cell_speed_inline(P.ph, o);
@@ -227,7 +248,7 @@ __global__ void __launch_bounds__(32 * NW2, 2) stage2d_kernel(const __grid_const
       // ---- x task: A2 own slope, right state from lane i+1, A3 + A4, low-face flux from lane i-1 ----
       if (full) {
 #pragma unroll
-        for (int r = 0; r < 8; ++r) {
+        for (int r = 0; r < NV; ++r) {
           const double a = ring[sc + r * RW2 + c - 1], b = ring[sc + r * RW2 + c], cc = ring[sc + r * RW2 + c + 1];
           const double hs = half_slope(limiter, hbeta, cc - b, b - a);
           L[r] = b + hs;
@@ -243,9 +264,15 @@ __global__ void __launch_bounds__(32 * NW2, 2) stage2d_kernel(const __grid_const
           const double dyBz = ((Bz[sp + c] - Bz[sm + c]) + (Bz[sp + cc1] - Bz[sm + cc1])) * h;
           Jr[0] = dyBz; Jr[1] = -dxBz; Jr[2] = dxBy - dyBx;              // rotated for n = 0: (Jx, Jy, Jz)
         }
+        if (GLM) {
+          bns = 0.5 * (L[5] + R[5]) - 0.5 * (R[NV - 1] - L[NV - 1]) * ich;
+          pss = 0.5 * (L[NV - 1] + R[NV - 1]) - 0.5 * ch * (R[5] - L[5]);
+          L[5] = bns; R[5] = bns;
+        }
         riemann_flux<RIEMANN, HALL>(P.ph, L, R, HALL ? Jr : nullptr, F);
+        if (GLM) { F[5] = pss; F[NV - 1] = ch * ch * bns; }
 #pragma unroll
-        for (int r = 0; r < 8; ++r) {
+        for (int r = 0; r < NV; ++r) {
           const double fl = __shfl_up_sync(0xffffffffu, F[r], 1);
           acc[r] -= cx * (F[r] - fl);
         }

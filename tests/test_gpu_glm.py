@@ -1,0 +1,106 @@
+"""GPU parity of the GLM path (NEXT-1: eqset IDEAL_GLM, 9 variables, 2-D strip kernel) against the oracle  (-m gpu).
+
+Same bar as the 8-variable path: relative L-inf per variable <= 1e-12 after one step, <= 1e-9 after the run, dt to
+1e-14 relative.  Scale of psi (R23): psi / c_h is the quantity that travels with B_n (the characteristic
+variables of eqs.10-11 are B_n -+ psi/c_h), and psi is built from differences of B times c_h, so its round-off is
+c_h |B| eps however small psi itself is: psi is measured against max(max|psi|, c_h max|B|)."""
+import numpy as np
+import pytest
+
+import oracle
+from workloads import make_workload
+
+pytestmark = pytest.mark.gpu
+
+TOL_1, TOL_N, TOL_DT = 1e-12, 1e-9, 1e-14
+
+
+@pytest.fixture(scope="module")
+def ag():
+    import paper_2503_20899_b200 as m
+    m.lib()
+    return m
+
+
+def rel_linf9(Ug, Ur, ch):
+    sc = np.empty(9)
+    sc[0] = np.max(np.abs(Ur[0])); sc[4] = np.max(np.abs(Ur[4]))
+    sc[1:4] = np.max(np.abs(Ur[1:4])); sc[5:8] = np.max(np.abs(Ur[5:8]))
+    sc[8] = max(np.max(np.abs(Ur[8])), ch * sc[5])
+    return np.array([np.max(np.abs(Ug[q] - Ur[q])) / (sc[q] if sc[q] > 0 else 1.0) for q in range(9)])
+
+
+@pytest.mark.parametrize("n,steps,riemann,grid", [(100, 12, None, 0), (64, 6, oracle.HLLD, 0), (100, 4, None, 40),
+                                                   (256, 3, None, 0)])
+def test_orszag_tang_glm_parity(ag, n, steps, riemann, grid, monkeypatch):
+    """Config 6 recipe (Orszag-Tang, + GLM) at reduced size: ragged strips (n=100: 3 x 30 + 10), short
+    segments (grid=40), HLL (the paper's default) and HLLD."""
+    if grid:
+        monkeypatch.setenv("AGATE_GRID", str(grid))
+    wl = make_workload(6, n=n)
+    over = {} if riemann is None else {"riemann": riemann}
+    ref = oracle.RefSolver.from_workload(wl, **over)
+    gpu = ag.Agate.from_workload(wl, **over)
+    e1 = None
+    for s in range(steps):
+        dtr, dtg = ref.compute_dt(), gpu.compute_dt()
+        assert abs(dtg - dtr) <= TOL_DT * dtr
+        ref.step(dtr)
+        assert gpu.step(0.0) == dtg
+        if s == 0:
+            e1 = rel_linf9(gpu.get_state(), ref.get_state(), ref.glm_ch())
+    eN = rel_linf9(gpu.get_state(), ref.get_state(), ref.glm_ch())
+    assert np.all(e1 <= TOL_1), e1
+    assert np.all(eN <= TOL_N), eN
+    assert np.max(np.abs(ref.get_state()[8])) > 0          # the cleaning field is live in this problem
+    ref.close(); gpu.close()
+
+
+@pytest.mark.parametrize("rk", [1, 2])
+def test_glm_sequences_and_advance(ag, rk):
+    """Host-chosen dt (c_h still 0.95 v_max of the current state), self-timed steps, agate_advance (graph replay)
+    and a second set_state, against the oracle doing the same."""
+    wl = make_workload(6, n=64)
+    U0 = wl.U.copy()
+    U0[8] = 0.01 * np.sin(2 * np.pi * (np.arange(64) + 0.5) / 64)[None, :, None]     # start with a live psi
+    ref = oracle.RefSolver.from_workload(wl, rk=rk); ref.set_state(U0)
+    gpu = ag.Agate.from_workload(wl, rk=rk); gpu.set_state(U0)
+    d = ref.compute_dt()
+    ref.step(0.5 * d); assert gpu.step(0.5 * d) == 0.5 * d
+    d = ref.compute_dt(); assert abs(gpu.compute_dt() - d) <= TOL_DT * d
+    ref.step(d); gpu.step(0.0)
+    tr, tg = ref.advance(4), gpu.advance(4)
+    assert abs(tg - tr) <= 1e-13 * tr
+    assert np.all(rel_linf9(gpu.get_state(), ref.get_state(), ref.glm_ch()) <= TOL_N)
+    ref.set_state(wl.U, 0.0); gpu.set_state(wl.U, 0.0)
+    tr, tg = ref.advance(2), gpu.advance(2)
+    assert abs(tg - tr) <= 1e-13 * tr
+    assert np.all(rel_linf9(gpu.get_state(), ref.get_state(), ref.glm_ch()) <= TOL_N)
+    ref.close(); gpu.close()
+
+
+def test_glm_uniform_state_exact_decay(ag):
+    """Pin G2 on the GPU: uniform state with psi = const: the 8 MHD variables stay bitwise fixed, psi is multiplied
+    by exp(-dt c_h/0.18) per step."""
+    W = np.array([1.3, 0.2, -0.1, 0.05, 0.9, 0.4, -0.3, 0.2, 0.37])
+    U1 = W.copy(); U1[1:4] = W[0] * W[1:4]
+    U1[4] = W[4] / (5 / 3 - 1) + 0.5 * W[0] * np.sum(W[1:4] ** 2) + 0.5 * np.sum(W[5:8] ** 2)
+    U = np.tile(U1[:, None, None, None], (1, 1, 50, 70))
+    gpu = ag.Agate(shape=(70, 50, 1), dx=(0.1, 0.1, 1), ndim=2, eqset=ag.IDEAL_GLM, riemann=0, beta=1.3)
+    ref = oracle.RefSolver(shape=(70, 50, 1), dx=(0.1, 0.1, 1), ndim=2, eqset=oracle.IDEAL_GLM, riemann=0, beta=1.3)
+    gpu.set_state(U); ref.set_state(U)
+    vm = ref.vmax()
+    psi = 0.37
+    for _ in range(3):
+        dt = gpu.step(0.0)
+        psi *= np.exp(-dt * 0.95 * vm / 0.18)
+    V = gpu.get_state()
+    assert np.array_equal(V[:8], U[:8])
+    assert np.allclose(V[8], psi, rtol=1e-14, atol=0)
+    gpu.close(); ref.close()
+
+
+def test_glm_rejected_where_not_built(ag):
+    with pytest.raises(ag.AgateError) as ei:
+        ag.Agate(shape=(8, 8, 8), dx=(1 / 8,) * 3, ndim=3, eqset=ag.IDEAL_GLM)
+    assert ei.value.code == ag.ERR_ARG

@@ -30,6 +30,7 @@ import numpy as np
 #                                primitive W = (rho, vx, vy, vz, p, Bx, By, Bz).
 NVAR = 8
 IDEAL, HALL = 0, 1
+IDEAL_GLM = 3          # 9 variables per cell: the GLM scalar psi behind the 8 MHD ones
 HLL, HLLD = 0, 1
 GAMMA = 5.0 / 3.0
 SEED_BASE = 2503208990
@@ -146,8 +147,10 @@ def _rms(*comps):
 
 def prim_to_cons(W: np.ndarray, gamma: float) -> np.ndarray:
     """Definition of the conserved vector (PAPER.md L140 with R2: p/(gamma-1))."""
-    rho, vx, vy, vz, p, bx, by, bz = W
+    rho, vx, vy, vz, p, bx, by, bz = W[:8]
     U = np.empty_like(W)
+    if W.shape[0] > 8:
+        U[8:] = W[8:]                 # the GLM scalar is its own conserved variable
     U[0] = rho
     U[1] = rho * vx
     U[2] = rho * vy
@@ -171,6 +174,10 @@ _CONFIGS = {
             name="cfg4: 2D Hall 1024^2 HLL minmod"),
     5: dict(ndim=3, n=512,  eqset=IDEAL, riemann=HLLD, beta=1.3, cfl=0.325, d_i=0.0,  n_steps=20,
             name="cfg5: 3D ideal 512^3 HLLD MC (headline)"),
+    # NEXT-1, not a BASELINE.json config: the workload of the paper's Table 2 -- Orszag-Tang vortex
+    # (IC printed at P:L282) with GLM divergence cleaning, "default settings": PLM + eq.4 beta=1.3, HLL, C=0.45.
+    6: dict(ndim=2, n=2048, eqset=IDEAL_GLM, riemann=HLL, beta=1.3, cfl=0.45,  d_i=0.0,  n_steps=100,
+            name="cfg6: 2D Orszag-Tang + GLM 2048^2 HLL MC (paper Table 2 workload)"),
 }
 
 
@@ -180,7 +187,7 @@ def config_settings(config_id: int) -> dict:
 
 def make_workload(config_id: int, n: int | None = None, n_steps: int | None = None,
                   scale_d_i: bool = True) -> Workload:
-    """Build config `config_id` (1..5). `n` overrides the per-dimension resolution (reduced-size
+    """Build config `config_id` (1..5: BASELINE.json; 6: Orszag-Tang + GLM, the paper's Table 2 workload). `n` overrides the per-dimension resolution (reduced-size
     parity cases use the same recipe and seed); for config 4, d_i is rescaled with n so that d_i/dx
     stays 51.2 cells (`scale_d_i`)."""
     c = config_settings(config_id)
@@ -192,10 +199,25 @@ def make_workload(config_id: int, n: int | None = None, n_steps: int | None = No
     rng = SplitMix64(SEED_BASE + config_id)
     g = GAMMA
     nx, ny, nz = shape
-    W = np.empty((NVAR, nz, ny, nx))
+    W = np.empty((NVAR + (1 if c["eqset"] == IDEAL_GLM else 0), nz, ny, nx))
     F = lambda M, K: _field(rng, M, K, ndim, shape)
 
-    if config_id in (1, 4):
+    if config_id == 6:
+        # rho = 25/(36 pi), p = 5/(12 pi), v = (-sin 2 pi y, sin 2 pi x, 0), B = B0 (-sin 2 pi y, sin 4 pi x, 0),
+        # B0 = 1/sqrt(4 pi), unit box, cell centres; psi = 0
+        xc = ((np.arange(nx) + 0.5) / nx)[None, None, :]
+        yc = ((np.arange(ny) + 0.5) / ny)[None, :, None]
+        B0 = 1.0 / math.sqrt(4.0 * math.pi)
+        W[0] = 25.0 / (36.0 * math.pi)
+        W[4] = 5.0 / (12.0 * math.pi)
+        W[1] = -np.sin(2.0 * math.pi * yc) + 0.0 * xc
+        W[2] = np.sin(2.0 * math.pi * xc) + 0.0 * yc
+        W[3] = 0.0
+        W[5] = -B0 * np.sin(2.0 * math.pi * yc) + 0.0 * xc
+        W[6] = B0 * np.sin(4.0 * math.pi * xc) + 0.0 * yc
+        W[7] = 0.0
+        W[8] = 0.0
+    elif config_id in (1, 4):
         W[0] = 1.0 + 0.1 * F(4, 4)
         W[1] = 0.1 * F(4, 4)
         W[2] = 0.1 * F(4, 4)
