@@ -37,9 +37,11 @@ UNIT = "zone-updates/s"
 # own as-written count (oracle.count_ops) is higher (1774 / 2265 / 3350 / 2072 / 3292) because it evaluates both
 # sides' fluxes and divides where a shared reciprocal serves.  The smaller figure is used so the fraction is not
 # flattered.
-FLOP_PER_ZONE_STEP = {1: 1430.0, 2: 1890.0, 3: 2770.0, 4: 1760.0, 5: 2770.0}
-FLOP_DT_PER_ZONE = {1: 45.0, 2: 45.0, 3: 45.0, 4: 60.0, 5: 45.0}
-BYTES_PER_ZONE_STEP = 320.0            # 5 x 8 variables x 8 B
+# config 6 (Orszag-Tang + GLM, NEXT-1): config 1's 2-D HLL count + 120 for the ninth variable (slopes, 2x2 face
+# problem, flux difference, source)
+FLOP_PER_ZONE_STEP = {1: 1430.0, 2: 1890.0, 3: 2770.0, 4: 1760.0, 5: 2770.0, 6: 1550.0}
+FLOP_DT_PER_ZONE = {1: 45.0, 2: 45.0, 3: 45.0, 4: 60.0, 5: 45.0, 6: 45.0}
+BYTES_PER_ZONE_STEP = 320.0            # 5 x 8 variables x 8 B; 360 with the GLM scalar (config 6)
 # DRAM bytes per launch of the dominant kernel (dram__bytes_read.sum + dram__bytes_write.sum, mean of the two stage
 # launches of one step) from the committed `ncu` capture of the same command: profiles/r1_stage3d.md
 NCU_TRAFFIC_BYTES = {5: 0.5 * (9617129216 + 8682435584 + 18299382528 + 8663042304),
@@ -47,7 +49,7 @@ NCU_TRAFFIC_BYTES = {5: 0.5 * (9617129216 + 8682435584 + 18299382528 + 866304230
 FP64_NOMINAL_TFLOPS = 148 * 64 * 2 * 1.965e9 / 1e12     # 148 SMs x 64 DFMA lanes x 2 x max SM clock = 37.2
 
 # reduced size of the bounded CPU sample per config (same recipe and seed), and its step count
-CPU_SAMPLE = {1: (128, 10), 2: (512, 8), 3: (96, 4), 4: (512, 8), 5: (96, 4)}
+CPU_SAMPLE = {1: (128, 10), 2: (512, 8), 3: (96, 4), 4: (512, 8), 5: (96, 4), 6: (512, 8)}
 
 
 def parse():
@@ -55,7 +57,11 @@ def parse():
     ap.add_argument("--gpus", type=int, default=1)
     ap.add_argument("--steps", type=int, default=20)
     ap.add_argument("--warmup", type=int, default=3)
-    ap.add_argument("--config", type=int, default=5, choices=[1, 2, 3, 4, 5])
+    ap.add_argument("--config", type=int, default=5, choices=[1, 2, 3, 4, 5, 6],
+                    help="1-5: BASELINE.json configs; 6: Orszag-Tang + GLM, the workload of the paper's Table 2")
+    ap.add_argument("--to-time", type=float, default=0.0,
+                    help="config 6: also run the problem from t=0 to this time (the paper ran to 0.5) and report the "
+                         "device wall time beside the paper's A100 figure")
     ap.add_argument("--n", type=int, default=0, help="override the per-dimension resolution (debugging)")
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--no-e2e", action="store_true")
@@ -222,10 +228,11 @@ def run_ours(args):
     flop_stage = (FLOP_PER_ZONE_STEP[cfg] - FLOP_DT_PER_ZONE[cfg]) / 2.0 * zones
     achieved = flop_stage / (stage_ms * 1e-3) / 1e12
     peaks, peak_src = measured_peaks()
-    hbm_frac = (BYTES_PER_ZONE_STEP / 5.0 * 2.5 * zones / (stage_ms * 1e-3) / 1e9) / peaks["hbm_gbs"]
+    bytes_step = BYTES_PER_ZONE_STEP * (9.0 / 8.0 if cfg == 6 else 1.0)
+    hbm_frac = (bytes_step / 5.0 * 2.5 * zones / (stage_ms * 1e-3) / 1e9) / peaks["hbm_gbs"]
     roofline = {"bound": "alu", "achieved": achieved, "peak": fp64_peak, "unit": "TFLOP/s",
                 "frac": achieved / fp64_peak, "traffic": NCU_TRAFFIC_BYTES.get(cfg) if not args.n else None,
-                "algorithmic_bytes": BYTES_PER_ZONE_STEP / 2.0 * zones,
+                "algorithmic_bytes": bytes_step / 2.0 * zones,
                 "kernel": {3: "stage3d_kernel", 2: "stage2d_kernel"}.get(wl.ndim, "stage_kernel"), "ms_per_launch": stage_ms, "launches_timed": st_n,
                 "stage_share_of_step": 2.0 * stage_ms * K / ms_max if st_n else None,
                 "peak_source": "FP64 DFMA micro-benchmark of this run (agate_measure_fp64_peak); nominal "
@@ -257,17 +264,40 @@ def run_ours(args):
                "d2h_bytes_per_step": nbytes, "steps": Ke,
                "note": "agate_set_state(host pinned) + agate_step + agate_get_state(host pinned) per step"}
 
+    # ---- config 6: the paper's own run (Table 2): Orszag-Tang + GLM from t = 0 to t_end -------------
+    table2 = None
+    if cfg == 6 and args.to_time > 0.0 and world == 1:
+        sim.set_state(Uh)
+        sim.advance(1)                                # graph instantiation outside the timed region
+        sim.set_state(Uh)
+        e0.record(sim.stream)
+        nst, t = 0, 0.0
+        while t < args.to_time:
+            t = sim.advance(50)
+            nst += 50
+        e1.record(sim.stream)
+        torch.cuda.synchronize()
+        paper = {32: 0.27, 64: 0.450, 128: 0.82, 256: 1.55, 512: 3.04, 1024: 12.0, 2048: 87.1}
+        table2 = {"t_end": t, "steps": nst, "wall_s": e0.elapsed_time(e1) * 1e-3, "n": wl.shape[0],
+                  "paper_kernel_mode_a100_s": paper.get(wl.shape[0]),
+                  "note": "paper: whole-run wall clock of AGATE's Kernel mode on one A100 (Table 2, P:L348-354; "
+                          "includes start-up and output); here: device time of the stepping only -- context, not a "
+                          "like-for-like benchmark"}
+
     if rank == 0:
         line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": Wm,
                 "ms_per_step": ms_max / K, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
                 "dtype": "f64", "data": "synthetic",
-                "config": {"workload": f"BASELINE.json config {cfg}: {wl.name}", "zones_per_gpu": zones,
+                "config": {"workload": (f"BASELINE.json config {cfg}: {wl.name}" if cfg <= 5 else
+                                        f"NEXT-1 (not a BASELINE.json config): {wl.name}"), "zones_per_gpu": zones,
                            "parallelism": "replicas only" if world > 1 else "single GPU",
                            "l2": "state (2 x %.2f GB) is larger than L2; no flush needed" % (zones * 64 / 1e9)
                                  if zones * 64 > 2.5e8 else "state fits L2 (small config); numbers are L2-resident",
                            "launch": info},
                 "roofline": roofline, "clocks": clk.summary(), "gpu_launches": info["launches_per_step"] * K,
                 "e2e": e2e}
+        if table2 is not None:
+            line["paper_table2_run"] = table2
         if not args.no_cpu and world >= 1:
             line["cpu_baseline"] = cpu_oracle_rate(cfg)[0]
         print(json.dumps(line))
