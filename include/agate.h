@@ -56,8 +56,8 @@ enum { AGATE_IDEAL = 0, AGATE_HALL = 1, AGATE_IDEAL_GLM = 3 };
 /* AGATE_IDEAL_GLM (NEXT-1; eqs.10-11, constants L142; R22): ideal MHD with GLM
  * divergence cleaning.  NINE variables per cell, the scalar psi last: every U below is U[9][nz][ny][nx].  Per step
  * c_h = 0.95 v_max(U^n), c_p^2 = 0.18 c_h; face (B_n, psi) from the 2x2 linear Riemann problem; psi is multiplied by
- * exp(-dt c_h^2/c_p^2) after the Runge-Kutta update.  2-D grids only in this build (agate_init returns AGATE_ERR_ARG
- * otherwise). */
+ * exp(-dt c_h^2/c_p^2) after the Runge-Kutta update.  2-D and 3-D grids (1-D: agate_init returns AGATE_ERR_ARG). */
+
 enum { AGATE_HLL = 0, AGATE_HLLD = 1 };
 enum {
   AGATE_OK = 0,

@@ -68,7 +68,7 @@ int check_args(const agate_grid* g, double gamma, int eqset, const agate_solver*
   if (!(g->dx > 0.0) || (g->ndim >= 2 && !(g->dy > 0.0)) || (g->ndim >= 3 && !(g->dz > 0.0))) return AGATE_ERR_ARG;
   if (!(gamma > 1.0)) return AGATE_ERR_ARG;
   if (eqset != AGATE_IDEAL && eqset != AGATE_HALL && eqset != AGATE_IDEAL_GLM) return AGATE_ERR_ARG;
-  if (eqset == AGATE_IDEAL_GLM && g->ndim != 2) return AGATE_ERR_ARG;            // GLM: 2-D strip kernel only so far
+  if (eqset == AGATE_IDEAL_GLM && g->ndim < 2) return AGATE_ERR_ARG;             // GLM: 2-D and 3-D kernels
   if (s->riemann < 0 || s->riemann > 1 || s->limiter < 0 || s->limiter > 2 || s->rk < 1 || s->rk > 2) return AGATE_ERR_ARG;
   if (s->limiter == 2 && !(s->beta >= 1.0 && s->beta <= 2.0)) return AGATE_ERR_ARG;
   if (eqset == AGATE_HALL && s->riemann == AGATE_HLLD) return AGATE_ERR_ARG;   // no Hall-HLLD in the paper
@@ -97,11 +97,11 @@ StageKernel make_stage() {
   return k;
 }
 
-template <int TY, int R, int LIM, int MINB>
+template <int TY, int R, int LIM, int MINB, bool GLM = false>
 StageKernel make_stage3d() {
   StageKernel k;
-  k.fn = stage3d_kernel<TY, R, LIM, MINB>;
-  k.ty = TY; k.np = 3; k.threads = Stage3dSmem<TY>::NT; k.smem = Stage3dSmem<TY>::BYTES;
+  k.fn = stage3d_kernel<TY, R, LIM, MINB, GLM>;
+  k.ty = TY; k.np = 3; k.threads = Stage3dSmem<TY, GLM ? 9 : 8>::NT; k.smem = Stage3dSmem<TY, GLM ? 9 : 8>::BYTES;
   k.even_split = true;
   k.fused_dt = true;
   return k;
@@ -123,6 +123,10 @@ StageKernel pick_stage(int ndim, int eqset, int riemann, int limiter) {
     if (getenv("AGATE_STAGE_V1")) {      // the pooled kernel of agate_kernels.cuh, kept for A/B measurements
       if (riemann == AGATE_HLLD) return make_stage<6, 3, 1, false, 2>();
       return make_stage<6, 3, 0, false, 2>();
+    }
+    if (eqset == AGATE_IDEAL_GLM) {
+      if (riemann == AGATE_HLLD) return (limiter == 2) ? make_stage3d<TY3, 1, 2, AGATE_MINB3, true>() : make_stage3d<TY3, 1, -1, AGATE_MINB3, true>();
+      return (limiter == 2) ? make_stage3d<TY3, 0, 2, AGATE_MINB3, true>() : make_stage3d<TY3, 0, -1, AGATE_MINB3, true>();
     }
     if (limiter == 2) {                  // eq.4 (every BASELINE config): limiter fixed at compile time
       if (riemann == AGATE_HLLD) return make_stage3d<TY3, 1, 2, AGATE_MINB3>();

@@ -60,7 +60,10 @@ __device__ __forceinline__ void await(const int* prog_w, int value, int* flag) {
 }
 __device__ __forceinline__ void prefetch_l2(const void* p) { asm volatile("prefetch.global.L2 [%0];" ::"l"(p)); }
 
-template <int TY>
+// rotated slot -> fixed variable; the GLM scalar (slot 8) is not rotated
+__host__ __device__ __forceinline__ int rv(int r, int n) { return (r < 8) ? rot_var(r, n) : r; }
+
+template <int TY, int NV = 8>
 struct Stage3dSmem {
   static_assert(TY >= 2 && TY <= 16, "the x-edge task packs two cells per row into one warp");
   static constexpr int NW = TY + 1;                 // warps: TY owners + H
@@ -71,22 +74,24 @@ struct Stage3dSmem {
   static constexpr int YS = (TY + 1) * 32;          // YR rows 0..TY;  YF rows -1..TY-1 (stored at j+1)
   static constexpr int ZS = TY * 32;                // z carry
   static constexpr int XS = TY;                     // x hand-over, one entry per row
-  static constexpr int OFF_YR = 8 * QS;
-  static constexpr int OFF_YF = OFF_YR + 8 * YS;
-  static constexpr int OFF_WLZ = OFF_YF + 8 * YS;
-  static constexpr int OFF_FZL = OFF_WLZ + 8 * ZS;
-  static constexpr int OFF_XR = OFF_FZL + 8 * ZS;
-  static constexpr int OFF_XF = OFF_XR + 8 * XS;
-  static constexpr int OFF_PROG = OFF_XF + 8 * XS;  // 16 ints: per-warp phase counters
+  static constexpr int OFF_YR = NV * QS;
+  static constexpr int OFF_YF = OFF_YR + NV * YS;
+  static constexpr int OFF_WLZ = OFF_YF + NV * YS;
+  static constexpr int OFF_FZL = OFF_WLZ + NV * ZS;
+  static constexpr int OFF_XR = OFF_FZL + NV * ZS;
+  static constexpr int OFF_XF = OFF_XR + NV * XS;
+  static constexpr int OFF_PROG = OFF_XF + NV * XS;  // 16 ints: per-warp phase counters
   static constexpr int TOTAL = OFF_PROG + 8;
   static constexpr size_t BYTES = sizeof(double) * (size_t)TOTAL;
 };
 
 // LIM >= 0 fixes the limiter at compile time (no branch per slope, one basic block for all eight variables);
 // LIM < 0 reads it from the parameters.
-template <int TY, int RIEMANN, int LIM, int MINB>
+// GLM = true: nine variables per cell, the scalar psi (index 8) behind the MHD ones (NEXT-1; eqs.10-11; R22).
+template <int TY, int RIEMANN, int LIM, int MINB, bool GLM = false>
 __global__ void __launch_bounds__(32 * (TY + 1), MINB) stage3d_kernel(const __grid_constant__ StageParams P) {
-  using SM = Stage3dSmem<TY>;
+  constexpr int NV = GLM ? 9 : 8;
+  using SM = Stage3dSmem<TY, NV>;
   constexpr int NT = SM::NT, PL = SM::PL, SB = SM::SB, QS = SM::QS, YS = SM::YS, ZS = SM::ZS, XS = SM::XS;
   extern __shared__ __align__(16) double smem[];
   double* const W = smem;                    // [8][QS]  primitives: ring planes + two y-halo buffers
@@ -106,6 +111,11 @@ __global__ void __launch_bounds__(32 * (TY + 1), MINB) stage3d_kernel(const __gr
   const double c0 = two ? P.a1 : 1.0;
   const int limiter = (LIM >= 0) ? LIM : P.limiter;
   const double hbeta = 0.5 * P.beta;
+  // GLM (R22): c_h of this step from the device scalar; the source term multiplies psi by exp(-dt c_h / 0.18)
+  // (c_h^2 / c_p^2 with c_p^2 = 0.18 c_h) in the stage that completes the step
+  const double ch = GLM ? *P.ch_ptr : 0.0;
+  const double ich = GLM ? 1.0 / ch : 0.0;
+  const double decay = (GLM && P.last_stage) ? exp(-dt * ch / 0.18) : 1.0;
 
   // Work = (x-y tile, plane) pairs, split EVENLY over the CTAs of a one-wave grid (no tail wave, whatever the grid
   // size).  First the rounds: in round r CTA b takes the whole column of tile r * grid + b, so the CTAs resident at
@@ -145,7 +155,7 @@ __global__ void __launch_bounds__(32 * (TY + 1), MINB) stage3d_kernel(const __gr
 
   auto slot_of = [](int p) { return ((p + 3) % 3) * PL; };     // p >= -2
   auto conv_in_place = [&](int off) {
-    double u[8], w[8];
+    double u[8], w[8];                       // the GLM scalar (index 8) is its own primitive
 #pragma unroll
     for (int q = 0; q < 8; ++q) u[q] = W[q * QS + off];
     cons_to_prim(P.ph, u, w);
@@ -155,7 +165,7 @@ __global__ void __launch_bounds__(32 * (TY + 1), MINB) stage3d_kernel(const __gr
   auto copy_cell = [&](int off, long long g) {
     const double* src = P.Uin + g;           // running pointer: one 64-bit add per variable
 #pragma unroll
-    for (int q = 0; q < 8; ++q, src += P.sq) cp_async8(W + q * QS + off, src);
+    for (int q = 0; q < NV; ++q, src += P.sq) cp_async8(W + q * QS + off, src);
   };
   // H's copy tasks for plane p: t < 4 TY -> x-halo columns of the ring rows;  else -> the four y-halo rows
   constexpr int NHT = 4 * TY + 4 * RS;
@@ -189,7 +199,7 @@ __global__ void __launch_bounds__(32 * (TY + 1), MINB) stage3d_kernel(const __gr
   };
 
   // ---- prologue: everything step k0 needs that the steady state would have produced earlier ----
-  for (int i = tid; i < 8 * QS; i += NT) W[i] = 1.0;           // cells outside the padded array (ragged tiles)
+  for (int i = tid; i < NV * QS; i += NT) W[i] = 1.0;           // cells outside the padded array (ragged tiles)
   __syncthreads();
   if (owner) {
     if (own_in) {
@@ -205,7 +215,7 @@ __global__ void __launch_bounds__(32 * (TY + 1), MINB) stage3d_kernel(const __gr
     }
     const int ca = slot_of(k0 - 2) + own_off, cb = slot_of(k0 - 1) + own_off, cc = slot_of(k0) + own_off;
 #pragma unroll
-    for (int q = 0; q < 8; ++q) {
+    for (int q = 0; q < NV; ++q) {
       const double a = W[q * QS + ca], b = W[q * QS + cb], c = W[q * QS + cc];
       WLz[q * ZS + tid] = b + half_slope(limiter, hbeta, c - b, b - a);
     }
@@ -219,9 +229,9 @@ __global__ void __launch_bounds__(32 * (TY + 1), MINB) stage3d_kernel(const __gr
   }
   __syncthreads();
 
-  double acc[8];
+  double acc[NV];
 #pragma unroll
-  for (int q = 0; q < 8; ++q) acc[q] = 0.0;
+  for (int q = 0; q < NV; ++q) acc[q] = 0.0;
 
   // ring slots of planes k-1, k, k+1 (rotated at the end of a step) and the own cell's offset in plane k-1
   int sm = slot_of(k0 - 1), sc = slot_of(k0), sp = slot_of(k0 + 1);
@@ -230,11 +240,11 @@ __global__ void __launch_bounds__(32 * (TY + 1), MINB) stage3d_kernel(const __gr
     const bool full = k < k1;       // plane k gets its x and y sweeps (step k1 only closes plane k1-1)
     const bool emit = k > k0;       // plane k-1 is completed in this step
     const int hb = 3 * PL + (k & 1) * SB;                 // y-halo rows of plane k
-    double Ly[8], ua[8], ub[8];
+    double Ly[NV], ua[NV], ub[NV];
 
 #pragma unroll
     for (int s = 0; s < 3; ++s) {
-      double L[8], R[8], F[8];
+      double L[NV], R[NV], F[NV];
       bool flux = false;
       // ---- hand-over: what this phase reads must be published, what it overwrites must have been read.  Every
       //      wait is on a phase EARLIER than the one about to start, so the waits cannot form a cycle.
@@ -265,15 +275,15 @@ __global__ void __launch_bounds__(32 * (TY + 1), MINB) stage3d_kernel(const __gr
           if (emit) {
             // A5 (y) of plane k-1: YF holds the rotated (n = 1) fluxes of the previous phase B
 #pragma unroll
-            for (int r = 0; r < 8; ++r)
-              acc[rot_var(r, 1)] -= cy * (YF[r * YS + (wid + 1) * 32 + lane] - YF[r * YS + wid * 32 + lane]);
+            for (int r = 0; r < NV; ++r)
+              acc[rv(r, 1)] -= cy * (YF[r * YS + (wid + 1) * 32 + lane] - YF[r * YS + wid * 32 + lane]);
           }
           cp_async_wait_all();
           if (own_in) conv_in_place(sp + own_off);          // A1 of the own cell of plane k+1
           // A2 (z): slope of plane k;  face k-1/2:  L carried,  R = W(k) - dW/2
 #pragma unroll
-          for (int r = 0; r < 8; ++r) {
-            const int v = rot_var(r, 2);
+          for (int r = 0; r < NV; ++r) {
+            const int v = rv(r, 2);
             const double a = W[v * QS + sm + own_off], b = W[v * QS + sc + own_off], c = W[v * QS + sp + own_off];
             const double hs = half_slope(limiter, hbeta, c - b, b - a);
             L[r] = WLz[v * ZS + tid];
@@ -284,17 +294,17 @@ __global__ void __launch_bounds__(32 * (TY + 1), MINB) stage3d_kernel(const __gr
         } else if (full) {
           if (s == 1) {
 #pragma unroll
-            for (int q = 0; q < 8; ++q) acc[q] += two ? (ua[q] + ub[q]) : ua[q];      // A6: Uin (+ U0)
+            for (int q = 0; q < NV; ++q) acc[q] += two ? (ua[q] + ub[q]) : ua[q];      // A6: Uin (+ U0)
 #pragma unroll
-            for (int r = 0; r < 8; ++r) {
+            for (int r = 0; r < NV; ++r) {
               L[r] = Ly[r];
-              R[r] = YR[rot_var(r, 1) * YS + (wid + 1) * 32 + lane];
+              R[r] = YR[rv(r, 1) * YS + (wid + 1) * 32 + lane];
             }
           } else {
             // A2 (x): own slope; the right state of face i+1/2 comes from lane i+1 (lane 31: from H)
             const int c = sc + own_off;
 #pragma unroll
-            for (int r = 0; r < 8; ++r) {
+            for (int r = 0; r < NV; ++r) {
               const double a = W[r * QS + c - 1], b = W[r * QS + c], cc = W[r * QS + c + 1];
               const double hs = half_slope(limiter, hbeta, cc - b, b - a);
               L[r] = b + hs;
@@ -310,7 +320,7 @@ __global__ void __launch_bounds__(32 * (TY + 1), MINB) stage3d_kernel(const __gr
           {
             const int cm = sc + (TY - 1) * RS + lane + 2, c0r = hb + 2 * RS + lane + 2, cp = hb + 3 * RS + lane + 2;
 #pragma unroll
-            for (int q = 0; q < 8; ++q) {
+            for (int q = 0; q < NV; ++q) {
               const double a = W[q * QS + cm], b = W[q * QS + c0r], c = W[q * QS + cp];
               YR[q * YS + TY * 32 + lane] = b - half_slope(limiter, hbeta, c - b, b - a);
             }
@@ -319,7 +329,7 @@ __global__ void __launch_bounds__(32 * (TY + 1), MINB) stage3d_kernel(const __gr
           if (lane < TY) {
             const int c = sc + lane * RS + 34;
 #pragma unroll
-            for (int q = 0; q < 8; ++q) {
+            for (int q = 0; q < NV; ++q) {
               const double a = W[q * QS + c - 1], b = W[q * QS + c], cc = W[q * QS + c + 1];
               XR[q * XS + lane] = b - half_slope(limiter, hbeta, cc - b, b - a);
             }
@@ -329,7 +339,7 @@ __global__ void __launch_bounds__(32 * (TY + 1), MINB) stage3d_kernel(const __gr
             const int row = min(lane & 15, TY - 1), half = lane >> 4;
             const int c = sc + row * RS + 1 + half;
 #pragma unroll
-            for (int r = 0; r < 8; ++r) {
+            for (int r = 0; r < NV; ++r) {
               const double a = W[r * QS + c - 1], b = W[r * QS + c], cc = W[r * QS + c + 1];
               const double hs = half_slope(limiter, hbeta, cc - b, b - a);
               L[r] = b + hs;
@@ -341,8 +351,8 @@ __global__ void __launch_bounds__(32 * (TY + 1), MINB) stage3d_kernel(const __gr
           // row -1: flux through face y = -1/2
           const int cm = hb + lane + 2, c0r = hb + RS + lane + 2, cp = sc + lane + 2;
 #pragma unroll
-          for (int r = 0; r < 8; ++r) {
-            const int v = rot_var(r, 1);
+          for (int r = 0; r < NV; ++r) {
+            const int v = rv(r, 1);
             const double a = W[v * QS + cm], b = W[v * QS + c0r], c = W[v * QS + cp];
             L[r] = b + half_slope(limiter, hbeta, c - b, b - a);
             R[r] = YR[v * YS + lane];
@@ -352,20 +362,32 @@ __global__ void __launch_bounds__(32 * (TY + 1), MINB) stage3d_kernel(const __gr
       }
 
       // ------------------------------------------------------------------ A3 + A4: the one Riemann call site
-      if (flux) riemann_flux<RIEMANN, false>(P.ph, L, R, nullptr, F);
+      if (GLM && flux) {
+        // (B_n, psi) at the face from the 2x2 linear Riemann problem (speeds -+c_h); the MHD solver sees B_n* on
+        // both sides, and  F[B_n] = psi*,  F[psi] = c_h^2 B_n*   (rotated slot 5 = B_n in every task)
+        const double bns = 0.5 * (L[5] + R[5]) - 0.5 * (R[NV - 1] - L[NV - 1]) * ich;
+        const double pss = 0.5 * (L[NV - 1] + R[NV - 1]) - 0.5 * ch * (R[5] - L[5]);
+        L[5] = bns; R[5] = bns;
+        riemann_flux<RIEMANN, false>(P.ph, L, R, nullptr, F);
+        F[5] = pss;
+        F[NV - 1] = ch * ch * bns;
+      } else if (flux) {
+        riemann_flux<RIEMANN, false>(P.ph, L, R, nullptr, F);
+      }
 
       // ------------------------------------------------------------------ consume the flux of task s
       if (owner) {
         if (s == 0) {
           // A5 (z) + A6: plane k-1 is complete;  the accumulator of plane k starts with its low z face
           double* po = P.Uout + gm;                                       // own cell of plane k-1
-          double o[8];
+          double o[NV];
 #pragma unroll
-          for (int v = 0; v < 8; ++v, po += P.sq) {
-            constexpr int inv2[8] = {0, 2, 3, 1, 4, 6, 7, 5};             // rot_var(inv2[v], 2) == v
+          for (int v = 0; v < NV; ++v, po += P.sq) {
+            constexpr int inv2[9] = {0, 2, 3, 1, 4, 6, 7, 5, 8};          // rv(inv2[v], 2) == v
             const int r = inv2[v];
             // the difference is formed before it meets U, so that a uniform state stays bitwise fixed (pin P1)
             o[v] = c0 * (acc[v] - cz * (F[r] - FzL[v * ZS + tid]));
+            if (GLM && v == NV - 1) o[v] *= decay;                        // eq.11's source, integrated exactly
             if (emit && cell_ok) *po = o[v];
             FzL[v * ZS + tid] = F[r];
             acc[v] = 0.0;
@@ -380,8 +402,8 @@ __global__ void __launch_bounds__(32 * (TY + 1), MINB) stage3d_kernel(const __gr
             const int cm = (wid == 0) ? hb + RS + lane + 2 : c - RS;
             const int cp = (wid == TY - 1) ? hb + 2 * RS + lane + 2 : c + RS;
 #pragma unroll
-            for (int r = 0; r < 8; ++r) {
-              const int v = rot_var(r, 1);
+            for (int r = 0; r < NV; ++r) {
+              const int v = rv(r, 1);
               const double a = W[v * QS + cm], b = W[v * QS + c], cc = W[v * QS + cp];
               const double hs = half_slope(limiter, hbeta, cc - b, b - a);
               YR[v * YS + wid * 32 + lane] = b - hs;
@@ -391,7 +413,7 @@ __global__ void __launch_bounds__(32 * (TY + 1), MINB) stage3d_kernel(const __gr
             const double* pa = P.Uin + gm + P.sz;
             const double* pb = P.U0 + gm + P.sz;
 #pragma unroll
-            for (int q = 0; q < 8; ++q, pa += P.sq, pb += P.sq) {
+            for (int q = 0; q < NV; ++q, pa += P.sq, pb += P.sq) {
               ua[q] = cell_ok ? __ldg(pa) : 0.0;
               ub[q] = (cell_ok && two) ? *pb : 0.0;
             }
@@ -399,11 +421,11 @@ __global__ void __launch_bounds__(32 * (TY + 1), MINB) stage3d_kernel(const __gr
         } else if (full) {
           if (s == 1) {
 #pragma unroll
-            for (int r = 0; r < 8; ++r) YF[r * YS + (wid + 1) * 32 + lane] = F[r];
+            for (int r = 0; r < NV; ++r) YF[r * YS + (wid + 1) * 32 + lane] = F[r];
           } else {
             // A5 (x): low-face flux from lane i-1 (lane 0: from H)
 #pragma unroll
-            for (int r = 0; r < 8; ++r) {
+            for (int r = 0; r < NV; ++r) {
               const double fl = __shfl_up_sync(0xffffffffu, F[r], 1);
               acc[r] -= cx * (F[r] - ((lane == 0) ? XF[r * XS + wid] : fl));
             }
@@ -413,7 +435,7 @@ __global__ void __launch_bounds__(32 * (TY + 1), MINB) stage3d_kernel(const __gr
             // lane per 64 bytes)
             if (two && cell_ok && (lane & 7) == 0 && k + 1 < k1) {
 #pragma unroll
-              for (int q = 0; q < 8; ++q) prefetch_l2(P.U0 + q * P.sq + gm + 2 * P.sz);
+              for (int q = 0; q < NV; ++q) prefetch_l2(P.U0 + q * P.sq + gm + 2 * P.sz);
             }
           }
         }
@@ -421,12 +443,12 @@ __global__ void __launch_bounds__(32 * (TY + 1), MINB) stage3d_kernel(const __gr
         if (s == 0) {
           if (full && lane < 16 && lane < TY) {
 #pragma unroll
-            for (int r = 0; r < 8; ++r) XF[r * XS + lane] = F[r];
+            for (int r = 0; r < NV; ++r) XF[r * XS + lane] = F[r];
           }
         } else if (s == 1) {
           if (full) {
 #pragma unroll
-            for (int r = 0; r < 8; ++r) YF[r * YS + lane] = F[r];
+            for (int r = 0; r < NV; ++r) YF[r * YS + lane] = F[r];
           }
         } else {
           // A1 for the halo cells of plane k+1 (copies issued one phase B ago), then the copies for plane k+2
