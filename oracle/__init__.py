@@ -21,6 +21,7 @@ _HDR = os.path.join(_HERE, "agate_ref.h")
 _LIB = os.path.join(_HERE, "libagate_ref.so")
 
 IDEAL, HALL = 0, 1
+CGL = 2              # CGL MHD: 9 variables per cell, U = (rho, m, E, B, A_log), W = (rho, v, p_par, B, p_perp) (R24)
 IDEAL_GLM = 3        # ideal MHD + GLM divergence cleaning: 9 variables per cell, psi last (eqs.10-11; R22)
 HLL, HLLD = 0, 1
 
@@ -45,7 +46,7 @@ class Grid(C.Structure):
 
 class SolverCfg(C.Structure):
     _fields_ = [("riemann", C.c_int32), ("limiter", C.c_int32), ("beta", C.c_double),
-                ("rk", C.c_int32), ("cfl", C.c_double), ("d_i", C.c_double)]
+                ("rk", C.c_int32), ("cfl", C.c_double), ("d_i", C.c_double), ("relax", C.c_double)]
 
 
 _lib = None
@@ -66,6 +67,16 @@ def lib():
         L.agate_ref_get_state.argtypes = [vp, _dp, _dp]
         L.agate_ref_rhs.argtypes = [vp, _dp]
         L.agate_ref_destroy.argtypes = [vp]
+        L.agate_ref_cgl_cons_to_prim.argtypes = [_dp, _dp]
+        L.agate_ref_cgl_cons_to_prim.restype = None
+        L.agate_ref_cgl_prim_to_cons.argtypes = [_dp, _dp]
+        L.agate_ref_cgl_prim_to_cons.restype = None
+        L.agate_ref_cgl_cfast.argtypes = [C.c_int, _dp]
+        L.agate_ref_cgl_cfast.restype = C.c_double
+        L.agate_ref_cgl_face_flux.argtypes = [C.c_int, _dp, _dp, _dp]
+        L.agate_ref_cgl_face_flux.restype = None
+        L.agate_ref_cgl_relax.argtypes = [C.c_double, C.c_double, _dp, _dp]
+        L.agate_ref_cgl_relax.restype = None
         L.agate_ref_nvar.argtypes = [vp]
         L.agate_ref_nvar.restype = C.c_int
         L.agate_ref_glm_ch.argtypes = [vp, _dp]
@@ -151,6 +162,31 @@ def face_flux(riemann, d, gamma, WL, WR, eqset=IDEAL, d_i=0.0, dxmin=1.0, J=None
     return F
 
 
+def cgl_cons_to_prim(U):
+    u, pu = _vec(U, 9); W = np.empty(9)
+    lib().agate_ref_cgl_cons_to_prim(pu, W.ctypes.data_as(_dp)); return W
+
+
+def cgl_prim_to_cons(W):
+    w, pw = _vec(W, 9); U = np.empty(9)
+    lib().agate_ref_cgl_prim_to_cons(pw, U.ctypes.data_as(_dp)); return U
+
+
+def cgl_cfast(d, W):
+    w, pw = _vec(W, 9); return float(lib().agate_ref_cgl_cfast(int(d), pw))
+
+
+def cgl_face_flux(d, WL, WR):
+    wl, pl = _vec(WL, 9); wr, pr = _vec(WR, 9); F = np.empty(9)
+    lib().agate_ref_cgl_face_flux(int(d), pl, pr, F.ctypes.data_as(_dp)); return F
+
+
+def cgl_relax(f, B2, ppar, pperp):
+    a, b = C.c_double(ppar), C.c_double(pperp)
+    lib().agate_ref_cgl_relax(float(f), float(B2), C.byref(a), C.byref(b))
+    return a.value, b.value
+
+
 def glm_face(ch, bnL, bnR, psL, psR):
     """(B_n*, psi*) of the 2x2 linear GLM Riemann problem at one face."""
     a, b = C.c_double(), C.c_double()
@@ -174,11 +210,11 @@ class RefSolver:
     """Host-memory solver with the same call shape as the product's C-ABI (agate_ref_* functions)."""
 
     def __init__(self, shape, dx, ndim, gamma=5.0 / 3.0, eqset=IDEAL, riemann=HLL, limiter=2, beta=1.3,
-                 rk=2, cfl=0.0, d_i=0.0):
+                 rk=2, cfl=0.0, d_i=0.0, relax=0.0):
         nx, ny, nz = (int(s) for s in shape)
         self.shape = (nx, ny, nz)
         self.grid = Grid(ndim, nx, ny, nz, dx[0], dx[1], dx[2])
-        self.cfg = SolverCfg(riemann, limiter, beta, rk, cfl, d_i)
+        self.cfg = SolverCfg(riemann, limiter, beta, rk, cfl, d_i, relax)
         self.gamma, self.eqset = float(gamma), int(eqset)
         self._h = C.c_void_p()
         rc = lib().agate_ref_create(C.byref(self.grid), self.gamma, self.eqset, C.byref(self.cfg), C.byref(self._h))

@@ -69,6 +69,10 @@ inline double val(double x) { return x; }
 inline double val(Counted x) { return x.v; }
 inline double tsqrt(double x) { return std::sqrt(x); }
 inline Counted tsqrt(Counted x) { g_ops.sqrt++; return Counted(std::sqrt(x.v)); }
+inline double texp(double x) { return std::exp(x); }
+inline Counted texp(Counted x) { g_ops.sqrt++; return Counted(std::exp(x.v)); }     // transcendental: counted with sqrt
+inline double tlog(double x) { return std::log(x); }
+inline Counted tlog(Counted x) { g_ops.sqrt++; return Counted(std::log(x.v)); }
 inline double tabs(double x) { return std::fabs(x); }
 inline Counted tabs(Counted x) { return Counted(std::fabs(x.v)); }
 template <class T> inline T tmin(T a, T b) { return (b < a) ? b : a; }
@@ -271,6 +275,81 @@ int flux_hlld(int n, double gamma, const T WLin[8], const T WRin[8], T F[8]) {
   return 3 + degenerate;
 }
 
+// ------------------------------------------------------------------------------------------------
+// CGL MHD (NEXT-2; R24).  Nine variables per cell:
+//   U = (rho, m, E, B, A_log)   with  E = rho v^2/2 + B^2/2 + p_par/2 + p_perp  and
+//                                     A_log = rho log[(rho^2/B^3)(p_perp/p_par)]      (eq.18)
+//   W = (rho, v, p_par, B, p_perp)    (p_par in slot 4, p_perp in slot 8)
+// ------------------------------------------------------------------------------------------------
+// eqs.26-27 (log form):  X = rho^2 exp(-A/rho);  p_par = 2 X e/(X + 2B^3),  p_perp = 2 B^3 e/(X + 2B^3)
+template <class T> void cgl_cons_to_prim(const T U[9], T W[9]) {
+  T rho = U[0];
+  T vx = U[1] / rho, vy = U[2] / rho, vz = U[3] / rho;
+  T v2 = vx * vx + vy * vy + vz * vz;
+  T b2 = U[5] * U[5] + U[6] * U[6] + U[7] * U[7];
+  T eint = U[4] - T(0.5) * rho * v2 - T(0.5) * b2;
+  T B3 = b2 * tsqrt(b2);
+  T X = rho * rho * texp(-U[8] / rho);
+  T den = X + T(2.0) * B3;
+  W[0] = rho; W[1] = vx; W[2] = vy; W[3] = vz;
+  W[4] = T(2.0) * X * eint / den;
+  W[5] = U[5]; W[6] = U[6]; W[7] = U[7];
+  W[8] = T(2.0) * B3 * eint / den;
+}
+template <class T> void cgl_prim_to_cons(const T W[9], T U[9]) {
+  T rho = W[0];
+  T v2 = W[1] * W[1] + W[2] * W[2] + W[3] * W[3];
+  T b2 = W[5] * W[5] + W[6] * W[6] + W[7] * W[7];
+  U[0] = rho; U[1] = rho * W[1]; U[2] = rho * W[2]; U[3] = rho * W[3];
+  U[4] = T(0.5) * rho * v2 + T(0.5) * b2 + T(0.5) * W[4] + W[8];
+  U[5] = W[5]; U[6] = W[6]; U[7] = W[7];
+  U[8] = rho * tlog((rho * rho / (b2 * tsqrt(b2))) * (W[8] / W[4]));
+}
+// eq.29, fast (+) branch, along direction d:  c^2 = (b1 + sqrt(b2^2 + c)) / (2 rho)
+template <class T> T cgl_cfast(int d, const T W[9]) {
+  T B2 = W[5] * W[5] + W[6] * W[6] + W[7] * W[7];
+  T cos2 = W[5 + d] * W[5 + d] / B2;
+  T b1 = B2 + T(2.0) * W[8] + cos2 * (T(2.0) * W[4] - W[8]);
+  T b2 = b1 - T(6.0) * cos2 * W[4];
+  T c = T(4.0) * W[8] * W[8] * cos2 * (T(1.0) - cos2);
+  return tsqrt((b1 + tsqrt(b2 * b2 + c)) / (T(2.0) * W[0]));
+}
+// eqs.19-22 with psi == 0 and eq.17 for A, along direction n;  Theta = 1 - (p_par - p_perp)/B^2
+template <class T> void cgl_phys_flux(int n, const T W[9], const T U[9], T F[9]) {
+  T B2 = W[5] * W[5] + W[6] * W[6] + W[7] * W[7];
+  T th = T(1.0) - (W[4] - W[8]) / B2;
+  T vn = W[1 + n], bn = W[5 + n];
+  T v2 = W[1] * W[1] + W[2] * W[2] + W[3] * W[3];
+  T vB = W[1] * W[5] + W[2] * W[6] + W[3] * W[7];
+  F[0] = W[0] * vn;
+  for (int c = 0; c < 3; ++c) F[1 + c] = W[0] * W[1 + c] * vn - th * W[5 + c] * bn;
+  F[1 + n] += W[8] + T(0.5) * B2;
+  F[4] = (T(0.5) * W[0] * v2 + T(0.5) * W[4] + T(2.0) * W[8] + B2) * vn - th * vB * bn;
+  for (int c = 0; c < 3; ++c) F[5 + c] = vn * W[5 + c] - bn * W[1 + c];
+  F[5 + n] = T(0.0);
+  F[8] = U[8] * vn;
+}
+// HLL eq.5 with the Davis speeds eq.6 and c = eq.29's fast speed; all nine components through eq.5
+template <class T> void cgl_flux_hll(int n, const T WL[9], const T WR[9], T F[9]) {
+  T UL[9], UR[9], fL[9], fR[9];
+  cgl_prim_to_cons(WL, UL); cgl_prim_to_cons(WR, UR);
+  cgl_phys_flux(n, WL, UL, fL); cgl_phys_flux(n, WR, UR, fR);
+  T cl = cgl_cfast(n, WL), cr = cgl_cfast(n, WR);
+  T sL = tmin(tmin(WL[1 + n] - cl, WR[1 + n] - cr), T(0.0));
+  T sR = tmax(tmax(WL[1 + n] + cl, WR[1 + n] + cr), T(0.0));
+  for (int q = 0; q < 9; ++q) F[q] = (sR * fL[q] - sL * fR[q] + sL * sR * (UR[q] - UL[q])) / (sR - sL);
+}
+// eqs.31-33: relaxation of the anisotropy dP = p_perp - p_par towards the stable range, at constant
+// (p_par + 2 p_perp)/3; f = dt/(dt + tau) (paper default 0.99), C1 = 0.3, C2 = 0.5
+inline void cgl_relax(double f, double B2, double* ppar, double* pperp) {
+  const double dP = *pperp - *ppar;
+  const double mirror = (*ppar / *pperp) * B2 / 2.0;
+  const double ic = 0.3 * *ppar * std::pow(B2 / (2.0 * *ppar), 0.5);
+  const double dPs = std::fmax(-B2, std::fmin(dP, std::fmin(mirror, ic)));
+  *ppar = *ppar - (2.0 / 3.0) * (dPs - dP) * f;
+  *pperp = *pperp + (1.0 / 3.0) * (dPs - dP) * f;
+}
+
 // GLM (eqs.10-11; R22).  Along the face normal, (B_n, psi) obey  dB_n/dt + dpsi/dx = 0,
 // dpsi/dt + c_h^2 dB_n/dx = 0: characteristic variables B_n -+ psi/c_h move at -+c_h, and the state
 // on the face (x/t = 0) is
@@ -305,6 +384,7 @@ template <class T> struct Solver {
   double dxmin, cfl;
   int nv;               // variables per cell: 8, or 9 with the GLM scalar psi (index 8) behind the MHD ones
   bool glm;
+  bool cgl = false;
   double ch = 0.0;      // GLM: c_h of the step being taken (R22: 0.95 v_max(U^n))
   std::vector<T> Un, U1, W, L;
   double t = 0.0;
@@ -323,7 +403,8 @@ template <class T> struct Solver {
     cfl = s.cfl;
     if (!(cfl > 0.0)) cfl = (g.ndim == 1) ? 0.8 : (g.ndim == 2 ? 0.45 : 0.325);
     glm = (eqset == AGATE_REF_IDEAL_GLM);
-    nv = glm ? 9 : 8;
+    cgl = (eqset == AGATE_REF_CGL);
+    nv = (glm || cgl) ? 9 : 8;
     Un.assign(nv * ntot, T(0.0)); U1.assign(nv * ntot, T(0.0)); W.assign(nv * ntot, T(0.0));
     L.assign(nv * nint, T(0.0));
   }
@@ -348,6 +429,13 @@ template <class T> struct Solver {
   void primitives(const std::vector<T>& U) {
 #pragma omp parallel for num_threads(g_threads) if (g_threads > 1)
     for (ptrdiff_t c = 0; c < (ptrdiff_t)ntot; ++c) {
+      if (cgl) {
+        T u9[9], w9[9];
+        for (int q = 0; q < 9; ++q) u9[q] = U[q * ntot + c];
+        cgl_cons_to_prim(u9, w9);
+        for (int q = 0; q < 9; ++q) W[q * ntot + c] = w9[q];
+        continue;
+      }
       T u[8], w[8];
       for (int q = 0; q < 8; ++q) u[q] = U[q * ntot + c];
       cons_to_prim(gamma, u, w);
@@ -399,7 +487,9 @@ template <class T> struct Solver {
             WR[q] = Wq[(c + 1) * sd] - T(0.5) * dW[q * (n + 2) + (c + 2)];       // eq.3
           }
           if (hall) face_current(d, base + c * sd, J);
-          if (glm) {
+          if (cgl) {
+            cgl_flux_hll<T>(d, WL, WR, Ff);
+          } else if (glm) {
             // eqs.10-11 (R22): (B_n, psi) decouple into a 2x2 linear system with speeds -+c_h; its Riemann
             // solution gives the single-valued face values, the MHD solver sees B_n* on both sides, and the two
             // GLM fluxes are  F[B_n] = psi*,  F[psi] = c_h^2 B_n*.
@@ -437,9 +527,19 @@ template <class T> struct Solver {
     for (int k = 0; k < nd[2]; ++k)
       for (int j = 0; j < nd[1]; ++j)
         for (int i = 0; i < nd[0]; ++i) {
-          T u[8], w[8];
+          T u[9], w[9];
           const ptrdiff_t c = pidx(i, j, k);
-          for (int q = 0; q < 8; ++q) u[q] = Un[q * ntot + c];
+          for (int q = 0; q < nv; ++q) u[q] = Un[q * ntot + c];
+          if (cgl) {
+            // eq.28: |v| + max_d c_cgl,d
+            cgl_cons_to_prim(u, w);
+            if (!(val(w[0]) > 0.0) || !(val(w[4]) > 0.0) || !(val(w[8]) > 0.0)) { bad = true; continue; }
+            T cm = tmax(tmax(cgl_cfast(0, w), cgl_cfast(1, w)), cgl_cfast(2, w));
+            T spc = tsqrt(w[1] * w[1] + w[2] * w[2] + w[3] * w[3]) + cm;
+            if (!std::isfinite(val(spc))) { bad = true; continue; }
+            vm = tmax(vm, spc);
+            continue;
+          }
           cons_to_prim(gamma, u, w);
           if (!(val(w[0]) > 0.0) || !(val(w[4]) > 0.0)) { bad = true; continue; }
           T cmax = tmax(tmax(cfast(0, gamma, w), cfast(1, gamma, w)), cfast(2, gamma, w));
@@ -469,6 +569,22 @@ template <class T> struct Solver {
       Un[p] = Un[p] * decay;
     }
   }
+  // CGL (R24): after the Runge-Kutta update every cell's anisotropy is relaxed (eqs.31-33) with
+  // f = dt/(dt+tau) = s.relax (0 = off); the total energy is unchanged, only A_log moves.
+  void cgl_source() {
+    if (!(s.relax > 0.0)) return;
+    for (int k = 0; k < nd[2]; ++k) for (int j = 0; j < nd[1]; ++j) for (int i = 0; i < nd[0]; ++i) {
+      const ptrdiff_t c = pidx(i, j, k);
+      T u[9], w[9];
+      for (int q = 0; q < 9; ++q) u[q] = Un[q * ntot + c];
+      cgl_cons_to_prim(u, w);
+      double ppar = val(w[4]), pperp = val(w[8]);
+      const double B2 = val(w[5] * w[5] + w[6] * w[6] + w[7] * w[7]);
+      cgl_relax(s.relax, B2, &ppar, &pperp);
+      const double rho = val(w[0]);
+      Un[8 * ntot + c] = T(rho * std::log((rho * rho / (B2 * std::sqrt(B2))) * (pperp / ppar)));
+    }
+  }
   void step(double dt) {
     if (glm) { double vm = 0.0; vmax(&vm); ch = 0.95 * vm; }
     fill_ghosts(Un);
@@ -479,6 +595,7 @@ template <class T> struct Solver {
         Un[p] = Un[p] + T(dt) * L[q * nint + iidx(i, j, k)];
       }
       if (glm) glm_source(dt);
+      if (cgl) cgl_source();
       t += dt;
       return;
     }
@@ -493,6 +610,7 @@ template <class T> struct Solver {
       Un[p] = T(0.5) * Un[p] + T(0.5) * (U1[p] + T(dt) * L[q * nint + iidx(i, j, k)]);   // stage 2
     }
     if (glm) glm_source(dt);
+    if (cgl) cgl_source();
     t += dt;
   }
 
@@ -515,7 +633,9 @@ int check_args(const agate_ref_grid* g, double gamma, int eqset, const agate_ref
   if (g->ndim < 2 && g->ny != 1) return 1;
   if (!(g->dx > 0.0) || (g->ndim >= 2 && !(g->dy > 0.0)) || (g->ndim >= 3 && !(g->dz > 0.0))) return 1;
   if (!(gamma > 1.0)) return 1;
-  if (eqset != AGATE_REF_IDEAL && eqset != AGATE_REF_HALL && eqset != AGATE_REF_IDEAL_GLM) return 1;
+  if (eqset != AGATE_REF_IDEAL && eqset != AGATE_REF_HALL && eqset != AGATE_REF_IDEAL_GLM && eqset != AGATE_REF_CGL) return 1;
+  if (eqset == AGATE_REF_CGL && s->riemann != 0) return 1;          // the paper's CGL runs use HLL
+  if (eqset == AGATE_REF_CGL && !(s->relax >= 0.0 && s->relax <= 1.0)) return 1;
   if (s->riemann < 0 || s->riemann > 1 || s->limiter < 0 || s->limiter > 2 || s->rk < 1 || s->rk > 2) return 1;
   if (s->limiter == 2 && !(s->beta >= 1.0 && s->beta <= 2.0)) return 1;
   if (eqset == AGATE_REF_HALL && s->riemann == 1) return 1;        // no Hall-HLLD in the paper
@@ -603,6 +723,11 @@ int agate_ref_rhs(agate_ref_ctx* c, double* Lout) {
   std::memcpy(Lout, c->s->L.data(), sizeof(double) * c->s->nv * c->s->nint);
   return 0;
 }
+void agate_ref_cgl_cons_to_prim(const double U[9], double W[9]) { cgl_cons_to_prim<double>(U, W); }
+void agate_ref_cgl_prim_to_cons(const double W[9], double U[9]) { cgl_prim_to_cons<double>(W, U); }
+double agate_ref_cgl_cfast(int dir, const double W[9]) { return cgl_cfast<double>(dir, W); }
+void agate_ref_cgl_face_flux(int dir, const double WL[9], const double WR[9], double F[9]) { cgl_flux_hll<double>(dir, WL, WR, F); }
+void agate_ref_cgl_relax(double f, double B2, double* ppar, double* pperp) { cgl_relax(f, B2, ppar, pperp); }
 int agate_ref_nvar(agate_ref_ctx* c) { return c ? c->s->nv : 0; }
 int agate_ref_glm_ch(agate_ref_ctx* c, double* ch_out) {
   if (!c || !ch_out) return 1;

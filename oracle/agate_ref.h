@@ -34,9 +34,13 @@ typedef struct {
   int32_t rk;            /* 1 = RK11 (forward Euler), 2 = SSP-RK2 (R11) */
   double  cfl;           /* Courant C; <=0 -> paper default 0.8/0.45/0.325 (L73) */
   double  d_i;           /* normalised ion inertial length (Hall) */
+  double  relax;         /* CGL: dt/(dt+tau) of eqs.32-33 (paper default 0.99, L254); 0 = no relaxation */
 } agate_ref_solver;
 
-enum { AGATE_REF_IDEAL = 0, AGATE_REF_HALL = 1, AGATE_REF_IDEAL_GLM = 3 };
+enum { AGATE_REF_IDEAL = 0, AGATE_REF_HALL = 1, AGATE_REF_CGL = 2, AGATE_REF_IDEAL_GLM = 3 };
+/* AGATE_REF_CGL (R24): 9 variables, U = (rho, m, E, B, A_log) with eq.18's A_log,
+ * W = (rho, v, p_par, B, p_perp); fluxes eqs.19-22 + eq.17, HLL only, speeds eq.29, dt eq.28, relaxation eqs.31-33
+ * after the Runge-Kutta update. */
 /* AGATE_REF_IDEAL_GLM (eqs.10-11; R22): 9 variables per cell, the GLM scalar psi
  * last: U[9][nz][ny][nx].  c_h = 0.95 v_max(U^n) per step, c_p^2 = 0.18 c_h; face (B_n, psi) from the 2x2
  * linear Riemann problem; psi <- psi exp(-dt c_h^2/c_p^2) after the Runge-Kutta update. */
@@ -50,6 +54,11 @@ int agate_ref_advance(agate_ref_ctx*, int32_t n_steps, double* t_out);    /* n s
 int agate_ref_get_state(agate_ref_ctx*, double* U_out, double* t_out);
 int agate_ref_rhs(agate_ref_ctx*, double* L_out);                         /* L(U) of eq.1, interior SoA */
 int agate_ref_vmax(agate_ref_ctx*, double* vmax_out);                     /* max_i(|v_i|+c_i) (L156)    */
+void   agate_ref_cgl_cons_to_prim(const double U[9], double W[9]);                      /* eqs.26-27 */
+void   agate_ref_cgl_prim_to_cons(const double W[9], double U[9]);                      /* L166, eq.18 */
+double agate_ref_cgl_cfast(int dir, const double W[9]);                                 /* eq.29 (+) */
+void   agate_ref_cgl_face_flux(int dir, const double WL[9], const double WR[9], double F[9]);
+void   agate_ref_cgl_relax(double f, double B2, double* p_par, double* p_perp);         /* eqs.31-33 */
 int agate_ref_nvar(agate_ref_ctx*);                                       /* 8, or 9 with GLM          */
 int agate_ref_glm_ch(agate_ref_ctx*, double* ch_out);                     /* c_h of the last step / rhs */
 void agate_ref_glm_face(double ch, double bnL, double bnR, double psL, double psR, double* bn_star, double* psi_star);

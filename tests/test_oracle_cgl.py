@@ -1,0 +1,204 @@
+"""Pins of the oracle's CGL MHD (NEXT-2; eqs.14-33, benchmarks L296, L318-334; R24).
+
+Hand values of the variable changes, textbook limits and the paper's printed number for eq.29, the paper's three CGL
+benchmarks (standing wave period, propagating wave speeds 5 +- 16.09, firehose growth rate 1.0472), the reduction to
+ideal MHD at zero anisotropy, conservation, and the relaxation step's defining properties.
+"""
+import numpy as np
+import pytest
+
+import oracle
+
+G = 5.0 / 3.0
+
+
+def cons_line(W):
+    return np.stack([oracle.cgl_prim_to_cons(W[:, i]) for i in range(W.shape[1])], axis=1)
+
+
+def solver_1d(n, length, relax=0.0, **kw):
+    return oracle.RefSolver(shape=(n, 1, 1), dx=(length / n, 1, 1), ndim=1, eqset=oracle.CGL, riemann=oracle.HLL,
+                            beta=1.3, relax=relax, **kw)
+
+
+def run_to(s, t_end):
+    t = 0.0
+    while t < t_end - 1e-14:
+        dt = min(s.compute_dt(), t_end - t)
+        s.step(dt)
+        t += dt
+
+
+def test_c1_variable_change_by_hand():
+    """rho = 2, |B| = 2 (B^3 = 8), p_perp/p_par = 2: (rho^2/B^3)(p_perp/p_par) = 1 so A_log = rho log 1 = 0 (eq.18);
+    E = rho v^2/2 + B^2/2 + p_par/2 + p_perp = 1 + 2 + 0.75 + 3 = 6.75.  And back (eqs.26-27)."""
+    W = np.array([2.0, 1.0, 0.0, 0.0, 1.5, 0.0, 2.0, 0.0, 3.0])
+    U = oracle.cgl_prim_to_cons(W)
+    assert U[8] == 0.0 and U[4] == 6.75 and U[1] == 2.0
+    assert np.allclose(oracle.cgl_cons_to_prim(U), W, rtol=1e-15, atol=1e-15)
+    # eq.16 vs eq.18: A_log = rho log( A / rho ) with A = (rho/B)^3 p_perp/p_par
+    W2 = np.array([1.3, 0.2, -0.4, 0.1, 0.7, 0.3, -0.8, 0.5, 1.9])
+    B = np.sqrt(0.3 ** 2 + 0.8 ** 2 + 0.5 ** 2)
+    A = (1.3 / B) ** 3 * 1.9 / 0.7
+    U2 = oracle.cgl_prim_to_cons(W2)
+    assert abs(U2[8] - 1.3 * np.log(A / 1.3)) <= 1e-14
+    assert np.allclose(oracle.cgl_cons_to_prim(U2), W2, rtol=1e-14, atol=1e-15)
+
+
+def test_c2_magnetosonic_speeds():
+    """eq.29 (+): the paper's propagating-wave state gives 16.09; perpendicular propagation gives
+    sqrt((B^2 + 2 p_perp)/rho); parallel propagation gives the larger of the CGL parallel sound speed
+    sqrt(3 p_par/rho) and the firehose-modified Alfven speed sqrt((B^2 + p_perp - p_par)/rho) (textbook CGL)."""
+    W = np.array([1, 5, 0, 0, 14, 0, 15, 0, 17.0])
+    assert abs(oracle.cgl_cfast(0, W) - 16.09) < 0.005
+    assert abs(oracle.cgl_cfast(0, W) - np.sqrt(15 ** 2 + 2 * 17)) <= 1e-13
+    for ppar, pperp, B in [(1.0, 2.0, 3.0), (5.0, 0.5, 1.0), (0.3, 0.3, 0.2)]:
+        Wp = np.array([0.8, 0, 0, 0, ppar, B, 0, 0, pperp])
+        want = np.sqrt(max(3 * ppar, B * B + pperp - ppar) / 0.8)
+        assert abs(oracle.cgl_cfast(0, Wp) - want) <= 1e-13 * want
+        # the same state seen along y and z is perpendicular
+        assert abs(oracle.cgl_cfast(1, Wp) - np.sqrt((B * B + 2 * pperp) / 0.8)) <= 1e-13
+        assert abs(oracle.cgl_cfast(2, Wp) - np.sqrt((B * B + 2 * pperp) / 0.8)) <= 1e-13
+
+
+@pytest.mark.parametrize("d", [0, 1, 2])
+def test_c3_zero_anisotropy_flux_is_ideal_mhd(d):
+    """with p_par = p_perp = p the CGL equations are ideal MHD with gamma = 5/3 (E carries 3p/2, the
+    enthalpy term 5p/2, Theta = 1).  HLL of two equal states is the physical flux, so the first 8 components must
+    be eqs.7-10's flux and the ninth A v_n."""
+    rng = np.random.default_rng(5 + d)
+    for _ in range(20):
+        W8 = np.concatenate([[0.5 + rng.random()], rng.normal(size=3), [0.2 + rng.random()], rng.normal(size=3)])
+        W9 = np.concatenate([W8, [W8[4]]])
+        F9 = oracle.cgl_face_flux(d, W9, W9)
+        F8 = oracle.phys_flux(d, G, W8)
+        assert np.max(np.abs(F9[:8] - F8)) <= 1e-13 * max(1.0, np.max(np.abs(F8)))
+        assert abs(F9[8] - oracle.cgl_prim_to_cons(W9)[8] * W8[1 + d]) <= 1e-13 * max(1.0, abs(F9[8]))
+
+
+@pytest.mark.parametrize("ap", [0.5, 1.0, 2.0])
+def test_c4_standing_wave_period(ap):
+    """rho = 1, B_y = 1, P = 0.5, v_x = 0.01 sin(2 pi x) on [-1, 1], N = 256, no relaxation; the wave
+    oscillates with period tau = lambda / c_ms, c_ms = sqrt(B^2 + 2 p_perp), lambda = 1: after tau/2 the velocity
+    pattern is reversed, after tau it is back."""
+    n = 256
+    x = -1 + (np.arange(n) + 0.5) * 2 / n
+    ppar = 1.5 / (1 + 2 * ap)
+    pperp = ap * ppar
+    W = np.zeros((9, n)); W[0] = 1; W[6] = 1; W[4] = ppar; W[8] = pperp; W[1] = 0.01 * np.sin(2 * np.pi * x)
+    s = solver_1d(n, 2.0)
+    s.set_state(cons_line(W).reshape(9, 1, 1, n))
+    tau = 1.0 / np.sqrt(1 + 2 * pperp)
+    proj = lambda: float(np.sum((s.get_state()[1] / s.get_state()[0]).ravel() * np.sin(2 * np.pi * x)))
+    a0 = proj()
+    run_to(s, tau / 2); a1 = proj()
+    run_to(s, tau / 2); a2 = proj()
+    assert -1.0 <= a1 / a0 <= -0.995
+    assert 0.995 <= a2 / a0 <= 1.0
+
+
+def test_c5_propagating_wave_speeds():
+    """the perturbation splits into fast waves at v_x +- 16.09 and a slow one at v_x = 5; at t = 1 the
+    B_y pulses sit at 21.09 and -11.09 and the density pulse that stays with the flow at 5."""
+    n = 600
+    x = -30 + (np.arange(n) + 0.5) * 60 / n
+    W = np.zeros((9, n)); W[0] = 1; W[1] = 5; W[6] = 15; W[4] = 14; W[8] = 17
+    m = np.abs(x) < 3
+    c = np.cos(2 * np.pi * x / 12)
+    W[0] += m * 0.01 * c; W[4] += m * 0.14 * c; W[8] += m * 0.17 * c; W[6] += m * 0.15 * c
+    s = solver_1d(n, 60.0)
+    s.set_state(cons_line(W).reshape(9, 1, 1, n))
+    run_to(s, 1.0)
+    V = s.get_state().reshape(9, n)
+    dBy = V[6] - 15
+    centroid = lambda sel, f: float(np.sum(x[sel] * f[sel]) / np.sum(f[sel]))
+    right, left, mid = (x > 16) & (x < 26), (x > -16) & (x < -6), (x > 1) & (x < 9)
+    assert abs(centroid(right, np.maximum(dBy, 0)) - 21.09) < 0.15
+    assert abs(centroid(left, np.maximum(dBy, 0)) + 11.09) < 0.15
+    # the CGL invariant p_perp/(rho B) (eq.15) is carried by the flow alone: its perturbation sits at x = v_x t = 5
+    Wt = np.stack([oracle.cgl_cons_to_prim(V[:, i]) for i in range(n)], axis=1)
+    inv = Wt[8] / (Wt[0] * np.abs(Wt[6]))
+    assert abs(centroid(mid, np.abs(inv - 17.0 / 15.0)) - 5.0) < 0.1
+    assert np.max(np.abs(inv - 17.0 / 15.0)[~mid]) < 0.02 * np.max(np.abs(inv - 17.0 / 15.0))
+
+
+@pytest.mark.parametrize("scale,t0,t1", [(1.0, 0.0, 0.5), (0.1, 0.0, 1.0), (0.01, 0.0, 0.25)])
+def test_c6_firehose_growth_rate(scale, t0, t1):
+    """rho = 1, B_x = 10, p_par = 104, p_perp = 3 (beyond the firehose threshold), Alfven mode of
+    wavelength 6 on [-6, 6], N = 512, no relaxation: v_y grows as exp(1.0472 t) from t = 0 (the initial phase relation
+    is the growing eigenmode).  With the paper's amplitude the growth is linear only early on (Theta = -0.01, so
+    B_y ~ 0.5 already changes it); smaller amplitudes follow the rate longer, until the grid-scale modes of this
+    ill-posed limit (growth ~ k) take over around t ~ 1.2 -- the deviations the paper mentions."""
+    n = 512
+    x = -6 + (np.arange(n) + 0.5) * 12 / n
+    W = np.zeros((9, n)); W[0] = 1; W[5] = 10; W[4] = 104; W[8] = 3
+    W[2] = scale * 0.01 * np.cos(2 * np.pi * x / 6)
+    W[6] = scale * 0.1 * np.cos(2 * np.pi * x / 6 + np.pi / 2)
+    s = solver_1d(n, 12.0)
+    s.set_state(cons_line(W).reshape(9, 1, 1, n))
+    amp = lambda: abs(np.fft.fft((s.get_state()[2] / s.get_state()[0]).ravel())[2]) / (n / 2)
+    run_to(s, t0); a0 = amp()
+    run_to(s, t1 - t0); a1 = amp()
+    rate = np.log(a1 / a0) / (t1 - t0)
+    assert abs(rate - 1.0472) < 0.03 * 1.0472, rate
+
+
+def _state2d(n, seed):
+    rng = np.random.default_rng(seed)
+    x = (np.arange(n) + 0.5) / n
+    X, Y = np.meshgrid(x, x, indexing="xy")
+    W = np.zeros((9, 1, n, n))
+    W[0] = 1.0 + 0.2 * np.sin(2 * np.pi * X) * np.cos(2 * np.pi * Y)
+    W[1] = 0.3 * np.sin(2 * np.pi * Y); W[2] = -0.3 * np.sin(2 * np.pi * X); W[3] = 0.1 * np.cos(2 * np.pi * (X + Y))
+    W[4] = 0.8 + 0.2 * np.cos(2 * np.pi * X); W[8] = 0.6 + 0.3 * np.sin(2 * np.pi * Y)
+    W[5] = 0.5 - 0.4 * np.sin(2 * np.pi * Y); W[6] = 0.4 * np.sin(4 * np.pi * X); W[7] = 0.2
+    U = np.empty_like(W)
+    for j in range(n):
+        for i in range(n):
+            U[:, 0, j, i] = oracle.cgl_prim_to_cons(W[:, 0, j, i])
+    return U
+
+
+@pytest.mark.parametrize("relax", [0.0, 0.99])
+def test_c7_conservation(relax):
+    """Flux form on a periodic box: every sum is conserved to round-off without relaxation; the relaxation keeps
+    (p_par + 2 p_perp)/3, hence e_int and E, so the first eight sums stay conserved with it too (eqs.32-33)."""
+    n = 20
+    U = _state2d(n, 3)
+    s = oracle.RefSolver(shape=(n, n, 1), dx=(1 / n, 1 / n, 1), ndim=2, eqset=oracle.CGL, riemann=oracle.HLL, beta=1.3,
+                         relax=relax)
+    s.set_state(U)
+    s0 = U.reshape(9, -1).sum(axis=1)
+    s.advance(6)
+    V = s.get_state()
+    s1 = V.reshape(9, -1).sum(axis=1)
+    scale = np.abs(V).reshape(9, -1).sum(axis=1) + 1e-300
+    nq = 9 if relax == 0.0 else 8
+    assert np.all(np.abs(s1[:nq] - s0[:nq]) <= 1e-13 * scale[:nq])
+
+
+def test_c8_relaxation_step():
+    """eqs.31-33 by hand.  Firehose side (the paper's 4.5 state): dP = -101 < -B^2 = -100, so dP* = -100 and with
+    f = 0.99: p_par = 104 - (2/3)(1)(0.99) = 103.34, p_perp = 3 + (1/3)(0.99) = 3.33.  Mirror side: p_par = 1,
+    p_perp = 3, B^2 = 1: mirror bound (1/3)(1/2) = 1/6 < ion-cyclotron bound 0.3 sqrt(1/2); with f = 1 the new
+    anisotropy is exactly the bound (hard wall).  A stable state is untouched; (p_par + 2 p_perp)/3 never moves."""
+    a, b = oracle.cgl_relax(0.99, 100.0, 104.0, 3.0)
+    assert abs(a - 103.34) <= 1e-12 and abs(b - 3.33) <= 1e-12
+    a, b = oracle.cgl_relax(1.0, 1.0, 1.0, 3.0)
+    assert abs((b - a) - 1.0 / 6.0) <= 1e-14
+    assert abs((a + 2 * b) / 3 - 7.0 / 3.0) <= 1e-14
+    assert oracle.cgl_relax(0.99, 4.0, 1.0, 1.2) == (1.0, 1.2)
+    # ion-cyclotron bound binding: p_par = 4, B^2 = 1: 0.3 * 4 * sqrt(1/8) = 0.4243 < mirror (4/p_perp)/2
+    a, b = oracle.cgl_relax(1.0, 1.0, 4.0, 5.0)
+    assert abs((b - a) - 0.3 * 4 * np.sqrt(1 / 8)) <= 1e-14
+
+
+def test_c9_uniform_state_is_fixed_and_hll_rejected_for_hlld():
+    W = np.array([1.1, 0.3, -0.2, 0.1, 0.9, 0.4, 0.2, -0.3, 0.5])
+    U = np.tile(oracle.cgl_prim_to_cons(W)[:, None, None, None], (1, 6, 7, 8))
+    s = oracle.RefSolver(shape=(8, 7, 6), dx=(0.1, 0.1, 0.1), ndim=3, eqset=oracle.CGL, riemann=oracle.HLL, relax=0.0)
+    s.set_state(U)
+    s.advance(3)
+    assert np.array_equal(s.get_state(), U)
+    with pytest.raises(oracle.RefError):
+        oracle.RefSolver(shape=(8, 1, 1), dx=(0.1, 1, 1), ndim=1, eqset=oracle.CGL, riemann=oracle.HLLD)
