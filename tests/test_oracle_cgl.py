@@ -188,9 +188,9 @@ def test_c8_relaxation_step():
     assert abs((b - a) - 1.0 / 6.0) <= 1e-14
     assert abs((a + 2 * b) / 3 - 7.0 / 3.0) <= 1e-14
     assert oracle.cgl_relax(0.99, 4.0, 1.0, 1.2) == (1.0, 1.2)
-    # ion-cyclotron bound binding: p_par = 4, B^2 = 1: 0.3 * 4 * sqrt(1/8) = 0.4243 < mirror (4/p_perp)/2
-    a, b = oracle.cgl_relax(1.0, 1.0, 4.0, 5.0)
-    assert abs((b - a) - 0.3 * 4 * np.sqrt(1 / 8)) <= 1e-14
+    # ion-cyclotron bound binding: p_par = 1, p_perp = 3, B^2 = 8: 0.3 * 1 * sqrt(8/2) = 0.6 < mirror (1/3)(8/2) = 1.33
+    a, b = oracle.cgl_relax(1.0, 8.0, 1.0, 3.0)
+    assert abs((b - a) - 0.6) <= 1e-14
 
 
 def test_c9_uniform_state_is_fixed_and_hll_rejected_for_hlld():
