@@ -22,6 +22,7 @@ import numpy as np
 from . import build as _build
 
 IDEAL, HALL = 0, 1
+CGL = 2              # CGL MHD: 9 variables per cell, U = (rho, m, E, B, A_log); see include/agate.h
 IDEAL_GLM = 3        # 9 variables per cell (psi last); see include/agate.h
 HLL, HLLD = 0, 1
 OK, ERR_ARG, ERR_STATE, ERR_UNPHYSICAL, ERR_CUDA, ERR_NOMEM = range(6)
@@ -40,7 +41,7 @@ class Grid(C.Structure):
 
 class SolverCfg(C.Structure):
     _fields_ = [("riemann", C.c_int32), ("limiter", C.c_int32), ("beta", C.c_double),
-                ("rk", C.c_int32), ("cfl", C.c_double), ("d_i", C.c_double)]
+                ("rk", C.c_int32), ("cfl", C.c_double), ("d_i", C.c_double), ("relax", C.c_double)]
 
 
 class AgateError(RuntimeError):
@@ -98,14 +99,14 @@ class Agate:
     """One simulation context (agate_ctx) on a dedicated CUDA stream.  Names follow include/agate.h."""
 
     def __init__(self, shape, dx, ndim, gamma=5.0 / 3.0, eqset=IDEAL, riemann=HLL, limiter=2, beta=1.3, rk=2,
-                 cfl=0.0, d_i=0.0, device="cuda:0", stream=None):
+                 cfl=0.0, d_i=0.0, relax=0.0, device="cuda:0", stream=None):
         torch = _torch_cuda()
         nx, ny, nz = (int(s) for s in shape)
         self.shape = (nx, ny, nz)
         self.zones = nx * ny * nz
-        self.nvar = 9 if int(eqset) == IDEAL_GLM else 8
+        self.nvar = 9 if int(eqset) in (IDEAL_GLM, CGL) else 8
         self.grid = Grid(ndim, nx, ny, nz, dx[0], dx[1], dx[2])
-        self.cfg = SolverCfg(riemann, limiter, beta, rk, cfl, d_i)
+        self.cfg = SolverCfg(riemann, limiter, beta, rk, cfl, d_i, relax)
         self.device = torch.device(device)
         L = lib()
         nbytes = L.agate_workspace_bytes(C.byref(self.grid), eqset, C.byref(self.cfg))

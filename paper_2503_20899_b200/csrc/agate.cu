@@ -67,7 +67,9 @@ int check_args(const agate_grid* g, double gamma, int eqset, const agate_solver*
   if (g->ndim < 2 && g->ny != 1) return AGATE_ERR_ARG;
   if (!(g->dx > 0.0) || (g->ndim >= 2 && !(g->dy > 0.0)) || (g->ndim >= 3 && !(g->dz > 0.0))) return AGATE_ERR_ARG;
   if (!(gamma > 1.0)) return AGATE_ERR_ARG;
-  if (eqset != AGATE_IDEAL && eqset != AGATE_HALL && eqset != AGATE_IDEAL_GLM) return AGATE_ERR_ARG;
+  if (eqset != AGATE_IDEAL && eqset != AGATE_HALL && eqset != AGATE_IDEAL_GLM && eqset != AGATE_CGL) return AGATE_ERR_ARG;
+  if (eqset == AGATE_CGL && (g->ndim != 2 || s->riemann != AGATE_HLL)) return AGATE_ERR_ARG;   // CGL: 2-D strip kernel, HLL
+  if (eqset == AGATE_CGL && !(s->relax >= 0.0 && s->relax <= 1.0)) return AGATE_ERR_ARG;
   if (eqset == AGATE_IDEAL_GLM && g->ndim < 2) return AGATE_ERR_ARG;             // GLM: 2-D and 3-D kernels
   if (s->riemann < 0 || s->riemann > 1 || s->limiter < 0 || s->limiter > 2 || s->rk < 1 || s->rk > 2) return AGATE_ERR_ARG;
   if (s->limiter == 2 && !(s->beta >= 1.0 && s->beta <= 2.0)) return AGATE_ERR_ARG;
@@ -107,14 +109,14 @@ StageKernel make_stage3d() {
   return k;
 }
 
-template <int R, int LIM, bool H, bool GLM = false>
+template <int R, int LIM, bool H, bool GLM = false, bool CGL = false>
 StageKernel make_stage2d() {
   StageKernel k;
-  k.fn = stage2d_kernel<R, LIM, H, GLM>;
-  k.ty = 1; k.np = 1; k.threads = 32 * Stage2dSmem<GLM>::NW; k.smem = Stage2dSmem<GLM>::BYTES;
-  k.warps2d = Stage2dSmem<GLM>::NW;
+  k.fn = stage2d_kernel<R, LIM, H, GLM, CGL>;
+  k.ty = 1; k.np = 1; k.threads = 32 * Stage2dSmem<GLM || CGL>::NW; k.smem = Stage2dSmem<GLM || CGL>::BYTES;
+  k.warps2d = Stage2dSmem<GLM || CGL>::NW;
   k.strips2d = true;
-  k.fused_dt = !H;           // the fused reduction evaluates the ideal-MHD speed; Hall keeps the dt_kernel pass
+  k.fused_dt = !H && !CGL;   // the fused reduction evaluates the ideal-MHD speed; Hall and CGL keep the dt_kernel pass
   return k;
 }
 
@@ -137,6 +139,7 @@ StageKernel pick_stage(int ndim, int eqset, int riemann, int limiter) {
   }
   if (ndim == 2 && !getenv("AGATE_STAGE_V1")) {   // warp-autonomous strips
     if (eqset == AGATE_HALL) return (limiter == 2) ? make_stage2d<0, 2, true>() : make_stage2d<0, -1, true>();
+    if (eqset == AGATE_CGL) return (limiter == 2) ? make_stage2d<0, 2, false, false, true>() : make_stage2d<0, -1, false, false, true>();
     if (eqset == AGATE_IDEAL_GLM) {
       if (riemann == AGATE_HLLD) return (limiter == 2) ? make_stage2d<1, 2, false, true>() : make_stage2d<1, -1, false, true>();
       return (limiter == 2) ? make_stage2d<0, 2, false, true>() : make_stage2d<0, -1, false, true>();
@@ -229,6 +232,7 @@ StageParams make_stage_params(const agate_ctx* c, const double* Uin, const doubl
   p.flag = c->flag;
   p.ch_ptr = c->scal + 3;
   p.last_stage = last_stage ? 1 : 0;
+  p.relax = (c->eqset == AGATE_CGL) ? c->s.relax : 0.0;
   p.lz = c->lz;
   p.ntx = (c->g.nx + TX - 1) / TX;
   p.nty = (c->g.ny + c->sk.ty - 1) / c->sk.ty;
@@ -252,6 +256,7 @@ int launch_dt(agate_ctx* c, int add_t) {
   p.ph = c->ph;
   p.scal = c->scal; p.flag = c->flag; p.ticket = c->ticket; p.partial = c->partial;
   p.add_t = add_t;
+  p.cgl = (c->eqset == AGATE_CGL) ? 1 : 0;
   if (c->eqset == AGATE_HALL) dt_kernel<true><<<c->dt_blocks, 256, 0, c->stream>>>(p);
   else dt_kernel<false><<<c->dt_blocks, 256, 0, c->stream>>>(p);
   CU_TRY(cudaGetLastError());
@@ -347,7 +352,7 @@ extern "C" {
 
 size_t agate_workspace_bytes(const agate_grid* grid, int eqset, const agate_solver* solver) {
   if (check_args(grid, 5.0 / 3.0, eqset, solver) != AGATE_OK) return 0;
-  return make_layout(*grid, eqset == AGATE_IDEAL_GLM ? 9 : 8).total;
+  return make_layout(*grid, (eqset == AGATE_IDEAL_GLM || eqset == AGATE_CGL) ? 9 : 8).total;
 }
 
 int agate_init(const agate_grid* grid, double gamma, int eqset, const agate_solver* solver, void* workspace,
@@ -356,7 +361,7 @@ int agate_init(const agate_grid* grid, double gamma, int eqset, const agate_solv
   int rc = check_args(grid, gamma, eqset, solver);
   if (rc) return rc;
   if (!workspace) return AGATE_ERR_ARG;
-  const int nv = (eqset == AGATE_IDEAL_GLM) ? 9 : 8;
+  const int nv = (eqset == AGATE_IDEAL_GLM || eqset == AGATE_CGL) ? 9 : 8;
   Layout L = make_layout(*grid, nv);
   if (workspace_bytes < L.total || ((uintptr_t)workspace & 255u)) return AGATE_ERR_NOMEM;
   int ndev = 0;

@@ -46,7 +46,8 @@ struct StageParams {
   unsigned long long* vnext;
   int* flag;
   const double* ch_ptr;  // GLM: c_h of this step (device scalar, scal[3])
-  int last_stage;        // GLM: the source term multiplies psi in the stage that completes the step
+  int last_stage;        // GLM / CGL: the source term acts in the stage that completes the step
+  double relax;          // CGL: dt/(dt+tau) of eqs.32-33; 0 = no relaxation
   int lz;                // z-chunk length per CTA (stage_kernel)
   int ntx, nty;          // x-y tiles (stage3d_kernel: work = ntx * nty * nz tile-planes, split evenly over the grid)
   Phys ph;
@@ -383,6 +384,7 @@ struct DtParams {
   Phys ph;
   double* scal;      // [0] dt, [1] vmax, [2] t
   int* flag;         // sticky: 1 = unphysical cell seen
+  int cgl;           // CGL MHD: nine variables per cell, speeds of eqs.28-29
   unsigned int* ticket;
   double* partial;   // [gridDim.x]
   int add_t;
@@ -406,12 +408,13 @@ __global__ void __launch_bounds__(256) dt_kernel(const __grid_constant__ DtParam
     const int kk = (int)(r / P.ny), jj = (int)(r - (long long)kk * P.ny);
     const long long base = (long long)(kk + P.ghz) * P.sz + (long long)(jj + P.ghy) * P.sy + 2;
     for (int i = threadIdx.x; i < P.nx; i += blockDim.x) {
-      double u[8];
+      double u[9];
 #pragma unroll
       for (int q = 0; q < 8; ++q) u[q] = __ldg(P.U + q * P.sq + base + i);
+      u[8] = P.cgl ? __ldg(P.U + 8 * P.sq + base + i) : 0.0;
       // ideal MHD: the same straight-line function the fused stage epilogue uses, so that a stand-alone
       // reduction and the fused one give the same dt bit for bit
-      const double sp = HALL ? cell_speed<HALL>(P.ph, u) : cell_speed_inline(P.ph, u);
+      const double sp = P.cgl ? cell_speed_cgl(u) : (HALL ? cell_speed<HALL>(P.ph, u) : cell_speed_inline(P.ph, u));
       if (sp < 0.0) bad = 1; else vm = fmax(vm, sp);
     }
   }

@@ -394,6 +394,97 @@ AG_HD double cell_speed(const Phys& ph, const double U[8]) {
   return (sp - sp == 0.0) ? sp : -1.0;     // finite test that survives fast-math-free builds
 }
 
+// ------------------------------------------------------------------------------------------------------------
+// CGL MHD (NEXT-2; R24).  Nine variables per cell:
+//   U = (rho, m, E, B, A_log),  E = rho v^2/2 + B^2/2 + p_par/2 + p_perp,  A_log as eq.18
+//   W = (rho, v, p_par, B, p_perp): p_par in slot 4, p_perp in slot 8 (slot 8 is not rotated)
+// IEEE division / sqrt / exp / log: this path is not the tuned one.
+// ------------------------------------------------------------------------------------------------------------
+AG_HD void cgl_cons_to_prim(const double U[9], double W[9]) {          // eqs.26-27
+  const double ir = 1.0 / U[0];
+  const double vx = U[1] * ir, vy = U[2] * ir, vz = U[3] * ir;
+  const double b2 = U[5] * U[5] + U[6] * U[6] + U[7] * U[7];
+  const double eint = U[4] - 0.5 * U[0] * (vx * vx + vy * vy + vz * vz) - 0.5 * b2;
+  const double B3 = b2 * sqrt(b2);
+  const double X = U[0] * U[0] * exp(-U[8] * ir);
+  const double iden = 1.0 / (X + 2.0 * B3);
+  W[0] = U[0]; W[1] = vx; W[2] = vy; W[3] = vz;
+  W[4] = 2.0 * X * eint * iden;
+  W[5] = U[5]; W[6] = U[6]; W[7] = U[7];
+  W[8] = 2.0 * B3 * eint * iden;
+}
+AG_HD double cgl_alog(double rho, double b2, double ppar, double pperp) {   // eq.18
+  return rho * log((rho * rho / (b2 * sqrt(b2))) * (pperp / ppar));
+}
+// eq.29, fast branch, along the face normal of a ROTATED state (w[5] = B_n)
+AG_HD double cgl_cfast(const double w[9]) {
+  const double B2 = w[5] * w[5] + w[6] * w[6] + w[7] * w[7];
+  const double cos2 = w[5] * w[5] / B2;
+  const double b1 = B2 + 2.0 * w[8] + cos2 * (2.0 * w[4] - w[8]);
+  const double b2 = b1 - 6.0 * cos2 * w[4];
+  const double c = 4.0 * w[8] * w[8] * cos2 * (1.0 - cos2);
+  return sqrt((b1 + sqrt(b2 * b2 + c)) / (2.0 * w[0]));
+}
+// eqs.19-22 (psi == 0) + eq.17 in the rotated frame; also returns the conserved vector of the state
+AG_HD void cgl_flux_and_cons(const double w[9], double f[9], double u[9]) {
+  const double B2 = w[5] * w[5] + w[6] * w[6] + w[7] * w[7];
+  const double th = 1.0 - (w[4] - w[8]) / B2;
+  const double v2 = w[1] * w[1] + w[2] * w[2] + w[3] * w[3];
+  const double vB = w[1] * w[5] + w[2] * w[6] + w[3] * w[7];
+  u[0] = w[0]; u[1] = w[0] * w[1]; u[2] = w[0] * w[2]; u[3] = w[0] * w[3];
+  u[4] = 0.5 * w[0] * v2 + 0.5 * B2 + 0.5 * w[4] + w[8];
+  u[5] = w[5]; u[6] = w[6]; u[7] = w[7];
+  u[8] = cgl_alog(w[0], B2, w[4], w[8]);
+  f[0] = w[0] * w[1];
+  f[1] = w[0] * w[1] * w[1] - th * w[5] * w[5] + (w[8] + 0.5 * B2);
+  f[2] = w[0] * w[2] * w[1] - th * w[6] * w[5];
+  f[3] = w[0] * w[3] * w[1] - th * w[7] * w[5];
+  f[4] = (0.5 * w[0] * v2 + 0.5 * w[4] + 2.0 * w[8] + B2) * w[1] - th * vB * w[5];
+  f[5] = 0.0;
+  f[6] = w[1] * w[6] - w[5] * w[2];
+  f[7] = w[1] * w[7] - w[5] * w[3];
+  f[8] = u[8] * w[1];
+}
+// HLL eq.5 with the Davis speeds eq.6 and eq.29's fast speed; all nine components through eq.5 (R9)
+AG_HD void flux_hll_cgl(const double L[9], const double R[9], double F[9]) {
+  double fl[9], fr[9], ul[9], ur[9];
+  cgl_flux_and_cons(L, fl, ul);
+  cgl_flux_and_cons(R, fr, ur);
+  const double cl = cgl_cfast(L), cr = cgl_cfast(R);
+  const double sL = dmin(dmin(L[1] - cl, R[1] - cr), 0.0);
+  const double sR = dmax(dmax(L[1] + cl, R[1] + cr), 0.0);
+  const double iw = 1.0 / (sR - sL);
+#pragma unroll
+  for (int q = 0; q < 9; ++q) F[q] = (sR * fl[q] - sL * fr[q] + sL * sR * (ur[q] - ul[q])) * iw;
+}
+// eqs.31-33 on a conserved cell: relax the anisotropy, keep E, return the new A_log (C1 = 0.3, C2 = 0.5)
+AG_HD double cgl_relaxed_alog(double f, const double U[9]) {
+  double w[9];
+  cgl_cons_to_prim(U, w);
+  const double B2 = w[5] * w[5] + w[6] * w[6] + w[7] * w[7];
+  const double dP = w[8] - w[4];
+  const double mirror = (w[4] / w[8]) * B2 / 2.0;
+  const double ic = 0.3 * w[4] * sqrt(B2 / (2.0 * w[4]));
+  const double dPs = fmax(-B2, fmin(dP, fmin(mirror, ic)));
+  const double ppar = w[4] - (2.0 / 3.0) * (dPs - dP) * f;
+  const double pperp = w[8] + (1.0 / 3.0) * (dPs - dP) * f;
+  return cgl_alog(w[0], B2, ppar, pperp);
+}
+// eq.28 per cell: |v| + max_d c_cgl,d; negative for an unphysical cell
+AG_HD double cell_speed_cgl(const double U[9]) {
+  double w[9], r[9];
+  cgl_cons_to_prim(U, w);
+  if (!(w[0] > 0.0) || !(w[4] > 0.0) || !(w[8] > 0.0)) return -1.0;
+  double cm = 0.0;
+  for (int d = 0; d < 3; ++d) {
+    for (int q = 0; q < 9; ++q) r[q] = w[q];
+    r[5] = w[5 + d]; r[5 + d] = w[5];                      // only B_n matters for the speed
+    cm = fmax(cm, cgl_cfast(r));
+  }
+  const double sp = sqrt(w[1] * w[1] + w[2] * w[2] + w[3] * w[3]) + cm;
+  return (sp - sp == 0.0) ? sp : -1.0;
+}
+
 // A7 inside the stage epilogue (ideal MHD): the same quantity as cell_speed<false> with the straight-line roots of
 // this file, evaluated on the conserved values the stage is about to store.
 AG_HD double cell_speed_inline(const Phys& ph, const double U[8]) {

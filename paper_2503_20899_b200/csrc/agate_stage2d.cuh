@@ -32,10 +32,10 @@ constexpr int RW2 = 34;        // cells per ring row: x = xs-2 .. xs+31
 constexpr int NW2 = 6;         // warps per CTA of the 8-variable kernels
 
 // GLM = true: nine variables per cell, the scalar psi (index 8) behind the MHD ones (NEXT-1; eqs.10-11; R22)
-template <bool GLM>
+template <bool NINE>
 struct Stage2dSmem {
-  static constexpr int NV = GLM ? 9 : 8;
-  static constexpr int NW = GLM ? 5 : 6;            // warps per CTA (two CTAs per SM must fit 227 KB)
+  static constexpr int NV = NINE ? 9 : 8;
+  static constexpr int NW = NINE ? 5 : 6;            // warps per CTA (two CTAs per SM must fit 227 KB)
   static constexpr int RING = 4 * NV * RW2;         // [slot][q][c]
   static constexpr int OFF_WLY = RING;              // [q][lane]
   static constexpr int OFF_FYL = OFF_WLY + NV * 32;
@@ -44,10 +44,11 @@ struct Stage2dSmem {
   static constexpr size_t BYTES = sizeof(double) * (size_t)PER_WARP * NW;
 };
 
-template <int RIEMANN, int LIM, bool HALL, bool GLM>
-__global__ void __launch_bounds__(32 * Stage2dSmem<GLM>::NW, 2) stage2d_kernel(const __grid_constant__ StageParams P) {
-  static_assert(!(HALL && GLM), "Hall + GLM is not built");
-  using SM = Stage2dSmem<GLM>;
+// CGL = true: CGL MHD (NEXT-2; R24): nine variables, W = (rho, v, p_par, B, p_perp), HLL only
+template <int RIEMANN, int LIM, bool HALL, bool GLM, bool CGL = false>
+__global__ void __launch_bounds__(32 * Stage2dSmem<GLM || CGL>::NW, 2) stage2d_kernel(const __grid_constant__ StageParams P) {
+  static_assert(!(HALL && GLM) && !(CGL && (HALL || GLM || RIEMANN != 0)), "combination not built");
+  using SM = Stage2dSmem<GLM || CGL>;
   constexpr int NV = SM::NV, NW2 = SM::NW;
   extern __shared__ __align__(16) double smem[];
   const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
@@ -94,6 +95,15 @@ __global__ void __launch_bounds__(32 * Stage2dSmem<GLM>::NW, 2) stage2d_kernel(c
 
   auto slot_of = [](int r) { return ((r + 4) & 3) * (NV * RW2); };     // r >= -4
   auto conv = [&](int off) {                                            // A1 in place; returns nothing
+    if (CGL) {
+      double u[9], w[9];
+#pragma unroll
+      for (int q = 0; q < 9; ++q) u[q] = ring[off + q * RW2];
+      cgl_cons_to_prim(u, w);
+#pragma unroll
+      for (int q = 0; q < 9; ++q) ring[off + q * RW2] = w[q];
+      return;
+    }
     double u[8], w[8];
 #pragma unroll
     for (int q = 0; q < 8; ++q) u[q] = ring[off + q * RW2];
@@ -219,7 +229,8 @@ __global__ void __launch_bounds__(32 * Stage2dSmem<GLM>::NW, 2) stage2d_kernel(c
         pss = 0.5 * (L[NV - 1] + R[NV - 1]) - 0.5 * ch * (R[5] - L[5]);
         L[5] = bns; R[5] = bns;
       }
-      riemann_flux<RIEMANN, HALL>(P.ph, L, R, HALL ? Jr : nullptr, F);
+      if (CGL) flux_hll_cgl(L, R, F);
+      else riemann_flux<RIEMANN, HALL>(P.ph, L, R, HALL ? Jr : nullptr, F);
       if (GLM) { F[5] = pss; F[NV - 1] = ch * ch * bns; }
       {
         // A5 (y) + A6: row j-1 is complete; the accumulator of row j starts from the raw Uin (+U0)
@@ -232,6 +243,8 @@ __global__ void __launch_bounds__(32 * Stage2dSmem<GLM>::NW, 2) stage2d_kernel(c
           // the difference is formed before it meets U, so that a uniform state stays bitwise fixed (pin P1)
           o[v] = c0 * (acc[v] - cy * (F[r] - FyL[v * 32 + lane]));
           if (GLM && v == NV - 1) o[v] *= decay;                          // eq.11's source, integrated exactly
+          if (CGL && v == NV - 1 && P.last_stage && P.relax > 0.0 && emit && cell_ok)
+            o[v] = cgl_relaxed_alog(P.relax, o);                          // eqs.31-33: E stays, A_log moves
           if (emit && cell_ok) *po = o[v];
           FyL[v * 32 + lane] = F[r];
           acc[v] = Uraw[((j & 1) * NV + v) * 32 + lane];
@@ -269,7 +282,8 @@ __global__ void __launch_bounds__(32 * Stage2dSmem<GLM>::NW, 2) stage2d_kernel(c
           pss = 0.5 * (L[NV - 1] + R[NV - 1]) - 0.5 * ch * (R[5] - L[5]);
           L[5] = bns; R[5] = bns;
         }
-        riemann_flux<RIEMANN, HALL>(P.ph, L, R, HALL ? Jr : nullptr, F);
+        if (CGL) flux_hll_cgl(L, R, F);
+        else riemann_flux<RIEMANN, HALL>(P.ph, L, R, HALL ? Jr : nullptr, F);
         if (GLM) { F[5] = pss; F[NV - 1] = ch * ch * bns; }
 #pragma unroll
         for (int r = 0; r < NV; ++r) {
