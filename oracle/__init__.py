@@ -225,7 +225,8 @@ class RefSolver:
     @classmethod
     def from_workload(cls, wl, **over):
         kw = dict(shape=wl.shape, dx=wl.dx, ndim=wl.ndim, gamma=wl.gamma, eqset=wl.eqset, riemann=wl.riemann,
-                  limiter=wl.limiter, beta=wl.beta, rk=wl.rk, cfl=wl.cfl, d_i=wl.d_i)
+                  limiter=wl.limiter, beta=wl.beta, rk=wl.rk, cfl=wl.cfl, d_i=wl.d_i,
+                  relax=getattr(wl, "relax", 0.0))
         kw.update(over)
         s = cls(**kw)
         s.set_state(wl.U)
@@ -297,7 +298,7 @@ def count_ops(wl):
     Returns dict(add, mul, div, sqrt, cmp, flops) per zone-update."""
     nx, ny, nz = wl.shape
     grid = Grid(wl.ndim, nx, ny, nz, wl.dx[0], wl.dx[1], wl.dx[2])
-    cfg = SolverCfg(wl.riemann, wl.limiter, wl.beta, wl.rk, wl.cfl, wl.d_i)
+    cfg = SolverCfg(wl.riemann, wl.limiter, wl.beta, wl.rk, wl.cfl, wl.d_i, getattr(wl, "relax", 0.0))
     U = np.ascontiguousarray(wl.U, dtype=np.float64)
     out = np.zeros(5)
     rc = lib().agate_ref_count_ops(C.byref(grid), wl.gamma, wl.eqset, C.byref(cfg), U.ctypes.data_as(_dp),

@@ -125,7 +125,8 @@ class Agate:
     @classmethod
     def from_workload(cls, wl, **over):
         kw = dict(shape=wl.shape, dx=wl.dx, ndim=wl.ndim, gamma=wl.gamma, eqset=wl.eqset, riemann=wl.riemann,
-                  limiter=wl.limiter, beta=wl.beta, rk=wl.rk, cfl=wl.cfl, d_i=wl.d_i)
+                  limiter=wl.limiter, beta=wl.beta, rk=wl.rk, cfl=wl.cfl, d_i=wl.d_i,
+                  relax=getattr(wl, "relax", 0.0))
         set_state = over.pop("set_state", True)
         kw.update(over)
         s = cls(**kw)

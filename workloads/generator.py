@@ -31,6 +31,7 @@ import numpy as np
 NVAR = 8
 IDEAL, HALL = 0, 1
 IDEAL_GLM = 3          # 9 variables per cell: the GLM scalar psi behind the 8 MHD ones
+CGL = 2                # 9 variables per cell: U = (rho, m, E, B, A_log), W = (rho, v, p_par, B, p_perp)
 HLL, HLLD = 0, 1
 GAMMA = 5.0 / 3.0
 SEED_BASE = 2503208990
@@ -76,6 +77,7 @@ class Workload:
     W: np.ndarray         # [8, nz, ny, nx] float64, primitive
     U: np.ndarray         # [8, nz, ny, nx] float64, conserved (x fastest)
     name: str = ""
+    relax: float = 0.0    # CGL: dt/(dt+tau) of eqs.32-33
 
     @property
     def zones(self) -> int:
@@ -163,6 +165,19 @@ def prim_to_cons(W: np.ndarray, gamma: float) -> np.ndarray:
 
 
 # Full-size grids and solver settings per config (BASELINE.json configs).
+def prim_to_cons_cgl(W: np.ndarray) -> np.ndarray:
+    """Definition of the CGL conserved vector from W = (rho, v, p_par, B, p_perp): E = rho v^2/2 + B^2/2 + p_par/2 +
+    p_perp, A_log = rho log[(rho^2/B^3)(p_perp/p_par)] (eq.18)."""
+    rho, vx, vy, vz, ppar, bx, by, bz, pperp = W
+    b2 = bx * bx + by * by + bz * bz
+    U = np.empty_like(W)
+    U[0] = rho; U[1] = rho * vx; U[2] = rho * vy; U[3] = rho * vz
+    U[4] = 0.5 * rho * (vx * vx + vy * vy + vz * vz) + 0.5 * b2 + 0.5 * ppar + pperp
+    U[5] = bx; U[6] = by; U[7] = bz
+    U[8] = rho * np.log((rho * rho / (b2 * np.sqrt(b2))) * (pperp / ppar))
+    return U
+
+
 _CONFIGS = {
     1: dict(ndim=2, n=128,  eqset=IDEAL, riemann=HLL,  beta=1.0, cfl=0.4,   d_i=0.0,  n_steps=10,
             name="cfg1: 2D ideal 128^2 HLL minmod"),
@@ -178,6 +193,10 @@ _CONFIGS = {
     # (IC printed at P:L282) with GLM divergence cleaning, "default settings": PLM + eq.4 beta=1.3, HLL, C=0.45.
     6: dict(ndim=2, n=2048, eqset=IDEAL_GLM, riemann=HLL, beta=1.3, cfl=0.45,  d_i=0.0,  n_steps=100,
             name="cfg6: 2D Orszag-Tang + GLM 2048^2 HLL MC (paper Table 2 workload)"),
+    # NEXT-2, not a BASELINE.json config: the Orszag-Tang vortex in CGL MHD ("In the CGL MHD version, we set
+    # the initial anisotropy to zero"), HLL, default relaxation dt/(dt+tau) = 0.99
+    7: dict(ndim=2, n=2048, eqset=CGL, riemann=HLL, beta=1.3, cfl=0.45, d_i=0.0, n_steps=100, relax=0.99,
+            name="cfg7: 2D Orszag-Tang CGL 2048^2 HLL MC"),
 }
 
 
@@ -199,10 +218,10 @@ def make_workload(config_id: int, n: int | None = None, n_steps: int | None = No
     rng = SplitMix64(SEED_BASE + config_id)
     g = GAMMA
     nx, ny, nz = shape
-    W = np.empty((NVAR + (1 if c["eqset"] == IDEAL_GLM else 0), nz, ny, nx))
+    W = np.empty((NVAR + (1 if c["eqset"] in (IDEAL_GLM, CGL) else 0), nz, ny, nx))
     F = lambda M, K: _field(rng, M, K, ndim, shape)
 
-    if config_id == 6:
+    if config_id in (6, 7):
         # rho = 25/(36 pi), p = 5/(12 pi), v = (-sin 2 pi y, sin 2 pi x, 0), B = B0 (-sin 2 pi y, sin 4 pi x, 0),
         # B0 = 1/sqrt(4 pi), unit box, cell centres; psi = 0
         xc = ((np.arange(nx) + 0.5) / nx)[None, None, :]
@@ -216,7 +235,7 @@ def make_workload(config_id: int, n: int | None = None, n_steps: int | None = No
         W[5] = -B0 * np.sin(2.0 * math.pi * yc) + 0.0 * xc
         W[6] = B0 * np.sin(4.0 * math.pi * xc) + 0.0 * yc
         W[7] = 0.0
-        W[8] = 0.0
+        W[8] = 0.0 if config_id == 6 else W[4]      # GLM: psi = 0;  CGL: p_perp = p_par = p
     elif config_id in (1, 4):
         W[0] = 1.0 + 0.1 * F(4, 4)
         W[1] = 0.1 * F(4, 4)
@@ -275,10 +294,10 @@ def make_workload(config_id: int, n: int | None = None, n_steps: int | None = No
     d_i = c["d_i"]
     if config_id == 4 and scale_d_i and n != nfull:
         d_i = d_i * nfull / n
-    U = prim_to_cons(W, g)
+    U = prim_to_cons_cgl(W) if c["eqset"] == CGL else prim_to_cons(W, g)
     return Workload(config_id=config_id, ndim=ndim, shape=shape, dx=dx, gamma=g, eqset=c["eqset"],
                     riemann=c["riemann"], limiter=2, beta=c["beta"], rk=2, cfl=c["cfl"], d_i=d_i,
-                    n_steps=c["n_steps"] if n_steps is None else n_steps, W=W, U=U,
+                    n_steps=c["n_steps"] if n_steps is None else n_steps, W=W, U=U, relax=c.get("relax", 0.0),
                     name=c["name"] + (f" @n={n}" if n != nfull else ""))
 
 
