@@ -386,7 +386,7 @@ template <class T> struct Solver {
   bool glm;
   bool cgl = false;
   double ch = 0.0;      // GLM: c_h of the step being taken (R22: 0.95 v_max(U^n))
-  std::vector<T> Un, U1, W, L;
+  std::vector<T> Un, U1, U2, W, L;
   double t = 0.0;
   bool have_state = false;
 
@@ -605,6 +605,24 @@ template <class T> struct Solver {
     }
     fill_ghosts(U1);
     rhs(U1);
+    if (s.rk == 3) {
+      // R25: SSP-RK33 in Shu-Osher form:  U2 = 3/4 Un + 1/4 (U1 + dt L(U1));  Un+1 = 1/3 Un + 2/3 (U2 + dt L(U2))
+      if (U2.empty()) U2.assign(nv * ntot, T(0.0));
+      for (int q = 0; q < nv; ++q) for (int k = 0; k < nd[2]; ++k) for (int j = 0; j < nd[1]; ++j) for (int i = 0; i < nd[0]; ++i) {
+        const size_t p = q * ntot + pidx(i, j, k);
+        U2[p] = T(0.75) * Un[p] + T(0.25) * (U1[p] + T(dt) * L[q * nint + iidx(i, j, k)]);
+      }
+      fill_ghosts(U2);
+      rhs(U2);
+      for (int q = 0; q < nv; ++q) for (int k = 0; k < nd[2]; ++k) for (int j = 0; j < nd[1]; ++j) for (int i = 0; i < nd[0]; ++i) {
+        const size_t p = q * ntot + pidx(i, j, k);
+        Un[p] = T(1.0 / 3.0) * Un[p] + T(2.0 / 3.0) * (U2[p] + T(dt) * L[q * nint + iidx(i, j, k)]);
+      }
+      if (glm) glm_source(dt);
+      if (cgl) cgl_source();
+      t += dt;
+      return;
+    }
     for (int q = 0; q < nv; ++q) for (int k = 0; k < nd[2]; ++k) for (int j = 0; j < nd[1]; ++j) for (int i = 0; i < nd[0]; ++i) {
       const size_t p = q * ntot + pidx(i, j, k);
       Un[p] = T(0.5) * Un[p] + T(0.5) * (U1[p] + T(dt) * L[q * nint + iidx(i, j, k)]);   // stage 2
@@ -636,7 +654,7 @@ int check_args(const agate_ref_grid* g, double gamma, int eqset, const agate_ref
   if (eqset != AGATE_REF_IDEAL && eqset != AGATE_REF_HALL && eqset != AGATE_REF_IDEAL_GLM && eqset != AGATE_REF_CGL) return 1;
   if (eqset == AGATE_REF_CGL && s->riemann != 0) return 1;          // the paper's CGL runs use HLL
   if (eqset == AGATE_REF_CGL && !(s->relax >= 0.0 && s->relax <= 1.0)) return 1;
-  if (s->riemann < 0 || s->riemann > 1 || s->limiter < 0 || s->limiter > 2 || s->rk < 1 || s->rk > 2) return 1;
+  if (s->riemann < 0 || s->riemann > 1 || s->limiter < 0 || s->limiter > 2 || s->rk < 1 || s->rk > 3) return 1;
   if (s->limiter == 2 && !(s->beta >= 1.0 && s->beta <= 2.0)) return 1;
   if (eqset == AGATE_REF_HALL && s->riemann == 1) return 1;        // no Hall-HLLD in the paper
   if (eqset == AGATE_REF_HALL && !(s->d_i >= 0.0)) return 1;

@@ -31,7 +31,7 @@ typedef struct {
   int32_t riemann;       /* 0 HLL (eq.5), 1 HLLD */
   int32_t limiter;       /* 0 none (dW=0), 1 central (unlimited), 2 eq.4 */
   double  beta;          /* eq.4 beta: 1.0 = minmod, 1.3 = paper default "MC" */
-  int32_t rk;            /* 1 = RK11 (forward Euler), 2 = SSP-RK2 (R11) */
+  int32_t rk;            /* 1 = RK11 (forward Euler), 2 = SSP-RK2 (R11), 3 = SSP-RK33 (R25) */
   double  cfl;           /* Courant C; <=0 -> paper default 0.8/0.45/0.325 (L73) */
   double  d_i;           /* normalised ion inertial length (Hall) */
   double  relax;         /* CGL: dt/(dt+tau) of eqs.32-33 (paper default 0.99, L254); 0 = no relaxation */

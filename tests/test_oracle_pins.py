@@ -406,15 +406,23 @@ def _amplification(lam, sL, sR, hlld, limiter, theta, dt_dx, rk):
     else:
         uL, uR = 1.0, cmath.exp(1j * theta)
     z = -dt_dx * (1 - cmath.exp(-1j * theta)) * (aL * uL + aR * uR)
-    return 1 + z + (0.5 * z * z if rk == 2 else 0.0)
+    return 1 + z + (0.5 * z * z if rk >= 2 else 0.0) + (z * z * z / 6.0 if rk == 3 else 0.0)
+
+
+@pytest.mark.parametrize("rk", [1, 3])
+@pytest.mark.parametrize("mode", ["alfven+", "entropy"])
+def test_p4_linear_eigenmode_rk1_rk3(rk, mode):
+    """The same closed form with the stability polynomial of forward Euler (1 + z) and of SSP-RK33 (R25:
+    1 + z + z^2/2 + z^3/6 -- any three-stage third-order scheme has it, so this pins the Shu-Osher weights)."""
+    test_p4_linear_eigenmode(oracle.HLLD, 0 if rk == 1 else 1, mode, 1, rk=rk)      # Euler + central slopes is unstable
 
 
 @pytest.mark.parametrize("riemann", [oracle.HLL, oracle.HLLD])
 @pytest.mark.parametrize("limiter", [0, 1])
 @pytest.mark.parametrize("mode", ["alfven+", "alfven-", "entropy"])
 @pytest.mark.parametrize("d", [0, 1, 2])
-def test_p4_linear_eigenmode(riemann, limiter, mode, d):
-    N, nsteps, eps, rk = 32, 25, 1e-7, 2
+def test_p4_linear_eigenmode(riemann, limiter, mode, d, rk=2):
+    N, nsteps, eps = 32, 25, 1e-7
     rho0, v0, p0, B0 = 1.3, 0.35, 0.7, 0.9
     gamma = G53
     ca = B0 / math.sqrt(rho0)
