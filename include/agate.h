@@ -47,7 +47,8 @@ typedef struct {
   int32_t riemann;      /* 0 = HLL (eq.5), 1 = HLLD (R10; not in the paper)              */
   int32_t limiter;      /* 0 = none (dU = 0), 1 = central (unlimited), 2 = eq.4   */
   double  beta;         /* eq.4 beta in [1,2]: 1.0 = minmod, 1.3 = the paper's "MC" default */
-  int32_t rk;           /* 1 = RK11 (forward Euler), 2 = SSP-RK22 (R11)                       */
+  int32_t rk;           /* 1 = RK11 (forward Euler), 2 = SSP-RK22 (R11), 3 = SSP-RK33 (R25;
+                           needs a third state copy in the workspace)                                  */
   double  cfl;          /* Courant number C; <= 0 selects the paper default 0.8/0.45/0.325   */
   double  d_i;          /* normalised ion inertial length (eqset AGATE_HALL only)            */
   double  relax;        /* eqset AGATE_CGL only: dt/(dt+tau) of eqs.32-33 in [0,1]; the paper's default is

@@ -36,10 +36,10 @@ struct Layout {
   int ghy, ghz, nxp, nyp, nzp;
   long long sy, sz, sq;
   size_t state_bytes;      // one padded copy of U (8 variables)
-  size_t off_A, off_B, off_scal, off_partial, total;
+  size_t off_A, off_B, off_C, off_scal, off_partial, total;   // off_C: third copy, SSP-RK33 only
 };
 
-Layout make_layout(const agate_grid& g, int nv) {
+Layout make_layout(const agate_grid& g, int nv, int rk = 2) {
   Layout L;
   L.ghy = (g.ndim >= 2) ? 2 : 0;
   L.ghz = (g.ndim >= 3) ? 2 : 0;
@@ -53,7 +53,8 @@ Layout make_layout(const agate_grid& g, int nv) {
   L.state_bytes = sizeof(double) * (size_t)nv * (size_t)L.sq;
   L.off_A = 0;
   L.off_B = align_up(L.off_A + L.state_bytes, 256);
-  L.off_scal = align_up(L.off_B + L.state_bytes, 256);
+  L.off_C = align_up(L.off_B + L.state_bytes, 256);
+  L.off_scal = (rk == 3) ? align_up(L.off_C + L.state_bytes, 256) : L.off_C;
   L.off_partial = L.off_scal + 256;                       // scal: 3 doubles + flag + ticket
   L.total = L.off_partial + align_up(sizeof(double) * kDtBlocksMax, 256);
   return L;
@@ -71,7 +72,7 @@ int check_args(const agate_grid* g, double gamma, int eqset, const agate_solver*
   if (eqset == AGATE_CGL && (g->ndim != 2 || s->riemann != AGATE_HLL)) return AGATE_ERR_ARG;   // CGL: 2-D strip kernel, HLL
   if (eqset == AGATE_CGL && !(s->relax >= 0.0 && s->relax <= 1.0)) return AGATE_ERR_ARG;
   if (eqset == AGATE_IDEAL_GLM && g->ndim < 2) return AGATE_ERR_ARG;             // GLM: 2-D and 3-D kernels
-  if (s->riemann < 0 || s->riemann > 1 || s->limiter < 0 || s->limiter > 2 || s->rk < 1 || s->rk > 2) return AGATE_ERR_ARG;
+  if (s->riemann < 0 || s->riemann > 1 || s->limiter < 0 || s->limiter > 2 || s->rk < 1 || s->rk > 3) return AGATE_ERR_ARG;
   if (s->limiter == 2 && !(s->beta >= 1.0 && s->beta <= 2.0)) return AGATE_ERR_ARG;
   if (eqset == AGATE_HALL && s->riemann == AGATE_HLLD) return AGATE_ERR_ARG;   // no Hall-HLLD in the paper
   if (eqset == AGATE_HALL && !(s->d_i >= 0.0)) return AGATE_ERR_ARG;
@@ -169,7 +170,7 @@ struct agate_ctx {
   double dxmin, cfl;
   cudaStream_t stream;
   char* ws;
-  double *UA, *UB, *scal, *partial;
+  double *UA, *UB, *UC, *scal, *partial;
   int* flag;
   unsigned int* ticket;
   unsigned long long* vnext;       // fused A7: bit pattern of v_max of the current state (valid iff vmax_valid)
@@ -180,7 +181,7 @@ struct agate_ctx {
   dim3 sgrid;
   int lz;
   int dt_blocks, ghost_blocks;
-  GhostParams gpA, gpB;
+  GhostParams gpA, gpB, gpC;
   cudaGraphExec_t graph = nullptr;
   bool timing = false;
   std::vector<cudaEvent_t> ev;     // pairs (start, stop) of timed stage launches
@@ -220,7 +221,7 @@ StageParams make_stage_params(const agate_ctx* c, const double* Uin, const doubl
   StageParams p;
   const Layout& L = c->L;
   p.Uin = Uin; p.U0 = U0; p.Uout = Uout; p.dt_ptr = c->scal;
-  p.a0 = a0; p.a1 = a1;
+  p.a0 = a0; p.a1 = a1; p.r0 = (a0 != 0.0) ? a0 / a1 : 0.0;
   p.nx = c->g.nx; p.ny = c->g.ny; p.nz = c->g.nz; p.ndim = c->g.ndim;
   p.ghy = L.ghy; p.ghz = L.ghz; p.nxp = L.nxp; p.nyp = L.nyp;
   p.sy = L.sy; p.sz = L.sz; p.sq = L.sq;
@@ -295,6 +296,13 @@ int enqueue_stages(agate_ctx* c) {
     return AGATE_OK;
   }
   if ((rc = launch_ghost(c, c->gpB))) return rc;
+  if (c->s.rk == 3) {
+    // R25, SSP-RK33:  U2 = 3/4 Un + 1/4 (U1 + dt L(U1))  into the third copy (U1's halos are still being read, Un is
+    // needed once more);  Un+1 = 1/3 Un + 2/3 (U2 + dt L(U2))  over Un
+    if ((rc = launch_stage(c, make_stage_params(c, c->UB, c->UA, c->UC, 0.75, 0.25, false)))) return rc;
+    if ((rc = launch_ghost(c, c->gpC))) return rc;
+    return launch_stage(c, make_stage_params(c, c->UC, c->UA, c->UA, 1.0 / 3.0, 2.0 / 3.0, true));
+  }
   return launch_stage(c, make_stage_params(c, c->UB, c->UA, c->UA, 0.5, 0.5, true));
 }
 
@@ -352,7 +360,7 @@ extern "C" {
 
 size_t agate_workspace_bytes(const agate_grid* grid, int eqset, const agate_solver* solver) {
   if (check_args(grid, 5.0 / 3.0, eqset, solver) != AGATE_OK) return 0;
-  return make_layout(*grid, (eqset == AGATE_IDEAL_GLM || eqset == AGATE_CGL) ? 9 : 8).total;
+  return make_layout(*grid, (eqset == AGATE_IDEAL_GLM || eqset == AGATE_CGL) ? 9 : 8, solver->rk).total;
 }
 
 int agate_init(const agate_grid* grid, double gamma, int eqset, const agate_solver* solver, void* workspace,
@@ -362,7 +370,7 @@ int agate_init(const agate_grid* grid, double gamma, int eqset, const agate_solv
   if (rc) return rc;
   if (!workspace) return AGATE_ERR_ARG;
   const int nv = (eqset == AGATE_IDEAL_GLM || eqset == AGATE_CGL) ? 9 : 8;
-  Layout L = make_layout(*grid, nv);
+  Layout L = make_layout(*grid, nv, solver->rk);
   if (workspace_bytes < L.total || ((uintptr_t)workspace & 255u)) return AGATE_ERR_NOMEM;
   int ndev = 0;
   if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev < 1) return AGATE_ERR_CUDA;   // no CPU fallback
@@ -380,6 +388,7 @@ int agate_init(const agate_grid* grid, double gamma, int eqset, const agate_solv
   c->ws = (char*)workspace;
   c->UA = (double*)(c->ws + L.off_A);
   c->UB = (double*)(c->ws + L.off_B);
+  c->UC = (double*)(c->ws + L.off_C);
   c->scal = (double*)(c->ws + L.off_scal);
   c->flag = (int*)(c->ws + L.off_scal + 64);
   c->ticket = (unsigned int*)(c->ws + L.off_scal + 128);
@@ -450,6 +459,7 @@ int agate_init(const agate_grid* grid, double gamma, int eqset, const agate_solv
   c->dt_blocks = (int)(nrows < kDtBlocksMax ? nrows : kDtBlocksMax);
   c->gpA = make_ghost(c, c->UA);
   c->gpB = make_ghost(c, c->UB);
+  c->gpC = make_ghost(c, c->UC);
   long long nghost = c->gpA.nzs + c->gpA.nys + c->gpA.nxs;
   long long gb = (nghost + 255) / 256;
   c->ghost_blocks = (int)(gb < 148 * 16 ? (gb < 1 ? 1 : gb) : 148 * 16);
@@ -515,7 +525,7 @@ int agate_advance(agate_ctx* c, int32_t n_steps, double* t_out) {
   if (!c->have_state) return AGATE_ERR_STATE;
   int rc;
   // stream capture is not allowed on the legacy default stream
-  const bool use_graph = (c->s.rk == 2) && !c->timing && c->stream != nullptr && !getenv("AGATE_NO_GRAPH");
+  const bool use_graph = (c->s.rk >= 2) && !c->timing && c->stream != nullptr && !getenv("AGATE_NO_GRAPH");
   if (n_steps > 0 && (rc = ensure_vmax(c))) return rc;
   if (use_graph && !c->graph && n_steps > 0) {
     cudaGraph_t g = nullptr;
@@ -570,7 +580,7 @@ int agate_launch_info(agate_ctx* c, int64_t out[8]) {
   if (!c || !out) return AGATE_ERR_ARG;
   out[0] = c->sgrid.x; out[1] = c->sgrid.y; out[2] = c->sgrid.z;
   out[3] = c->sk.threads; out[4] = (int64_t)c->sk.smem; out[5] = c->regs; out[6] = c->occ;
-  out[7] = (c->s.rk == 2) ? 5 : 3;   // dt + (ghost + stage) per RK stage
+  out[7] = 1 + 2 * c->s.rk;          // dt + (ghost + stage) per RK stage
   return AGATE_OK;
 }
 

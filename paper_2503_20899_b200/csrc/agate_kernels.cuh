@@ -32,7 +32,9 @@ struct StageParams {
   const double* U0;      // U^n for the combine (may alias Uout); unused when a0 == 0
   double* Uout;
   const double* dt_ptr;  // device scalar
-  double a0, a1;         // a0 == 0: Uout = Uin + dt*L;  a0 == a1: Uout = a1*(U0 + Uin + dt*L)  (SSP-RK22: 1/2)
+  double a0, a1;         // Uout = a0 U0 + a1 (Uin + dt L), evaluated as a1 ((a0/a1) U0 + Uin + dt L); a0 == 0: no U0.
+                         // SSP-RK22: (1/2, 1/2);  SSP-RK33 (R25): (3/4, 1/4) then (1/3, 2/3)
+  double r0;             // a0 / a1
   int nx, ny, nz, ndim;
   int ghy, ghz;          // ghost widths (2 if the dimension is active, else 0)
   int nxp, nyp;          // padded extents
@@ -160,7 +162,7 @@ __global__ void __launch_bounds__(32 * (TY + 2), MINB) stage_kernel(const __grid
       for (int q = 0; q < 8; ++q) acc[q] = __ldg(P.Uin + q * P.sq + gcell);
       if (P.a0 != 0.0) {
 #pragma unroll
-        for (int q = 0; q < 8; ++q) acc[q] += P.U0[q * P.sq + gcell];
+        for (int q = 0; q < 8; ++q) acc[q] = fma(P.r0, P.U0[q * P.sq + gcell], acc[q]);
       }
     } else {
 #pragma unroll

@@ -155,7 +155,7 @@ __global__ void __launch_bounds__(32 * Stage2dSmem<GLM || CGL>::NW, 2) stage2d_k
           for (int q = 0; q < NV; ++q) {
             const int a = ((r & 1) * NV + q) * 32 + lane;
             const double u = ring[so + q * RW2 + lane + 1];
-            Uraw[a] = two ? (u + Uraw[a]) : u;
+            Uraw[a] = two ? fma(P.r0, Uraw[a], u) : u;          // Uin + (a0/a1) U0
           }
         }
         conv(so + lane + 1);

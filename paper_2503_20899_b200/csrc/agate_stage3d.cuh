@@ -294,7 +294,7 @@ __global__ void __launch_bounds__(32 * (TY + 1), MINB) stage3d_kernel(const __gr
         } else if (full) {
           if (s == 1) {
 #pragma unroll
-            for (int q = 0; q < NV; ++q) acc[q] += two ? (ua[q] + ub[q]) : ua[q];      // A6: Uin (+ U0)
+            for (int q = 0; q < NV; ++q) acc[q] += two ? fma(P.r0, ub[q], ua[q]) : ua[q];      // A6: Uin (+ (a0/a1) U0)
 #pragma unroll
             for (int r = 0; r < NV; ++r) {
               L[r] = Ly[r];

@@ -184,7 +184,7 @@ def test_advance_matches_oracle_advance(ag):
     assert abs(gpu.t - tr) <= 1e-13 * tr
 
 
-@pytest.mark.parametrize("rk", [1, 2])
+@pytest.mark.parametrize("rk", [1, 2, 3])
 def test_fused_dt_sequences_3d(ag, rk):
     """3-D path: the Courant reduction of step n+1 runs inside the last stage of step n (A7 fused).  Every way into a
     step must see the right v_max: after set_state (stand-alone reduction), after a self-timed step (fused), after a
@@ -247,10 +247,37 @@ def test_3d_run_to_run_bitwise(ag):
         assert np.array_equal(U, outs[0][1])
 
 
+@pytest.mark.parametrize("cfg,n", [(2, 100), (4, 64), (1, 32)])
+def test_ssp_rk33_2d(ag, cfg, n):
+    """SSP-RK33 (NEXT-3, R25) through the 2-D strip kernel (ideal HLLD, Hall HLL) -- three stages, third state copy,
+    weights (3/4, 1/4) and (1/3, 2/3), A7 fused into the third stage."""
+    wl = make_workload(cfg, n=n)
+    assert_parity(*run_pair(ag, wl, 6, rk=3))
+    ref = oracle.RefSolver.from_workload(wl, rk=3)
+    gpu = ag.Agate.from_workload(wl, rk=3)
+    tr, tg = ref.advance(5), gpu.advance(5)
+    assert abs(tg - tr) <= 1e-13 * tr
+    assert np.all(rel_linf(gpu.get_state(), ref.get_state()) <= TOL_N)
+    assert gpu.launch_info()["launches_per_step"] == 7
+    ref.close(); gpu.close()
+
+
+def test_ssp_rk33_1d_pooled_kernel(ag):
+    wl = make_workload(1, n=32)
+    U = wl.U[:, :, :1, :].copy()
+    kw = dict(shape=(32, 1, 1), dx=(1 / 32, 1, 1), ndim=1, riemann=HLLD, beta=1.3, rk=3)
+    ref = oracle.RefSolver(**kw); gpu = ag.Agate(**kw)
+    ref.set_state(U); gpu.set_state(U)
+    tr, tg = ref.advance(8), gpu.advance(8)
+    assert abs(tg - tr) <= 1e-13 * tr
+    assert np.all(rel_linf(gpu.get_state(), ref.get_state()) <= TOL_N)
+    ref.close(); gpu.close()
+
+
 # ---- solver options and edge cases --------------------------------------------------------------------------
 @pytest.mark.parametrize("riemann", [HLL, HLLD])
 @pytest.mark.parametrize("limiter,beta", [(0, 1.0), (1, 1.0), (2, 1.0), (2, 2.0)])
-@pytest.mark.parametrize("rk", [1, 2])
+@pytest.mark.parametrize("rk", [1, 2, 3])
 def test_options_3d(ag, riemann, limiter, beta, rk):
     W, U = random_state(21, (20, 14, 9), 3, amp=0.3)
     dx = (1 / 20, 1 / 14, 1 / 9)
