@@ -53,6 +53,8 @@ typedef struct {
   double  d_i;          /* normalised ion inertial length (eqset AGATE_HALL only)            */
   double  relax;        /* eqset AGATE_CGL only: dt/(dt+tau) of eqs.32-33 in [0,1]; the paper's default is
                            0.99; 0 = no relaxation                                            */
+  int32_t bc[3];        /* ghost rule per dimension (x, y, z): 0 = periodic, 1 = zero-gradient /
+                           open end (R26: ghost = nearest interior zone)                       */
 } agate_solver;
 
 enum { AGATE_IDEAL = 0, AGATE_HALL = 1, AGATE_CGL = 2, AGATE_IDEAL_GLM = 3 };

@@ -46,7 +46,8 @@ class Grid(C.Structure):
 
 class SolverCfg(C.Structure):
     _fields_ = [("riemann", C.c_int32), ("limiter", C.c_int32), ("beta", C.c_double),
-                ("rk", C.c_int32), ("cfl", C.c_double), ("d_i", C.c_double), ("relax", C.c_double)]
+                ("rk", C.c_int32), ("cfl", C.c_double), ("d_i", C.c_double), ("relax", C.c_double),
+                ("bc", C.c_int32 * 3)]
 
 
 _lib = None
@@ -210,11 +211,11 @@ class RefSolver:
     """Host-memory solver with the same call shape as the product's C-ABI (agate_ref_* functions)."""
 
     def __init__(self, shape, dx, ndim, gamma=5.0 / 3.0, eqset=IDEAL, riemann=HLL, limiter=2, beta=1.3,
-                 rk=2, cfl=0.0, d_i=0.0, relax=0.0):
+                 rk=2, cfl=0.0, d_i=0.0, relax=0.0, bc=(0, 0, 0)):
         nx, ny, nz = (int(s) for s in shape)
         self.shape = (nx, ny, nz)
         self.grid = Grid(ndim, nx, ny, nz, dx[0], dx[1], dx[2])
-        self.cfg = SolverCfg(riemann, limiter, beta, rk, cfl, d_i, relax)
+        self.cfg = SolverCfg(riemann, limiter, beta, rk, cfl, d_i, relax, (C.c_int32 * 3)(*[int(b) for b in bc]))
         self.gamma, self.eqset = float(gamma), int(eqset)
         self._h = C.c_void_p()
         rc = lib().agate_ref_create(C.byref(self.grid), self.gamma, self.eqset, C.byref(self.cfg), C.byref(self._h))

@@ -420,7 +420,10 @@ template <class T> struct Solver {
       for (int k = -gh[2]; k < nd[2] + gh[2]; ++k)
         for (int j = -gh[1]; j < nd[1] + gh[1]; ++j)
           for (int i = -gh[0]; i < nd[0] + gh[0]; ++i) {
-            int iw = ((i % nd[0]) + nd[0]) % nd[0], jw = ((j % nd[1]) + nd[1]) % nd[1], kw = ((k % nd[2]) + nd[2]) % nd[2];
+            // periodic: wrapped index;  zero-gradient (R26): the nearest interior zone
+            int iw = s.bc[0] ? std::min(std::max(i, 0), nd[0] - 1) : ((i % nd[0]) + nd[0]) % nd[0];
+            int jw = s.bc[1] ? std::min(std::max(j, 0), nd[1] - 1) : ((j % nd[1]) + nd[1]) % nd[1];
+            int kw = s.bc[2] ? std::min(std::max(k, 0), nd[2] - 1) : ((k % nd[2]) + nd[2]) % nd[2];
             if (iw != i || jw != j || kw != k) U[q * ntot + pidx(i, j, k)] = U[q * ntot + pidx(iw, jw, kw)];
           }
   }
@@ -656,6 +659,7 @@ int check_args(const agate_ref_grid* g, double gamma, int eqset, const agate_ref
   if (eqset == AGATE_REF_CGL && !(s->relax >= 0.0 && s->relax <= 1.0)) return 1;
   if (s->riemann < 0 || s->riemann > 1 || s->limiter < 0 || s->limiter > 2 || s->rk < 1 || s->rk > 3) return 1;
   if (s->limiter == 2 && !(s->beta >= 1.0 && s->beta <= 2.0)) return 1;
+  for (int d = 0; d < 3; ++d) if (s->bc[d] < 0 || s->bc[d] > 1) return 1;
   if (eqset == AGATE_REF_HALL && s->riemann == 1) return 1;        // no Hall-HLLD in the paper
   if (eqset == AGATE_REF_HALL && !(s->d_i >= 0.0)) return 1;
   return 0;

@@ -35,6 +35,7 @@ typedef struct {
   double  cfl;           /* Courant C; <=0 -> paper default 0.8/0.45/0.325 (L73) */
   double  d_i;           /* normalised ion inertial length (Hall) */
   double  relax;         /* CGL: dt/(dt+tau) of eqs.32-33 (paper default 0.99, L254); 0 = no relaxation */
+  int32_t bc[3];         /* per dimension: 0 periodic, 1 zero-gradient (open end, L314: ghost = nearest interior zone) */
 } agate_ref_solver;
 
 enum { AGATE_REF_IDEAL = 0, AGATE_REF_HALL = 1, AGATE_REF_CGL = 2, AGATE_REF_IDEAL_GLM = 3 };

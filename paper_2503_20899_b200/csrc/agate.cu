@@ -74,6 +74,7 @@ int check_args(const agate_grid* g, double gamma, int eqset, const agate_solver*
   if (eqset == AGATE_IDEAL_GLM && g->ndim < 2) return AGATE_ERR_ARG;             // GLM: 2-D and 3-D kernels
   if (s->riemann < 0 || s->riemann > 1 || s->limiter < 0 || s->limiter > 2 || s->rk < 1 || s->rk > 3) return AGATE_ERR_ARG;
   if (s->limiter == 2 && !(s->beta >= 1.0 && s->beta <= 2.0)) return AGATE_ERR_ARG;
+  for (int d = 0; d < 3; ++d) if (s->bc[d] < 0 || s->bc[d] > 1) return AGATE_ERR_ARG;
   if (eqset == AGATE_HALL && s->riemann == AGATE_HLLD) return AGATE_ERR_ARG;   // no Hall-HLLD in the paper
   if (eqset == AGATE_HALL && !(s->d_i >= 0.0)) return AGATE_ERR_ARG;
   if (eqset == AGATE_HALL && g->ndim == 3) return AGATE_ERR_ARG;               // 3-D Hall: not built yet
@@ -207,6 +208,7 @@ GhostParams make_ghost(const agate_ctx* c, double* U) {
   const Layout& L = c->L;
   p.U = U;
   p.nv = c->nv;
+  p.bcx = c->s.bc[0]; p.bcy = c->s.bc[1]; p.bcz = c->s.bc[2];
   p.nx = c->g.nx; p.ny = c->g.ny; p.nz = c->g.nz;
   p.ghy = L.ghy; p.ghz = L.ghz; p.nxp = L.nxp; p.nyp = L.nyp; p.nzp = L.nzp;
   p.sy = L.sy; p.sz = L.sz; p.sq = L.sq;

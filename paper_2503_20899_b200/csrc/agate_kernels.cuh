@@ -328,6 +328,7 @@ __global__ void __launch_bounds__(32 * (TY + 2), MINB) stage_kernel(const __grid
 struct GhostParams {
   double* U;
   int nv;
+  int bcx, bcy, bcz;         // 0 periodic, 1 zero-gradient (R26)
   int nx, ny, nz, ghy, ghz, nxp, nyp, nzp;
   long long sy, sz, sq;
   long long nzs, nys, nxs;   // cells in the z-, y-, x-slabs
@@ -363,9 +364,10 @@ __global__ void __launch_bounds__(256) ghost_fill_kernel(const __grid_constant__
       jp = (int)(row - (long long)kk * P.ny) + P.ghy;
       ip = (s < 2) ? s : P.nxp - 4 + s;
     }
-    int i = (ip - 2) % P.nx;          if (i < 0) i += P.nx;
-    int j = (jp - P.ghy) % P.ny;      if (j < 0) j += P.ny;
-    int k = (kp - P.ghz) % P.nz;      if (k < 0) k += P.nz;
+    int i = ip - 2, j = jp - P.ghy, k = kp - P.ghz;
+    if (P.bcx) i = min(max(i, 0), P.nx - 1); else { i %= P.nx; if (i < 0) i += P.nx; }
+    if (P.bcy) j = min(max(j, 0), P.ny - 1); else { j %= P.ny; if (j < 0) j += P.ny; }
+    if (P.bcz) k = min(max(k, 0), P.nz - 1); else { k %= P.nz; if (k < 0) k += P.nz; }
     const long long dst = (long long)kp * P.sz + (long long)jp * P.sy + ip;
     const long long src = (long long)(k + P.ghz) * P.sz + (long long)(j + P.ghy) * P.sy + (i + 2);
     for (int q = 0; q < P.nv; ++q) P.U[q * P.sq + dst] = P.U[q * P.sq + src];

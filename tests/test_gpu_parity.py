@@ -378,3 +378,31 @@ def test_call_order_and_bad_args(ag):
     assert ei.value.code == ag.ERR_STATE
     with pytest.raises(ag.AgateError):
         ag.Agate(shape=(32, 32, 1), dx=(1, 1, 1), ndim=2, eqset=HALL, riemann=HLLD)
+
+
+# ---- NEXT-3 (R26): zero-gradient / open boundaries ------------------------------------------------------------
+@pytest.mark.parametrize("riemann", [HLL, HLLD])
+def test_open_boundaries_brio_wu(ag, riemann):
+    """The paper's Brio-Wu tube (gamma = 2) as four identical rows, open in x and periodic in y, run until
+    the fast waves have left through both ends: GPU against the oracle, ghost rule included."""
+    n = 128
+    x = (np.arange(n) + 0.5) / n
+    W = np.zeros((8, 1, 4, n))
+    left = (x < 0.5)[None, None, :]
+    W[0] = np.where(left, 1.0, 0.125); W[4] = np.where(left, 1.0, 0.1); W[5] = 0.75; W[6] = np.where(left, 1.0, -1.0)
+    import workloads
+    U = workloads.prim_to_cons(W, 2.0)
+    kw = dict(shape=(n, 4, 1), dx=(1 / n, 1 / n, 1), ndim=2, gamma=2.0, riemann=riemann, beta=1.3, bc=(1, 0, 0))
+    ref = oracle.RefSolver(**kw); gpu = ag.Agate(**kw)
+    ref.set_state(U); gpu.set_state(U)
+    tr, tg = ref.advance(450), gpu.advance(450)
+    assert abs(tg - tr) <= 1e-12 * tr and tr > 0.3
+    assert np.all(rel_linf(gpu.get_state(), ref.get_state()) <= TOL_N)
+    assert abs(gpu.get_state()[0].sum() - U[0].sum()) > 1e-3 * U[0].sum()        # mass has left the tube
+    ref.close(); gpu.close()
+
+
+def test_open_boundaries_3d(ag):
+    """Open in z and x, periodic in y, on the 3-D kernel (config 3 recipe at 40^3)."""
+    wl = make_workload(3, n=40)
+    assert_parity(*run_pair(ag, wl, 4, bc=(1, 0, 1)))

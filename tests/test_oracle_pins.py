@@ -703,3 +703,54 @@ def test_op_counts_are_reported():
     wl = workloads.make_workload(5, n=8)
     c = oracle.count_ops(wl)
     assert 2000 < c["flops"] < 6000 and c["div"] > 10 and c["sqrt"] > 10
+
+
+# ------------------------------------------------------------------------------------------------
+# P13 (NEXT-3, R26): zero-gradient / open boundaries, on the Brio-Wu tube of P:L276
+# ------------------------------------------------------------------------------------------------
+def _brio_wu(n, gamma=2.0):
+    x = (np.arange(n) + 0.5) / n
+    W = np.zeros((8, 1, 1, n))
+    left = x < 0.5
+    W[0] = np.where(left, 1.0, 0.125); W[4] = np.where(left, 1.0, 0.1)
+    W[5] = 0.75; W[6] = np.where(left, 1.0, -1.0)
+    return W, workloads.prim_to_cons(W, gamma)
+
+
+@pytest.mark.parametrize("riemann", [oracle.HLL, oracle.HLLD])
+def test_p13_open_ends_equal_a_longer_tube(riemann):
+    """Until a wave reaches an end, a tube with zero-gradient ends must evolve bit for bit like the middle of a
+    longer periodic tube whose outer parts continue the end states: the ghost zones hold exactly what the longer
+    tube has there.  (With periodic ends instead, the jump between the end states sits on the boundary and the
+    result differs at once.)"""
+    n, pad, gamma = 64, 64, 2.0
+    W, U = _brio_wu(n, gamma)
+    Ubig = np.concatenate([np.repeat(U[..., :1], pad, axis=-1), U, np.repeat(U[..., -1:], pad, axis=-1)], axis=-1)
+    kw = dict(ndim=1, gamma=gamma, riemann=riemann, beta=1.3)
+    a = oracle.RefSolver(shape=(n, 1, 1), dx=(1.0 / n, 1, 1), bc=(1, 0, 0), **kw); a.set_state(U)
+    b = oracle.RefSolver(shape=(n + 2 * pad, 1, 1), dx=(1.0 / n, 1, 1), **kw); b.set_state(Ubig)
+    p = oracle.RefSolver(shape=(n, 1, 1), dx=(1.0 / n, 1, 1), **kw); p.set_state(U)
+    for _ in range(10):                 # fastest wave: c_f,R = 3.68 (tests/golden/brio_wu_hll.txt): 10 steps stay inside
+        dt = b.compute_dt()
+        a.step(dt); b.step(dt); p.step(dt)
+    Va, Vb, Vp = a.get_state(), b.get_state(), p.get_state()
+    assert np.array_equal(Va, Vb[..., pad:pad + n])
+    assert not np.array_equal(Va, Vp)
+    # the end zones have not moved yet, and the run is still well-posed at the ends
+    assert np.array_equal(Va[..., 0], U[..., 0]) and np.array_equal(Va[..., -1], U[..., -1])
+
+
+def test_p13_open_ends_let_waves_out():
+    """Run the tube until the fast waves have left through both ends: the state stays within the initial extremes, no
+    jump piles up at the ends (as it would at a wall), and total mass is no longer conserved."""
+    n, gamma = 128, 2.0
+    W, U = _brio_wu(n, gamma)
+    s = oracle.RefSolver(shape=(n, 1, 1), dx=(1.0 / n, 1, 1), ndim=1, gamma=gamma, riemann=oracle.HLLD, beta=1.3, bc=(1, 0, 0))
+    s.set_state(U)
+    t = 0.0
+    while t < 0.4:
+        t += s.step(0.0)
+    V = s.get_state()
+    assert np.all(np.isfinite(V)) and V[0].min() > 0.1 and V[0].max() < 1.0 + 1e-12
+    assert abs(V[0].sum() - U[0].sum()) > 1e-3 * U[0].sum()
+    assert abs(V[0, 0, 0, 0] - V[0, 0, 0, 1]) < 0.05 and abs(V[0, 0, 0, -1] - V[0, 0, 0, -2]) < 0.05   # no wall-like pile-up
