@@ -61,7 +61,7 @@ enum { AGATE_IDEAL = 0, AGATE_HALL = 1, AGATE_CGL = 2, AGATE_IDEAL_GLM = 3 };
 /* AGATE_CGL (NEXT-2; eqs.14-33; R24): CGL MHD with the logarithmic state variable of
  * eq.18.  NINE variables per cell: U = (rho, m, E, B, A_log) with E = rho v^2/2 + B^2/2 + p_par/2 + p_perp.  HLL only,
  * speeds eq.29, dt eq.28, anisotropy relaxation eqs.31-33 (C1 = 0.3, C2 = 0.5) after the Runge-Kutta update.  2-D
- * grids only in this build (a 1-D problem runs as a few identical rows). */
+ * and 3-D grids (a 1-D problem runs as a few identical rows). */
 /* AGATE_IDEAL_GLM (NEXT-1; eqs.10-11, constants L142; R22): ideal MHD with GLM
  * divergence cleaning.  NINE variables per cell, the scalar psi last: every U below is U[9][nz][ny][nx].  Per step
  * c_h = 0.95 v_max(U^n), c_p^2 = 0.18 c_h; face (B_n, psi) from the 2x2 linear Riemann problem; psi is multiplied by

@@ -69,7 +69,7 @@ int check_args(const agate_grid* g, double gamma, int eqset, const agate_solver*
   if (!(g->dx > 0.0) || (g->ndim >= 2 && !(g->dy > 0.0)) || (g->ndim >= 3 && !(g->dz > 0.0))) return AGATE_ERR_ARG;
   if (!(gamma > 1.0)) return AGATE_ERR_ARG;
   if (eqset != AGATE_IDEAL && eqset != AGATE_HALL && eqset != AGATE_IDEAL_GLM && eqset != AGATE_CGL) return AGATE_ERR_ARG;
-  if (eqset == AGATE_CGL && (g->ndim != 2 || s->riemann != AGATE_HLL)) return AGATE_ERR_ARG;   // CGL: 2-D strip kernel, HLL
+  if (eqset == AGATE_CGL && (g->ndim < 2 || s->riemann != AGATE_HLL)) return AGATE_ERR_ARG;    // CGL: 2-D and 3-D kernels, HLL
   if (eqset == AGATE_CGL && !(s->relax >= 0.0 && s->relax <= 1.0)) return AGATE_ERR_ARG;
   if (eqset == AGATE_IDEAL_GLM && g->ndim < 2) return AGATE_ERR_ARG;             // GLM: 2-D and 3-D kernels
   if (s->riemann < 0 || s->riemann > 1 || s->limiter < 0 || s->limiter > 2 || s->rk < 1 || s->rk > 3) return AGATE_ERR_ARG;
@@ -101,13 +101,14 @@ StageKernel make_stage() {
   return k;
 }
 
-template <int TY, int R, int LIM, int MINB, bool GLM = false>
+template <int TY, int R, int LIM, int MINB, bool GLM = false, bool CGL = false>
 StageKernel make_stage3d() {
   StageKernel k;
-  k.fn = stage3d_kernel<TY, R, LIM, MINB, GLM>;
-  k.ty = TY; k.np = 3; k.threads = Stage3dSmem<TY, GLM ? 9 : 8>::NT; k.smem = Stage3dSmem<TY, GLM ? 9 : 8>::BYTES;
+  k.fn = stage3d_kernel<TY, R, LIM, MINB, GLM, CGL>;
+  k.ty = TY; k.np = 3; k.threads = Stage3dSmem<TY, (GLM || CGL) ? 9 : 8>::NT;
+  k.smem = Stage3dSmem<TY, (GLM || CGL) ? 9 : 8>::BYTES;
   k.even_split = true;
-  k.fused_dt = true;
+  k.fused_dt = !CGL;         // the fused reduction evaluates the ideal-MHD speed; CGL keeps the dt_kernel pass
   return k;
 }
 
@@ -128,6 +129,8 @@ StageKernel pick_stage(int ndim, int eqset, int riemann, int limiter) {
       if (riemann == AGATE_HLLD) return make_stage<6, 3, 1, false, 2>();
       return make_stage<6, 3, 0, false, 2>();
     }
+    if (eqset == AGATE_CGL)
+      return (limiter == 2) ? make_stage3d<TY3, 0, 2, AGATE_MINB3, false, true>() : make_stage3d<TY3, 0, -1, AGATE_MINB3, false, true>();
     if (eqset == AGATE_IDEAL_GLM) {
       if (riemann == AGATE_HLLD) return (limiter == 2) ? make_stage3d<TY3, 1, 2, AGATE_MINB3, true>() : make_stage3d<TY3, 1, -1, AGATE_MINB3, true>();
       return (limiter == 2) ? make_stage3d<TY3, 0, 2, AGATE_MINB3, true>() : make_stage3d<TY3, 0, -1, AGATE_MINB3, true>();

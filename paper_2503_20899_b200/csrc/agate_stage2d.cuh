@@ -102,14 +102,14 @@ __global__ void __launch_bounds__(32 * Stage2dSmem<GLM || CGL>::NW, 2) stage2d_k
       cgl_cons_to_prim(u, w);
 #pragma unroll
       for (int q = 0; q < 9; ++q) ring[off + q * RW2] = w[q];
-      return;
+    } else {
+      double u[8], w[8];
+#pragma unroll
+      for (int q = 0; q < 8; ++q) u[q] = ring[off + q * RW2];
+      cons_to_prim(P.ph, u, w);
+#pragma unroll
+      for (int q = 0; q < 8; ++q) ring[off + q * RW2] = w[q];
     }
-    double u[8], w[8];
-#pragma unroll
-    for (int q = 0; q < 8; ++q) u[q] = ring[off + q * RW2];
-    cons_to_prim(P.ph, u, w);
-#pragma unroll
-    for (int q = 0; q < 8; ++q) ring[off + q * RW2] = w[q];
   };
 
   while (wpos < wend) {

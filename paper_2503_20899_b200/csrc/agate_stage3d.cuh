@@ -88,9 +88,11 @@ struct Stage3dSmem {
 // LIM >= 0 fixes the limiter at compile time (no branch per slope, one basic block for all eight variables);
 // LIM < 0 reads it from the parameters.
 // GLM = true: nine variables per cell, the scalar psi (index 8) behind the MHD ones (NEXT-1; eqs.10-11; R22).
-template <int TY, int RIEMANN, int LIM, int MINB, bool GLM = false>
+// CGL = true: CGL MHD (NEXT-2; R24): nine variables, W = (rho, v, p_par, B, p_perp), HLL only.
+template <int TY, int RIEMANN, int LIM, int MINB, bool GLM = false, bool CGL = false>
 __global__ void __launch_bounds__(32 * (TY + 1), MINB) stage3d_kernel(const __grid_constant__ StageParams P) {
-  constexpr int NV = GLM ? 9 : 8;
+  static_assert(!(CGL && (GLM || RIEMANN != 0)), "combination not built");
+  constexpr int NV = (GLM || CGL) ? 9 : 8;
   using SM = Stage3dSmem<TY, NV>;
   constexpr int NT = SM::NT, PL = SM::PL, SB = SM::SB, QS = SM::QS, YS = SM::YS, ZS = SM::ZS, XS = SM::XS;
   extern __shared__ __align__(16) double smem[];
@@ -155,12 +157,21 @@ __global__ void __launch_bounds__(32 * (TY + 1), MINB) stage3d_kernel(const __gr
 
   auto slot_of = [](int p) { return ((p + 3) % 3) * PL; };     // p >= -2
   auto conv_in_place = [&](int off) {
-    double u[8], w[8];                       // the GLM scalar (index 8) is its own primitive
+    if (CGL) {
+      double u[9], w[9];
 #pragma unroll
-    for (int q = 0; q < 8; ++q) u[q] = W[q * QS + off];
-    cons_to_prim(P.ph, u, w);
+      for (int q = 0; q < 9; ++q) u[q] = W[q * QS + off];
+      cgl_cons_to_prim(u, w);
 #pragma unroll
-    for (int q = 0; q < 8; ++q) W[q * QS + off] = w[q];
+      for (int q = 0; q < 9; ++q) W[q * QS + off] = w[q];
+    } else {
+      double u[8], w[8];                     // the GLM scalar (index 8) is its own primitive
+#pragma unroll
+      for (int q = 0; q < 8; ++q) u[q] = W[q * QS + off];
+      cons_to_prim(P.ph, u, w);
+#pragma unroll
+      for (int q = 0; q < 8; ++q) W[q * QS + off] = w[q];
+    }
   };
   auto copy_cell = [&](int off, long long g) {
     const double* src = P.Uin + g;           // running pointer: one 64-bit add per variable
@@ -372,7 +383,8 @@ __global__ void __launch_bounds__(32 * (TY + 1), MINB) stage3d_kernel(const __gr
         F[5] = pss;
         F[NV - 1] = ch * ch * bns;
       } else if (flux) {
-        riemann_flux<RIEMANN, false>(P.ph, L, R, nullptr, F);
+        if (CGL) flux_hll_cgl(L, R, F);
+        else riemann_flux<RIEMANN, false>(P.ph, L, R, nullptr, F);
       }
 
       // ------------------------------------------------------------------ consume the flux of task s
@@ -388,6 +400,8 @@ __global__ void __launch_bounds__(32 * (TY + 1), MINB) stage3d_kernel(const __gr
             // the difference is formed before it meets U, so that a uniform state stays bitwise fixed (pin P1)
             o[v] = c0 * (acc[v] - cz * (F[r] - FzL[v * ZS + tid]));
             if (GLM && v == NV - 1) o[v] *= decay;                        // eq.11's source, integrated exactly
+            if (CGL && v == NV - 1 && P.last_stage && P.relax > 0.0 && emit && cell_ok)
+              o[v] = cgl_relaxed_alog(P.relax, o);                        // eqs.31-33: E stays, A_log moves
             if (emit && cell_ok) *po = o[v];
             FzL[v * ZS + tid] = F[r];
             acc[v] = 0.0;
