@@ -170,6 +170,22 @@ def run_reference(args):
     print(json.dumps(line))
 
 
+def max_over_ranks(x, world, device):
+    """Timing rule for N > 1 (replicas only, no data-path collective): every rank times its own K steps on the
+    device, the job's time is the MAX over ranks."""
+    import torch
+    import torch.distributed as dist
+    t = torch.tensor([x], dtype=torch.float64, device=device)
+    if world > 1:
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return float(t.item())
+
+
+def aggregate_rate(zones_per_rank, world, steps, ms_max):
+    """Whole-job zone-updates/s: every rank advanced its own replica (weak scaling) in the slowest rank's time."""
+    return zones_per_rank * world * steps / (ms_max * 1e-3)
+
+
 def run_ours(args):
     import numpy as np
     import torch
@@ -215,11 +231,8 @@ def run_ours(args):
         barrier()
     ms = e0.elapsed_time(e1)
     sim.poll()
-    t_ms = torch.tensor([ms], dtype=torch.float64, device=dev)
-    if world > 1:
-        dist.all_reduce(t_ms, op=dist.ReduceOp.MAX)
-    ms_max = float(t_ms.item())
-    value = zones * world * K / (ms_max * 1e-3)
+    ms_max = max_over_ranks(ms, world, dev)
+    value = aggregate_rate(zones, world, K, ms_max)
 
     # ---- per-launch duration of the dominant kernel (fused stage), CUDA events on its own stream ---------
     sim.set_state(Uh)
@@ -259,11 +272,9 @@ def run_ours(args):
             a, b = b, a
         barrier()
         te = time.perf_counter() - t0
-        t_e = torch.tensor([te], dtype=torch.float64, device=dev)
-        if world > 1:
-            dist.all_reduce(t_e, op=dist.ReduceOp.MAX)
+        te_max = max_over_ranks(te, world, dev)
         nbytes = Uh.numel() * 8
-        e2e = {"value": zones * world * Ke / float(t_e.item()), "unit": UNIT, "h2d_bytes_per_step": nbytes,
+        e2e = {"value": aggregate_rate(zones, world, Ke, te_max * 1e3), "unit": UNIT, "h2d_bytes_per_step": nbytes,
                "d2h_bytes_per_step": nbytes, "steps": Ke,
                "note": "agate_set_state(host pinned) + agate_step + agate_get_state(host pinned) per step"}
 
