@@ -398,37 +398,37 @@ AG_HD double cell_speed(const Phys& ph, const double U[8]) {
 // CGL MHD (NEXT-2; R24).  Nine variables per cell:
 //   U = (rho, m, E, B, A_log),  E = rho v^2/2 + B^2/2 + p_par/2 + p_perp,  A_log as eq.18
 //   W = (rho, v, p_par, B, p_perp): p_par in slot 4, p_perp in slot 8 (slot 8 is not rotated)
-// IEEE division / sqrt / exp / log: this path is not the tuned one.
+// Reciprocals and roots as in the ideal path (MUFU seed + Newton, a few ulp); exp / log from the CUDA math library.
 // ------------------------------------------------------------------------------------------------------------
 AG_HD void cgl_cons_to_prim(const double U[9], double W[9]) {          // eqs.26-27
-  const double ir = 1.0 / U[0];
+  const double ir = rcp(U[0]);
   const double vx = U[1] * ir, vy = U[2] * ir, vz = U[3] * ir;
   const double b2 = U[5] * U[5] + U[6] * U[6] + U[7] * U[7];
   const double eint = U[4] - 0.5 * U[0] * (vx * vx + vy * vy + vz * vz) - 0.5 * b2;
-  const double B3 = b2 * sqrt(b2);
+  const double B3 = b2 * sqrt_pos(dmax(b2, kTiny));
   const double X = U[0] * U[0] * exp(-U[8] * ir);
-  const double iden = 1.0 / (X + 2.0 * B3);
+  const double iden = rcp(X + 2.0 * B3);
   W[0] = U[0]; W[1] = vx; W[2] = vy; W[3] = vz;
   W[4] = 2.0 * X * eint * iden;
   W[5] = U[5]; W[6] = U[6]; W[7] = U[7];
   W[8] = 2.0 * B3 * eint * iden;
 }
 AG_HD double cgl_alog(double rho, double b2, double ppar, double pperp) {   // eq.18
-  return rho * log((rho * rho / (b2 * sqrt(b2))) * (pperp / ppar));
+  return rho * log((rho * rho * pperp) * rcp(b2 * sqrt_pos(dmax(b2, kTiny)) * ppar));
 }
 // eq.29, fast branch, along the face normal of a ROTATED state (w[5] = B_n)
 AG_HD double cgl_cfast(const double w[9]) {
   const double B2 = w[5] * w[5] + w[6] * w[6] + w[7] * w[7];
-  const double cos2 = w[5] * w[5] / B2;
+  const double cos2 = w[5] * w[5] * rcp(B2);
   const double b1 = B2 + 2.0 * w[8] + cos2 * (2.0 * w[4] - w[8]);
   const double b2 = b1 - 6.0 * cos2 * w[4];
   const double c = 4.0 * w[8] * w[8] * cos2 * (1.0 - cos2);
-  return sqrt((b1 + sqrt(b2 * b2 + c)) / (2.0 * w[0]));
+  return sqrt_pos((b1 + sqrt_pos(dmax(b2 * b2 + c, kTiny))) * (0.5 * rcp(w[0])));
 }
 // eqs.19-22 (psi == 0) + eq.17 in the rotated frame; also returns the conserved vector of the state
 AG_HD void cgl_flux_and_cons(const double w[9], double f[9], double u[9]) {
   const double B2 = w[5] * w[5] + w[6] * w[6] + w[7] * w[7];
-  const double th = 1.0 - (w[4] - w[8]) / B2;
+  const double th = 1.0 - (w[4] - w[8]) * rcp(B2);
   const double v2 = w[1] * w[1] + w[2] * w[2] + w[3] * w[3];
   const double vB = w[1] * w[5] + w[2] * w[6] + w[3] * w[7];
   u[0] = w[0]; u[1] = w[0] * w[1]; u[2] = w[0] * w[2]; u[3] = w[0] * w[3];
@@ -453,7 +453,7 @@ AG_HD void flux_hll_cgl(const double L[9], const double R[9], double F[9]) {
   const double cl = cgl_cfast(L), cr = cgl_cfast(R);
   const double sL = dmin(dmin(L[1] - cl, R[1] - cr), 0.0);
   const double sR = dmax(dmax(L[1] + cl, R[1] + cr), 0.0);
-  const double iw = 1.0 / (sR - sL);
+  const double iw = rcp(sR - sL);
 #pragma unroll
   for (int q = 0; q < 9; ++q) F[q] = (sR * fl[q] - sL * fr[q] + sL * sR * (ur[q] - ul[q])) * iw;
 }
