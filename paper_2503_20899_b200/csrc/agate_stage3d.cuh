@@ -24,8 +24,9 @@
 //   * A6: the accumulator of plane k gets Uin (+U0 in the second SSP stage) right after
 //     barrier 1 (the loads are issued just before it), then the x and y differences; plane k leaves in step k+1.
 //
-// Shared memory per CTA: ring 3 planes x 8 x TY x 36, y-halo rows 2 x 8 x 4 x 36, YR/YF 8 x (TY+1) x 32 each,
-// z carries 2 x 8 x TY x 32, XR/XF 8 x TY each:  TY = 6 -> 111 KB (2 CTAs/SM, 14 warps),  TY = 14 -> 227 KB (1 CTA, 15).
+// Shared memory per CTA (NV = 8 variables; 9 with GLM or CGL): ring 3 planes x NV x TY x 36, y-halo rows
+// 2 x NV x 4 x 36, YR / YF NV x (TY+1) x 32 each, z carries 2 x NV x TY x 32, XR / XF NV x TY each, 16 phase counters:
+// TY = 11 -> 186 KB (214 KB with 9 variables), one CTA of 12 warps per SM, <= 168 registers.
 #pragma once
 #include <cuda_runtime.h>
 #include <stdint.h>
