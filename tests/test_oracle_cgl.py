@@ -8,8 +8,10 @@ import numpy as np
 import pytest
 
 import oracle
+from conftest import read_golden
 
 G = 5.0 / 3.0
+GOLD = read_golden("cgl.txt")          # the numbers PAPER.md prints for its CGL benchmarks (L318-334)
 
 
 def cons_line(W):
@@ -50,7 +52,7 @@ def test_c2_magnetosonic_speeds():
     sqrt((B^2 + 2 p_perp)/rho); parallel propagation gives the larger of the CGL parallel sound speed
     sqrt(3 p_par/rho) and the firehose-modified Alfven speed sqrt((B^2 + p_perp - p_par)/rho) (textbook CGL)."""
     W = np.array([1, 5, 0, 0, 14, 0, 15, 0, 17.0])
-    assert abs(oracle.cgl_cfast(0, W) - 16.09) < 0.005
+    assert abs(oracle.cgl_cfast(0, W) - GOLD["prop_vms"][0]) < 0.005
     assert abs(oracle.cgl_cfast(0, W) - np.sqrt(15 ** 2 + 2 * 17)) <= 1e-13
     for ppar, pperp, B in [(1.0, 2.0, 3.0), (5.0, 0.5, 1.0), (0.3, 0.3, 0.2)]:
         Wp = np.array([0.8, 0, 0, 0, ppar, B, 0, 0, pperp])
@@ -113,12 +115,12 @@ def test_c5_propagating_wave_speeds():
     dBy = V[6] - 15
     centroid = lambda sel, f: float(np.sum(x[sel] * f[sel]) / np.sum(f[sel]))
     right, left, mid = (x > 16) & (x < 26), (x > -16) & (x < -6), (x > 1) & (x < 9)
-    assert abs(centroid(right, np.maximum(dBy, 0)) - 21.09) < 0.15
-    assert abs(centroid(left, np.maximum(dBy, 0)) + 11.09) < 0.15
+    assert abs(centroid(right, np.maximum(dBy, 0)) - GOLD["prop_fast_plus"][0]) < 0.15
+    assert abs(centroid(left, np.maximum(dBy, 0)) - GOLD["prop_fast_minus"][0]) < 0.15
     # the CGL invariant p_perp/(rho B) (eq.15) is carried by the flow alone: its perturbation sits at x = v_x t = 5
     Wt = np.stack([oracle.cgl_cons_to_prim(V[:, i]) for i in range(n)], axis=1)
     inv = Wt[8] / (Wt[0] * np.abs(Wt[6]))
-    assert abs(centroid(mid, np.abs(inv - 17.0 / 15.0)) - 5.0) < 0.1
+    assert abs(centroid(mid, np.abs(inv - 17.0 / 15.0)) - GOLD["prop_vx"][0]) < 0.1
     assert np.max(np.abs(inv - 17.0 / 15.0)[~mid]) < 0.02 * np.max(np.abs(inv - 17.0 / 15.0))
 
 
@@ -140,7 +142,7 @@ def test_c6_firehose_growth_rate(scale, t0, t1):
     run_to(s, t0); a0 = amp()
     run_to(s, t1 - t0); a1 = amp()
     rate = np.log(a1 / a0) / (t1 - t0)
-    assert abs(rate - 1.0472) < 0.03 * 1.0472, rate
+    assert abs(rate - GOLD["firehose_rate"][0]) < 0.03 * GOLD["firehose_rate"][0], rate
 
 
 def _state2d(n, seed):
