@@ -179,36 +179,28 @@ __global__ void __launch_bounds__(32 * (TY + 1), MINB) stage3d_kernel(const __gr
 #pragma unroll
     for (int q = 0; q < NV; ++q, src += P.sq) cp_async8(W + q * QS + off, src);
   };
-  // H's copy tasks for plane p: t < 4 TY -> x-halo columns of the ring rows;  else -> the four y-halo rows
-  constexpr int NHT = 4 * TY + 4 * RS;
-  auto htask = [&](int t, int p, int slot, int& off, long long& g) -> bool {
-    int j, c;
-    if (t < 4 * TY) {
-      j = t >> 2;
-      c = t & 3;
-      c = (c < 2) ? c : 32 + c;
-      off = slot + j * RS + c;
-    } else {
-      const int u = t - 4 * TY, r = u / RS;
-      c = u - r * RS;
-      j = (r < 2) ? r - 2 : TY + r - 2;
-      off = 3 * PL + (p & 1) * SB + u;
+  // H's halo cells of plane p.  The four y-halo rows: one pass per row, lane = column of the tile (the row's own
+  // x-halo corners are never read).  The x-halo columns of the ring rows: four cells per row, ceil(4 TY / 32) passes.
+  // Fully unrolled with closed-form offsets: this work sits on H's critical path in phase B.
+  constexpr int NHC = (4 * TY + 31) / 32;
+  auto h_cells = [&](int p, int slot, auto&& fn) {
+    const long long gp = (long long)(p + 2) * P.sz + x0;
+    const bool xin = x0 + lane + 2 < P.nxp;
+#pragma unroll
+    for (int r = 0; r < 4; ++r) {
+      const int j = (r < 2) ? r - 2 : TY + r - 2;
+      if (xin && y0 + j + 2 < P.nyp)
+        fn(3 * PL + (p & 1) * SB + r * RS + lane + 2, gp + (long long)(y0 + j + 2) * P.sy + lane + 2);
     }
-    g = (long long)(p + 2) * P.sz + (long long)(y0 + j + 2) * P.sy + (x0 + c);
-    return (x0 + c < P.nxp) && (y0 + j + 2 < P.nyp);
-  };
-  auto h_copy = [&](int p, int slot) {
-    for (int t = lane; t < NHT; t += 32) {
-      int off; long long g;
-      if (htask(t, p, slot, off, g)) copy_cell(off, g);
+#pragma unroll
+    for (int i = 0; i < NHC; ++i) {
+      const int t = lane + 32 * i, j = t >> 2, cc = t & 3, c = (cc < 2) ? cc : 32 + cc;
+      if (t < 4 * TY && x0 + c < P.nxp && y0 + j + 2 < P.nyp)
+        fn(slot + j * RS + c, gp + (long long)(y0 + j + 2) * P.sy + c);
     }
   };
-  auto h_conv = [&](int p, int slot) {
-    for (int t = lane; t < NHT; t += 32) {
-      int off; long long g;
-      if (htask(t, p, slot, off, g)) conv_in_place(off);
-    }
-  };
+  auto h_copy = [&](int p, int slot) { h_cells(p, slot, [&](int off, long long g) { copy_cell(off, g); }); };
+  auto h_conv = [&](int p, int slot) { h_cells(p, slot, [&](int off, long long) { conv_in_place(off); }); };
 
   // ---- prologue: everything step k0 needs that the steady state would have produced earlier ----
   for (int i = tid; i < NV * QS; i += NT) W[i] = 1.0;           // cells outside the padded array (ragged tiles)
