@@ -46,8 +46,8 @@ FLOP_DT_PER_ZONE = {1: 45.0, 2: 45.0, 3: 45.0, 4: 60.0, 5: 45.0, 6: 45.0, 7: 90.
 BYTES_PER_ZONE_STEP = 320.0            # 5 x 8 variables x 8 B; 360 with the GLM scalar (config 6)
 # DRAM bytes per launch of the dominant kernel (dram__bytes_read.sum + dram__bytes_write.sum, mean of the two stage
 # launches of one step) from the committed `ncu` capture of the same command: profiles/r1_stage3d.md
-NCU_TRAFFIC_BYTES = {5: 0.5 * (9617129216 + 8682435584 + 18299382528 + 8663042304),
-                     2: 0.5 * (285912064 + 227066880 + 561840896 + 226612736)}
+NCU_TRAFFIC_BYTES = {5: 0.5 * (9532646144 + 8676093184 + 20187381504 + 8776886784),
+                     2: 0.5 * (285508864 + 226625280 + 561331200 + 226205952)}
 FP64_NOMINAL_TFLOPS = 148 * 64 * 2 * 1.965e9 / 1e12     # 148 SMs x 64 DFMA lanes x 2 x max SM clock = 37.2
 
 # reduced size of the bounded CPU sample per config (same recipe and seed), and its step count
