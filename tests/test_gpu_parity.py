@@ -406,3 +406,36 @@ def test_open_boundaries_3d(ag):
     """Open in z and x, periodic in y, on the 3-D kernel (config 3 recipe at 40^3)."""
     wl = make_workload(3, n=40)
     assert_parity(*run_pair(ag, wl, 4, bc=(1, 0, 1)))
+
+
+# ---- seeded sweep over shapes, options and work splits ----------------------------------------------------------
+@pytest.mark.parametrize("seed", range(24))
+def test_random_shapes_and_options(ag, seed, monkeypatch):
+    """Ragged sizes around the tile / strip / segment boundaries (nx around 30, 32, 60, 64; ny around 11, 22; small nz),
+    every solver option, periodic and open ends, default and forced work splits -- 3 steps against the oracle."""
+    rng = np.random.default_rng(9000 + seed)
+    ndim = int(rng.choice([2, 3]))
+    nx = int(rng.choice([5, 29, 30, 31, 32, 33, 59, 61, 64, 65, 70]))
+    ny = int(rng.choice([3, 10, 11, 12, 21, 23, 34]))
+    nz = int(rng.choice([3, 7, 16, 19])) if ndim == 3 else 1
+    hall = ndim == 2 and rng.random() < 0.25
+    riemann = HLL if hall else int(rng.choice([HLL, HLLD]))
+    limiter, beta = [(0, 1.0), (1, 1.0), (2, 1.0), (2, 1.3), (2, 2.0)][int(rng.integers(5))]
+    rk = int(rng.choice([1, 2, 3]))
+    bc = tuple(int(b) for b in rng.integers(0, 2, 3))
+    if rng.random() < 0.5:
+        monkeypatch.setenv("AGATE_GRID", str(int(rng.choice([1, 3, 17, 80]))))
+    import workloads
+    W, U = workloads.random_state(100 + seed, (nx, ny, nz), ndim, amp=0.3)
+    kw = dict(shape=(nx, ny, nz), dx=(1.0 / nx, 1.3 / ny, 0.7 / nz if ndim == 3 else 1.0), ndim=ndim, riemann=riemann,
+              limiter=limiter, beta=beta, rk=rk, bc=bc, eqset=(ag.HALL if hall else ag.IDEAL), d_i=(0.02 if hall else 0.0))
+    ref = oracle.RefSolver(**kw); gpu = ag.Agate(**kw)
+    ref.set_state(U); gpu.set_state(U)
+    for s in range(3):
+        dtr, dtg = ref.compute_dt(), gpu.compute_dt()
+        assert abs(dtg - dtr) <= TOL_DT * dtr, (kw, s)
+        ref.step(0.5 * dtr)                     # random cell-to-cell data: half the Courant step keeps it physical
+        gpu.step(0.5 * dtr)
+        e = rel_linf(gpu.get_state(), ref.get_state())
+        assert np.all(e <= 1e-11), (kw, s, e)
+    ref.close(); gpu.close()
