@@ -119,7 +119,7 @@ StageKernel make_stage2d() {
   k.ty = 1; k.np = 1; k.threads = 32 * Stage2dSmem<GLM || CGL>::NW; k.smem = Stage2dSmem<GLM || CGL>::BYTES;
   k.warps2d = Stage2dSmem<GLM || CGL>::NW;
   k.strips2d = true;
-  k.fused_dt = !H && !CGL;   // the fused reduction evaluates the ideal-MHD speed; Hall and CGL keep the dt_kernel pass
+  k.fused_dt = !CGL;         // the fused reduction evaluates the ideal / Hall speed; CGL keeps the dt_kernel pass
   return k;
 }
 

@@ -485,8 +485,9 @@ AG_HD double cell_speed_cgl(const double U[9]) {
   return (sp - sp == 0.0) ? sp : -1.0;
 }
 
-// A7 inside the stage epilogue (ideal MHD): the same quantity as cell_speed<false> with the straight-line roots of
+// A7 inside the stage epilogue (ideal and Hall MHD): the same quantity as cell_speed<HALL> with the straight-line roots of
 // this file, evaluated on the conserved values the stage is about to store.
+template <bool HALL = false>
 AG_HD double cell_speed_inline(const Phys& ph, const double U[8]) {
   const double ir = rcp(U[0]);
   const double v2 = (U[1] * U[1] + U[2] * U[2] + U[3] * U[3]) * (ir * ir);
@@ -496,7 +497,13 @@ AG_HD double cell_speed_inline(const Phys& ph, const double U[8]) {
   if (!(U[0] > 0.0) || !(p > 0.0)) return -1.0;
   const double a2 = ph.gamma * p * ir, sm = a2 + B2 * ir;
   const double rad = dmax(sm * sm - 4.0 * a2 * (dmin(dmin(bx2, by2), bz2) * ir), kTiny);
-  const double sp = sqrt_pos(dmax(v2, kTiny)) + sqrt_pos(0.5 * (sm + sqrt_pos(rad)));
+  double c = sqrt_pos(0.5 * (sm + sqrt_pos(rad)));
+  if (HALL) {
+    // eq.13: c_w = aw + sqrt(aw^2 + v_A^2),  aw = d_i pi |B| / (2 rho dx_min)
+    const double aw = ph.cwk * sqrt_pos(dmax(B2, kTiny)) * ir;
+    c = dmax(c, aw + sqrt_pos(dmax(aw * aw + B2 * ir, kTiny)));
+  }
+  const double sp = sqrt_pos(dmax(v2, kTiny)) + c;
   return (sp - sp == 0.0) ? sp : -1.0;
 }
 

@@ -14,7 +14,7 @@
 //     primitives in place (A1); the raw Uin (+U0, copied straight into the same slot) of the own cell is kept for A6.
 //   * work = (strip, row) pairs over the warps of a one-wave grid: every strip cut into the same row ranges,
 //     consecutive warps on consecutive strips (L2 serves the shared halo columns).
-//   * A7 of the next step rides in the last stage, as in stage3d_kernel (ideal MHD; Hall keeps the dt_kernel pass).
+//   * A7 of the next step rides in the last stage, as in stage3d_kernel (ideal, Hall, GLM; CGL keeps the dt_kernel pass).
 //   * Hall (A8): the face current comes from the cell-centred B of the three ring rows around the face.
 //
 // Shared memory per warp: ring 4 x 8 x 34, two y carries 8 x 32, raw U 2 x 8 x 32  =  16.5 KB;  6 warps per CTA,
@@ -250,7 +250,7 @@ __global__ void __launch_bounds__(32 * Stage2dSmem<GLM || CGL>::NW, 2) stage2d_k
           acc[v] = Uraw[((j & 1) * NV + v) * 32 + lane];
         }
         if (P.vnext != nullptr && emit && cell_ok) {                      // A7 on the values just stored
-          const double sp2 = cell_speed_inline(P.ph, o);
+          const double sp2 = cell_speed_inline<HALL>(P.ph, o);
           if (sp2 < 0.0) bad = 1; else vmx = dmax(vmx, sp2);
         }
       }
