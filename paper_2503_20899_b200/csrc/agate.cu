@@ -143,13 +143,15 @@ StageKernel pick_stage(int ndim, int eqset, int riemann, int limiter) {
     return make_stage3d<TY3, 0, -1, AGATE_MINB3>();
   }
   if (ndim == 2 && !getenv("AGATE_STAGE_V1")) {   // warp-autonomous strips
-    if (eqset == AGATE_HALL) return (limiter == 2) ? make_stage2d<0, 2, true>() : make_stage2d<0, -1, true>();
+    if (eqset == AGATE_HALL)
+      return (limiter == 3) ? make_stage2d<0, 3, true>() : ((limiter == 2) ? make_stage2d<0, 2, true>() : make_stage2d<0, -1, true>());
     if (eqset == AGATE_CGL) return (limiter == 2) ? make_stage2d<0, 2, false, false, true>() : make_stage2d<0, -1, false, false, true>();
     if (eqset == AGATE_IDEAL_GLM) {
       if (riemann == AGATE_HLLD) return (limiter == 2) ? make_stage2d<1, 2, false, true>() : make_stage2d<1, -1, false, true>();
       return (limiter == 2) ? make_stage2d<0, 2, false, true>() : make_stage2d<0, -1, false, true>();
     }
-    if (limiter == 2) {
+    if (limiter == 3 && riemann == AGATE_HLL) return make_stage2d<0, 3, false>();     // eq.4 at beta = 1: minmod
+    if (limiter >= 2) {
       if (riemann == AGATE_HLLD) return make_stage2d<1, 2, false>();
       return make_stage2d<0, 2, false>();
     }
@@ -400,7 +402,10 @@ int agate_init(const agate_grid* grid, double gamma, int eqset, const agate_solv
   c->vnext = (unsigned long long*)(c->ws + L.off_scal + 192);
   c->partial = (double*)(c->ws + L.off_partial);
 
-  c->sk = pick_stage(grid->ndim, eqset, solver->riemann, solver->limiter);
+  // eq.4 at beta = 1 is plain minmod: the 2-D HLL kernels (configs 1 and 4) have a variant without its third argument
+  c->sk = pick_stage(grid->ndim, eqset, solver->riemann,
+                     (solver->limiter == 2 && solver->beta == 1.0 && grid->ndim == 2 && solver->riemann == AGATE_HLL &&
+                      (eqset == AGATE_IDEAL || eqset == AGATE_HALL)) ? 3 : solver->limiter);
   cudaError_t e = cudaFuncSetAttribute((const void*)c->sk.fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)c->sk.smem);
   cudaFuncAttributes fa;
   if (e == cudaSuccess) e = cudaFuncGetAttributes(&fa, (const void*)c->sk.fn);

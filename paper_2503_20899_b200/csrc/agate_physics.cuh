@@ -164,10 +164,12 @@ AG_HD double limited_slope(int limiter, double beta, double dp, double dm) {
 
 // Half of the eq.4 slope (what the face states W -+ dW/2 use), with the factor folded into the constants:
 // hbeta = beta / 2.  Scaling by a power of two is exact, so this is 0.5 * limited_slope bit for bit.
+// limiter 3 = eq.4 at beta = 1 (minmod): min(|dp|,|dm|)/2 never exceeds (|dp|+|dm|)/4, rounding included (the sum of
+// two doubles is at least twice the smaller one), so the third argument of eq.4 drops out bit for bit.
 AG_HD double half_slope(int limiter, double hbeta, double dp, double dm) {
-  if (limiter == 2) {
+  if (limiter >= 2) {
     const double a = fabs(dp), b = fabs(dm);
-    const double m = dmin(hbeta * dmin(a, b), 0.25 * (a + b));
+    const double m = (limiter == 3) ? 0.5 * dmin(a, b) : dmin(hbeta * dmin(a, b), 0.25 * (a + b));
 #if defined(__CUDA_ARCH__)
     const int hp = __double2hiint(dp), hm = __double2hiint(dm);
     const int hi = (__double2hiint(m) | (hp & 0x80000000)) & ~((hp ^ hm) >> 31);
