@@ -297,8 +297,13 @@ __global__ void __launch_bounds__(32 * (TY + 1), MINB) stage3d_kernel(const __gr
           flux = true;
         } else if (full) {
           if (s == 1) {
+            if (two) {                                                     // A6: Uin + (a0/a1) U0  (uniform branch)
 #pragma unroll
-            for (int q = 0; q < NV; ++q) acc[q] += two ? fma(P.r0, ub[q], ua[q]) : ua[q];      // A6: Uin (+ (a0/a1) U0)
+              for (int q = 0; q < NV; ++q) acc[q] += fma(P.r0, ub[q], ua[q]);
+            } else {
+#pragma unroll
+              for (int q = 0; q < NV; ++q) acc[q] += ua[q];
+            }
 #pragma unroll
             for (int r = 0; r < NV; ++r) {
               L[r] = Ly[r];
@@ -420,9 +425,16 @@ __global__ void __launch_bounds__(32 * (TY + 1), MINB) stage3d_kernel(const __gr
             const double* pa = P.Uin + gm + P.sz;
             const double* pb = P.U0 + gm + P.sz;
 #pragma unroll
-            for (int q = 0; q < NV; ++q, pa += P.sq, pb += P.sq) {
-              ua[q] = cell_ok ? __ldg(pa) : 0.0;
-              ub[q] = (cell_ok && two) ? *pb : 0.0;
+            for (int q = 0; q < NV; ++q) { ua[q] = 0.0; ub[q] = 0.0; }
+            if (cell_ok) {
+              // uniform branches on the stage kind: the first stage issues no U0 loads and no selects
+              if (two) {
+#pragma unroll
+                for (int q = 0; q < NV; ++q, pa += P.sq, pb += P.sq) { ua[q] = __ldg(pa); ub[q] = *pb; }
+              } else {
+#pragma unroll
+                for (int q = 0; q < NV; ++q, pa += P.sq) ua[q] = __ldg(pa);
+              }
             }
           }
         } else if (full) {
