@@ -73,11 +73,12 @@ enum {
   AGATE_ERR_ARG = 1,          /* null pointer, bad size, unsupported combination (Hall + HLLD)       */
   AGATE_ERR_STATE = 2,        /* call order: no state set yet                                        */
   AGATE_ERR_UNPHYSICAL = 3,   /* rho <= 0, p <= 0 or a non-finite speed seen by the dt reduction (R14) */
-  AGATE_ERR_CUDA = 4,         /* CUDA runtime error, or no CUDA device                               */
+  AGATE_ERR_CUDA = 4,         /* CUDA runtime error, no CUDA device, or a hand-over wait inside a kernel ran out */
   AGATE_ERR_NOMEM = 5         /* workspace too small or misaligned                                   */
 };
 
-/* Bytes of device workspace agate_init needs for this problem (0 on invalid arguments). */
+/* Bytes of device workspace agate_init needs for this problem (0 on invalid arguments): two ghost-padded copies of
+ * the state (three with rk = 3), 8 or 9 variables each, plus a few hundred bytes of device scalars. */
 size_t agate_workspace_bytes(const agate_grid* grid, int eqset, const agate_solver* solver);
 
 /* Create a context.  `workspace`: DEVICE pointer, caller-owned, >= agate_workspace_bytes(), 256-byte aligned,
@@ -87,9 +88,11 @@ size_t agate_workspace_bytes(const agate_grid* grid, int eqset, const agate_solv
 int agate_init(const agate_grid* grid, double gamma, int eqset, const agate_solver* solver,
                void* workspace, size_t workspace_bytes, void* stream, agate_ctx** out);
 
-/* Copy an interior-only SoA state U[8][nz][ny][nx] into the context and set the time to t0.
+/* Copy an interior-only SoA state U[8][nz][ny][nx] (U[9]... for AGATE_IDEAL_GLM / AGATE_CGL) into the context and set
+ * the time to t0.
  * `U` is a HOST pointer when src_is_device == 0 (pinned memory makes the copy asynchronous), else a DEVICE
- * pointer.  Fills the periodic ghost layers (A0).  Validates nothing physical (the dt reduction does). */
+ * pointer.  Fills the ghost layers (A0; periodic or zero-gradient per solver->bc).  Validates nothing physical (the
+ * dt reduction does). */
 int agate_set_state(agate_ctx*, const double* U, int src_is_device, double t0);
 
 /* A7: dt = C dx_min / max_cells(|v| + max(c_f, c_w)) of the current state -> *dt_out (HOST).
