@@ -145,3 +145,56 @@ def test_cgl_rejected_where_not_built(ag):
         with pytest.raises(ag.AgateError) as ei:
             ag.Agate(eqset=ag.CGL, **kw)
         assert ei.value.code == ag.ERR_ARG
+
+
+def test_cgl_brio_wu_open_ends(ag):
+    """The paper's CGL shock tube (the Brio-Wu states with zero initial anisotropy), four identical rows, open
+    in x, default relaxation, run until the fast waves have left: GPU against the oracle."""
+    n = 128
+    x = (np.arange(n) + 0.5) / n
+    left = (x < 0.5)[None, None, :]
+    W = np.zeros((9, 1, 4, n))
+    W[0] = np.where(left, 1.0, 0.125); W[4] = np.where(left, 1.0, 0.1); W[8] = W[4]
+    W[5] = 0.75; W[6] = np.where(left, 1.0, -1.0)
+    U = cons_field(W)
+    ref, gpu = pair(ag, (n, 4, 1), (1 / n, 1 / n, 1), 0.99, bc=(1, 0, 0))
+    ref.set_state(U); gpu.set_state(U)
+    tr, tg = ref.advance(300), gpu.advance(300)
+    assert abs(tg - tr) <= 1e-12 * tr and tr > 0.15
+    assert np.all(rel_linf9(gpu.get_state(), ref.get_state()) <= TOL_N)
+    ref.close(); gpu.close()
+
+
+@pytest.mark.parametrize("seed", range(6))
+def test_cgl_random_shapes_and_options(ag, seed, monkeypatch):
+    """Seeded sweep for the CGL path: ragged 2-D and 3-D shapes, every limiter and RK scheme, relaxation on and off,
+    periodic and open ends, default and forced work splits -- 3 steps against the oracle."""
+    rng = np.random.default_rng(8000 + seed)
+    ndim = int(rng.choice([2, 3]))
+    nx, ny = int(rng.choice([29, 31, 33, 61, 64])), int(rng.choice([5, 11, 12, 23]))
+    nz = int(rng.choice([4, 9, 17])) if ndim == 3 else 1
+    limiter, beta = [(0, 1.0), (1, 1.0), (2, 1.0), (2, 1.3)][int(rng.integers(4))]
+    rk = int(rng.choice([1, 2, 3]))
+    relax = float(rng.choice([0.0, 0.5, 0.99]))
+    bc = tuple(int(b) for b in rng.integers(0, 2, 3))
+    if rng.random() < 0.5:
+        monkeypatch.setenv("AGATE_GRID", str(int(rng.choice([1, 5, 40]))))
+    shp = (nz, ny, nx)
+    W = np.empty((9,) + shp)
+    W[0] = 0.5 + rng.random(shp); W[4] = 0.5 + rng.random(shp); W[8] = 0.5 + rng.random(shp)
+    for q in (1, 2, 3):
+        W[q] = 0.3 * (2 * rng.random(shp) - 1)
+    for q in (5, 6, 7):
+        W[q] = 0.4 + 0.3 * (2 * rng.random(shp) - 1)               # |B| bounded away from zero (A_log needs it)
+    U = cons_field(W)
+    kw = dict(shape=(nx, ny, nz), dx=(1.0 / nx, 1.3 / ny, 0.7 / nz if ndim == 3 else 1.0), ndim=ndim, riemann=0,
+              limiter=limiter, beta=beta, rk=rk, bc=bc, relax=relax)
+    ref = oracle.RefSolver(eqset=oracle.CGL, **kw); gpu = ag.Agate(eqset=ag.CGL, **kw)
+    ref.set_state(U); gpu.set_state(U)
+    for s in range(3):
+        dtr, dtg = ref.compute_dt(), gpu.compute_dt()
+        assert abs(dtg - dtr) <= TOL_DT * dtr, (kw, s)
+        ref.step(0.5 * dtr); gpu.step(0.5 * dtr)
+        e = rel_linf9(gpu.get_state(), ref.get_state())
+        assert np.all(e <= 1e-11), (kw, s, e)
+    ref.close(); gpu.close()
