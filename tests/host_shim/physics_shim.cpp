@@ -26,6 +26,24 @@ void shim_cons_to_prim(double gamma, const double* U, double* W) {
 
 double shim_slope(int limiter, double beta, double dp, double dm) { return limited_slope(limiter, beta, dp, dm); }
 
+double shim_half_slope(int limiter, double hbeta, double dp, double dm) { return half_slope(limiter, hbeta, dp, dm); }
+
+double shim_cell_speed_inline(int eqset, double gamma, double d_i, double dxmin, const double* U) {
+  Phys ph = make_phys(gamma, eqset == 1 ? d_i : 0.0, dxmin);
+  return eqset == 1 ? cell_speed_inline<true>(ph, U) : cell_speed_inline<false>(ph, U);
+}
+
+// CGL (R24): the kernels' point functions, rotated frame handled here as the kernels do
+void shim_cgl_cons_to_prim(const double* U, double* W) { cgl_cons_to_prim(U, W); }
+void shim_cgl_face_flux(int dir, const double* WL, const double* WR, double* F) {
+  double L[9], R[9], Fr[9];
+  for (int r = 0; r < 9; ++r) { const int v = (r < 8) ? rot_var(r, dir) : r; L[r] = WL[v]; R[r] = WR[v]; }
+  flux_hll_cgl(L, R, Fr);
+  for (int r = 0; r < 9; ++r) F[(r < 8) ? rot_var(r, dir) : r] = Fr[r];
+}
+double shim_cgl_relaxed_alog(double f, const double* U) { return cgl_relaxed_alog(f, U); }
+double shim_cell_speed_cgl(const double* U) { return cell_speed_cgl(U); }
+
 double shim_cell_speed(int eqset, double gamma, double d_i, double dxmin, const double* U) {
   Phys ph = make_phys(gamma, eqset == 1 ? d_i : 0.0, dxmin);
   return eqset == 1 ? cell_speed<true>(ph, U) : cell_speed<false>(ph, U);

@@ -39,6 +39,18 @@ def shim():
     L.shim_slope.restype = C.c_double
     L.shim_cell_speed.argtypes = [C.c_int, C.c_double, C.c_double, C.c_double, _dp]
     L.shim_cell_speed.restype = C.c_double
+    L.shim_half_slope.argtypes = [C.c_int, C.c_double, C.c_double, C.c_double]
+    L.shim_half_slope.restype = C.c_double
+    L.shim_cell_speed_inline.argtypes = [C.c_int, C.c_double, C.c_double, C.c_double, _dp]
+    L.shim_cell_speed_inline.restype = C.c_double
+    L.shim_cgl_cons_to_prim.argtypes = [_dp, _dp]
+    L.shim_cgl_cons_to_prim.restype = None
+    L.shim_cgl_face_flux.argtypes = [C.c_int, _dp, _dp, _dp]
+    L.shim_cgl_face_flux.restype = None
+    L.shim_cgl_relaxed_alog.argtypes = [C.c_double, _dp]
+    L.shim_cgl_relaxed_alog.restype = C.c_double
+    L.shim_cell_speed_cgl.argtypes = [_dp]
+    L.shim_cell_speed_cgl.restype = C.c_double
     return L
 
 
@@ -163,3 +175,55 @@ def test_cons_to_prim_slope_speed(shim):
         assert abs(vsh - voh) <= 2e-15 * voh
     Ubad = oracle.prim_to_cons(np.array([1.0, 0, 0, 0, 1.0, 0, 0, 0]), G); Ubad[0] = -1.0
     assert shim.shim_cell_speed(0, G, 0.0, 1.0, _p(Ubad)) < 0
+
+
+def test_half_slope_and_inline_speed(shim):
+    """The kernels' own forms: half_slope (limiter constants folded, minmod variant 3) is half of eq.4 bit for bit;
+    cell_speed_inline (straight-line roots in the device build, IEEE here) is the A7 speed."""
+    rng = np.random.default_rng(4)
+    for n in range(2000):
+        dp, dm = rng.normal(), rng.normal()
+        if n % 5 == 0:
+            dm = 0.0
+        if n % 7 == 0:
+            dm = dp
+        for lim, beta in ((0, 1.0), (1, 1.0), (2, 1.0), (2, 1.3), (2, 2.0)):
+            assert shim.shim_half_slope(lim, 0.5 * beta, dp, dm) == 0.5 * oracle.slope(lim, beta, dp, dm)
+        assert shim.shim_half_slope(3, 0.5, dp, dm) == 0.5 * oracle.slope(2, 1.0, dp, dm)
+        W = rand_state(rng)
+        U = oracle.prim_to_cons(W, G)
+        vo = np.sqrt(np.sum(W[1:4] ** 2)) + max(oracle.cfast(d, G, W) for d in range(3))
+        assert abs(shim.shim_cell_speed_inline(0, G, 0.0, 1.0, _p(U)) - vo) <= 3e-15 * vo
+        cw = oracle.cwhistler(0.05, 1.0 / 64, W)
+        voh = np.sqrt(np.sum(W[1:4] ** 2)) + max(max(oracle.cfast(d, G, W) for d in range(3)), cw)
+        assert abs(shim.shim_cell_speed_inline(1, G, 0.05, 1.0 / 64, _p(U)) - voh) <= 3e-15 * voh
+
+
+def test_cgl_point_functions(shim):
+    """CGL (R24): recovery, HLL flux in all three directions, relaxed A_log and the eq.28 cell speed of the kernels'
+    header against the oracle."""
+    rng = np.random.default_rng(6)
+    def rand9():
+        W = np.empty(9)
+        W[0] = 0.3 + 2 * rng.random(); W[4] = 0.2 + 2 * rng.random(); W[8] = 0.2 + 2 * rng.random()
+        W[1:4] = rng.normal(size=3) * 0.5
+        W[5:8] = 0.3 + rng.random(3)
+        return W
+    for _ in range(500):
+        WL, WR = rand9(), rand9()
+        U = oracle.cgl_prim_to_cons(WL)
+        Ws = np.empty(9)
+        shim.shim_cgl_cons_to_prim(_p(U), _p(Ws))
+        assert relerr(Ws, oracle.cgl_cons_to_prim(U)) < 1e-14
+        for d in range(3):
+            F = np.empty(9)
+            shim.shim_cgl_face_flux(d, _p(WL), _p(WR), _p(F))
+            assert relerr(F, oracle.cgl_face_flux(d, WL, WR)) < 5e-14
+        for f in (0.5, 0.99):
+            W2 = oracle.cgl_cons_to_prim(U)
+            B2 = float(np.sum(W2[5:8] ** 2))
+            a, b = oracle.cgl_relax(f, B2, W2[4], W2[8])
+            want = W2[0] * np.log((W2[0] ** 2 / (B2 * np.sqrt(B2))) * (b / a))
+            assert abs(shim.shim_cgl_relaxed_alog(f, _p(U)) - want) <= 1e-13 * max(1.0, abs(want))
+        vo = np.sqrt(np.sum(WL[1:4] ** 2)) + max(oracle.cgl_cfast(d, WL) for d in range(3))
+        assert abs(shim.shim_cell_speed_cgl(_p(U)) - vo) <= 5e-15 * vo
