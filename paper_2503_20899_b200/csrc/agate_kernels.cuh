@@ -1,7 +1,9 @@
-// agate_kernels.cuh — the three hot-path kernels (A0 ghost fill, A1-A6 fused stage, A7 dt reduction) plus the
-// two diagnostic kernels.  sm_100a, fp64, SoA, ghost-padded storage  U[8][nz+2gz][ny+2gy][nx+4].
+// agate_kernels.cuh — shared pieces of the hot path: the stage-kernel parameter block, A0 ghost fill, A7 dt reduction
+// and step-head kernels, the POOLED fused stage kernel (1-D grids; 2-D / 3-D only with AGATE_STAGE_V1 -- the 3-D grids
+// run agate_stage3d.cuh, the 2-D grids agate_stage2d.cuh) and the two diagnostic kernels.
+// sm_100a, fp64, SoA, ghost-padded storage  U[NV][nz+2gz][ny+2gy][nx+4]  (NV = 8; 9 with GLM or CGL).
 //
-// Fused stage kernel (one launch per Runge-Kutta stage; SURVEY §8(a) rows A1-A6[+A8]):
+// Pooled stage kernel (one launch per Runge-Kutta stage; SURVEY §8(a) rows A1-A6[+A8]):
 //   * a CTA owns an x-y tile of TX=32 x TY cells and MARCHES along z over a chunk of planes (2.5-D streaming).
 //     Primitive variables W live only in shared memory: a ring of NP x-extended planes (TY rows of TX+4 cells)
 //     plus the four y-halo rows ("strips") of the current plane.  U is read from HBM/L2 once per stage per cell
