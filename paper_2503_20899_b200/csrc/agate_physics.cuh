@@ -37,6 +37,7 @@ struct Phys {
   double gm1;     // gamma - 1
   double igm1;    // 1 / (gamma - 1)
   double gogm1;   // gamma / (gamma - 1)
+  double hgamma;  // gamma / 2
   double d_i;     // Hall: normalised ion inertial length
   double cwk;     // Hall: d_i * pi / (2 dx_min)   (eq.13 with k_max = pi / dx_min, R15)
 };
@@ -47,6 +48,7 @@ AG_HD Phys make_phys(double gamma, double d_i, double dxmin) {
   ph.gm1 = gamma - 1.0;
   ph.igm1 = 1.0 / (gamma - 1.0);
   ph.gogm1 = gamma / (gamma - 1.0);
+  ph.hgamma = 0.5 * gamma;
   ph.d_i = d_i;
   ph.cwk = d_i * 3.14159265358979323846264338327950288 / (2.0 * dxmin);
   return ph;
@@ -183,6 +185,62 @@ AG_HD double half_slope(int limiter, double hbeta, double dp, double dm) {
   return 0.0;
 }
 
+// x with its sign flipped when bit 31 of hmask is set (hmask = 0 or 0x80000000): one logic op on the high word
+AG_HD double flipsign_hi(double x, int hmask) {
+#if defined(__CUDA_ARCH__)
+  return __hiloint2double(__double2hiint(x) ^ hmask, __double2loint(x));
+#else
+  return hmask ? -x : x;
+#endif
+}
+AG_HD int signbit_hi(double x) {
+#if defined(__CUDA_ARCH__)
+  return __double2hiint(x) & (int)0x80000000;
+#else
+  return signbit(x) ? (int)0x80000000 : 0;
+#endif
+}
+
+// A2 in one piece (eqs.2-4, R7): the two face states of cell b with neighbours a (low) and c (high),
+//   lo = W - dW/2  (right state of the low face),   hi = W + dW/2  (left state of the high face).
+// limiter 2 (eq.4):  dW = minmod[beta dp, beta dm, (dp+dm)/2],  dp = c-b, dm = b-a.  For dp, dm of one sign the
+// candidate of smaller magnitude of {dp, dm} is picked WITH its sign, scaled by 2 beta, and compared in magnitude
+// with the centred difference c - a (which carries the same sign), so the result needs no sign fix-up; opposite
+// signs (or a zero) give 0.  The common factor 1/4 rides in the two fused multiply-adds that form the states:
+// 8 FP64-pipe instructions per variable and direction (12 with half_slope and separate adds).  The scalings are by
+// powers of two, so the only difference from half_slope is c - a against dp + dm (one rounding of the centred term).
+// limiter 3 = eq.4 at beta = 1 (minmod; the centred term never binds, see half_slope).  beta2 = 2 beta.
+AG_HD void plm_faces(int limiter, double beta2, double a, double b, double c, double& lo, double& hi) {
+  if (limiter >= 2) {
+    const double dp = c - b, dm = b - a;
+    double m = (fabs(dp) < fabs(dm)) ? dp : dm;            // smaller magnitude, with its sign
+#if defined(__CUDA_ARCH__)
+    const bool opp = (__double2hiint(dp) ^ __double2hiint(dm)) < 0;
+#else
+    const bool opp = signbit(dp) != signbit(dm);
+#endif
+    m = opp ? 0.0 : m;
+    if (limiter == 3) {
+      lo = fma(-0.5, m, b);
+      hi = fma(0.5, m, b);
+    } else {
+      const double t = beta2 * m, cen = c - a;
+      const double x = (fabs(t) < fabs(cen)) ? t : cen;    // opp: t = 0 -> x = 0 (cen = 0 too if it is not picked)
+      lo = fma(-0.25, x, b);
+      hi = fma(0.25, x, b);
+    }
+    return;
+  }
+  if (limiter == 1) {
+    const double cen = c - a;
+    lo = fma(-0.25, cen, b);
+    hi = fma(0.25, cen, b);
+    return;
+  }
+  lo = b;
+  hi = b;
+}
+
 // Per-side quantities every solver needs.
 struct Side {
   double ir;    // 1/rho
@@ -293,7 +351,7 @@ AG_HD Star star_of(const double a[8], double S, double m, double SM, double bn, 
 // their terms on and off through the wave speed that multiplies them, so there is no branch and no divergence.
 AG_HD double sel(bool c, double a, double b) { return c ? a : b; }
 
-AG_HD void flux_hlld(const Phys& ph, const double L[8], const double R[8], double F[8]) {
+AG_HD void flux_hlld_general(const Phys& ph, const double L[8], const double R[8], double F[8]) {
   const double bn = 0.5 * (L[5] + R[5]);                     // single-valued Bn: arithmetic mean
   const double bn2 = bn * bn;
   // per-side speeds with Bn := bn (the caller's L[5], R[5] are not used below)
@@ -366,6 +424,111 @@ AG_HD void flux_hlld(const Phys& ph, const double L[8], const double R[8], doubl
   F[5] = 0.0;                                                // F[Bn] = 0 in every branch (R10)
   F[6] = fa[6] + SAe * (a.b1 - A[6]) + Sse * (b1ss - a.b1);
   F[7] = fa[7] + SAe * (a.b2 - A[7]) + Sse * (b2ss - a.b2);
+}
+
+// HLLD (R10), the common case: a face inside the Riemann fan (S_L < 0 < S_R) whose star states are regular
+// (|den| >= eps pt*).  Returns true when the face is NOT of that kind (supersonic or degenerate) -- its F is then
+// meaningless and the caller takes flux_hlld_general.  What makes it lean:
+//   * 1/rho is only needed inside the fast speed:  c_f = sqrt(N / rho),  N = H + sqrt(H^2 - gamma p Bn^2),
+//     H = (gamma p + B^2)/2, evaluated as N * rsqrt(N rho): one root-type Newton chain less per side, no reciprocal.
+//   * pt* = pt_L + m_L (S_M - u_L), the Rankine-Hugoniot condition across S_L (equal to the symmetric formula of
+//     R10 up to rounding): one FMA.
+//   * the star states satisfy the jump conditions, so the flux behind a wave is the physical flux function of the
+//     state behind it:  F = (rho* S_M,  rho* S_M^2 + pt* - Bn^2,  rho* S_M v_t - Bn B_t,  (E + pt*) S_M - Bn (v.B),
+//     0,  B_t S_M - Bn v_t)  with (v_t, B_t, E) of the single- or double-star state.  No physical flux of the outer
+//     state, no jump terms.
+//   * star transverse parts from one ratio  g = (S_M - u)/den:  v* = v - Bn B_t g,  B_t* = B_t (1 + m g).
+AG_HD bool flux_hlld_fast(const Phys& ph, const double L[8], const double R[8], double F[8]) {
+  const double bn = 0.5 * (L[5] + R[5]);                     // single-valued Bn: arithmetic mean
+  const double bn2 = bn * bn, bn2x2 = bn2 + bn2, hbn2 = 0.5 * bn2;
+  // Davis speeds eq.6 with eq.12 (R3) of the states with Bn := bn
+  const double hBl = fma(0.5, fma(L[6], L[6], L[7] * L[7]), hbn2);       // |B|^2 / 2
+  const double hBr = fma(0.5, fma(R[6], R[6], R[7] * R[7]), hbn2);
+  const double ptl = L[4] + hBl, ptr = R[4] + hBr;
+  const double gl = ph.hgamma * L[4], gr = ph.hgamma * R[4];             // gamma p / 2
+  const double Hl = gl + hBl, Hr = gr + hBr;
+  const double Ql = dmax(fma(Hl, Hl, -(gl * bn2x2)), kTiny), Qr = dmax(fma(Hr, Hr, -(gr * bn2x2)), kTiny);
+  const double Nl = Hl + sqrt_pos(Ql), Nr = Hr + sqrt_pos(Qr);           // rho c_f^2
+  const double cfl = Nl * rsq(Nl * L[0]), cfr = Nr * rsq(Nr * R[0]);
+  const double SL = dmin(L[1] - cfl, R[1] - cfr);
+  const double SR = dmax(L[1] + cfl, R[1] + cfr);
+  const double dl = SL - L[1], dr = SR - R[1];
+  const double mL = L[0] * dl, mR = R[0] * dr;                           // mL < 0 < mR
+  const double idm = rcp(mR - mL);
+  const double SM = fma(-mL, L[1], fma(mR, R[1], ptl - ptr)) * idm;
+  const double eL = SM - L[1], eR = SM - R[1];
+  const double pts = fma(mL, eL, ptl);
+  const double epts = kHlldEps * pts;
+  // star states behind the two outer waves
+  const double dSl = SL - SM, dSr = SR - SM;
+  const double denl = fma(mL, dSl, -bn2), denr = fma(mR, dSr, -bn2);
+  const double r1l = rcp(dSl * denl), r1r = rcp(dSr * denr);             // one reciprocal serves 1/dS and 1/den
+  const double idSl = denl * r1l, idSr = denr * r1r;
+  const double rsl = mL * idSl, rsr = mR * idSr;                         // rho*
+  const double ggl = eL * (dSl * r1l), ggr = eR * (dSr * r1r);
+  const double tl = bn * ggl, tr = bn * ggr;
+  const double fl = fma(mL, ggl, 1.0), fr = fma(mR, ggr, 1.0);
+  const double vl = fma(-L[6], tl, L[2]), wl = fma(-L[7], tl, L[3]), b1l = L[6] * fl, b2l = L[7] * fl;
+  const double vr = fma(-R[6], tr, R[2]), wr = fma(-R[7], tr, R[3]), b1r = R[6] * fr, b2r = R[7] * fr;
+  const bool slow = !(SL < 0.0) || !(SR > 0.0) || (fabs(denl) < epts) || (fabs(denr) < epts);
+  // double-star state (symmetric in L, R)
+  const double ql = rsl * rsq(rsl), qr = rsr * rsq(rsr);                 // sqrt(rho*)
+  const int sbn = signbit_hi(bn);                                        // sgn(Bn) = -1
+  const double I = rcp(ql + qr), sI = flipsign_hi(I, sbn);
+  const double qlI = ql * I, qrI = qr * I, qqI = ql * flipsign_hi(qrI, sbn);
+  const double vss = fma(qlI, vl, fma(qrI, vr, sI * (b1r - b1l)));
+  const double wss = fma(qlI, wl, fma(qrI, wr, sI * (b2r - b2l)));
+  const double b1ss = fma(qlI, b1r, fma(qrI, b1l, qqI * (vr - vl)));
+  const double b2ss = fma(qlI, b2r, fma(qrI, b2l, qqI * (wr - wl)));
+  // upwind side alpha: L if S_M >= 0, else R
+  const bool rt = SM < 0.0;
+  const double rA = sel(rt, R[0], L[0]), uA = sel(rt, R[1], L[1]), vA = sel(rt, R[2], L[2]), wA = sel(rt, R[3], L[3]);
+  const double pA = sel(rt, R[4], L[4]), b1A = sel(rt, R[6], L[6]), b2A = sel(rt, R[7], L[7]);
+  const double hBA = sel(rt, hBr, hBl), ptA = sel(rt, ptr, ptl), dA = sel(rt, dr, dl);
+  const double rsA = sel(rt, rsr, rsl), idSA = sel(rt, idSr, idSl), qA = sel(rt, qr, ql);
+  const double vsA = sel(rt, vr, vl), wsA = sel(rt, wr, wl), b1sA = sel(rt, b1r, b1l), b2sA = sel(rt, b2r, b2l);
+  const double EA = fma(pA, ph.igm1, fma(0.5 * rA, fma(uA, uA, fma(vA, vA, wA * wA)), hBA));
+  const double SMbn = SM * bn;
+  const double vBA = fma(uA, bn, fma(vA, b1A, wA * b2A));
+  const double vBsA = fma(vsA, b1sA, fma(wsA, b2sA, SMbn));
+  const double EsA = (fma(dA, EA, -(ptA * uA)) + fma(pts, SM, bn * (vBA - vBsA))) * idSA;
+  // S*_alpha lies on the far side of zero  <=>  S_M^2 rho*_alpha < Bn^2;  no rotational waves when Bn^2/2 < eps pt*
+  const bool twostar = (SM * SM * rsA < bn2) && !(hbn2 < epts);
+  const double vBss = fma(vss, b1ss, fma(wss, b2ss, SMbn));
+  // E** = E* -+ sqrt(rho*) (v*.B* - v**.B**) sgn(Bn):  - for alpha = L, + for alpha = R
+  const double EssA = fma(-flipsign_hi(qA, sbn ^ (rt ? (int)0x80000000 : 0)), vBsA - vBss, EsA);
+  const double vf = sel(twostar, vss, vsA), wf = sel(twostar, wss, wsA);
+  const double b1f = sel(twostar, b1ss, b1sA), b2f = sel(twostar, b2ss, b2sA);
+  const double Ef = sel(twostar, EssA, EsA), vBf = sel(twostar, vBss, vBsA);
+  const double rSM = rsA * SM;
+  F[0] = rSM;
+  F[1] = fma(rSM, SM, pts - bn2);
+  F[2] = fma(rSM, vf, -(bn * b1f));
+  F[3] = fma(rSM, wf, -(bn * b2f));
+  F[4] = fma(Ef + pts, SM, -(bn * vBf));
+  F[5] = 0.0;                                                            // F[Bn] = 0 in every branch (R10)
+  F[6] = fma(b1f, SM, -(bn * vf));
+  F[7] = fma(b2f, SM, -(bn * wf));
+  return slow;
+}
+
+// HLLD (R10): the lean form for regular faces inside the fan, the general straight-line form for a warp that holds a
+// supersonic or degenerate face (rare: strong shocks, field-aligned states with B_t = 0).  A lane's result depends
+// on its own face only, so the grid decomposition does not change the bits.
+AG_HD void flux_hlld(const Phys& ph, const double L[8], const double R[8], double F[8]) {
+  const bool slow = flux_hlld_fast(ph, L, R, F);
+#if defined(__CUDA_ARCH__)
+  if (__any_sync(__activemask(), slow)) {
+    double G[8];
+    flux_hlld_general(ph, L, R, G);
+    if (slow) {
+#pragma unroll
+      for (int q = 0; q < 8; ++q) F[q] = G[q];
+    }
+  }
+#else
+  if (slow) flux_hlld_general(ph, L, R, F);
+#endif
 }
 
 template <int RIEMANN, bool HALL>

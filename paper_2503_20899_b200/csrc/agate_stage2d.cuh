@@ -62,7 +62,7 @@ __global__ void __launch_bounds__(32 * Stage2dSmem<GLM || CGL>::NW, 2) stage2d_k
   const bool two = (P.a0 != 0.0);
   const double c0 = two ? P.a1 : 1.0;
   const int limiter = (LIM >= 0) ? LIM : P.limiter;
-  const double hbeta = 0.5 * P.beta;
+  const double beta2 = 2.0 * P.beta;
   double vmx = 0.0;
   int bad = 0;
   // GLM (R22): c_h of this step from the device scalar; the source term multiplies psi by exp(-dt c_h / 0.18)
@@ -178,7 +178,9 @@ __global__ void __launch_bounds__(32 * Stage2dSmem<GLM || CGL>::NW, 2) stage2d_k
       for (int q = 0; q < NV; ++q) {
         const double a = ring[slot_of(j0 - 2) + q * RW2 + c], b = ring[slot_of(j0 - 1) + q * RW2 + c];
         const double cc = ring[slot_of(j0) + q * RW2 + c];
-        WLy[q * 32 + lane] = b + half_slope(limiter, hbeta, cc - b, b - a);
+        double lo, hi;
+        plm_faces(limiter, beta2, a, b, cc, lo, hi);
+        WLy[q * 32 + lane] = hi;
       }
     }
     copy_row(j0 + 1, true);
@@ -205,10 +207,11 @@ __global__ void __launch_bounds__(32 * Stage2dSmem<GLM || CGL>::NW, 2) stage2d_k
       for (int r = 0; r < NV; ++r) {
         const int v = (r < 8) ? rot_var(r, 1) : r;
         const double a = ring[sm + v * RW2 + c], b = ring[sc + v * RW2 + c], cc = ring[sp + v * RW2 + c];
-        const double hs = half_slope(limiter, hbeta, cc - b, b - a);
+        double lo, hi;
+        plm_faces(limiter, beta2, a, b, cc, lo, hi);
         L[r] = WLy[v * 32 + lane];
-        R[r] = b - hs;
-        WLy[v * 32 + lane] = b + hs;
+        R[r] = lo;
+        WLy[v * 32 + lane] = hi;
       }
       double Jr[3];
       if (HALL) {
@@ -263,9 +266,10 @@ __global__ void __launch_bounds__(32 * Stage2dSmem<GLM || CGL>::NW, 2) stage2d_k
 #pragma unroll
         for (int r = 0; r < NV; ++r) {
           const double a = ring[sc + r * RW2 + c - 1], b = ring[sc + r * RW2 + c], cc = ring[sc + r * RW2 + c + 1];
-          const double hs = half_slope(limiter, hbeta, cc - b, b - a);
-          L[r] = b + hs;
-          R[r] = __shfl_down_sync(0xffffffffu, b - hs, 1);
+          double lo, hi;
+          plm_faces(limiter, beta2, a, b, cc, lo, hi);
+          L[r] = hi;
+          R[r] = __shfl_down_sync(0xffffffffu, lo, 1);
         }
         if (HALL) {
           // A8: J at the x-face between columns c and c+1 of row j; transverse differences from rows j-1, j+1

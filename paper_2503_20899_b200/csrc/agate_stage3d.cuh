@@ -113,7 +113,7 @@ __global__ void __launch_bounds__(32 * (TY + 1), MINB) stage3d_kernel(const __gr
   const bool two = (P.a0 != 0.0);                       // second SSP stage: Uout = a1 (U0 + Uin + dt L)
   const double c0 = two ? P.a1 : 1.0;
   const int limiter = (LIM >= 0) ? LIM : P.limiter;
-  const double hbeta = 0.5 * P.beta;
+  const double beta2 = 2.0 * P.beta;
   // GLM (R22): c_h of this step from the device scalar; the source term multiplies psi by exp(-dt c_h / 0.18)
   // (c_h^2 / c_p^2 with c_p^2 = 0.18 c_h) in the stage that completes the step
   const double ch = GLM ? *P.ch_ptr : 0.0;
@@ -221,7 +221,9 @@ __global__ void __launch_bounds__(32 * (TY + 1), MINB) stage3d_kernel(const __gr
 #pragma unroll
     for (int q = 0; q < NV; ++q) {
       const double a = W[q * QS + ca], b = W[q * QS + cb], c = W[q * QS + cc];
-      WLz[q * ZS + tid] = b + half_slope(limiter, hbeta, c - b, b - a);
+      double lo, hi;
+      plm_faces(limiter, beta2, a, b, c, lo, hi);
+      WLz[q * ZS + tid] = hi;
     }
     // plane k0+1 goes into the slot plane k0-2 just left (own cell only: no other thread touches it)
     if (own_in) copy_cell(slot_of(k0 + 1) + own_off, own_g + (long long)(k0 + 3) * P.sz);
@@ -289,10 +291,11 @@ __global__ void __launch_bounds__(32 * (TY + 1), MINB) stage3d_kernel(const __gr
           for (int r = 0; r < NV; ++r) {
             const int v = rv(r, 2);
             const double a = W[v * QS + sm + own_off], b = W[v * QS + sc + own_off], c = W[v * QS + sp + own_off];
-            const double hs = half_slope(limiter, hbeta, c - b, b - a);
+            double lo, hi;
+            plm_faces(limiter, beta2, a, b, c, lo, hi);
             L[r] = WLz[v * ZS + tid];
-            R[r] = b - hs;
-            WLz[v * ZS + tid] = b + hs;
+            R[r] = lo;
+            WLz[v * ZS + tid] = hi;
           }
           flux = true;
         } else if (full) {
@@ -315,9 +318,10 @@ __global__ void __launch_bounds__(32 * (TY + 1), MINB) stage3d_kernel(const __gr
 #pragma unroll
             for (int r = 0; r < NV; ++r) {
               const double a = W[r * QS + c - 1], b = W[r * QS + c], cc = W[r * QS + c + 1];
-              const double hs = half_slope(limiter, hbeta, cc - b, b - a);
-              L[r] = b + hs;
-              const double rn = __shfl_down_sync(0xffffffffu, b - hs, 1);
+              double lo, hi;
+              plm_faces(limiter, beta2, a, b, cc, lo, hi);
+              L[r] = hi;
+              const double rn = __shfl_down_sync(0xffffffffu, lo, 1);
               R[r] = (lane == 31) ? XR[r * XS + wid] : rn;
             }
           }
@@ -331,7 +335,9 @@ __global__ void __launch_bounds__(32 * (TY + 1), MINB) stage3d_kernel(const __gr
 #pragma unroll
             for (int q = 0; q < NV; ++q) {
               const double a = W[q * QS + cm], b = W[q * QS + c0r], c = W[q * QS + cp];
-              YR[q * YS + TY * 32 + lane] = b - half_slope(limiter, hbeta, c - b, b - a);
+              double lo, hi;
+              plm_faces(limiter, beta2, a, b, c, lo, hi);
+              YR[q * YS + TY * 32 + lane] = lo;
             }
           }
           // column x = 32: right state for lane 31 of every row
@@ -340,7 +346,9 @@ __global__ void __launch_bounds__(32 * (TY + 1), MINB) stage3d_kernel(const __gr
 #pragma unroll
             for (int q = 0; q < NV; ++q) {
               const double a = W[q * QS + c - 1], b = W[q * QS + c], cc = W[q * QS + c + 1];
-              XR[q * XS + lane] = b - half_slope(limiter, hbeta, cc - b, b - a);
+              double lo, hi;
+              plm_faces(limiter, beta2, a, b, cc, lo, hi);
+              XR[q * XS + lane] = lo;
             }
           }
           // face x = -1/2 of every row: lanes 0..15 hold cell -1 (left state), lanes 16..31 cell 0 (right state)
@@ -350,9 +358,10 @@ __global__ void __launch_bounds__(32 * (TY + 1), MINB) stage3d_kernel(const __gr
 #pragma unroll
             for (int r = 0; r < NV; ++r) {
               const double a = W[r * QS + c - 1], b = W[r * QS + c], cc = W[r * QS + c + 1];
-              const double hs = half_slope(limiter, hbeta, cc - b, b - a);
-              L[r] = b + hs;
-              R[r] = __shfl_down_sync(0xffffffffu, b - hs, 16);
+              double lo, hi;
+              plm_faces(limiter, beta2, a, b, cc, lo, hi);
+              L[r] = hi;
+              R[r] = __shfl_down_sync(0xffffffffu, lo, 16);
             }
           }
           flux = true;
@@ -363,7 +372,9 @@ __global__ void __launch_bounds__(32 * (TY + 1), MINB) stage3d_kernel(const __gr
           for (int r = 0; r < NV; ++r) {
             const int v = rv(r, 1);
             const double a = W[v * QS + cm], b = W[v * QS + c0r], c = W[v * QS + cp];
-            L[r] = b + half_slope(limiter, hbeta, c - b, b - a);
+            double lo, hi;
+            plm_faces(limiter, beta2, a, b, c, lo, hi);
+            L[r] = hi;
             R[r] = YR[v * YS + lane];
           }
           flux = true;
@@ -417,9 +428,10 @@ __global__ void __launch_bounds__(32 * (TY + 1), MINB) stage3d_kernel(const __gr
             for (int r = 0; r < NV; ++r) {
               const int v = rv(r, 1);
               const double a = W[v * QS + cm], b = W[v * QS + c], cc = W[v * QS + cp];
-              const double hs = half_slope(limiter, hbeta, cc - b, b - a);
-              YR[v * YS + wid * 32 + lane] = b - hs;
-              Ly[r] = b + hs;
+              double lo, hi;
+              plm_faces(limiter, beta2, a, b, cc, lo, hi);
+              YR[v * YS + wid * 32 + lane] = lo;
+              Ly[r] = hi;
             }
             // Uin (+U0) of the own cell of plane k: in flight across barrier 1
             const double* pa = P.Uin + gm + P.sz;

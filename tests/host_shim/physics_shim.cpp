@@ -28,6 +28,26 @@ double shim_slope(int limiter, double beta, double dp, double dm) { return limit
 
 double shim_half_slope(int limiter, double hbeta, double dp, double dm) { return half_slope(limiter, hbeta, dp, dm); }
 
+// A2 in one piece (limited slope + both face states), and the two HLLD bodies on their own
+void shim_plm_faces(int limiter, double beta2, double a, double b, double c, double* lo, double* hi) {
+  plm_faces(limiter, beta2, a, b, c, *lo, *hi);
+}
+int shim_hlld_fast(int dir, double gamma, const double* WL, const double* WR, double* F) {
+  Phys ph = make_phys(gamma, 0.0, 1.0);
+  double L[8], R[8], Fr[8];
+  for (int r = 0; r < 8; ++r) { L[r] = WL[rot_var(r, dir)]; R[r] = WR[rot_var(r, dir)]; }
+  const bool slow = flux_hlld_fast(ph, L, R, Fr);
+  unrotate(dir, Fr, F);
+  return slow ? 1 : 0;
+}
+void shim_hlld_general(int dir, double gamma, const double* WL, const double* WR, double* F) {
+  Phys ph = make_phys(gamma, 0.0, 1.0);
+  double L[8], R[8], Fr[8];
+  for (int r = 0; r < 8; ++r) { L[r] = WL[rot_var(r, dir)]; R[r] = WR[rot_var(r, dir)]; }
+  flux_hlld_general(ph, L, R, Fr);
+  unrotate(dir, Fr, F);
+}
+
 double shim_cell_speed_inline(int eqset, double gamma, double d_i, double dxmin, const double* U) {
   Phys ph = make_phys(gamma, eqset == 1 ? d_i : 0.0, dxmin);
   return eqset == 1 ? cell_speed_inline<true>(ph, U) : cell_speed_inline<false>(ph, U);

@@ -43,6 +43,12 @@ def shim():
     L.shim_half_slope.restype = C.c_double
     L.shim_cell_speed_inline.argtypes = [C.c_int, C.c_double, C.c_double, C.c_double, _dp]
     L.shim_cell_speed_inline.restype = C.c_double
+    L.shim_plm_faces.argtypes = [C.c_int, C.c_double, C.c_double, C.c_double, C.c_double, _dp, _dp]
+    L.shim_plm_faces.restype = None
+    L.shim_hlld_fast.argtypes = [C.c_int, C.c_double, _dp, _dp, _dp]
+    L.shim_hlld_fast.restype = C.c_int
+    L.shim_hlld_general.argtypes = [C.c_int, C.c_double, _dp, _dp, _dp]
+    L.shim_hlld_general.restype = None
     L.shim_cgl_cons_to_prim.argtypes = [_dp, _dp]
     L.shim_cgl_cons_to_prim.restype = None
     L.shim_cgl_face_flux.argtypes = [C.c_int, _dp, _dp, _dp]
@@ -127,6 +133,62 @@ def test_hlld_degenerate_cases(shim):
             Fo = oracle.face_flux(1, d, G, wl, wr)
             Fs = shim_flux(shim, 0, 1, d, G, wl, wr)
             assert relerr(Fs, Fo) < 1e-13, (WL, WR, d, Fs, Fo)
+
+
+def test_hlld_fast_and_general_bodies(shim):
+    """The two HLLD bodies of the CUDA path on their own.  The lean body (star-region flux function, one-sided pt*,
+    c_f = N rsqrt(N rho)) must agree with the oracle on every face it accepts, and it must hand every supersonic
+    or degenerate face (oracle branches 0, 5 and the eps-guarded star states) to the general body, which must agree
+    with the oracle everywhere."""
+    rng = np.random.default_rng(77)
+    worst_fast, worst_gen, nslow, seen = 0.0, 0.0, 0, set()
+    Ff, Fg = np.empty(8), np.empty(8)
+    for n in range(6000):
+        amp = [0.1, 0.5, 2.0, 6.0][n % 4]
+        WL, WR = rand_state(rng, amp), rand_state(rng, amp)
+        if n % 7 == 0:
+            WR = WL + 1e-3 * (rand_state(rng) - 1.0)
+            WR[0] = abs(WR[0]) + 0.1; WR[4] = abs(WR[4]) + 0.1
+        if n % 11 == 0:
+            WL[5:8] *= [1.0, 0.0, 0.0][n % 3]; WR[5:8] = WL[5:8]        # B = 0, or B along one axis on both sides
+        d = n % 3
+        Fo = oracle.face_flux(1, d, G, WL, WR)
+        br = oracle.hlld_branch(d, G, WL, WR) % 10
+        slow = shim.shim_hlld_fast(d, G, _p(WL), _p(WR), _p(Ff))
+        shim.shim_hlld_general(d, G, _p(WL), _p(WR), _p(Fg))
+        worst_gen = max(worst_gen, relerr(Fg, Fo))
+        if br in (0, 5):
+            assert slow == 1, (n, br)                                   # supersonic faces never stay in the lean body
+        if slow:
+            nslow += 1
+        else:
+            seen.add(br)
+            worst_fast = max(worst_fast, relerr(Ff, Fo))
+    assert worst_gen < 2e-13 and worst_fast < 2e-13, (worst_gen, worst_fast)
+    assert seen >= {1, 2, 3, 4}, seen           # both single-star and both double-star branches ran through the lean body
+    assert 0 < nslow < 3000, nslow
+
+
+def test_plm_faces(shim):
+    """plm_faces (slope and both face states in one piece) against W -+ slope/2 of the oracle's eq.4: equal up to
+    one rounding of the centred difference (c - a against dp + dm), exact zeros where eq.4 gives zero."""
+    rng = np.random.default_rng(5)
+    lo, hi = C.c_double(), C.c_double()
+    for n in range(4000):
+        a, b, c = rng.normal(size=3) * [1.0, 1e-3, 1e3][n % 3]
+        if n % 5 == 0:
+            a = b
+        if n % 7 == 0:
+            c = 2 * b - a
+        if n % 13 == 0:
+            a = b = c
+        for lim, beta in ((0, 1.0), (1, 1.0), (2, 1.0), (2, 1.3), (2, 2.0), (3, 1.0)):
+            shim.shim_plm_faces(lim, 2.0 * beta, a, b, c, C.byref(lo), C.byref(hi))
+            so = oracle.slope(2 if lim == 3 else lim, beta, c - b, b - a)
+            tol = 4e-16 * max(abs(c - b), abs(b - a)) + 2e-16 * abs(b)
+            assert abs(hi.value - (b + 0.5 * so)) <= tol and abs(lo.value - (b - 0.5 * so)) <= tol, (lim, beta, a, b, c)
+            if so == 0.0:
+                assert hi.value == b and lo.value == b
 
 
 def test_hall_hll_flux(shim):
