@@ -213,21 +213,24 @@ AG_HD int signbit_hi(double x) {
 AG_HD void plm_faces(int limiter, double beta2, double a, double b, double c, double& lo, double& hi) {
   if (limiter >= 2) {
     const double dp = c - b, dm = b - a;
-    double m = (fabs(dp) < fabs(dm)) ? dp : dm;            // smaller magnitude, with its sign
+    const double m = (fabs(dp) < fabs(dm)) ? dp : dm;      // smaller magnitude, with its sign
+    // the factor of the fused multiply-adds carries the zero for opposite signs: 0.25 (0.5) and 0.0 differ in the
+    // high word only, so that is one 32-bit select
 #if defined(__CUDA_ARCH__)
     const bool opp = (__double2hiint(dp) ^ __double2hiint(dm)) < 0;
+    const double q = __hiloint2double(opp ? 0 : ((limiter == 3) ? 0x3FE00000 : 0x3FD00000), 0);
 #else
     const bool opp = signbit(dp) != signbit(dm);
+    const double q = opp ? 0.0 : ((limiter == 3) ? 0.5 : 0.25);
 #endif
-    m = opp ? 0.0 : m;
     if (limiter == 3) {
-      lo = fma(-0.5, m, b);
-      hi = fma(0.5, m, b);
+      lo = fma(-q, m, b);
+      hi = fma(q, m, b);
     } else {
       const double t = beta2 * m, cen = c - a;
-      const double x = (fabs(t) < fabs(cen)) ? t : cen;    // opp: t = 0 -> x = 0 (cen = 0 too if it is not picked)
-      lo = fma(-0.25, x, b);
-      hi = fma(0.25, x, b);
+      const double x = (fabs(t) < fabs(cen)) ? t : cen;    // a zero difference of one sign: m = 0 -> t = 0 -> x = 0
+      lo = fma(-q, x, b);
+      hi = fma(q, x, b);
     }
     return;
   }
@@ -512,6 +515,19 @@ AG_HD bool flux_hlld_fast(const Phys& ph, const double L[8], const double R[8], 
   return slow;
 }
 
+#if defined(__CUDACC__)
+// One out-of-line copy of the general body for all call sites of a kernel: the path is cold, and inlining it at
+// every call site would put ~6 KB of never-executed code between the hot loops of the stage kernels.
+static __device__ __noinline__ void flux_hlld_general_cold(const Phys* ph, const double* L, const double* R, double* F) {
+  double l[8], r[8], f[8];
+#pragma unroll
+  for (int q = 0; q < 8; ++q) { l[q] = L[q]; r[q] = R[q]; }
+  flux_hlld_general(*ph, l, r, f);
+#pragma unroll
+  for (int q = 0; q < 8; ++q) F[q] = f[q];
+}
+#endif
+
 // HLLD (R10): the lean form for regular faces inside the fan, the general straight-line form for a warp that holds a
 // supersonic or degenerate face (rare: strong shocks, field-aligned states with B_t = 0).  A lane's result depends
 // on its own face only, so the grid decomposition does not change the bits.
@@ -519,8 +535,11 @@ AG_HD void flux_hlld(const Phys& ph, const double L[8], const double R[8], doubl
   const bool slow = flux_hlld_fast(ph, L, R, F);
 #if defined(__CUDA_ARCH__)
   if (__any_sync(__activemask(), slow)) {
-    double G[8];
-    flux_hlld_general(ph, L, R, G);
+    // copies in local memory for the call, so that L, R, F themselves stay in registers on the hot path
+    double Lc[8], Rc[8], G[8];
+#pragma unroll
+    for (int q = 0; q < 8; ++q) { Lc[q] = L[q]; Rc[q] = R[q]; }
+    flux_hlld_general_cold(&ph, Lc, Rc, G);
     if (slow) {
 #pragma unroll
       for (int q = 0; q < 8; ++q) F[q] = G[q];
