@@ -386,7 +386,7 @@ template <class T> struct Solver {
   bool glm;
   bool cgl = false;
   double ch = 0.0;      // GLM: c_h of the step being taken (R22: 0.95 v_max(U^n))
-  std::vector<T> Un, U1, U2, W, L;
+  std::vector<T> Un, U1, U2, U3, W, L;
   double t = 0.0;
   bool have_state = false;
 
@@ -424,6 +424,14 @@ template <class T> struct Solver {
             int iw = s.bc[0] ? std::min(std::max(i, 0), nd[0] - 1) : ((i % nd[0]) + nd[0]) % nd[0];
             int jw = s.bc[1] ? std::min(std::max(j, 0), nd[1] - 1) : ((j % nd[1]) + nd[1]) % nd[1];
             int kw = s.bc[2] ? std::min(std::max(k, 0), nd[2] - 1) : ((k % nd[2]) + nd[2]) % nd[2];
+            if (s.bc[1] == 2 && (j < 0 || j >= nd[1])) {
+              // sheared zero-gradient ends in y (R28): the ghost zone (i, j) takes the value of zone
+              // (i-1, j+2) at the down side and (i+1, j-2) at the up side, x wrapped periodically.  With two
+              // ghost layers the source row j+-2 is an interior row.
+              const int sh = (j < 0) ? -1 : 1;
+              jw = j - 2 * sh;
+              iw = (((i + sh) % nd[0]) + nd[0]) % nd[0];
+            }
             if (iw != i || jw != j || kw != k) U[q * ntot + pidx(i, j, k)] = U[q * ntot + pidx(iw, jw, kw)];
           }
   }
@@ -588,10 +596,56 @@ template <class T> struct Solver {
       Un[8 * ntot + c] = T(rho * std::log((rho * rho / (B2 * std::sqrt(B2))) * (pperp / ppar)));
     }
   }
+  // Uout = a0 Uref + a1 (Uin + c dt L)  on the interior, L = L(Uin) as left by rhs()
+  void combine(std::vector<T>& Uout, double a0, const std::vector<T>& Uref, double a1, const std::vector<T>& Uin, double cdt) {
+    for (int q = 0; q < nv; ++q) for (int k = 0; k < nd[2]; ++k) for (int j = 0; j < nd[1]; ++j) for (int i = 0; i < nd[0]; ++i) {
+      const size_t p = q * ntot + pidx(i, j, k);
+      const T up = Uin[p] + T(cdt) * L[q * nint + iidx(i, j, k)];
+      Uout[p] = (a0 == 0.0) ? up : T(a0) * Uref[p] + T(a1) * up;
+    }
+  }
+  // R27: the higher-order SSP schemes the paper names without a tableau (ref.[25]), in Shu-Osher form; the
+  // first stage's L(U^n) has been evaluated by the caller.  dt once per step (R11).
+  //   RK43 (4 stages, order 3, c = 1/2):
+  //     U1 = Un + c dt L(Un);  U2 = U1 + c dt L(U1);  U3 = 2/3 Un + 1/3 (U2 + c dt L(U2));  Un+1 = U3 + c dt L(U3)
+  //   RK53 (5 stages, order 3, Ruuth's form of the optimal scheme, c = 0.377268915331368):
+  //     U1 = Un + c dt L(Un);  U2 = U1 + c dt L(U1);
+  //     U3 = 0.355909775063327 Un + 0.644090224936674 (U2 + c dt L(U2));
+  //     U4 = 0.367933791638137 Un + 0.632066208361863 (U3 + c dt L(U3));
+  //     Un+1 = 0.237593836598569 U2 + 0.762406163401431 (U4 + c dt L(U4))
+  void step_ssp_high(double dt) {
+    if (U2.empty()) U2.assign(nv * ntot, T(0.0));
+    if (s.rk == 4) {
+      const double c = 0.5;
+      combine(U1, 0.0, Un, 1.0, Un, c * dt);                                   // U1
+      fill_ghosts(U1); rhs(U1);
+      combine(U2, 0.0, Un, 1.0, U1, c * dt);                                   // U2
+      fill_ghosts(U2); rhs(U2);
+      combine(U1, 2.0 / 3.0, Un, 1.0 / 3.0, U2, c * dt);                       // U3 (over U1)
+      fill_ghosts(U1); rhs(U1);
+      combine(Un, 0.0, Un, 1.0, U1, c * dt);                                   // Un+1
+    } else {
+      const double c = 0.377268915331368;
+      if (U3.empty()) U3.assign(nv * ntot, T(0.0));
+      combine(U1, 0.0, Un, 1.0, Un, c * dt);                                   // U1
+      fill_ghosts(U1); rhs(U1);
+      combine(U2, 0.0, Un, 1.0, U1, c * dt);                                   // U2 (kept for the last stage)
+      fill_ghosts(U2); rhs(U2);
+      combine(U1, 0.355909775063327, Un, 0.644090224936674, U2, c * dt);       // U3 (over U1)
+      fill_ghosts(U1); rhs(U1);
+      combine(U3, 0.367933791638137, Un, 0.632066208361863, U1, c * dt);       // U4
+      fill_ghosts(U3); rhs(U3);
+      combine(Un, 0.237593836598569, U2, 0.762406163401431, U3, c * dt);       // Un+1
+    }
+    if (glm) glm_source(dt);
+    if (cgl) cgl_source();
+    t += dt;
+  }
   void step(double dt) {
     if (glm) { double vm = 0.0; vmax(&vm); ch = 0.95 * vm; }
     fill_ghosts(Un);
     rhs(Un);
+    if (s.rk == 4 || s.rk == 5) { step_ssp_high(dt); return; }
     if (s.rk == 1) {
       for (int q = 0; q < nv; ++q) for (int k = 0; k < nd[2]; ++k) for (int j = 0; j < nd[1]; ++j) for (int i = 0; i < nd[0]; ++i) {
         const size_t p = q * ntot + pidx(i, j, k);
@@ -657,9 +711,10 @@ int check_args(const agate_ref_grid* g, double gamma, int eqset, const agate_ref
   if (eqset != AGATE_REF_IDEAL && eqset != AGATE_REF_HALL && eqset != AGATE_REF_IDEAL_GLM && eqset != AGATE_REF_CGL) return 1;
   if (eqset == AGATE_REF_CGL && s->riemann != 0) return 1;          // the paper's CGL runs use HLL
   if (eqset == AGATE_REF_CGL && !(s->relax >= 0.0 && s->relax <= 1.0)) return 1;
-  if (s->riemann < 0 || s->riemann > 1 || s->limiter < 0 || s->limiter > 2 || s->rk < 1 || s->rk > 3) return 1;
+  if (s->riemann < 0 || s->riemann > 1 || s->limiter < 0 || s->limiter > 2 || s->rk < 1 || s->rk > 5) return 1;
   if (s->limiter == 2 && !(s->beta >= 1.0 && s->beta <= 2.0)) return 1;
-  for (int d = 0; d < 3; ++d) if (s->bc[d] < 0 || s->bc[d] > 1) return 1;
+  for (int d = 0; d < 3; ++d) if (s->bc[d] < 0 || s->bc[d] > ((d == 1) ? 2 : 1)) return 1;
+  if (s->bc[1] == 2 && (g->ndim < 2 || s->bc[0] != 0)) return 1;   // sheared ends in y need a periodic x (R28)
   if (eqset == AGATE_REF_HALL && s->riemann == 1) return 1;        // no Hall-HLLD in the paper
   if (eqset == AGATE_REF_HALL && !(s->d_i >= 0.0)) return 1;
   return 0;

@@ -31,11 +31,12 @@ typedef struct {
   int32_t riemann;       /* 0 HLL (eq.5), 1 HLLD */
   int32_t limiter;       /* 0 none (dW=0), 1 central (unlimited), 2 eq.4 */
   double  beta;          /* eq.4 beta: 1.0 = minmod, 1.3 = paper default "MC" */
-  int32_t rk;            /* 1 = RK11 (forward Euler), 2 = SSP-RK2 (R11), 3 = SSP-RK33 (R25) */
+  int32_t rk;            /* 1 = RK11 (forward Euler), 2 = SSP-RK2 (R11), 3 = SSP-RK33 (R25), 4 = RK43, 5 = RK53 (R27) */
   double  cfl;           /* Courant C; <=0 -> paper default 0.8/0.45/0.325 (L73) */
   double  d_i;           /* normalised ion inertial length (Hall) */
   double  relax;         /* CGL: dt/(dt+tau) of eqs.32-33 (paper default 0.99, L254); 0 = no relaxation */
-  int32_t bc[3];         /* per dimension: 0 periodic, 1 zero-gradient (open end, L314: ghost = nearest interior zone) */
+  int32_t bc[3];         /* per dimension: 0 periodic, 1 zero-gradient (open end, L314: ghost = nearest interior zone);
+                            bc[1] = 2: sheared zero-gradient ends in y (L314, R28), x periodic */
 } agate_ref_solver;
 
 enum { AGATE_REF_IDEAL = 0, AGATE_REF_HALL = 1, AGATE_REF_CGL = 2, AGATE_REF_IDEAL_GLM = 3 };

@@ -55,7 +55,10 @@ __device__ __forceinline__ int peek(const int* prog_w) {
 __device__ __forceinline__ void await(const int* prog_w, int value, int* flag) {
   int spins = 0;
   while (peek(prog_w) < value) {
-    __nanosleep(40);                              // the wait is for ~a phase of another warp; keep the issue slots free
+#ifndef AGATE_SPIN_NS
+#define AGATE_SPIN_NS 40
+#endif
+    if (AGATE_SPIN_NS > 0) __nanosleep(AGATE_SPIN_NS);   // the wait is for ~a phase of another warp; keep the issue slots free
     if (++spins > (1 << 22)) { atomicOr(flag, 2); break; }
   }
 }
