@@ -18,7 +18,12 @@
 using namespace agate;
 
 #ifndef AGATE_TY3
-#define AGATE_TY3 11    // 3-D tile height: 11 owner warps + 1 helper = 12 warps (3 per scheduler, 168 registers), 186 KB
+#define AGATE_TY3 11    // 3-D tile height: 11 owner warps + 1 helper = 12 warps (3 per scheduler, <= 168 registers), 162 KB.
+                        // Measured at 512^3 (profiles/r2_stage3d.md): TY = 15 (16 warps, 128 registers, no spills) 32.9 ms
+                        // per step, TY = 12 (13 warps, 128 registers) 35.2, TY = 11 31.5
+#endif
+#ifndef AGATE_TY3N
+#define AGATE_TY3N 11   // ... with nine variables (GLM, CGL): 182 KB
 #endif
 #ifndef AGATE_MINB3
 #define AGATE_MINB3 1
@@ -27,6 +32,7 @@ using namespace agate;
 namespace {
 
 constexpr int TY3 = AGATE_TY3;   // 3-D tile height (rows); CTA = 32 x (TY3+1) threads (agate_stage3d.cuh)
+constexpr int TY3N = AGATE_TY3N;
 constexpr int TY2 = 6;    // 1-D / 2-D: 32x6 tile, 8 warps, 2 CTAs / SM
 constexpr int kDtBlocksMax = 148 * 8;
 
@@ -130,10 +136,10 @@ StageKernel pick_stage(int ndim, int eqset, int riemann, int limiter) {
       return make_stage<6, 3, 0, false, 2>();
     }
     if (eqset == AGATE_CGL)
-      return (limiter == 2) ? make_stage3d<TY3, 0, 2, AGATE_MINB3, false, true>() : make_stage3d<TY3, 0, -1, AGATE_MINB3, false, true>();
+      return (limiter == 2) ? make_stage3d<TY3N, 0, 2, AGATE_MINB3, false, true>() : make_stage3d<TY3N, 0, -1, AGATE_MINB3, false, true>();
     if (eqset == AGATE_IDEAL_GLM) {
-      if (riemann == AGATE_HLLD) return (limiter == 2) ? make_stage3d<TY3, 1, 2, AGATE_MINB3, true>() : make_stage3d<TY3, 1, -1, AGATE_MINB3, true>();
-      return (limiter == 2) ? make_stage3d<TY3, 0, 2, AGATE_MINB3, true>() : make_stage3d<TY3, 0, -1, AGATE_MINB3, true>();
+      if (riemann == AGATE_HLLD) return (limiter == 2) ? make_stage3d<TY3N, 1, 2, AGATE_MINB3, true>() : make_stage3d<TY3N, 1, -1, AGATE_MINB3, true>();
+      return (limiter == 2) ? make_stage3d<TY3N, 0, 2, AGATE_MINB3, true>() : make_stage3d<TY3N, 0, -1, AGATE_MINB3, true>();
     }
     if (limiter == 2) {                  // eq.4 (every BASELINE config): limiter fixed at compile time
       if (riemann == AGATE_HLLD) return make_stage3d<TY3, 1, 2, AGATE_MINB3>();

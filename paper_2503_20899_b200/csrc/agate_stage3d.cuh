@@ -6,27 +6,30 @@
 //     HIGH face in x and y and its LOW face in z, so every slope and every flux is computed once.
 //   * x: neighbours are lanes of the same warp -> the right state and the low-face flux travel by warp shuffles.
 //     The cells outside the row (x = -1, 32) belong to H, which hands  R(32)  and  F(-1/2)  over in XR / XF.
-//   * y: neighbours are adjacent warps -> the right state travels through YR, the flux through YF.  Row -1 (its
-//     flux through face -1/2) and row TY (its right state) belong to H.
+//   * y: neighbours are adjacent warps -> one hand-over row per tile row, Y[r]: first the right state of row r, then,
+//     written over it by its only reader (the owner of row r-1), the flux through face r-1/2.  Row -1 (its flux
+//     through face -1/2) and row TY (its right state) belong to H.
 //   * z: private column, one plane behind: step k computes F(k-1/2) from planes k-1, k, k+1 and completes plane
-//     k-1.  The left state W(k-1)+dW(k-1)/2 is carried in a per-thread shared slot, the accumulator in registers.
-//   * NO CTA-wide barrier in the steady state: two phases per plane, and at each phase boundary a warp publishes a
-//     phase counter (st.release) and waits (ld.acquire) only for the warps whose data it reads or overwrites -- its
-//     two neighbours and H; H waits for all owners once per plane.  Phase A: y-difference of the previous plane, z slope + flux, store of
-//     plane k-1, y slope -> YR.  Phase B: y flux -> YF, x slope + flux + difference.  H mirrors the owners with the
-//     tile-edge tasks (one Riemann call per phase), so no warp idles while the others solve.
+//     k-1.  The left state W(k-1)+dW(k-1)/2 is carried in a per-thread shared slot.
+//   * no register state across the Riemann calls: the flux differences of the plane being assembled live in a
+//     per-thread shared slot (ACC), seeded with +dt/dz F(k-1/2) when that flux is formed and closed with the same
+//     rounded product of F(k+1/2) one step later, so a uniform state stays bitwise fixed; Uin (+U0) of the own cell
+//     is read when the plane is completed (A6).
+//   * NO CTA-wide barrier in the steady state: three sub-phases per plane, and at each boundary a warp publishes a
+//     counter (st.release) and waits (ld.acquire) only for the warps whose data it reads or overwrites -- its
+//     two neighbours and H; H waits for all owners once per plane.  Phase A: z slope + flux, completion and store of
+//     plane k-1, y slope -> Y.  Phase B1: y flux -> Y.  Phase B2: x slope + flux, x and y differences -> ACC.  H mirrors
+//     the owners with the tile-edge tasks (one Riemann call in A and in B1, the halo cells in B2).
 //   * no global-load latency on the critical path: conserved cells are brought in by cp.async (LDGSTS) one phase
 //     ahead, straight into their final shared-memory slot, and turned into primitives IN PLACE (A1) by the thread
 //     that issued the copy: owners their own cell of plane k+2, H the x-halo columns and the y-halo rows.
 //   * the three tasks of a warp per plane run through one loop that is unrolled: three inlined copies of the solver,
-//     each with its direction's variable permutation resolved at compile time (3 % faster than one call site with
-//     the states marshalled into common registers; 91 KB of SASS, no instruction-fetch stalls measured).
-//   * A6: the accumulator of plane k gets Uin (+U0 in the second SSP stage) right after
-//     barrier 1 (the loads are issued just before it), then the x and y differences; plane k leaves in step k+1.
+//     each with its direction's variable permutation resolved at compile time.
 //
 // Shared memory per CTA (NV = 8 variables; 9 with GLM or CGL): ring 3 planes x NV x TY x 36, y-halo rows
-// 2 x NV x 4 x 36, YR / YF NV x (TY+1) x 32 each, z carries 2 x NV x TY x 32, XR / XF NV x TY each, 16 phase counters:
-// TY = 11 -> 186 KB (214 KB with 9 variables), one CTA of 12 warps per SM, <= 168 registers.
+// 2 x NV x 4 x 36, Y NV x (TY+1) x 32, z carry and accumulator NV x TY x 32 each, XR / XF NV x TY each, 16 counters:
+// TY = 11 -> 162 KB (182 KB with 9 variables), one CTA of 12 warps per SM, <= 168 registers.  (TY = 15, 16 warps at
+// 128 registers without spills, fits in 213 KB and was measured slower: profiles/r2_stage3d.md.)
 #pragma once
 #include <cuda_runtime.h>
 #include <stdint.h>
@@ -55,10 +58,7 @@ __device__ __forceinline__ int peek(const int* prog_w) {
 __device__ __forceinline__ void await(const int* prog_w, int value, int* flag) {
   int spins = 0;
   while (peek(prog_w) < value) {
-#ifndef AGATE_SPIN_NS
-#define AGATE_SPIN_NS 40
-#endif
-    if (AGATE_SPIN_NS > 0) __nanosleep(AGATE_SPIN_NS);   // the wait is for ~a phase of another warp; keep the issue slots free
+    __nanosleep(40);                              // the wait is for ~a phase of another warp; keep the issue slots free
     if (++spins > (1 << 22)) { atomicOr(flag, 2); break; }
   }
 }
@@ -75,14 +75,13 @@ struct Stage3dSmem {
   static constexpr int PL = TY * RS;                // one ring plane of one variable
   static constexpr int SB = 4 * RS;                 // one y-halo buffer of one variable (rows -2,-1,TY,TY+1)
   static constexpr int QS = 3 * PL + 2 * SB;        // per-variable stride of W
-  static constexpr int YS = (TY + 1) * 32;          // YR rows 0..TY;  YF rows -1..TY-1 (stored at j+1)
-  static constexpr int ZS = TY * 32;                // z carry
+  static constexpr int YS = (TY + 1) * 32;          // y hand-over rows 0..TY (right state of row r, then flux of face r-1/2)
+  static constexpr int ZS = TY * 32;                // per-thread slots: z carry, accumulator
   static constexpr int XS = TY;                     // x hand-over, one entry per row
-  static constexpr int OFF_YR = NV * QS;
-  static constexpr int OFF_YF = OFF_YR + NV * YS;
-  static constexpr int OFF_WLZ = OFF_YF + NV * YS;
-  static constexpr int OFF_FZL = OFF_WLZ + NV * ZS;
-  static constexpr int OFF_XR = OFF_FZL + NV * ZS;
+  static constexpr int OFF_Y = NV * QS;
+  static constexpr int OFF_WLZ = OFF_Y + NV * YS;
+  static constexpr int OFF_ACC = OFF_WLZ + NV * ZS;
+  static constexpr int OFF_XR = OFF_ACC + NV * ZS;
   static constexpr int OFF_XF = OFF_XR + NV * XS;
   static constexpr int OFF_PROG = OFF_XF + NV * XS;  // 16 ints: per-warp phase counters
   static constexpr int TOTAL = OFF_PROG + 8;
@@ -101,10 +100,12 @@ __global__ void __launch_bounds__(32 * (TY + 1), MINB) stage3d_kernel(const __gr
   constexpr int NT = SM::NT, PL = SM::PL, SB = SM::SB, QS = SM::QS, YS = SM::YS, ZS = SM::ZS, XS = SM::XS;
   extern __shared__ __align__(16) double smem[];
   double* const W = smem;                    // [8][QS]  primitives: ring planes + two y-halo buffers
-  double* const YR = smem + SM::OFF_YR;      // [8][YS]  right state  W(j) - dW_y(j)/2  of rows 0..TY   (fixed order)
-  double* const YF = smem + SM::OFF_YF;      // [8][YS]  y flux through face j+1/2, rows -1..TY-1       (rotated, n=1)
+  // Y row r holds, in turn, the right state  W(r) - dW_y(r)/2  of row r (fixed variable order; written in phase A by
+  // the owner of row r, H for r = TY) and the y flux through face r-1/2 (rotated order, n = 1; written over it in phase
+  // B1 by the only reader of that state, the owner of row r-1, H for r = 0)
+  double* const Y = smem + SM::OFF_Y;        // [8][YS]
   double* const WLz = smem + SM::OFF_WLZ;    // [8][ZS]  z: left state of the next face                (fixed order)
-  double* const FzL = smem + SM::OFF_FZL;    // [8][ZS]  z: flux through the low face of plane k-1     (fixed order)
+  double* const ACC = smem + SM::OFF_ACC;    // [8][ZS]  -dt (flux differences) of the plane being assembled (fixed order)
   double* const XR = smem + SM::OFF_XR;      // [8][XS]  right state of cell x = 32, per row
   double* const XF = smem + SM::OFF_XF;      // [8][XS]  x flux through face -1/2, per row
   int* const prog = reinterpret_cast<int*>(smem + SM::OFF_PROG);   // [TY+1] phases completed, per warp
@@ -238,10 +239,6 @@ __global__ void __launch_bounds__(32 * (TY + 1), MINB) stage3d_kernel(const __gr
   }
   __syncthreads();
 
-  double acc[NV];
-#pragma unroll
-  for (int q = 0; q < NV; ++q) acc[q] = 0.0;
-
   // ring slots of planes k-1, k, k+1 (rotated at the end of a step) and the own cell's offset in plane k-1
   int sm = slot_of(k0 - 1), sc = slot_of(k0), sp = slot_of(k0 + 1);
   long long gm = own_g + (long long)(k0 + 1) * P.sz;
@@ -249,44 +246,44 @@ __global__ void __launch_bounds__(32 * (TY + 1), MINB) stage3d_kernel(const __gr
     const bool full = k < k1;       // plane k gets its x and y sweeps (step k1 only closes plane k1-1)
     const bool emit = k > k0;       // plane k-1 is completed in this step
     const int hb = 3 * PL + (k & 1) * SB;                 // y-halo rows of plane k
+    const int ph0 = ph;                                   // sub-phases completed when this plane starts
     double Ly[NV], ua[NV], ub[NV];
 
 #pragma unroll
     for (int s = 0; s < 3; ++s) {
       double L[NV], R[NV], F[NV];
       bool flux = false;
-      // ---- hand-over: what this phase reads must be published, what it overwrites must have been read.  Every
-      //      wait is on a phase EARLIER than the one about to start, so the waits cannot form a cycle.
+      // ---- hand-over: what this sub-phase reads must be published, what it overwrites must have been read.  Every
+      //      wait is on a sub-phase EARLIER than the one about to start, so the waits cannot form a cycle.
       if (s == 0) {
-        // phase A.  owner j: YF / YR row pair with the warp below (H for row 0), ring rows j+-1 of plane k, and the
-        // y-halo rows (H) for the top row.  H: every owner is done with XR / XF / YR[TY] and the halo columns.
+        // phase A.  owner j: the row below is done with plane k-1 (it has read Y[j], the state this phase replaces,
+        // and converted its ring row); the row above has converted its ring row of plane k (its phase A of plane
+        // k-1), H its y-halo rows (all of plane k-1).  H: every owner is done with XR / XF / Y[TY] / the halo columns.
         if (owner) {
-          await(prog + (wid == 0 ? TY : wid - 1), ph, P.flag);
-          await(prog + (wid == TY - 1 ? TY : wid + 1), wid == TY - 1 ? ph : ph - 1, P.flag);
+          await(prog + (wid == 0 ? TY : wid - 1), ph0, P.flag);
+          await(prog + (wid == TY - 1 ? TY : wid + 1), wid == TY - 1 ? ph0 : ph0 - 2, P.flag);
         } else {
-          await(prog + min(lane, TY - 1), ph, P.flag);
+          await(prog + min(lane, TY - 1), ph0, P.flag);
           __syncwarp();
         }
       } else if (s == 1) {
-        // phase B.  owner j: YR of the row above (H for the top row), XR / XF and the halo columns (H).
-        // H: YR[0] (owner 0), and both edge owners are done with the y-halo rows H is about to refill.
+        // phase B1.  owner j: the right state in Y[j+1] (phase A of the row above, H for the top row).
+        // H: Y[0] (owner 0).
+        if (owner) await(prog + (wid == TY - 1 ? TY : wid + 1), ph0 + 1, P.flag);
+        else await(prog + 0, ph0 + 1, P.flag);
+      } else {
+        // phase B2.  owner j: XR / XF and the halo columns (phase A of H).
+        // H: both edge owners are done with the y-halo rows H is about to refill (their phase A).
         if (owner) {
-          await(prog + (wid == TY - 1 ? TY : wid + 1), ph, P.flag);
-          await(prog + TY, ph, P.flag);
+          await(prog + TY, ph0 + 1, P.flag);
         } else {
-          await(prog + 0, ph, P.flag);
-          await(prog + TY - 1, ph, P.flag);
+          await(prog + 0, ph0 + 1, P.flag);
+          await(prog + TY - 1, ph0 + 1, P.flag);
         }
       }
       // ------------------------------------------------------------------ prepare the face states of task s
       if (owner) {
         if (s == 0) {
-          if (emit) {
-            // A5 (y) of plane k-1: YF holds the rotated (n = 1) fluxes of the previous phase B
-#pragma unroll
-            for (int r = 0; r < NV; ++r)
-              acc[rv(r, 1)] -= cy * (YF[r * YS + (wid + 1) * 32 + lane] - YF[r * YS + wid * 32 + lane]);
-          }
           cp_async_wait_all();
           if (own_in) conv_in_place(sp + own_off);          // A1 of the own cell of plane k+1
           // A2 (z): slope of plane k;  face k-1/2:  L carried,  R = W(k) - dW/2
@@ -303,17 +300,10 @@ __global__ void __launch_bounds__(32 * (TY + 1), MINB) stage3d_kernel(const __gr
           flux = true;
         } else if (full) {
           if (s == 1) {
-            if (two) {                                                     // A6: Uin + (a0/a1) U0  (uniform branch)
-#pragma unroll
-              for (int q = 0; q < NV; ++q) acc[q] += fma(P.r0, ub[q], ua[q]);
-            } else {
-#pragma unroll
-              for (int q = 0; q < NV; ++q) acc[q] += ua[q];
-            }
 #pragma unroll
             for (int r = 0; r < NV; ++r) {
               L[r] = Ly[r];
-              R[r] = YR[rv(r, 1) * YS + (wid + 1) * 32 + lane];
+              R[r] = Y[rv(r, 1) * YS + (wid + 1) * 32 + lane];
             }
           } else {
             // A2 (x): own slope; the right state of face i+1/2 comes from lane i+1 (lane 31: from H)
@@ -340,7 +330,7 @@ __global__ void __launch_bounds__(32 * (TY + 1), MINB) stage3d_kernel(const __gr
               const double a = W[q * QS + cm], b = W[q * QS + c0r], c = W[q * QS + cp];
               double lo, hi;
               plm_faces(limiter, beta2, a, b, c, lo, hi);
-              YR[q * YS + TY * 32 + lane] = lo;
+              Y[q * YS + TY * 32 + lane] = lo;
             }
           }
           // column x = 32: right state for lane 31 of every row
@@ -378,7 +368,7 @@ __global__ void __launch_bounds__(32 * (TY + 1), MINB) stage3d_kernel(const __gr
             double lo, hi;
             plm_faces(limiter, beta2, a, b, c, lo, hi);
             L[r] = hi;
-            R[r] = YR[v * YS + lane];
+            R[r] = Y[v * YS + lane];
           }
           flux = true;
         }
@@ -402,28 +392,24 @@ __global__ void __launch_bounds__(32 * (TY + 1), MINB) stage3d_kernel(const __gr
       // ------------------------------------------------------------------ consume the flux of task s
       if (owner) {
         if (s == 0) {
-          // A5 (z) + A6: plane k-1 is complete;  the accumulator of plane k starts with its low z face
-          double* po = P.Uout + gm;                                       // own cell of plane k-1
-          double o[NV];
+          // Uin (+U0) of the own cell of plane k-1, needed when the plane is completed below: the loads are in
+          // flight while the y slopes are formed.  Uniform branches on the stage kind: the first stage issues no U0
+          // loads and no selects.
 #pragma unroll
-          for (int v = 0; v < NV; ++v, po += P.sq) {
-            constexpr int inv2[9] = {0, 2, 3, 1, 4, 6, 7, 5, 8};          // rv(inv2[v], 2) == v
-            const int r = inv2[v];
-            // the difference is formed before it meets U, so that a uniform state stays bitwise fixed (pin P1)
-            o[v] = c0 * (acc[v] - cz * (F[r] - FzL[v * ZS + tid]));
-            if (GLM && v == NV - 1) o[v] *= decay;                        // eq.11's source, integrated exactly
-            if (CGL && v == NV - 1 && P.last_stage && P.relax > 0.0 && emit && cell_ok)
-              o[v] = cgl_relaxed_alog(P.relax, o);                        // eqs.31-33: E stays, A_log moves
-            if (emit && cell_ok) *po = o[v];
-            FzL[v * ZS + tid] = F[r];
-            acc[v] = 0.0;
-          }
-          if (P.vnext != nullptr && emit && cell_ok) {                    // A7 on the values just stored
-            const double sp = cell_speed_inline(P.ph, o);
-            if (sp < 0.0) bad = 1; else vmx = dmax(vmx, sp);
+          for (int q = 0; q < NV; ++q) { ua[q] = 0.0; ub[q] = 0.0; }
+          if (emit && cell_ok) {
+            const double* pa = P.Uin + gm;
+            const double* pb = P.U0 + gm;
+            if (two) {
+#pragma unroll
+              for (int q = 0; q < NV; ++q, pa += P.sq, pb += P.sq) { ua[q] = __ldg(pa); ub[q] = *pb; }
+            } else {
+#pragma unroll
+              for (int q = 0; q < NV; ++q, pa += P.sq) ua[q] = __ldg(pa);
+            }
           }
           if (full) {
-            // A2 (y): own slope -> right state for the row below, left state kept for phase B
+            // A2 (y): own slope -> right state for the row below, left state kept for phase B1
             const int c = sc + own_off;
             const int cm = (wid == 0) ? hb + RS + lane + 2 : c - RS;
             const int cp = (wid == TY - 1) ? hb + 2 * RS + lane + 2 : c + RS;
@@ -433,43 +419,59 @@ __global__ void __launch_bounds__(32 * (TY + 1), MINB) stage3d_kernel(const __gr
               const double a = W[v * QS + cm], b = W[v * QS + c], cc = W[v * QS + cp];
               double lo, hi;
               plm_faces(limiter, beta2, a, b, cc, lo, hi);
-              YR[v * YS + wid * 32 + lane] = lo;
+              Y[v * YS + wid * 32 + lane] = lo;
               Ly[r] = hi;
             }
-            // Uin (+U0) of the own cell of plane k: in flight across barrier 1
-            const double* pa = P.Uin + gm + P.sz;
-            const double* pb = P.U0 + gm + P.sz;
+          }
+          // A5 (z) + A6: plane k-1 is complete:  Uout = a1 ((a0/a1) U0 + Uin + [-dt (flux differences)]);  the
+          // accumulator of plane k starts with its low z face.  The flux terms are summed on their own and the two
+          // z terms are the same rounded product, so a uniform state stays bitwise fixed (pin P1).
+          double* po = P.Uout + gm;                                       // own cell of plane k-1
+          double o[NV];
 #pragma unroll
-            for (int q = 0; q < NV; ++q) { ua[q] = 0.0; ub[q] = 0.0; }
-            if (cell_ok) {
-              // uniform branches on the stage kind: the first stage issues no U0 loads and no selects
-              if (two) {
-#pragma unroll
-                for (int q = 0; q < NV; ++q, pa += P.sq, pb += P.sq) { ua[q] = __ldg(pa); ub[q] = *pb; }
-              } else {
-#pragma unroll
-                for (int q = 0; q < NV; ++q, pa += P.sq) ua[q] = __ldg(pa);
-              }
-            }
+          for (int v = 0; v < NV; ++v, po += P.sq) {
+            constexpr int inv2[9] = {0, 2, 3, 1, 4, 6, 7, 5, 8};          // rv(inv2[v], 2) == v
+            const double t = cz * F[inv2[v]];
+            const double d = ACC[v * ZS + tid] - t;
+            o[v] = c0 * ((two ? fma(P.r0, ub[v], ua[v]) : ua[v]) + d);
+            if (GLM && v == NV - 1) o[v] *= decay;                        // eq.11's source, integrated exactly
+            if (CGL && v == NV - 1 && P.last_stage && P.relax > 0.0 && emit && cell_ok)
+              o[v] = cgl_relaxed_alog(P.relax, o);                        // eqs.31-33: E stays, A_log moves
+            if (emit && cell_ok) *po = o[v];
+            ACC[v * ZS + tid] = t;
+          }
+          if (P.vnext != nullptr && emit && cell_ok) {                    // A7 on the values just stored
+            const double sp = cell_speed_inline(P.ph, o);
+            if (sp < 0.0) bad = 1; else vmx = dmax(vmx, sp);
           }
         } else if (full) {
           if (s == 1) {
 #pragma unroll
-            for (int r = 0; r < NV; ++r) YF[r * YS + (wid + 1) * 32 + lane] = F[r];
+            for (int r = 0; r < NV; ++r) Y[r * YS + (wid + 1) * 32 + lane] = F[r];
           } else {
             // A5 (x): low-face flux from lane i-1 (lane 0: from H)
+            double dFx[NV];
 #pragma unroll
             for (int r = 0; r < NV; ++r) {
               const double fl = __shfl_up_sync(0xffffffffu, F[r], 1);
-              acc[r] -= cx * (F[r] - ((lane == 0) ? XF[r * XS + wid] : fl));
+              dFx[r] = F[r] - ((lane == 0) ? XF[r * XS + wid] : fl);
             }
             // own cell of plane k+2 -> the slot plane k-1 left in phase A
             if (own_in && k + 2 <= k1 + 1) copy_cell(sm + own_off, gm + 3 * P.sz);
-            // second SSP stage: U0 of plane k+1 is first touched one step from now; pull its lines into L2 (one
+            // second SSP stage: U0 of plane k+1 is first touched two steps from now; pull its lines into L2 (one
             // lane per 64 bytes)
             if (two && cell_ok && (lane & 7) == 0 && k + 1 < k1) {
 #pragma unroll
               for (int q = 0; q < NV; ++q) prefetch_l2(P.U0 + q * P.sq + gm + 2 * P.sz);
+            }
+            // A5 (y): Y[j+1] holds this row's own flux (phase B1), Y[j] the flux of the row below (its phase B1)
+            await(prog + (wid == 0 ? TY : wid - 1), ph0 + 2, P.flag);
+#pragma unroll
+            for (int v = 0; v < NV; ++v) {
+              constexpr int inv1[9] = {0, 3, 1, 2, 4, 7, 5, 6, 8};        // rv(inv1[v], 1) == v
+              const int r = inv1[v];
+              const double dFy = Y[r * YS + (wid + 1) * 32 + lane] - Y[r * YS + wid * 32 + lane];
+              ACC[v * ZS + tid] = fma(-cx, dFx[v], fma(-cy, dFy, ACC[v * ZS + tid]));
             }
           }
         }
@@ -482,16 +484,16 @@ __global__ void __launch_bounds__(32 * (TY + 1), MINB) stage3d_kernel(const __gr
         } else if (s == 1) {
           if (full) {
 #pragma unroll
-            for (int r = 0; r < NV; ++r) YF[r * YS + lane] = F[r];
+            for (int r = 0; r < NV; ++r) Y[r * YS + lane] = F[r];
           }
         } else {
-          // A1 for the halo cells of plane k+1 (copies issued one phase B ago), then the copies for plane k+2
+          // A1 for the halo cells of plane k+1 (copies issued one phase B2 ago), then the copies for plane k+2
           cp_async_wait_all();
           if (k + 1 < k1) h_conv(k + 1, sp);
           if (k + 2 < k1) h_copy(k + 2, sm);
         }
       }
-      if (s != 1) publish(prog + wid, ++ph, lane);   // end of phase A (s = 0) and of phase B (s = 2)
+      publish(prog + wid, ++ph, lane);   // end of phase A, B1, B2
     }
     { const int t = sm; sm = sc; sc = sp; sp = t; }
   }
