@@ -6,7 +6,7 @@
  *
  *   A0 ghost fill (periodic, 2 layers)      A4 Riemann flux: HLL eq.5-6 or HLLD (R10)
  *   A1 primitive recovery (R2)                     A5 flux difference, eq.1
- *   A2 PLM reconstruction + eq.4 limiter       A6 Runge-Kutta stage combine (RK11 / SSP-RK22, R11)
+ *   A2 PLM reconstruction + eq.4 limiter       A6 Runge-Kutta stage combine (RK11 ... RK53, R11/R25/R27)
  *   A3 Davis signal speeds eq.6 + fast speed eq.12 (R3)    A7 global Courant reduction dt = C dx_min / v_max
  *   A8 Hall terms: face current J, v_H = -d_i J / rho, whistler speed eq.13
  *
@@ -47,14 +47,17 @@ typedef struct {
   int32_t riemann;      /* 0 = HLL (eq.5), 1 = HLLD (R10; not in the paper)              */
   int32_t limiter;      /* 0 = none (dU = 0), 1 = central (unlimited), 2 = eq.4   */
   double  beta;         /* eq.4 beta in [1,2]: 1.0 = minmod, 1.3 = the paper's "MC" default */
-  int32_t rk;           /* 1 = RK11 (forward Euler), 2 = SSP-RK22 (R11), 3 = SSP-RK33 (R25;
-                           needs a third state copy in the workspace)                                  */
+  int32_t rk;           /* stages: 1 = RK11 (forward Euler), 2 = SSP-RK22 (R11), 3 = SSP-RK33 (R25),
+                           4 = RK43, 5 = RK53 (P:L55 names them, ref.[25]; Shu-Osher forms of R27, third order);
+                           rk >= 3 needs a third state copy in the workspace                             */
   double  cfl;          /* Courant number C; <= 0 selects the paper default 0.8/0.45/0.325   */
   double  d_i;          /* normalised ion inertial length (eqset AGATE_HALL only)            */
   double  relax;        /* eqset AGATE_CGL only: dt/(dt+tau) of eqs.32-33 in [0,1]; the paper's default is
                            0.99; 0 = no relaxation                                            */
   int32_t bc[3];        /* ghost rule per dimension (x, y, z): 0 = periodic, 1 = zero-gradient /
-                           open end (R26: ghost = nearest interior zone)                       */
+                           open end (R26: ghost = nearest interior zone); bc[1] = 2: the sheared
+                           zero-gradient ends of the 2-D whistler test (R28: ghost (i,j) = zone (i-1,j+2)
+                           at the down side, (i+1,j-2) at the up side, x periodic: needs bc[0] = 0, ndim >= 2) */
 } agate_solver;
 
 enum { AGATE_IDEAL = 0, AGATE_HALL = 1, AGATE_CGL = 2, AGATE_IDEAL_GLM = 3 };
@@ -78,7 +81,7 @@ enum {
 };
 
 /* Bytes of device workspace agate_init needs for this problem (0 on invalid arguments): two ghost-padded copies of
- * the state (three with rk = 3), 8 or 9 variables each, plus a few hundred bytes of device scalars. */
+ * the state (three with rk >= 3), 8 or 9 variables each, plus a few hundred bytes of device scalars. */
 size_t agate_workspace_bytes(const agate_grid* grid, int eqset, const agate_solver* solver);
 
 /* Create a context.  `workspace`: DEVICE pointer, caller-owned, >= agate_workspace_bytes(), 256-byte aligned,
@@ -90,9 +93,11 @@ int agate_init(const agate_grid* grid, double gamma, int eqset, const agate_solv
 
 /* Copy an interior-only SoA state U[8][nz][ny][nx] (U[9]... for AGATE_IDEAL_GLM / AGATE_CGL) into the context and set
  * the time to t0.
- * `U` is a HOST pointer when src_is_device == 0 (pinned memory makes the copy asynchronous), else a DEVICE
- * pointer.  Fills the ghost layers (A0; periodic or zero-gradient per solver->bc).  Validates nothing physical (the
- * dt reduction does). */
+ * `U` is a HOST pointer when src_is_device == 0 (borrowed for the call only: the call synchronises the stream), else
+ * a DEVICE pointer, read in stream order without any synchronisation: whatever produced it must be ordered before
+ * this call on the context's stream (an event wait if it ran on another stream), and it must stay untouched until the
+ * copy has run.  The same holds for a DEVICE destination of agate_get_state.  Fills the ghost layers (A0; per
+ * solver->bc).  Validates nothing physical (the dt reduction does). */
 int agate_set_state(agate_ctx*, const double* U, int src_is_device, double t0);
 
 /* A7: dt = C dx_min / max_cells(|v| + max(c_f, c_w)) of the current state -> *dt_out (HOST).
@@ -127,6 +132,15 @@ int agate_launch_info(agate_ctx*, int64_t out[8]);
 int agate_set_timing(agate_ctx*, int enabled);
 int agate_stage_time(agate_ctx*, double* ms_out, int64_t* launches_out, int reset);
 
+/* Launch tuning of one context (optional; call before stepping).  No process-wide state, no environment variables. */
+typedef struct {
+  int32_t stage_grid;   /* CTAs of the 2-D / 3-D stage kernel's one-wave grid; 0 = automatic (every resident slot,
+                           fewer on tiny grids).  The result does not depend on it bit for bit; the tests use it to
+                           reach ragged work splits.  Ignored on 1-D grids.                                       */
+  int32_t no_graph;     /* != 0: agate_advance enqueues the kernels directly instead of replaying its CUDA graph  */
+} agate_tuning;
+int agate_set_tuning(agate_ctx*, const agate_tuning*);
+
 int agate_destroy(agate_ctx*);
 const char* agate_strerror(int status);
 
@@ -140,8 +154,9 @@ int agate_test_face_flux(int eqset, int riemann, int dir, double gamma, double d
 
 /* FP64 FMA throughput micro-benchmark (8 independent DFMA chains per thread on every SM): returns the sustained
  * TFLOP/s (FMA = 2 flop) over `iters` launches in *tflops_out.  Gives the ALU roofline denominator, which
- * MEASURED_PEAKS.json does not hold. */
-int agate_measure_fp64_peak(int iters, double* tflops_out, void* stream);
+ * MEASURED_PEAKS.json does not hold.  `scratch`: >= 8 bytes of the caller's DEVICE memory (the library allocates
+ * none). */
+int agate_measure_fp64_peak(int iters, double* tflops_out, void* scratch, void* stream);
 
 #ifdef __cplusplus
 }

@@ -30,7 +30,7 @@ OK, ERR_ARG, ERR_STATE, ERR_UNPHYSICAL, ERR_CUDA, ERR_NOMEM = range(6)
 # every symbol include/agate.h declares (tests check that the library exports each of them)
 SYMBOLS = ("agate_workspace_bytes", "agate_init", "agate_set_state", "agate_compute_dt", "agate_step",
            "agate_advance", "agate_get_state", "agate_poll", "agate_launch_info", "agate_set_timing",
-           "agate_stage_time", "agate_destroy", "agate_strerror", "agate_test_face_flux",
+           "agate_stage_time", "agate_set_tuning", "agate_destroy", "agate_strerror", "agate_test_face_flux",
            "agate_measure_fp64_peak")
 
 
@@ -43,6 +43,10 @@ class SolverCfg(C.Structure):
     _fields_ = [("riemann", C.c_int32), ("limiter", C.c_int32), ("beta", C.c_double),
                 ("rk", C.c_int32), ("cfl", C.c_double), ("d_i", C.c_double), ("relax", C.c_double),
                 ("bc", C.c_int32 * 3)]
+
+
+class Tuning(C.Structure):
+    _fields_ = [("stage_grid", C.c_int32), ("no_graph", C.c_int32)]
 
 
 class AgateError(RuntimeError):
@@ -79,12 +83,13 @@ def lib():
         L.agate_launch_info.argtypes = [_vp, C.POINTER(C.c_int64)]
         L.agate_set_timing.argtypes = [_vp, C.c_int]
         L.agate_stage_time.argtypes = [_vp, _dp, C.POINTER(C.c_int64), C.c_int]
+        L.agate_set_tuning.argtypes = [_vp, C.POINTER(Tuning)]
         L.agate_destroy.argtypes = [_vp]
         L.agate_strerror.argtypes = [C.c_int]
         L.agate_strerror.restype = C.c_char_p
         L.agate_test_face_flux.argtypes = [C.c_int, C.c_int, C.c_int, C.c_double, C.c_double, C.c_double,
                                            _vp, _vp, _vp, _vp, C.c_int64, _vp]
-        L.agate_measure_fp64_peak.argtypes = [C.c_int, _dp, _vp]
+        L.agate_measure_fp64_peak.argtypes = [C.c_int, _dp, _vp, _vp]
         _lib = L
     return _lib
 
@@ -100,7 +105,7 @@ class Agate:
     """One simulation context (agate_ctx) on a dedicated CUDA stream.  Names follow include/agate.h."""
 
     def __init__(self, shape, dx, ndim, gamma=5.0 / 3.0, eqset=IDEAL, riemann=HLL, limiter=2, beta=1.3, rk=2,
-                 cfl=0.0, d_i=0.0, relax=0.0, bc=(0, 0, 0), device="cuda:0", stream=None):
+                 cfl=0.0, d_i=0.0, relax=0.0, bc=(0, 0, 0), device="cuda:0", stream=None, stage_grid=0, no_graph=False):
         torch = _torch_cuda()
         nx, ny, nz = (int(s) for s in shape)
         self.shape = (nx, ny, nz)
@@ -122,6 +127,9 @@ class Agate:
                               _vp(self.workspace.data_ptr()), nbytes, _vp(self.stream.cuda_stream), C.byref(self._h))
         if rc:
             raise AgateError(rc, "agate_init")
+        if stage_grid or no_graph:
+            tun = Tuning(int(stage_grid), 1 if no_graph else 0)
+            self._chk(L.agate_set_tuning(self._h, C.byref(tun)), "agate_set_tuning")
 
     @classmethod
     def from_workload(cls, wl, **over):
@@ -154,6 +162,8 @@ class Agate:
             self._keep = U
             ptr, on_dev = U.ctypes.data, False
         with torch.cuda.device(self.device):
+            if on_dev:      # the copy runs on the context's stream: order it after whatever produced U (include/agate.h)
+                self.stream.wait_stream(torch.cuda.current_stream())
             self._chk(lib().agate_set_state(self._h, _vp(ptr), int(on_dev), float(t0)), "agate_set_state")
 
     def get_state(self, out=None):
@@ -171,6 +181,8 @@ class Agate:
             ptr, on_dev = out.ctypes.data, False
         with torch.cuda.device(self.device):
             self._chk(lib().agate_get_state(self._h, _vp(ptr), int(on_dev), C.byref(t)), "agate_get_state")
+            if on_dev:      # later work on torch's current stream sees the copied state
+                torch.cuda.current_stream().wait_stream(self.stream)
         self.t = t.value
         return out
 
@@ -238,9 +250,11 @@ def test_face_flux(eqset, riemann, d, gamma, WL, WR, J=None, d_i=0.0, dxmin=1.0)
 
 
 def measure_fp64_peak(iters=20):
-    _torch_cuda()
+    torch = _torch_cuda()
     v = C.c_double()
-    rc = lib().agate_measure_fp64_peak(int(iters), C.byref(v), None)
+    scratch = torch.zeros(8, dtype=torch.float64, device="cuda")
+    torch.cuda.synchronize()
+    rc = lib().agate_measure_fp64_peak(int(iters), C.byref(v), _vp(scratch.data_ptr()), None)
     if rc:
         raise AgateError(rc, "agate_measure_fp64_peak")
     return v.value

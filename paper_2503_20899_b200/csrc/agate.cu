@@ -60,7 +60,7 @@ Layout make_layout(const agate_grid& g, int nv, int rk = 2) {
   L.off_A = 0;
   L.off_B = align_up(L.off_A + L.state_bytes, 256);
   L.off_C = align_up(L.off_B + L.state_bytes, 256);
-  L.off_scal = (rk == 3) ? align_up(L.off_C + L.state_bytes, 256) : L.off_C;
+  L.off_scal = (rk >= 3) ? align_up(L.off_C + L.state_bytes, 256) : L.off_C;
   L.off_partial = L.off_scal + 256;                       // scal: 3 doubles + flag + ticket
   L.total = L.off_partial + align_up(sizeof(double) * kDtBlocksMax, 256);
   return L;
@@ -78,9 +78,10 @@ int check_args(const agate_grid* g, double gamma, int eqset, const agate_solver*
   if (eqset == AGATE_CGL && (g->ndim < 2 || s->riemann != AGATE_HLL)) return AGATE_ERR_ARG;    // CGL: 2-D and 3-D kernels, HLL
   if (eqset == AGATE_CGL && !(s->relax >= 0.0 && s->relax <= 1.0)) return AGATE_ERR_ARG;
   if (eqset == AGATE_IDEAL_GLM && g->ndim < 2) return AGATE_ERR_ARG;             // GLM: 2-D and 3-D kernels
-  if (s->riemann < 0 || s->riemann > 1 || s->limiter < 0 || s->limiter > 2 || s->rk < 1 || s->rk > 3) return AGATE_ERR_ARG;
+  if (s->riemann < 0 || s->riemann > 1 || s->limiter < 0 || s->limiter > 2 || s->rk < 1 || s->rk > 5) return AGATE_ERR_ARG;
   if (s->limiter == 2 && !(s->beta >= 1.0 && s->beta <= 2.0)) return AGATE_ERR_ARG;
-  for (int d = 0; d < 3; ++d) if (s->bc[d] < 0 || s->bc[d] > 1) return AGATE_ERR_ARG;
+  for (int d = 0; d < 3; ++d) if (s->bc[d] < 0 || s->bc[d] > ((d == 1) ? 2 : 1)) return AGATE_ERR_ARG;
+  if (s->bc[1] == 2 && (g->ndim < 2 || s->bc[0] != 0)) return AGATE_ERR_ARG;   // sheared ends in y need a periodic x (R28)
   if (eqset == AGATE_HALL && s->riemann == AGATE_HLLD) return AGATE_ERR_ARG;   // no Hall-HLLD in the paper
   if (eqset == AGATE_HALL && !(s->d_i >= 0.0)) return AGATE_ERR_ARG;
   if (eqset == AGATE_HALL && g->ndim == 3) return AGATE_ERR_ARG;               // 3-D Hall: not built yet
@@ -131,10 +132,6 @@ StageKernel make_stage2d() {
 
 StageKernel pick_stage(int ndim, int eqset, int riemann, int limiter) {
   if (ndim == 3) {
-    if (getenv("AGATE_STAGE_V1")) {      // the pooled kernel of agate_kernels.cuh, kept for A/B measurements
-      if (riemann == AGATE_HLLD) return make_stage<6, 3, 1, false, 2>();
-      return make_stage<6, 3, 0, false, 2>();
-    }
     if (eqset == AGATE_CGL)
       return (limiter == 2) ? make_stage3d<TY3N, 0, 2, AGATE_MINB3, false, true>() : make_stage3d<TY3N, 0, -1, AGATE_MINB3, false, true>();
     if (eqset == AGATE_IDEAL_GLM) {
@@ -148,7 +145,7 @@ StageKernel pick_stage(int ndim, int eqset, int riemann, int limiter) {
     if (riemann == AGATE_HLLD) return make_stage3d<TY3, 1, -1, AGATE_MINB3>();
     return make_stage3d<TY3, 0, -1, AGATE_MINB3>();
   }
-  if (ndim == 2 && !getenv("AGATE_STAGE_V1")) {   // warp-autonomous strips
+  if (ndim == 2) {   // warp-autonomous strips
     if (eqset == AGATE_HALL)
       return (limiter == 3) ? make_stage2d<0, 3, true>() : ((limiter == 2) ? make_stage2d<0, 2, true>() : make_stage2d<0, -1, true>());
     if (eqset == AGATE_CGL) return (limiter == 2) ? make_stage2d<0, 2, false, false, true>() : make_stage2d<0, -1, false, false, true>();
@@ -196,6 +193,7 @@ struct agate_ctx {
   GhostParams gpA, gpB, gpC;
   cudaGraphExec_t graph = nullptr;
   bool timing = false;
+  bool no_graph = false;           // agate_set_tuning: launch the kernels directly
   std::vector<cudaEvent_t> ev;     // pairs (start, stop) of timed stage launches
   size_t ev_used = 0;
   double stage_ms = 0.0;
@@ -230,11 +228,11 @@ GhostParams make_ghost(const agate_ctx* c, double* U) {
 }
 
 StageParams make_stage_params(const agate_ctx* c, const double* Uin, const double* U0, double* Uout, double a0,
-                              double a1, bool last_stage) {
+                              double a1, double cdt, bool last_stage) {
   StageParams p;
   const Layout& L = c->L;
   p.Uin = Uin; p.U0 = U0; p.Uout = Uout; p.dt_ptr = c->scal;
-  p.a0 = a0; p.a1 = a1; p.r0 = (a0 != 0.0) ? a0 / a1 : 0.0;
+  p.a0 = a0; p.a1 = a1; p.r0 = (a0 != 0.0) ? a0 / a1 : 0.0; p.cdt = cdt;
   p.nx = c->g.nx; p.ny = c->g.ny; p.nz = c->g.nz; p.ndim = c->g.ndim;
   p.ghy = L.ghy; p.ghz = L.ghz; p.nxp = L.nxp; p.nyp = L.nyp;
   p.sy = L.sy; p.sz = L.sz; p.sq = L.sq;
@@ -297,26 +295,59 @@ int launch_stage(agate_ctx* c, const StageParams& sp) {
   return AGATE_OK;
 }
 
-// One full time step enqueued on the stream; dt is already in scal[0].
-// SSP-RK22 (R11):  U1 = Un + dt L(Un);  Un+1 = Un/2 + (U1 + dt L(U1))/2.   RK11: Un+1 = Un + dt L(Un).
+// One full time step enqueued on the stream; dt is already in scal[0].  Every stage is
+//     Uout = a0 Uref + a1 (Uin + c dt L(Uin))                                   (Shu-Osher form, dt once per step: R11)
+// with the ghost fill of Uin in front of it.  A, B, C are the state copies; the step starts and ends with U^n in A.
+//   RK11:      B = A + dt L(A)                                                   (then A <-> B)
+//   SSP-RK22:  B = A + dt L(A);  A = 1/2 A + 1/2 (B + dt L(B))                                              (R11)
+//   SSP-RK33:  B = A + dt L(A);  C = 3/4 A + 1/4 (B + dt L(B));  A = 1/3 A + 2/3 (C + dt L(C))             (R25)
+//   RK43:      c = 1/2:  B = A + c dt L(A);  C = B + c dt L(B);  B = 2/3 A + 1/3 (C + c dt L(C));  A = B + c dt L(B)   (R27)
+//   RK53:      c = 0.377268915331368:  B = A + c dt L(A);  C = B + c dt L(B);  B = a30 A + a32 (C + c dt L(C));
+//              A = a40 A + a43 (B + c dt L(B));  B = a52 C + a54 (A + c dt L(A))   (then A <-> B)             (R27)
+// Uref may be the output buffer (the combine is pointwise); Uin never is (the stage reads its neighbours).
+struct RkStage { int in, ref, out; double a0, a1, c; };
+int rk_table(int rk, RkStage st[5], bool* swap_ab) {
+  *swap_ab = false;
+  switch (rk) {
+    case 1: st[0] = {0, -1, 1, 0.0, 1.0, 1.0}; *swap_ab = true; return 1;
+    case 2: st[0] = {0, -1, 1, 0.0, 1.0, 1.0}; st[1] = {1, 0, 0, 0.5, 0.5, 1.0}; return 2;
+    case 3:
+      st[0] = {0, -1, 1, 0.0, 1.0, 1.0}; st[1] = {1, 0, 2, 0.75, 0.25, 1.0}; st[2] = {2, 0, 0, 1.0 / 3.0, 2.0 / 3.0, 1.0};
+      return 3;
+    case 4:
+      st[0] = {0, -1, 1, 0.0, 1.0, 0.5}; st[1] = {1, -1, 2, 0.0, 1.0, 0.5};
+      st[2] = {2, 0, 1, 2.0 / 3.0, 1.0 / 3.0, 0.5}; st[3] = {1, -1, 0, 0.0, 1.0, 0.5};
+      return 4;
+    default: {
+      const double c = 0.377268915331368;
+      st[0] = {0, -1, 1, 0.0, 1.0, c}; st[1] = {1, -1, 2, 0.0, 1.0, c};
+      st[2] = {2, 0, 1, 0.355909775063327, 0.644090224936674, c};
+      st[3] = {1, 0, 0, 0.367933791638137, 0.632066208361863, c};
+      st[4] = {0, 2, 1, 0.237593836598569, 0.762406163401431, c};
+      *swap_ab = true;
+      return 5;
+    }
+  }
+}
+
 int enqueue_stages(agate_ctx* c) {
+  RkStage st[5];
+  bool swap_ab;
+  const int ns = rk_table(c->s.rk, st, &swap_ab);
+  double* U[3] = {c->UA, c->UB, c->UC};
+  const GhostParams* gp[3] = {&c->gpA, &c->gpB, &c->gpC};
   int rc;
-  if ((rc = launch_ghost(c, c->gpA))) return rc;
-  if ((rc = launch_stage(c, make_stage_params(c, c->UA, nullptr, c->UB, 0.0, 1.0, c->s.rk == 1)))) return rc;
-  if (c->s.rk == 1) {
+  for (int i = 0; i < ns; ++i) {
+    if ((rc = launch_ghost(c, *gp[st[i].in]))) return rc;
+    const double* ref = (st[i].ref >= 0) ? U[st[i].ref] : nullptr;
+    if ((rc = launch_stage(c, make_stage_params(c, U[st[i].in], ref, U[st[i].out], st[i].a0, st[i].a1, st[i].c, i == ns - 1))))
+      return rc;
+  }
+  if (swap_ab) {
     std::swap(c->UA, c->UB);
     std::swap(c->gpA, c->gpB);
-    return AGATE_OK;
   }
-  if ((rc = launch_ghost(c, c->gpB))) return rc;
-  if (c->s.rk == 3) {
-    // R25, SSP-RK33:  U2 = 3/4 Un + 1/4 (U1 + dt L(U1))  into the third copy (U1's halos are still being read, Un is
-    // needed once more);  Un+1 = 1/3 Un + 2/3 (U2 + dt L(U2))  over Un
-    if ((rc = launch_stage(c, make_stage_params(c, c->UB, c->UA, c->UC, 0.75, 0.25, false)))) return rc;
-    if ((rc = launch_ghost(c, c->gpC))) return rc;
-    return launch_stage(c, make_stage_params(c, c->UC, c->UA, c->UA, 1.0 / 3.0, 2.0 / 3.0, true));
-  }
-  return launch_stage(c, make_stage_params(c, c->UB, c->UA, c->UA, 0.5, 0.5, true));
+  return AGATE_OK;
 }
 
 // Head of a self-timed step: dt = C dx_min / v_max(U^n), t += dt  (R11).  Separate reduction pass, or -- when the
@@ -365,6 +396,35 @@ int copy_state(agate_ctx* c, double* padded, double* ext, bool to_device, bool e
     CU_TRY(cudaMemcpy3DAsync(&m, c->stream));
   }
   return AGATE_OK;
+}
+
+// Launch grid of the stage kernel.  The pooled kernel (1-D grids) takes one CTA per tile; the 2-D and 3-D kernels
+// run as one resident wave whose CTAs (warps) split the work evenly: `forced` > 0 fixes the number of CTAs
+// (agate_set_tuning; the tests use it to reach ragged splits), 0 = as many as are resident, fewer on tiny grids.
+void set_stage_grid(agate_ctx* c, int forced) {
+  const agate_grid& g = c->g;
+  const int ntx = (g.nx + TX - 1) / TX, nty = (g.ny + c->sk.ty - 1) / c->sk.ty;
+  c->sgrid = dim3(ntx, nty, 1);
+  if (!c->sk.strips2d && !c->sk.even_split) return;
+  int dev = 0, sms = 148;
+  cudaGetDevice(&dev);
+  cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
+  const long long slots = (long long)sms * (c->occ > 0 ? c->occ : 1);
+  long long n;
+  if (c->sk.strips2d) {
+    // a warp gets at least ~4 rows of its 30-column strip
+    const long long work = (long long)((g.nx + SW2 - 1) / SW2) * g.ny;
+    n = (work + 4 * c->sk.warps2d - 1) / (4 * c->sk.warps2d);
+  } else {
+    // a CTA gets at least ~16 tile-planes so that a segment's start-up (three plane loads and the step that
+    // closes its last plane) stays small on tiny grids
+    const long long work = (long long)ntx * nty * g.nz;
+    n = (work + 15) / 16;
+  }
+  if (n > slots) n = slots;
+  if (n < 1) n = 1;
+  if (forced > 0) n = forced;
+  c->sgrid = dim3((unsigned)n, 1, 1);
 }
 
 }  // namespace
@@ -419,58 +479,8 @@ int agate_init(const agate_grid* grid, double gamma, int eqset, const agate_solv
   if (e != cudaSuccess) { delete c; return AGATE_ERR_CUDA; }
   c->regs = fa.numRegs;
 
-  // z-chunk length: the grid is (x-y tiles) x (z chunks).  Pick the chunk count that minimises
-  //   waves x (planes per chunk + start-up),  waves = ceil(CTAs / resident CTAs):  whole waves, short start-up
-  //   (a chunk costs about four extra planes: three loads and the step that closes its last plane).
   c->lz = grid->nz;
-  if (grid->ndim == 3 && !c->sk.even_split) {
-    int dev = 0, sms = 148;
-    cudaGetDevice(&dev);
-    cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
-    const long long slots = (long long)sms * (c->occ > 0 ? c->occ : 1);
-    const long long tiles = (long long)((grid->nx + TX - 1) / TX) * ((grid->ny + c->sk.ty - 1) / c->sk.ty);
-    int best_n = 1;
-    double best_t = 1e300;
-    for (int n = 1; n <= grid->nz && n <= 64; ++n) {
-      const int lz = (grid->nz + n - 1) / n;
-      if (lz < 8 && n > 1) break;
-      const int nn = (grid->nz + lz - 1) / lz;
-      const long long waves = (tiles * nn + slots - 1) / slots;
-      const double t = (double)waves * (lz + 4.0);
-      if (t < best_t * 0.999) { best_t = t; best_n = nn; }
-    }
-    c->lz = (grid->nz + best_n - 1) / best_n;
-    if (const char* s = getenv("AGATE_LZ")) { int v = atoi(s); if (v > 0 && v <= grid->nz) c->lz = v; }
-  }
-  c->sgrid = dim3((grid->nx + TX - 1) / TX, (grid->ny + c->sk.ty - 1) / c->sk.ty,
-                  (grid->ndim == 3) ? (grid->nz + c->lz - 1) / c->lz : 1);
-  if (c->sk.strips2d) {
-    // one resident wave of 6-warp CTAs; a warp gets at least ~4 rows of its 30-column strip
-    int dev = 0, sms = 148;
-    cudaGetDevice(&dev);
-    cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
-    const long long slots = (long long)sms * (c->occ > 0 ? c->occ : 1);
-    const long long work = (long long)((grid->nx + SW2 - 1) / SW2) * grid->ny;
-    long long g = (work + 4 * c->sk.warps2d - 1) / (4 * c->sk.warps2d);
-    if (g > slots) g = slots;
-    if (g < 1) g = 1;
-    if (const char* s = getenv("AGATE_GRID")) { int v = atoi(s); if (v > 0) g = v; }
-    c->sgrid = dim3((unsigned)g, 1, 1);
-  }
-  if (c->sk.even_split) {
-    // one resident wave; a CTA gets at least ~16 tile-planes so that a segment's start-up (three plane loads and
-    // the step that closes its last plane) stays small on tiny grids
-    int dev = 0, sms = 148;
-    cudaGetDevice(&dev);
-    cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
-    const long long slots = (long long)sms * (c->occ > 0 ? c->occ : 1);
-    const long long work = (long long)c->sgrid.x * c->sgrid.y * grid->nz;
-    long long g = (work + 15) / 16;
-    if (g > slots) g = slots;
-    if (g < 1) g = 1;
-    if (const char* s = getenv("AGATE_GRID")) { int v = atoi(s); if (v > 0) g = v; }
-    c->sgrid = dim3((unsigned)g, 1, 1);
-  }
+  set_stage_grid(c, 0);
   long long nrows = (long long)grid->ny * grid->nz;
   c->dt_blocks = (int)(nrows < kDtBlocksMax ? nrows : kDtBlocksMax);
   c->gpA = make_ghost(c, c->UA);
@@ -489,10 +499,10 @@ int agate_set_state(agate_ctx* c, const double* U, int src_is_device, double t0)
   if (!c || !U) return AGATE_ERR_ARG;
   int rc = copy_state(c, c->UA, const_cast<double*>(U), true, src_is_device != 0);
   if (rc) return rc;
-  const double sc[3] = {0.0, 0.0, t0};
-  CU_TRY(cudaMemcpyAsync(c->scal, sc, sizeof(sc), cudaMemcpyHostToDevice, c->stream));
-  CU_TRY(cudaMemsetAsync(c->flag, 0, sizeof(int), c->stream));
-  CU_TRY(cudaStreamSynchronize(c->stream));   // `sc` and the caller's U are borrowed only for this call
+  reset_scalars_kernel<<<1, 1, 0, c->stream>>>(c->scal, c->flag, t0);
+  CU_TRY(cudaGetLastError());
+  // a HOST array is borrowed only for this call; a DEVICE source is read in stream order, no synchronisation
+  if (!src_is_device) CU_TRY(cudaStreamSynchronize(c->stream));
   if ((rc = launch_ghost(c, c->gpA))) return rc;
   c->have_state = true;
   c->vmax_valid = false;
@@ -541,7 +551,7 @@ int agate_advance(agate_ctx* c, int32_t n_steps, double* t_out) {
   if (!c->have_state) return AGATE_ERR_STATE;
   int rc;
   // stream capture is not allowed on the legacy default stream
-  const bool use_graph = (c->s.rk >= 2) && !c->timing && c->stream != nullptr && !getenv("AGATE_NO_GRAPH");
+  const bool use_graph = (c->s.rk >= 2 && c->s.rk <= 4) && !c->timing && c->stream != nullptr && !c->no_graph;
   if (n_steps > 0 && (rc = ensure_vmax(c))) return rc;
   if (use_graph && !c->graph && n_steps > 0) {
     cudaGraph_t g = nullptr;
@@ -596,13 +606,21 @@ int agate_launch_info(agate_ctx* c, int64_t out[8]) {
   if (!c || !out) return AGATE_ERR_ARG;
   out[0] = c->sgrid.x; out[1] = c->sgrid.y; out[2] = c->sgrid.z;
   out[3] = c->sk.threads; out[4] = (int64_t)c->sk.smem; out[5] = c->regs; out[6] = c->occ;
-  out[7] = 1 + 2 * c->s.rk;          // dt + (ghost + stage) per RK stage
+  out[7] = 1 + 2 * c->s.rk;          // dt + (ghost + stage) per RK stage (rk = number of stages)
   return AGATE_OK;
 }
 
 int agate_set_timing(agate_ctx* c, int enabled) {
   if (!c) return AGATE_ERR_ARG;
   c->timing = enabled != 0;
+  return AGATE_OK;
+}
+
+int agate_set_tuning(agate_ctx* c, const agate_tuning* t) {
+  if (!c || !t || t->stage_grid < 0) return AGATE_ERR_ARG;
+  set_stage_grid(c, t->stage_grid);
+  c->no_graph = t->no_graph != 0;
+  if (c->graph) { cudaGraphExecDestroy(c->graph); c->graph = nullptr; }      // captured with the old grid
   return AGATE_OK;
 }
 
@@ -661,15 +679,14 @@ int agate_test_face_flux(int eqset, int riemann, int dir, double gamma, double d
   return AGATE_OK;
 }
 
-int agate_measure_fp64_peak(int iters, double* tflops_out, void* stream) {
-  if (!tflops_out || iters < 1) return AGATE_ERR_ARG;
+int agate_measure_fp64_peak(int iters, double* tflops_out, void* scratch, void* stream) {
+  if (!tflops_out || !scratch || iters < 1) return AGATE_ERR_ARG;
   int ndev = 0, dev = 0, sms = 0;
   if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev < 1) return AGATE_ERR_CUDA;
   cudaGetDevice(&dev);
   cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
   cudaStream_t st = (cudaStream_t)stream;
-  double* d = nullptr;
-  if (cudaMalloc(&d, 64) != cudaSuccess) return AGATE_ERR_CUDA;   // diagnostic only: 64 bytes, freed below
+  double* d = (double*)scratch;     // 8 bytes of the caller's device memory (never written in practice)
   const int blocks = sms * 8, trips = 4096;
   cudaEvent_t e0, e1;
   cudaEventCreate(&e0); cudaEventCreate(&e1);
@@ -681,7 +698,6 @@ int agate_measure_fp64_peak(int iters, double* tflops_out, void* stream) {
   float ms = 0.f;
   cudaEventElapsedTime(&ms, e0, e1);
   cudaEventDestroy(e0); cudaEventDestroy(e1);
-  cudaFree(d);
   if (e != cudaSuccess || !(ms > 0.f)) return AGATE_ERR_CUDA;
   const double flops = 2.0 * 8 * 16 * (double)trips * 256.0 * blocks * iters;
   *tflops_out = flops / (ms * 1e-3) / 1e12;

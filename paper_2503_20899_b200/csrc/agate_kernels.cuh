@@ -37,6 +37,7 @@ struct StageParams {
   double a0, a1;         // Uout = a0 U0 + a1 (Uin + dt L), evaluated as a1 ((a0/a1) U0 + Uin + dt L); a0 == 0: no U0.
                          // SSP-RK22: (1/2, 1/2);  SSP-RK33 (R25): (3/4, 1/4) then (1/3, 2/3)
   double r0;             // a0 / a1
+  double cdt;            // the stage's fraction c of dt (1 except RK43 / RK53, R27): Uin + c dt L
   int nx, ny, nz, ndim;
   int ghy, ghz;          // ghost widths (2 if the dimension is active, else 0)
   int nxp, nyp;          // padded extents
@@ -88,7 +89,7 @@ __global__ void __launch_bounds__(32 * (TY + 2), MINB) stage_kernel(const __grid
   const bool threeD = (NP > 1);
   const int k0 = threeD ? blockIdx.z * P.lz : 0;
   const int k1 = threeD ? min(P.nz, k0 + P.lz) : 1;
-  const double dt = *P.dt_ptr;
+  const double dt = *P.dt_ptr * P.cdt;
   const int ci = tid & 31, cj = tid >> 5;
   const bool cell_ok = (tid < NCELL) && (ci < tw) && (cj < th);
   const int limiter = P.limiter;
@@ -330,7 +331,7 @@ __global__ void __launch_bounds__(32 * (TY + 2), MINB) stage_kernel(const __grid
 struct GhostParams {
   double* U;
   int nv;
-  int bcx, bcy, bcz;         // 0 periodic, 1 zero-gradient (R26)
+  int bcx, bcy, bcz;         // 0 periodic, 1 zero-gradient (R26); bcy = 2: sheared zero-gradient (R28)
   int nx, ny, nz, ghy, ghz, nxp, nyp, nzp;
   long long sy, sz, sq;
   long long nzs, nys, nxs;   // cells in the z-, y-, x-slabs
@@ -368,7 +369,14 @@ __global__ void __launch_bounds__(256) ghost_fill_kernel(const __grid_constant__
     }
     int i = ip - 2, j = jp - P.ghy, k = kp - P.ghz;
     if (P.bcx) i = min(max(i, 0), P.nx - 1); else { i %= P.nx; if (i < 0) i += P.nx; }
-    if (P.bcy) j = min(max(j, 0), P.ny - 1); else { j %= P.ny; if (j < 0) j += P.ny; }
+    if (P.bcy == 2 && (j < 0 || j >= P.ny)) {
+      // sheared zero-gradient ends in y (R28): ghost (i, j) = zone (i-1, j+2) at the down side, (i+1, j-2) at
+      // the up side, x wrapped periodically
+      const int sh = (j < 0) ? -1 : 1;
+      j -= 2 * sh;
+      i = (ip - 2 + sh) % P.nx;
+      if (i < 0) i += P.nx;
+    } else if (P.bcy) j = min(max(j, 0), P.ny - 1); else { j %= P.ny; if (j < 0) j += P.ny; }
     if (P.bcz) k = min(max(k, 0), P.nz - 1); else { k %= P.nz; if (k < 0) k += P.nz; }
     const long long dst = (long long)kp * P.sz + (long long)jp * P.sy + ip;
     const long long src = (long long)(k + P.ghz) * P.sz + (long long)(j + P.ghy) * P.sy + (i + 2);
@@ -485,6 +493,12 @@ __global__ void begin_step_kernel(double* scal, unsigned long long* vnext, doubl
   scal[2] += dt;
   scal[3] = 0.95 * v;                                              // GLM (R22): c_h
   *vnext = 0ull;
+}
+
+// agate_set_state: dt = 0, v_max = 0, t = t0, flag cleared (no host buffer is borrowed past the call)
+__global__ void reset_scalars_kernel(double* scal, int* flag, double t0) {
+  scal[0] = 0.0; scal[1] = 0.0; scal[2] = t0;
+  *flag = 0;
 }
 
 // after a stand-alone dt_kernel: hand its v_max to the fused path

@@ -57,7 +57,7 @@ __global__ void __launch_bounds__(32 * Stage2dSmem<GLM || CGL>::NW, 2) stage2d_k
   double* const FyL = ring + SM::OFF_FYL;
   double* const Uraw = ring + SM::OFF_URAW;
 
-  const double dt = *P.dt_ptr;
+  const double dtf = *P.dt_ptr, dt = dtf * P.cdt;      // full step, and the stage's share of it (R27)
   const double cx = dt * P.idx, cy = dt * P.idy;
   const bool two = (P.a0 != 0.0);
   const double c0 = two ? P.a1 : 1.0;
@@ -69,7 +69,7 @@ __global__ void __launch_bounds__(32 * Stage2dSmem<GLM || CGL>::NW, 2) stage2d_k
   // (c_h^2 / c_p^2 with c_p^2 = 0.18 c_h) in the stage that completes the step
   const double ch = GLM ? *P.ch_ptr : 0.0;
   const double ich = GLM ? 1.0 / ch : 0.0;
-  const double decay = (GLM && P.last_stage) ? exp(-dt * ch / 0.18) : 1.0;
+  const double decay = (GLM && P.last_stage) ? exp(-dtf * ch / 0.18) : 1.0;
 
   const int nstrip = (P.nx + SW2 - 1) / SW2;
   const long long wtot = (long long)nstrip * P.ny;

@@ -112,7 +112,7 @@ __global__ void __launch_bounds__(32 * (TY + 1), MINB) stage3d_kernel(const __gr
 
   const int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5;
   const bool owner = wid < TY;
-  const double dt = *P.dt_ptr;
+  const double dtf = *P.dt_ptr, dt = dtf * P.cdt;      // full step, and the stage's share of it (R27)
   const double cx = dt * P.idx, cy = dt * P.idy, cz = dt * P.idz;
   const bool two = (P.a0 != 0.0);                       // second SSP stage: Uout = a1 (U0 + Uin + dt L)
   const double c0 = two ? P.a1 : 1.0;
@@ -122,7 +122,7 @@ __global__ void __launch_bounds__(32 * (TY + 1), MINB) stage3d_kernel(const __gr
   // (c_h^2 / c_p^2 with c_p^2 = 0.18 c_h) in the stage that completes the step
   const double ch = GLM ? *P.ch_ptr : 0.0;
   const double ich = GLM ? 1.0 / ch : 0.0;
-  const double decay = (GLM && P.last_stage) ? exp(-dt * ch / 0.18) : 1.0;
+  const double decay = (GLM && P.last_stage) ? exp(-dtf * ch / 0.18) : 1.0;
 
   // Work = (x-y tile, plane) pairs, split EVENLY over the CTAs of a one-wave grid (no tail wave, whatever the grid
   // size).  First the rounds: in round r CTA b takes the whole column of tile r * grid + b, so the CTAs resident at

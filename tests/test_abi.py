@@ -59,4 +59,5 @@ def test_no_cpu_fallback_without_cuda():
     with pytest.raises(RuntimeError):
         ag.Agate(shape=(32, 32, 1), dx=(1 / 32, 1 / 32, 1.0), ndim=2)
     v = C.c_double()
-    assert L.agate_measure_fp64_peak(1, C.byref(v), None) == ag.ERR_CUDA
+    assert L.agate_measure_fp64_peak(1, C.byref(v), C.c_void_p(addr), None) == ag.ERR_CUDA
+    assert L.agate_measure_fp64_peak(1, C.byref(v), None, None) == ag.ERR_ARG        # the caller supplies the scratch

@@ -48,10 +48,10 @@ def smooth_state(n):
     return cons_field(W)
 
 
-def pair(ag, shape, dx, relax, **kw):
+def pair(ag, shape, dx, relax, stage_grid=0, **kw):
     args = dict(shape=shape, dx=dx, ndim=2, riemann=0, limiter=2, beta=1.3, rk=2, relax=relax)
     args.update(kw)
-    return oracle.RefSolver(eqset=oracle.CGL, **args), ag.Agate(eqset=ag.CGL, **args)
+    return oracle.RefSolver(eqset=oracle.CGL, **args), ag.Agate(eqset=ag.CGL, stage_grid=stage_grid, **args)
 
 
 def march(ref, gpu, steps):
@@ -68,13 +68,11 @@ def march(ref, gpu, steps):
 
 @pytest.mark.parametrize("relax", [0.0, 0.99])
 @pytest.mark.parametrize("n,grid", [(100, 0), (64, 30)])
-def test_cgl_smooth_2d_parity(ag, relax, n, grid, monkeypatch):
+def test_cgl_smooth_2d_parity(ag, relax, n, grid):
     """Smooth anisotropic 2-D state, ragged strips (n=100) and short segments (grid=30), with and without the
     relaxation of eqs.31-33 (the state crosses the mirror bound in places, so the relaxation is live)."""
-    if grid:
-        monkeypatch.setenv("AGATE_GRID", str(grid))
     U = smooth_state(n)
-    ref, gpu = pair(ag, (n, n, 1), (1 / n, 1 / n, 1), relax)
+    ref, gpu = pair(ag, (n, n, 1), (1 / n, 1 / n, 1), relax, stage_grid=grid)
     ref.set_state(U); gpu.set_state(U)
     e1, eN = march(ref, gpu, 8)
     assert np.all(e1 <= TOL_1), e1
@@ -166,7 +164,7 @@ def test_cgl_brio_wu_open_ends(ag):
 
 
 @pytest.mark.parametrize("seed", range(6))
-def test_cgl_random_shapes_and_options(ag, seed, monkeypatch):
+def test_cgl_random_shapes_and_options(ag, seed):
     """Seeded sweep for the CGL path: ragged 2-D and 3-D shapes, every limiter and RK scheme, relaxation on and off,
     periodic and open ends, default and forced work splits -- 3 steps against the oracle."""
     rng = np.random.default_rng(8000 + seed)
@@ -174,11 +172,10 @@ def test_cgl_random_shapes_and_options(ag, seed, monkeypatch):
     nx, ny = int(rng.choice([29, 31, 33, 61, 64])), int(rng.choice([5, 11, 12, 23]))
     nz = int(rng.choice([4, 9, 17])) if ndim == 3 else 1
     limiter, beta = [(0, 1.0), (1, 1.0), (2, 1.0), (2, 1.3)][int(rng.integers(4))]
-    rk = int(rng.choice([1, 2, 3]))
+    rk = int(rng.choice([1, 2, 3, 4, 5]))
     relax = float(rng.choice([0.0, 0.5, 0.99]))
     bc = tuple(int(b) for b in rng.integers(0, 2, 3))
-    if rng.random() < 0.5:
-        monkeypatch.setenv("AGATE_GRID", str(int(rng.choice([1, 5, 40]))))
+    sg = int(rng.choice([1, 5, 40])) if rng.random() < 0.5 else 0
     shp = (nz, ny, nx)
     W = np.empty((9,) + shp)
     W[0] = 0.5 + rng.random(shp); W[4] = 0.5 + rng.random(shp); W[8] = 0.5 + rng.random(shp)
@@ -189,7 +186,7 @@ def test_cgl_random_shapes_and_options(ag, seed, monkeypatch):
     U = cons_field(W)
     kw = dict(shape=(nx, ny, nz), dx=(1.0 / nx, 1.3 / ny, 0.7 / nz if ndim == 3 else 1.0), ndim=ndim, riemann=0,
               limiter=limiter, beta=beta, rk=rk, bc=bc, relax=relax)
-    ref = oracle.RefSolver(eqset=oracle.CGL, **kw); gpu = ag.Agate(eqset=ag.CGL, **kw)
+    ref = oracle.RefSolver(eqset=oracle.CGL, **kw); gpu = ag.Agate(eqset=ag.CGL, stage_grid=sg, **kw)
     ref.set_state(U); gpu.set_state(U)
     for s in range(3):
         dtr, dtg = ref.compute_dt(), gpu.compute_dt()

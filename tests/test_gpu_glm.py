@@ -32,15 +32,13 @@ def rel_linf9(Ug, Ur, ch):
 
 @pytest.mark.parametrize("n,steps,riemann,grid", [(100, 12, None, 0), (64, 6, oracle.HLLD, 0), (100, 4, None, 40),
                                                    (256, 3, None, 0)])
-def test_orszag_tang_glm_parity(ag, n, steps, riemann, grid, monkeypatch):
+def test_orszag_tang_glm_parity(ag, n, steps, riemann, grid):
     """Config 6 recipe (Orszag-Tang, + GLM) at reduced size: ragged strips (n=100: 3 x 30 + 10), short
     segments (grid=40), HLL (the paper's default) and HLLD."""
-    if grid:
-        monkeypatch.setenv("AGATE_GRID", str(grid))
     wl = make_workload(6, n=n)
     over = {} if riemann is None else {"riemann": riemann}
     ref = oracle.RefSolver.from_workload(wl, **over)
-    gpu = ag.Agate.from_workload(wl, **over)
+    gpu = ag.Agate.from_workload(wl, stage_grid=grid, **over)
     e1 = None
     for s in range(steps):
         dtr, dtg = ref.compute_dt(), gpu.compute_dt()
@@ -102,11 +100,9 @@ def test_glm_uniform_state_exact_decay(ag):
 
 @pytest.mark.parametrize("riemann", [oracle.HLL, oracle.HLLD])
 @pytest.mark.parametrize("grid", [0, 23])
-def test_glm_3d_parity(ag, riemann, grid, monkeypatch):
+def test_glm_3d_parity(ag, riemann, grid):
     """GLM through the 3-D row-owner kernel: config 3's seeded state at 40^3 (ragged tiles) plus a smooth psi and a
     divergence error in B_x; default segmentation and short segments."""
-    if grid:
-        monkeypatch.setenv("AGATE_GRID", str(grid))
     wl = make_workload(3, n=40)
     n = 40
     x = (np.arange(n) + 0.5) / n
@@ -117,7 +113,7 @@ def test_glm_3d_parity(ag, riemann, grid, monkeypatch):
     U[8] = 0.01 * np.sin(2 * np.pi * x)[None, None, :] * np.cos(2 * np.pi * x)[:, None, None]
     kw = dict(shape=wl.shape, dx=wl.dx, ndim=3, gamma=wl.gamma, riemann=riemann, limiter=2, beta=1.3, rk=2, cfl=wl.cfl)
     ref = oracle.RefSolver(eqset=oracle.IDEAL_GLM, **kw); ref.set_state(U)
-    gpu = ag.Agate(eqset=ag.IDEAL_GLM, **kw); gpu.set_state(U)
+    gpu = ag.Agate(eqset=ag.IDEAL_GLM, stage_grid=grid, **kw); gpu.set_state(U)
     e1 = None
     for s_ in range(4):
         dtr, dtg = ref.compute_dt(), gpu.compute_dt()
@@ -141,7 +137,7 @@ def test_glm_rejected_where_not_built(ag):
 
 
 @pytest.mark.parametrize("seed", range(8))
-def test_glm_random_shapes_and_options(ag, seed, monkeypatch):
+def test_glm_random_shapes_and_options(ag, seed):
     """Seeded sweep for the 9-variable GLM path: ragged 2-D and 3-D shapes, both solvers, every limiter and RK scheme,
     periodic and open ends, default and forced work splits -- 3 steps against the oracle."""
     import workloads
@@ -151,15 +147,14 @@ def test_glm_random_shapes_and_options(ag, seed, monkeypatch):
     nz = int(rng.choice([4, 9, 17])) if ndim == 3 else 1
     riemann = int(rng.choice([oracle.HLL, oracle.HLLD]))
     limiter, beta = [(0, 1.0), (1, 1.0), (2, 1.0), (2, 1.3)][int(rng.integers(4))]
-    rk = int(rng.choice([1, 2, 3]))
+    rk = int(rng.choice([1, 2, 3, 4, 5]))
     bc = tuple(int(b) for b in rng.integers(0, 2, 3))
-    if rng.random() < 0.5:
-        monkeypatch.setenv("AGATE_GRID", str(int(rng.choice([1, 5, 40]))))
+    sg = int(rng.choice([1, 5, 40])) if rng.random() < 0.5 else 0
     W, U8 = workloads.random_state(300 + seed, (nx, ny, nz), ndim, amp=0.3)
     U = np.concatenate([U8, 0.05 * rng.standard_normal((1,) + U8.shape[1:])], axis=0)
     kw = dict(shape=(nx, ny, nz), dx=(1.0 / nx, 1.3 / ny, 0.7 / nz if ndim == 3 else 1.0), ndim=ndim, riemann=riemann,
               limiter=limiter, beta=beta, rk=rk, bc=bc)
-    ref = oracle.RefSolver(eqset=oracle.IDEAL_GLM, **kw); gpu = ag.Agate(eqset=ag.IDEAL_GLM, **kw)
+    ref = oracle.RefSolver(eqset=oracle.IDEAL_GLM, **kw); gpu = ag.Agate(eqset=ag.IDEAL_GLM, stage_grid=sg, **kw)
     ref.set_state(U); gpu.set_state(U)
     for s in range(3):
         dtr, dtg = ref.compute_dt(), gpu.compute_dt()

@@ -39,14 +39,14 @@ def rel_linf(Ug, Ur):
     sc[1:4] = np.max(np.abs(Ur[1:4])); sc[5:8] = np.max(np.abs(Ur[5:8]))
     for q in range(8):
         d = np.max(np.abs(Ug[q] - Ur[q]))
-        err[q] = d / sc[q] if sc[q] > 0 else d
+        err[q] = d / sc[q] if sc[q] > 0 else (0.0 if d == 0 else np.inf)     # R19: exact zeros stay exact zeros
     return err
 
 
-def run_pair(ag, wl, n_steps, check_each=True, **over):
+def run_pair(ag, wl, n_steps, check_each=True, gpu_kw=None, **over):
     """Advance the oracle and the GPU side by side; returns (err after step 1, err after n_steps, worst dt err)."""
     ref = oracle.RefSolver.from_workload(wl, **over)
-    gpu = ag.Agate.from_workload(wl, **over)
+    gpu = ag.Agate.from_workload(wl, **over, **(gpu_kw or {}))      # gpu_kw: launch tuning (stage_grid)
     worst_dt, e1 = 0.0, None
     for s in range(n_steps):
         dtr = ref.compute_dt()
@@ -118,46 +118,23 @@ def test_config1_full(ag):
 
 
 @pytest.mark.parametrize("n,steps,grid", [(100, 12, 0), (256, 4, 0), (100, 4, 1), (100, 4, 5), (100, 4, 40)])
-def test_config2_reduced(ag, n, steps, grid, monkeypatch):
+def test_config2_reduced(ag, n, steps, grid):
     """Config 2 recipe (2D HLLD, beta=1.3, shear layer) through the strip kernel.  n=100: 3 full 30-column strips + a
     ragged one of 10.  `grid` CTAs of 6 warps share the (strip, row) pairs evenly: 1 = 16-17 rows per warp, segments
     that cross from one strip into the next; 5 / 40 = ever shorter segments (40: one or two rows each, every row
     through the segment prologue and the closing step); 0 = the library's own choice."""
-    if grid:
-        monkeypatch.setenv("AGATE_GRID", str(grid))
     wl = make_workload(2, n=n)
-    assert_parity(*run_pair(ag, wl, steps))
-
-
-@pytest.mark.parametrize("cfg", [2, 4])
-def test_config2_4_reduced_pooled_kernel(ag, cfg, monkeypatch):
-    """The pooled kernel of agate_kernels.cuh (1-D grids; 2-D kept for A/B measurements) on the 2-D recipes."""
-    monkeypatch.setenv("AGATE_STAGE_V1", "1")
-    wl = make_workload(cfg, n=100)
-    assert_parity(*run_pair(ag, wl, 4))
+    assert_parity(*run_pair(ag, wl, steps, gpu_kw=dict(stage_grid=grid)))
 
 
 @pytest.mark.parametrize("n,grid", [(40, 0), (40, 1), (40, 7), (40, 37), (40, 160), (72, 0)])
-def test_config3_reduced(ag, n, grid, monkeypatch):
+def test_config3_reduced(ag, n, grid):
     """Config 3 recipe (3D HLLD) through the row-owner kernel.  n=40: ragged in x (32+8) and y (3*11+7).  The work
     (tile-planes) is split evenly over `grid` CTAs: 1 = every tile a whole segment of one CTA, 7 / 37 = segments that
     start and end in the middle of a tile column, 160 = one or two planes per segment (every plane through the segment
     prologue and the closing step), 0 = the library's own choice."""
-    if grid:
-        monkeypatch.setenv("AGATE_GRID", str(grid))
     wl = make_workload(3, n=n)
-    assert_parity(*run_pair(ag, wl, 5 if n == 40 else 2))
-
-
-@pytest.mark.parametrize("lz", [0, 16])
-def test_config3_reduced_pooled_kernel(ag, lz, monkeypatch):
-    """Same recipe through the pooled 3-D kernel of agate_kernels.cuh (kept for A/B measurements); lz=16 forces three
-    z-chunks per column."""
-    monkeypatch.setenv("AGATE_STAGE_V1", "1")
-    if lz:
-        monkeypatch.setenv("AGATE_LZ", str(lz))
-    wl = make_workload(3, n=40)
-    assert_parity(*run_pair(ag, wl, 3))
+    assert_parity(*run_pair(ag, wl, 5 if n == 40 else 2, gpu_kw=dict(stage_grid=grid)))
 
 
 @pytest.mark.parametrize("n", [64, 100])
@@ -410,7 +387,7 @@ def test_open_boundaries_3d(ag):
 
 # ---- seeded sweep over shapes, options and work splits ----------------------------------------------------------
 @pytest.mark.parametrize("seed", range(24))
-def test_random_shapes_and_options(ag, seed, monkeypatch):
+def test_random_shapes_and_options(ag, seed):
     """Ragged sizes around the tile / strip / segment boundaries (nx around 30, 32, 60, 64; ny around 11, 22; small nz),
     every solver option, periodic and open ends, default and forced work splits -- 3 steps against the oracle."""
     rng = np.random.default_rng(9000 + seed)
@@ -421,15 +398,17 @@ def test_random_shapes_and_options(ag, seed, monkeypatch):
     hall = ndim == 2 and rng.random() < 0.25
     riemann = HLL if hall else int(rng.choice([HLL, HLLD]))
     limiter, beta = [(0, 1.0), (1, 1.0), (2, 1.0), (2, 1.3), (2, 2.0)][int(rng.integers(5))]
-    rk = int(rng.choice([1, 2, 3]))
-    bc = tuple(int(b) for b in rng.integers(0, 2, 3))
-    if rng.random() < 0.5:
-        monkeypatch.setenv("AGATE_GRID", str(int(rng.choice([1, 3, 17, 80]))))
+    rk = int(rng.choice([1, 2, 3, 4, 5]))
+    bc = [int(b) for b in rng.integers(0, 2, 3)]
+    if bc[0] == 0 and rng.random() < 0.4:
+        bc[1] = 2                               # sheared zero-gradient ends in y (R28)
+    bc = tuple(bc)
+    sg = int(rng.choice([1, 3, 17, 80])) if rng.random() < 0.5 else 0
     import workloads
     W, U = workloads.random_state(100 + seed, (nx, ny, nz), ndim, amp=0.3)
     kw = dict(shape=(nx, ny, nz), dx=(1.0 / nx, 1.3 / ny, 0.7 / nz if ndim == 3 else 1.0), ndim=ndim, riemann=riemann,
               limiter=limiter, beta=beta, rk=rk, bc=bc, eqset=(ag.HALL if hall else ag.IDEAL), d_i=(0.02 if hall else 0.0))
-    ref = oracle.RefSolver(**kw); gpu = ag.Agate(**kw)
+    ref = oracle.RefSolver(**kw); gpu = ag.Agate(stage_grid=sg, **kw)
     ref.set_state(U); gpu.set_state(U)
     for s in range(3):
         dtr, dtg = ref.compute_dt(), gpu.compute_dt()
