@@ -48,6 +48,18 @@ BYTES_PER_ZONE_STEP = 320.0            # 5 x 8 variables x 8 B; 
 # launches of one step) from the committed `ncu` capture of the same command: profiles/r1_stage3d.md
 NCU_TRAFFIC_BYTES = {5: 0.5 * (9532646144 + 8676093184 + 20187381504 + 8776886784),
                      2: 0.5 * (285508864 + 226625280 + 561331200 + 226205952)}
+# ... and the kernels they were captured on: sha256 over csrc/*.cu* at capture time.  When the kernels have changed
+# since, the figure is stale and the line reports "traffic": null instead (profiles/ names the capture).
+NCU_TRAFFIC_CSRC_SHA = "unset"
+
+
+def csrc_sha():
+    import glob
+    import hashlib
+    h = hashlib.sha256()
+    for f in sorted(glob.glob(os.path.join(ROOT, "paper_2503_20899_b200", "csrc", "*.cu*"))):
+        h.update(open(f, "rb").read())
+    return h.hexdigest()[:16]
 FP64_NOMINAL_TFLOPS = 148 * 64 * 2 * 1.965e9 / 1e12     # 148 SMs x 64 DFMA lanes x 2 x max SM clock = 37.2
 
 # reduced size of the bounded CPU sample per config (same recipe and seed), and its step count
@@ -67,6 +79,10 @@ def parse():
                          "device wall time beside the paper's A100 figure")
     ap.add_argument("--n", type=int, default=0, help="override the per-dimension resolution (debugging)")
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--decomp", action="store_true",
+                    help="NEXT-4: slab domain decomposition along the last active dimension instead of replicas: every "
+                         "rank holds one full-size slab of a domain N times as long (weak scaling), halo exchange per "
+                         "stage, one all-reduce(max) per step; at N = 1 the slab is its own periodic neighbour")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu", action="store_true")
     return ap.parse_args()
@@ -135,7 +151,17 @@ class ClockSampler:
                 "samples": len(sm)}
 
 
-def cpu_oracle_rate(config, steps=None, warmup=0):
+def cpu_model():
+    try:
+        for line in open("/proc/cpuinfo"):
+            if line.startswith("model name"):
+                return line.split(":", 1)[1].strip()
+    except Exception:
+        pass
+    return "unknown"
+
+
+def cpu_oracle_rate(config, steps=None, warmup=0, all_cores=False):
     """The oracle as it stands (single-threaded build default) on a bounded sample; returns dict for the JSON."""
     import oracle
     from workloads import make_workload
@@ -149,10 +175,27 @@ def cpu_oracle_rate(config, steps=None, warmup=0):
     t0 = time.perf_counter()
     ref.advance(nst)
     dt = time.perf_counter() - t0
+    cores1 = oracle.get_threads()
+    allc = None
+    if all_cores and (os.cpu_count() or 1) > 1:
+        # the same loops under OpenMP on every host core (bitwise identical results, tests/test_oracle_pins.py)
+        oracle.set_threads(os.cpu_count())
+        try:
+            ref.set_state(wl.U)
+            ref.advance(1)
+            t0 = time.perf_counter()
+            ref.advance(nst)
+            dta = time.perf_counter() - t0
+            allc = {"value": wl.zones * nst / dta, "unit": UNIT, "cores": oracle.get_threads(), "cpu": cpu_model()}
+        finally:
+            oracle.set_threads(1)
     ref.close()
-    return {"value": wl.zones * nst / dt, "unit": UNIT, "cores": oracle.get_threads(), "kind": "oracle",
-            "sample": f"config {config} recipe at {wl.shape[0]}^{wl.ndim}, {nst} full steps, "
-                      f"{os.cpu_count()} host cores present"}, dt / nst, wl
+    out = {"value": wl.zones * nst / dt, "unit": UNIT, "cores": cores1, "kind": "oracle",
+           "sample": f"config {config} recipe at {wl.shape[0]}^{wl.ndim}, {nst} full steps, "
+                     f"{os.cpu_count()} host cores present"}
+    if allc is not None:
+        out["all_cores"] = allc
+    return out, dt / nst, wl
 
 
 def run_reference(args):
@@ -213,6 +256,8 @@ def run_ours(args):
     zones = wl.zones
     wl.W = None                                       # only U is needed; frees one state-sized host array
     K, Wm = args.steps, args.warmup
+    if args.decomp:
+        return run_decomp(args, ag, wl, world, rank, local, dev, barrier)
     sim = ag.Agate.from_workload(wl, device=dev, set_state=False)
     Uh = torch.from_numpy(wl.U).pin_memory()
     info = sim.launch_info()
@@ -247,7 +292,9 @@ def run_ours(args):
     bytes_step = BYTES_PER_ZONE_STEP * (9.0 / 8.0 if cfg >= 6 else 1.0)
     hbm_frac = (bytes_step / 5.0 * 2.5 * zones / (stage_ms * 1e-3) / 1e9) / peaks["hbm_gbs"]
     roofline = {"bound": "alu", "achieved": achieved, "peak": fp64_peak, "unit": "TFLOP/s",
-                "frac": achieved / fp64_peak, "traffic": NCU_TRAFFIC_BYTES.get(cfg) if not args.n else None,
+                "frac": achieved / fp64_peak, "traffic": (NCU_TRAFFIC_BYTES.get(cfg) if (not args.n and csrc_sha() == NCU_TRAFFIC_CSRC_SHA) else None),
+                "traffic_source": f"ncu --set full capture of kernels with csrc sha {NCU_TRAFFIC_CSRC_SHA} (profiles/); "
+                                  f"this run's csrc sha {csrc_sha()}",
                 "algorithmic_bytes": bytes_step / 2.0 * zones,
                 "kernel": {3: "stage3d_kernel", 2: "stage2d_kernel"}.get(wl.ndim, "stage_kernel"), "ms_per_launch": stage_ms, "launches_timed": st_n,
                 "stage_share_of_step": 2.0 * stage_ms * K / ms_max if st_n else None,
@@ -313,7 +360,63 @@ def run_ours(args):
         if table2 is not None:
             line["paper_table2_run"] = table2
         if not args.no_cpu and world >= 1:
-            line["cpu_baseline"] = cpu_oracle_rate(cfg)[0]
+            line["cpu_baseline"] = cpu_oracle_rate(cfg, all_cores=True)[0]
+        print(json.dumps(line))
+    sim.close()
+    if world > 1:
+        dist.barrier()
+        dist.destroy_process_group()
+
+
+def run_decomp(args, ag, wl, world, rank, local, dev, barrier):
+    """NEXT-4 arm: one slab per rank (weak scaling: the domain is N slabs long in its last active dimension, every
+    slab carries the config's seeded state, which is periodic, so the stacked state is smooth across the cut faces).
+    Per step: one all-reduce(max) of the device-resident v_max; per stage: ghost fill, pack, halo exchange (NCCL
+    send/recv between neighbours; two device copies when N = 1), unpack, stage kernel."""
+    import torch
+    import torch.distributed as dist
+    from paper_2503_20899_b200 import slab
+    if wl.ndim < 2:
+        raise SystemExit("--decomp needs a 2-D or 3-D config")
+    K, Wm, zones, cfg = args.steps, args.warmup, wl.zones, args.config
+    sim = ag.Agate.from_workload(wl, device=dev, set_state=False)
+    Uh = torch.from_numpy(wl.U).pin_memory()
+    st = slab.SlabStepper(sim, rank, world, True)
+    info = sim.launch_info()
+    sim.set_state(Uh); st.reset()
+    for _ in range(Wm):
+        st.step()
+    sim.set_state(Uh); st.reset()
+    st.step()                                          # the first step takes v_max through the host; time the steady state
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    barrier()
+    with ClockSampler(local) as clk:
+        e0.record(sim.stream)
+        for _ in range(K):
+            st.step()
+        e1.record(sim.stream)
+        barrier()
+    ms = e0.elapsed_time(e1)
+    sim.poll()
+    ms_max = max_over_ranks(ms, world, dev)
+    value = aggregate_rate(zones, world, K, ms_max)
+    halo = sim.halo_bytes()
+    if rank == 0:
+        rk = int(sim.cfg.rk)
+        line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": Wm,
+                "ms_per_step": ms_max / K, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+                "dtype": "f64", "data": "synthetic",
+                "config": {"workload": f"BASELINE.json config {cfg} recipe as one slab per GPU: {wl.name}",
+                           "zones_per_gpu": zones,
+                           "parallelism": f"slab decomposition along {'z' if wl.ndim == 3 else 'y'} over {world} rank(s): "
+                                          "halo exchange per stage (2 layers x all variables per cut face, "
+                                          + ("NCCL send/recv" if world > 1 else "device copies: the slab is its own neighbour")
+                                          + "), one all-reduce(max) of v_max per step",
+                           "halo_bytes_per_face_per_stage": halo, "launch": info},
+                "clocks": clk.summary(), "gpu_launches": (1 + 2 * rk) * K,
+                "roofline": None, "e2e": None,
+                "note": "NEXT-4 arm; the headline line is the default (replicas) arm.  No scaling curve exists until "
+                        "this runs on a multi-GPU node."}
         print(json.dumps(line))
     sim.close()
     if world > 1:

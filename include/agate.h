@@ -141,6 +141,38 @@ typedef struct {
 } agate_tuning;
 int agate_set_tuning(agate_ctx*, const agate_tuning*);
 
+/* ---- NEXT-4: slab decomposition of the grid along its last active dimension ----------------------
+ * A rank holds an ordinary context over its slab (grid.nz = planes of the slab on a 3-D grid, grid.ny = rows on a 2-D
+ * one) and steps it stage by stage, exchanging the two ghost layers of each cut face with its neighbours in between:
+ *
+ *   v = agate_get_vmax;  v = max over ranks;  agate_set_vmax(v)          (A7: one allreduce(max) of one double per step)
+ *   agate_step_begin(ctx, 0)                                             dt = C dx_min / v,  t += dt,  GLM: c_h = 0.95 v
+ *   for stage = 0 .. rk-1:
+ *     agate_stage_pre(ctx, stage, send_lo, send_hi)    A0 on the ends that are not cut, then the two interior layers
+ *                                                       next to each cut face -> the caller's DEVICE buffers
+ *     (send_hi -> the upper neighbour's recv_lo,  send_lo -> the lower neighbour's recv_hi: NCCL send/recv, peer
+ *      copies, or plain device copies between two contexts of one GPU)
+ *     agate_stage_post(ctx, stage, recv_lo, recv_hi)   the neighbours' layers -> this slab's ghost layers, then the
+ *                                                       stage kernel (A1-A6); after the last stage the step is complete
+ *
+ * Every zone's new value depends on the ghost-padded stage input only, so the slabs reproduce the undivided run bit
+ * for bit.  A halo buffer holds [nv][2][padded plane] doubles (agate_halo_bytes; whole padded planes, so edges and
+ * corners travel with them: the Hall current needs them).  All calls enqueue on the context's stream and, except
+ * agate_get_vmax, do not synchronise; the buffers must stay untouched until the enqueued copies have run.
+ * agate_step / agate_advance return AGATE_ERR_STATE on a context with a cut face.  Call order errors (a stage out of
+ * turn, a step begun twice) return AGATE_ERR_STATE. */
+int agate_set_slab(agate_ctx*, int cut_lo, int cut_hi);        /* which ends of the last active dimension are cut faces */
+size_t agate_halo_bytes(const agate_ctx*);                     /* bytes of ONE halo buffer (0: 1-D grid)               */
+int agate_get_vmax(agate_ctx*, double* vmax_out);              /* max_cells(|v| + c) of this slab (HOST); synchronises */
+int agate_set_vmax(agate_ctx*, double vmax);                   /* the maximum over all slabs, for the next step_begin  */
+int agate_vmax_device(agate_ctx*, void** ptr_out);             /* DEVICE address of that maximum (8 bytes, a positive
+                                                                  double): an in-place ncclAllReduce(max) on it replaces
+                                                                  the get / set pair without a host round trip.  Only on
+                                                                  2-D / 3-D grids with the fused reduction (not CGL).    */
+int agate_step_begin(agate_ctx*, double dt);                   /* dt > 0: use it;  dt <= 0: from the device v_max       */
+int agate_stage_pre(agate_ctx*, int stage, void* send_lo, void* send_hi);
+int agate_stage_post(agate_ctx*, int stage, const void* recv_lo, const void* recv_hi);
+
 int agate_destroy(agate_ctx*);
 const char* agate_strerror(int status);
 

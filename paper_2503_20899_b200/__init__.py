@@ -30,7 +30,9 @@ OK, ERR_ARG, ERR_STATE, ERR_UNPHYSICAL, ERR_CUDA, ERR_NOMEM = range(6)
 # every symbol include/agate.h declares (tests check that the library exports each of them)
 SYMBOLS = ("agate_workspace_bytes", "agate_init", "agate_set_state", "agate_compute_dt", "agate_step",
            "agate_advance", "agate_get_state", "agate_poll", "agate_launch_info", "agate_set_timing",
-           "agate_stage_time", "agate_set_tuning", "agate_destroy", "agate_strerror", "agate_test_face_flux",
+           "agate_stage_time", "agate_set_tuning", "agate_set_slab", "agate_halo_bytes", "agate_get_vmax",
+           "agate_set_vmax", "agate_vmax_device", "agate_step_begin", "agate_stage_pre", "agate_stage_post",
+           "agate_destroy", "agate_strerror", "agate_test_face_flux",
            "agate_measure_fp64_peak")
 
 
@@ -84,6 +86,15 @@ def lib():
         L.agate_set_timing.argtypes = [_vp, C.c_int]
         L.agate_stage_time.argtypes = [_vp, _dp, C.POINTER(C.c_int64), C.c_int]
         L.agate_set_tuning.argtypes = [_vp, C.POINTER(Tuning)]
+        L.agate_set_slab.argtypes = [_vp, C.c_int, C.c_int]
+        L.agate_halo_bytes.argtypes = [_vp]
+        L.agate_halo_bytes.restype = C.c_size_t
+        L.agate_get_vmax.argtypes = [_vp, _dp]
+        L.agate_set_vmax.argtypes = [_vp, C.c_double]
+        L.agate_vmax_device.argtypes = [_vp, C.POINTER(_vp)]
+        L.agate_step_begin.argtypes = [_vp, C.c_double]
+        L.agate_stage_pre.argtypes = [_vp, C.c_int, _vp, _vp]
+        L.agate_stage_post.argtypes = [_vp, C.c_int, _vp, _vp]
         L.agate_destroy.argtypes = [_vp]
         L.agate_strerror.argtypes = [C.c_int]
         L.agate_strerror.restype = C.c_char_p
@@ -204,6 +215,47 @@ class Agate:
 
     def poll(self):
         self._chk(lib().agate_poll(self._h), "agate_poll")
+
+    # -- NEXT-4: slab decomposition (include/agate.h) ---------------------------------------------------------
+    def set_slab(self, cut_lo, cut_hi):
+        self._chk(lib().agate_set_slab(self._h, int(bool(cut_lo)), int(bool(cut_hi))), "agate_set_slab")
+        self.rk = int(self.cfg.rk)
+
+    def halo_bytes(self):
+        return int(lib().agate_halo_bytes(self._h))
+
+    def halo_buffers(self):
+        """Four device buffers (send_lo, send_hi, recv_lo, recv_hi) of halo_bytes() each, as float64 tensors."""
+        torch = _torch_cuda()
+        n = self.halo_bytes() // 8
+        return tuple(torch.zeros(n, dtype=torch.float64, device=self.device) for _ in range(4))
+
+    def get_vmax(self):
+        v = C.c_double()
+        self._chk(lib().agate_get_vmax(self._h, C.byref(v)), "agate_get_vmax")
+        return v.value
+
+    def set_vmax(self, v):
+        self._chk(lib().agate_set_vmax(self._h, float(v)), "agate_set_vmax")
+
+    def vmax_tensor(self):
+        """The device-resident v_max as a one-element float64 view of the workspace (for an in-place all-reduce)."""
+        torch = _torch_cuda()
+        p = _vp()
+        self._chk(lib().agate_vmax_device(self._h, C.byref(p)), "agate_vmax_device")
+        off = p.value - self.workspace.data_ptr()
+        return self.workspace[off:off + 8].view(torch.float64)
+
+    def step_begin(self, dt=0.0):
+        self._chk(lib().agate_step_begin(self._h, float(dt)), "agate_step_begin")
+
+    def stage_pre(self, stage, send_lo=None, send_hi=None):
+        p = lambda t: _vp(t.data_ptr()) if t is not None else None
+        self._chk(lib().agate_stage_pre(self._h, int(stage), p(send_lo), p(send_hi)), "agate_stage_pre")
+
+    def stage_post(self, stage, recv_lo=None, recv_hi=None):
+        p = lambda t: _vp(t.data_ptr()) if t is not None else None
+        self._chk(lib().agate_stage_post(self._h, int(stage), p(recv_lo), p(recv_hi)), "agate_stage_post")
 
     # -- bookkeeping ---------------------------------------------------------------------------------------
     def launch_info(self):

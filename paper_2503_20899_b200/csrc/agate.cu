@@ -194,6 +194,10 @@ struct agate_ctx {
   cudaGraphExec_t graph = nullptr;
   bool timing = false;
   bool no_graph = false;           // agate_set_tuning: launch the kernels directly
+  bool ext_lo = false, ext_hi = false;   // NEXT-4: cut faces of a slab decomposition (last active dimension)
+  bool vmax_given = false;         // agate_set_vmax: the device v_max is the caller's global maximum
+  int next_stage = -1;             // split-phase stepping: stage expected next (-1: no step open)
+  bool pre_done = false;           // ... and whether its agate_stage_pre has run
   std::vector<cudaEvent_t> ev;     // pairs (start, stop) of timed stage launches
   size_t ev_used = 0;
   double stage_ms = 0.0;
@@ -224,6 +228,9 @@ GhostParams make_ghost(const agate_ctx* c, double* U) {
   p.nzs = (long long)2 * L.ghz * L.nyp * L.nxp;
   p.nys = (long long)c->g.nz * 2 * L.ghy * L.nxp;
   p.nxs = (long long)c->g.nz * c->g.ny * 4;
+  p.dcut = (c->g.ndim == 3) ? 2 : 1;
+  p.skip_lo = c->ext_lo ? 1 : 0;
+  p.skip_hi = c->ext_hi ? 1 : 0;
   return p;
 }
 
@@ -330,22 +337,42 @@ int rk_table(int rk, RkStage st[5], bool* swap_ab) {
   }
 }
 
-int enqueue_stages(agate_ctx* c) {
+// First half of stage i: ghost fill of the stage input (A0).  Second half: the stage kernel (A1-A6), and after the
+// last stage the buffer rotation.  The slab decomposition (NEXT-4) puts its halo exchange between the two.
+int stage_pre(agate_ctx* c, int i) {
+  RkStage st[5];
+  bool swap_ab;
+  rk_table(c->s.rk, st, &swap_ab);
+  const GhostParams* gp[3] = {&c->gpA, &c->gpB, &c->gpC};
+  return launch_ghost(c, *gp[st[i].in]);
+}
+int stage_post(agate_ctx* c, int i) {
   RkStage st[5];
   bool swap_ab;
   const int ns = rk_table(c->s.rk, st, &swap_ab);
   double* U[3] = {c->UA, c->UB, c->UC};
-  const GhostParams* gp[3] = {&c->gpA, &c->gpB, &c->gpC};
-  int rc;
-  for (int i = 0; i < ns; ++i) {
-    if ((rc = launch_ghost(c, *gp[st[i].in]))) return rc;
-    const double* ref = (st[i].ref >= 0) ? U[st[i].ref] : nullptr;
-    if ((rc = launch_stage(c, make_stage_params(c, U[st[i].in], ref, U[st[i].out], st[i].a0, st[i].a1, st[i].c, i == ns - 1))))
-      return rc;
-  }
-  if (swap_ab) {
+  const double* ref = (st[i].ref >= 0) ? U[st[i].ref] : nullptr;
+  int rc = launch_stage(c, make_stage_params(c, U[st[i].in], ref, U[st[i].out], st[i].a0, st[i].a1, st[i].c, i == ns - 1));
+  if (rc) return rc;
+  if (i == ns - 1 && swap_ab) {
     std::swap(c->UA, c->UB);
     std::swap(c->gpA, c->gpB);
+  }
+  return AGATE_OK;
+}
+double* stage_input(agate_ctx* c, int i) {
+  RkStage st[5];
+  bool swap_ab;
+  rk_table(c->s.rk, st, &swap_ab);
+  double* U[3] = {c->UA, c->UB, c->UC};
+  return U[st[i].in];
+}
+
+int enqueue_stages(agate_ctx* c) {
+  int rc;
+  for (int i = 0; i < c->s.rk; ++i) {
+    if ((rc = stage_pre(c, i))) return rc;
+    if ((rc = stage_post(c, i))) return rc;
   }
   return AGATE_OK;
 }
@@ -506,6 +533,9 @@ int agate_set_state(agate_ctx* c, const double* U, int src_is_device, double t0)
   if ((rc = launch_ghost(c, c->gpA))) return rc;
   c->have_state = true;
   c->vmax_valid = false;
+  c->vmax_given = false;
+  c->next_stage = -1;
+  c->pre_done = false;
   if (c->sticky == AGATE_ERR_UNPHYSICAL) c->sticky = AGATE_OK;
   return AGATE_OK;
 }
@@ -525,7 +555,7 @@ int agate_compute_dt(agate_ctx* c, double* dt_out) {
 
 int agate_step(agate_ctx* c, double dt, double* dt_used) {
   if (!c) return AGATE_ERR_ARG;
-  if (!c->have_state) return AGATE_ERR_STATE;
+  if (!c->have_state || c->ext_lo || c->ext_hi) return AGATE_ERR_STATE;   // a slab steps through agate_stage_pre / _post
   int rc;
   if (dt > 0.0) {
     if (c->eqset == AGATE_IDEAL_GLM && (rc = ensure_vmax(c))) return rc;      // c_h = 0.95 v_max(U^n) whoever chose dt
@@ -548,7 +578,7 @@ int agate_step(agate_ctx* c, double dt, double* dt_used) {
 
 int agate_advance(agate_ctx* c, int32_t n_steps, double* t_out) {
   if (!c || n_steps < 0) return AGATE_ERR_ARG;
-  if (!c->have_state) return AGATE_ERR_STATE;
+  if (!c->have_state || c->ext_lo || c->ext_hi) return AGATE_ERR_STATE;
   int rc;
   // stream capture is not allowed on the legacy default stream
   const bool use_graph = (c->s.rk >= 2 && c->s.rk <= 4) && !c->timing && c->stream != nullptr && !c->no_graph;
@@ -637,6 +667,121 @@ int agate_stage_time(agate_ctx* c, double* ms_out, int64_t* launches_out, int re
   if (ms_out) *ms_out = c->stage_ms;
   if (launches_out) *launches_out = c->stage_launches;
   if (reset) { c->stage_ms = 0.0; c->stage_launches = 0; }
+  return AGATE_OK;
+}
+
+// ---- NEXT-4: slab decomposition along the last active dimension -------------------------------------
+int agate_set_slab(agate_ctx* c, int ext_lo, int ext_hi) {
+  if (!c) return AGATE_ERR_ARG;
+  if (c->g.ndim < 2) return AGATE_ERR_ARG;
+  c->ext_lo = ext_lo != 0; c->ext_hi = ext_hi != 0;
+  c->gpA = make_ghost(c, c->UA); c->gpB = make_ghost(c, c->UB); c->gpC = make_ghost(c, c->UC);
+  if (c->graph) { cudaGraphExecDestroy(c->graph); c->graph = nullptr; }
+  return AGATE_OK;
+}
+
+size_t agate_halo_bytes(const agate_ctx* c) {
+  if (!c || c->g.ndim < 2) return 0;
+  const long long plane = (c->g.ndim == 3) ? c->L.sz : c->L.sy;      // one padded plane (row) incl. its own ghosts
+  return sizeof(double) * (size_t)c->nv * 2 * (size_t)plane;
+}
+
+int agate_get_vmax(agate_ctx* c, double* vmax_out) {
+  if (!c || !vmax_out) return AGATE_ERR_ARG;
+  if (!c->have_state) return AGATE_ERR_STATE;
+  int rc;
+  double v;
+  if (c->sk.fused_dt && c->vmax_valid) {
+    if ((rc = collect_status(c))) return rc;
+    CU_TRY(cudaMemcpy(&v, c->vnext, sizeof(double), cudaMemcpyDeviceToHost));     // bit pattern of a positive double
+  } else {
+    if ((rc = launch_dt(c, 0))) return rc;
+    if ((rc = collect_status(c))) return rc;
+    CU_TRY(cudaMemcpy(&v, c->scal + 1, sizeof(double), cudaMemcpyDeviceToHost));
+  }
+  *vmax_out = v;
+  return AGATE_OK;
+}
+
+int agate_set_vmax(agate_ctx* c, double vmax) {
+  if (!c || !(vmax > 0.0)) return AGATE_ERR_ARG;
+  if (!c->have_state) return AGATE_ERR_STATE;
+  set_vnext_kernel<<<1, 1, 0, c->stream>>>(c->scal, c->vnext, vmax);
+  CU_TRY(cudaGetLastError());
+  c->vmax_given = true;
+  return AGATE_OK;
+}
+
+int agate_vmax_device(agate_ctx* c, void** ptr_out) {
+  if (!c || !ptr_out) return AGATE_ERR_ARG;
+  if (!c->sk.fused_dt) return AGATE_ERR_ARG;      // only the kernels with the fused reduction keep v_max there
+  *ptr_out = c->vnext;
+  return AGATE_OK;
+}
+
+int agate_step_begin(agate_ctx* c, double dt) {
+  if (!c) return AGATE_ERR_ARG;
+  if (!c->have_state || c->next_stage != -1) return AGATE_ERR_STATE;
+  int rc;
+  const bool have_v = c->vmax_given || (c->sk.fused_dt && c->vmax_valid);
+  if (dt > 0.0) {
+    if (c->eqset == AGATE_IDEAL_GLM && !have_v && (rc = ensure_vmax(c))) return rc;
+    set_dt_kernel<<<1, 1, 0, c->stream>>>(c->scal, dt, (c->sk.fused_dt || c->vmax_given) ? c->vnext : nullptr);
+    CU_TRY(cudaGetLastError());
+  } else {
+    if (!have_v) {                                   // local v_max: a slab wants agate_set_vmax with the global one
+      if ((rc = launch_dt(c, 0))) return rc;
+      seed_vnext_kernel<<<1, 1, 0, c->stream>>>(c->scal, c->vnext);
+      CU_TRY(cudaGetLastError());
+    }
+    begin_step_kernel<<<1, 1, 0, c->stream>>>(c->scal, c->vnext, c->cfl * c->dxmin);
+    CU_TRY(cudaGetLastError());
+  }
+  c->vmax_given = false;
+  c->vmax_valid = false;
+  c->next_stage = 0;
+  c->pre_done = false;
+  return AGATE_OK;
+}
+
+int agate_stage_pre(agate_ctx* c, int stage, void* send_lo, void* send_hi) {
+  if (!c || stage < 0 || stage >= c->s.rk) return AGATE_ERR_ARG;
+  if ((c->ext_lo && !send_lo) || (c->ext_hi && !send_hi)) return AGATE_ERR_ARG;
+  if (!c->have_state || c->next_stage != stage || c->pre_done) return AGATE_ERR_STATE;
+  int rc = stage_pre(c, stage);                      // A0 on the ends that are not cut faces
+  if (rc) return rc;
+  // the two interior layers next to each cut face, whole padded planes (their x / y ghosts were just filled), every
+  // variable: [nv][2 planes] contiguous in the caller's buffer
+  const double* U = stage_input(c, stage);
+  const long long plane = (c->g.ndim == 3) ? c->L.sz : c->L.sy;
+  const int gh = 2, n = (c->g.ndim == 3) ? c->g.nz : c->g.ny;
+  const size_t w = sizeof(double) * 2 * (size_t)plane;
+  if (c->ext_lo) CU_TRY(cudaMemcpy2DAsync(send_lo, w, U + (long long)gh * plane, sizeof(double) * (size_t)c->L.sq, w, c->nv,
+                                          cudaMemcpyDeviceToDevice, c->stream));
+  if (c->ext_hi) CU_TRY(cudaMemcpy2DAsync(send_hi, w, U + (long long)n * plane, sizeof(double) * (size_t)c->L.sq, w, c->nv,
+                                          cudaMemcpyDeviceToDevice, c->stream));
+  c->pre_done = true;
+  return AGATE_OK;
+}
+
+int agate_stage_post(agate_ctx* c, int stage, const void* recv_lo, const void* recv_hi) {
+  if (!c || stage < 0 || stage >= c->s.rk) return AGATE_ERR_ARG;
+  if ((c->ext_lo && !recv_lo) || (c->ext_hi && !recv_hi)) return AGATE_ERR_ARG;
+  if (!c->have_state || c->next_stage != stage || !c->pre_done) return AGATE_ERR_STATE;
+  double* U = stage_input(c, stage);
+  const long long plane = (c->g.ndim == 3) ? c->L.sz : c->L.sy;
+  const int gh = 2, n = (c->g.ndim == 3) ? c->g.nz : c->g.ny;
+  const size_t w = sizeof(double) * 2 * (size_t)plane;
+  // the neighbour's layers become this slab's ghost layers: below the low cut face, above the high one
+  if (c->ext_lo) CU_TRY(cudaMemcpy2DAsync(U, sizeof(double) * (size_t)c->L.sq, recv_lo, w, w, c->nv, cudaMemcpyDeviceToDevice,
+                                          c->stream));
+  if (c->ext_hi) CU_TRY(cudaMemcpy2DAsync(U + (long long)(n + gh) * plane, sizeof(double) * (size_t)c->L.sq, recv_hi, w, w, c->nv,
+                                          cudaMemcpyDeviceToDevice, c->stream));
+  int rc = stage_post(c, stage);
+  if (rc) return rc;
+  c->pre_done = false;
+  c->next_stage = (stage == c->s.rk - 1) ? -1 : stage + 1;
+  if (c->next_stage == -1) c->vmax_valid = c->sk.fused_dt;
   return AGATE_OK;
 }
 

@@ -335,6 +335,8 @@ struct GhostParams {
   int nx, ny, nz, ghy, ghz, nxp, nyp, nzp;
   long long sy, sz, sq;
   long long nzs, nys, nxs;   // cells in the z-, y-, x-slabs
+  int dcut, skip_lo, skip_hi; // NEXT-4: ends of dimension dcut that are cut faces of a slab decomposition: their ghost
+                              // layers come from the neighbouring slab (agate_stage_post), not from this kernel
 };
 
 __global__ void __launch_bounds__(256) ghost_fill_kernel(const __grid_constant__ GhostParams P) {
@@ -368,6 +370,10 @@ __global__ void __launch_bounds__(256) ghost_fill_kernel(const __grid_constant__
       ip = (s < 2) ? s : P.nxp - 4 + s;
     }
     int i = ip - 2, j = jp - P.ghy, k = kp - P.ghz;
+    {
+      const int c = (P.dcut == 2) ? k : j, nc = (P.dcut == 2) ? P.nz : P.ny;
+      if ((P.skip_lo && c < 0) || (P.skip_hi && c >= nc)) continue;
+    }
     if (P.bcx) i = min(max(i, 0), P.nx - 1); else { i %= P.nx; if (i < 0) i += P.nx; }
     if (P.bcy == 2 && (j < 0 || j >= P.ny)) {
       // sheared zero-gradient ends in y (R28): ghost (i, j) = zone (i-1, j+2) at the down side, (i+1, j-2) at
@@ -499,6 +505,12 @@ __global__ void begin_step_kernel(double* scal, unsigned long long* vnext, doubl
 __global__ void reset_scalars_kernel(double* scal, int* flag, double t0) {
   scal[0] = 0.0; scal[1] = 0.0; scal[2] = t0;
   *flag = 0;
+}
+
+// agate_set_vmax: the caller's (global) v_max for the next step head
+__global__ void set_vnext_kernel(double* scal, unsigned long long* vnext, double v) {
+  scal[1] = v;
+  *vnext = (unsigned long long)__double_as_longlong(v);
 }
 
 // after a stand-alone dt_kernel: hand its v_max to the fused path

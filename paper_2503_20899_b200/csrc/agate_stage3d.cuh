@@ -67,14 +67,14 @@ __device__ __forceinline__ void prefetch_l2(const void* p) { asm volatile("prefe
 // rotated slot -> fixed variable; the GLM scalar (slot 8) is not rotated
 __host__ __device__ __forceinline__ int rv(int r, int n) { return (r < 8) ? rot_var(r, n) : r; }
 
-template <int TY, int NV = 8>
+template <int TY, int NV = 8, int NHB = 2>
 struct Stage3dSmem {
   static_assert(TY >= 2 && TY <= 16, "the x-edge task packs two cells per row into one warp");
   static constexpr int NW = TY + 1;                 // warps: TY owners + H
   static constexpr int NT = 32 * NW;
   static constexpr int PL = TY * RS;                // one ring plane of one variable
   static constexpr int SB = 4 * RS;                 // one y-halo buffer of one variable (rows -2,-1,TY,TY+1)
-  static constexpr int QS = 3 * PL + 2 * SB;        // per-variable stride of W
+  static constexpr int QS = 3 * PL + NHB * SB;      // per-variable stride of W (NHB y-halo buffers: 3 with Hall)
   static constexpr int YS = (TY + 1) * 32;          // y hand-over rows 0..TY (right state of row r, then flux of face r-1/2)
   static constexpr int ZS = TY * 32;                // per-thread slots: z carry, accumulator
   static constexpr int XS = TY;                     // x hand-over, one entry per row
@@ -88,15 +88,41 @@ struct Stage3dSmem {
   static constexpr size_t BYTES = sizeof(double) * (size_t)TOTAL;
 };
 
+// A8 (R15): rotated face current (J_n, J_t1, J_t2), J = curl B, at the face between cells C and D = C + e_n from
+// the cell-centred B of the stage input: central difference across the face along n; along a transverse direction
+// the mean of the two cells' central differences.  o* are offsets into one variable's shared array (stride QS per
+// variable): C, D, and their neighbours at +-1 along t1 = n+1 and t2 = n+2 (cyclic).  q1 = 1/(4 h_t1), q2 = 1/(4 h_t2).
+template <int N>
+__device__ __forceinline__ void hall_current(const double* W, int QS, int oC, int oD, int oCp1, int oCm1, int oDp1,
+                                             int oDm1, int oCp2, int oCm2, int oDp2, int oDm2, double idn, double q1,
+                                             double q2, double Jr[3]) {
+  constexpr int a1 = (N + 1) % 3, a2 = (N + 2) % 3;
+  const double* Bn = W + (5 + N) * QS;
+  const double* B1 = W + (5 + a1) * QS;
+  const double* B2 = W + (5 + a2) * QS;
+  const double dnB1 = (B1[oD] - B1[oC]) * idn, dnB2 = (B2[oD] - B2[oC]) * idn;
+  const double d1Bn = ((Bn[oCp1] - Bn[oCm1]) + (Bn[oDp1] - Bn[oDm1])) * q1;
+  const double d1B2 = ((B2[oCp1] - B2[oCm1]) + (B2[oDp1] - B2[oDm1])) * q1;
+  const double d2Bn = ((Bn[oCp2] - Bn[oCm2]) + (Bn[oDp2] - Bn[oDm2])) * q2;
+  const double d2B1 = ((B1[oCp2] - B1[oCm2]) + (B1[oDp2] - B1[oDm2])) * q2;
+  Jr[0] = d1B2 - d2B1;
+  Jr[1] = d2Bn - dnB2;
+  Jr[2] = dnB1 - d1Bn;
+}
+
 // LIM >= 0 fixes the limiter at compile time (no branch per slope, one basic block for all eight variables);
 // LIM < 0 reads it from the parameters.
 // GLM = true: nine variables per cell, the scalar psi (index 8) behind the MHD ones (NEXT-1; eqs.10-11; R22).
 // CGL = true: CGL MHD (NEXT-2; R24): nine variables, W = (rho, v, p_par, B, p_perp), HLL only.
-template <int TY, int RIEMANN, int LIM, int MINB, bool GLM = false, bool CGL = false>
+// HALL = true: Hall MHD (A8; R15): HLL with the Hall velocity in the induction and energy fluxes and
+// max(c_f, c_w) in the Davis speeds; the face current needs B one zone around every face, so the y-halo rows keep
+// three planes, carry their x-halo corners, and a few more hand-overs guard the planes k-1 and k+1.
+template <int TY, int RIEMANN, int LIM, int MINB, bool GLM = false, bool CGL = false, bool HALL = false>
 __global__ void __launch_bounds__(32 * (TY + 1), MINB) stage3d_kernel(const __grid_constant__ StageParams P) {
-  static_assert(!(CGL && (GLM || RIEMANN != 0)), "combination not built");
+  static_assert(!(CGL && (GLM || RIEMANN != 0)) && !(HALL && (GLM || CGL || RIEMANN != 0)), "combination not built");
   constexpr int NV = (GLM || CGL) ? 9 : 8;
-  using SM = Stage3dSmem<TY, NV>;
+  constexpr int NHB = HALL ? 3 : 2;
+  using SM = Stage3dSmem<TY, NV, NHB>;
   constexpr int NT = SM::NT, PL = SM::PL, SB = SM::SB, QS = SM::QS, YS = SM::YS, ZS = SM::ZS, XS = SM::XS;
   extern __shared__ __align__(16) double smem[];
   double* const W = smem;                    // [8][QS]  primitives: ring planes + two y-halo buffers
@@ -168,14 +194,15 @@ __global__ void __launch_bounds__(32 * (TY + 1), MINB) stage3d_kernel(const __gr
       for (int q = 0; q < 9; ++q) u[q] = W[q * QS + off];
       cgl_cons_to_prim(u, w);
 #pragma unroll
-      for (int q = 0; q < 9; ++q) W[q * QS + off] = w[q];
+      for (int q = 0; q < 9; ++q)
+        if (q < 5 || q > 7) W[q * QS + off] = w[q];       // B is its own primitive: the copied value stays
     } else {
       double u[8], w[8];                     // the GLM scalar (index 8) is its own primitive
 #pragma unroll
       for (int q = 0; q < 8; ++q) u[q] = W[q * QS + off];
       cons_to_prim(P.ph, u, w);
 #pragma unroll
-      for (int q = 0; q < 8; ++q) W[q * QS + off] = w[q];
+      for (int q = 0; q < 5; ++q) W[q * QS + off] = w[q];       // B is its own primitive: the copied value stays
     }
   };
   auto copy_cell = [&](int off, long long g) {
@@ -186,7 +213,9 @@ __global__ void __launch_bounds__(32 * (TY + 1), MINB) stage3d_kernel(const __gr
   // H's halo cells of plane p.  The four y-halo rows: one pass per row, lane = column of the tile (the row's own
   // x-halo corners are never read).  The x-halo columns of the ring rows: four cells per row, ceil(4 TY / 32) passes.
   // Fully unrolled with closed-form offsets: this work sits on H's critical path in phase B.
-  constexpr int NHC = (4 * TY + 31) / 32;
+  // Hall: also the x-halo corners (columns -1 and 32) of the four y-halo rows, for the transverse differences of J
+  constexpr int NHC = (4 * TY + (HALL ? 8 : 0) + 31) / 32;
+  auto hbuf_of = [](int p) { return 3 * PL + ((p + NHB) % NHB) * SB; };       // y-halo rows of plane p >= -2
   auto h_cells = [&](int p, int slot, auto&& fn) {
     const long long gp = (long long)(p + 2) * P.sz + x0;
     const bool xin = x0 + lane + 2 < P.nxp;
@@ -194,13 +223,18 @@ __global__ void __launch_bounds__(32 * (TY + 1), MINB) stage3d_kernel(const __gr
     for (int r = 0; r < 4; ++r) {
       const int j = (r < 2) ? r - 2 : TY + r - 2;
       if (xin && y0 + j + 2 < P.nyp)
-        fn(3 * PL + (p & 1) * SB + r * RS + lane + 2, gp + (long long)(y0 + j + 2) * P.sy + lane + 2);
+        fn(hbuf_of(p) + r * RS + lane + 2, gp + (long long)(y0 + j + 2) * P.sy + lane + 2);
     }
 #pragma unroll
     for (int i = 0; i < NHC; ++i) {
-      const int t = lane + 32 * i, j = t >> 2, cc = t & 3, c = (cc < 2) ? cc : 32 + cc;
-      if (t < 4 * TY && x0 + c < P.nxp && y0 + j + 2 < P.nyp)
-        fn(slot + j * RS + c, gp + (long long)(y0 + j + 2) * P.sy + c);
+      const int t = lane + 32 * i;
+      if (t < 4 * TY) {
+        const int j = t >> 2, cc = t & 3, c = (cc < 2) ? cc : 32 + cc;
+        if (x0 + c < P.nxp && y0 + j + 2 < P.nyp) fn(slot + j * RS + c, gp + (long long)(y0 + j + 2) * P.sy + c);
+      } else if (HALL && t < 4 * TY + 8) {
+        const int u = t - 4 * TY, r = u >> 1, c = (u & 1) ? 34 : 1, j = (r < 2) ? r - 2 : TY + r - 2;
+        if (x0 + c < P.nxp && y0 + j + 2 < P.nyp) fn(hbuf_of(p) + r * RS + c, gp + (long long)(y0 + j + 2) * P.sy + c);
+      }
     }
   };
   auto h_copy = [&](int p, int slot) { h_cells(p, slot, [&](int off, long long g) { copy_cell(off, g); }); };
@@ -232,6 +266,7 @@ __global__ void __launch_bounds__(32 * (TY + 1), MINB) stage3d_kernel(const __gr
     // plane k0+1 goes into the slot plane k0-2 just left (own cell only: no other thread touches it)
     if (own_in) copy_cell(slot_of(k0 + 1) + own_off, own_g + (long long)(k0 + 3) * P.sz);
   } else {
+    if (HALL) h_copy(k0 - 1, slot_of(k0 - 1));        // only its B is read (the current at face k0 - 1/2): no conversion
     h_copy(k0, slot_of(k0));
     cp_async_wait_all();
     h_conv(k0, slot_of(k0));
@@ -245,7 +280,7 @@ __global__ void __launch_bounds__(32 * (TY + 1), MINB) stage3d_kernel(const __gr
   for (int k = k0; k <= k1; ++k, gm += P.sz) {
     const bool full = k < k1;       // plane k gets its x and y sweeps (step k1 only closes plane k1-1)
     const bool emit = k > k0;       // plane k-1 is completed in this step
-    const int hb = 3 * PL + (k & 1) * SB;                 // y-halo rows of plane k
+    const int hb = hbuf_of(k);                            // y-halo rows of plane k
     const int ph0 = ph;                                   // sub-phases completed when this plane starts
     double Ly[NV], ua[NV], ub[NV];
 

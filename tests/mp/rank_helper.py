@@ -15,5 +15,7 @@ ms = 10.0 + 5.0 * rank                                  # rank r "measured" 10 +
 ms_max = bench.max_over_ranks(ms, world, "cpu")
 rate = bench.aggregate_rate(1000, world, 4, ms_max)
 dist.barrier()
-print(json.dumps({"rank": rank, "world": world, "ms_max": ms_max, "rate": rate}), flush=True)
+# one file per rank: two ranks printing to one captured stdout can interleave their lines
+with open(os.path.join(os.environ["AGATE_MP_OUT"], f"rank{rank}.json"), "w") as f:
+    json.dump({"rank": rank, "world": world, "ms_max": ms_max, "rate": rate}, f)
 dist.destroy_process_group()
