@@ -84,7 +84,6 @@ int check_args(const agate_grid* g, double gamma, int eqset, const agate_solver*
   if (s->bc[1] == 2 && (g->ndim < 2 || s->bc[0] != 0)) return AGATE_ERR_ARG;   // sheared ends in y need a periodic x (R28)
   if (eqset == AGATE_HALL && s->riemann == AGATE_HLLD) return AGATE_ERR_ARG;   // no Hall-HLLD in the paper
   if (eqset == AGATE_HALL && !(s->d_i >= 0.0)) return AGATE_ERR_ARG;
-  if (eqset == AGATE_HALL && g->ndim == 3) return AGATE_ERR_ARG;               // 3-D Hall: not built yet
   return AGATE_OK;
 }
 
@@ -108,12 +107,13 @@ StageKernel make_stage() {
   return k;
 }
 
-template <int TY, int R, int LIM, int MINB, bool GLM = false, bool CGL = false>
+template <int TY, int R, int LIM, int MINB, bool GLM = false, bool CGL = false, bool HALL = false>
 StageKernel make_stage3d() {
   StageKernel k;
-  k.fn = stage3d_kernel<TY, R, LIM, MINB, GLM, CGL>;
-  k.ty = TY; k.np = 3; k.threads = Stage3dSmem<TY, (GLM || CGL) ? 9 : 8>::NT;
-  k.smem = Stage3dSmem<TY, (GLM || CGL) ? 9 : 8>::BYTES;
+  k.fn = stage3d_kernel<TY, R, LIM, MINB, GLM, CGL, HALL>;
+  using SM = Stage3dSmem<TY, (GLM || CGL) ? 9 : 8, HALL ? 3 : 2>;
+  k.ty = TY; k.np = 3; k.threads = SM::NT;
+  k.smem = SM::BYTES;
   k.even_split = true;
   k.fused_dt = !CGL;         // the fused reduction evaluates the ideal-MHD speed; CGL keeps the dt_kernel pass
   return k;
@@ -132,6 +132,9 @@ StageKernel make_stage2d() {
 
 StageKernel pick_stage(int ndim, int eqset, int riemann, int limiter) {
   if (ndim == 3) {
+    if (eqset == AGATE_HALL)
+      return (limiter == 2) ? make_stage3d<TY3, 0, 2, AGATE_MINB3, false, false, true>()
+                            : make_stage3d<TY3, 0, -1, AGATE_MINB3, false, false, true>();
     if (eqset == AGATE_CGL)
       return (limiter == 2) ? make_stage3d<TY3N, 0, 2, AGATE_MINB3, false, true>() : make_stage3d<TY3N, 0, -1, AGATE_MINB3, false, true>();
     if (eqset == AGATE_IDEAL_GLM) {

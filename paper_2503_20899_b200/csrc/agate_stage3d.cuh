@@ -270,7 +270,7 @@ __global__ void __launch_bounds__(32 * (TY + 1), MINB) stage3d_kernel(const __gr
     h_copy(k0, slot_of(k0));
     cp_async_wait_all();
     h_conv(k0, slot_of(k0));
-    if (k0 + 1 < k1) h_copy(k0 + 1, slot_of(k0 + 1));
+    if (!HALL && k0 + 1 < k1) h_copy(k0 + 1, slot_of(k0 + 1));
   }
   __syncthreads();
 
@@ -286,7 +286,7 @@ __global__ void __launch_bounds__(32 * (TY + 1), MINB) stage3d_kernel(const __gr
 
 #pragma unroll
     for (int s = 0; s < 3; ++s) {
-      double L[NV], R[NV], F[NV];
+      double L[NV], R[NV], F[NV], Jr[3];
       bool flux = false;
       // ---- hand-over: what this sub-phase reads must be published, what it overwrites must have been read.  Every
       //      wait is on a sub-phase EARLIER than the one about to start, so the waits cannot form a cycle.
@@ -300,6 +300,10 @@ __global__ void __launch_bounds__(32 * (TY + 1), MINB) stage3d_kernel(const __gr
         } else {
           await(prog + min(lane, TY - 1), ph0, P.flag);
           __syncwarp();
+          // Hall: the owners read the B of plane k-1's halo cells until the end of their phase B2 (currents at the x
+          // faces), so the halo cells of plane k+1 cannot take that slot before now; they are read (raw B) from phase
+          // B1 on, so the copies are awaited before this phase is published
+          if (HALL && k + 1 <= k1) h_copy(k + 1, sp);
         }
       } else if (s == 1) {
         // phase B1.  owner j: the right state in Y[j+1] (phase A of the row above, H for the top row).
@@ -311,7 +315,7 @@ __global__ void __launch_bounds__(32 * (TY + 1), MINB) stage3d_kernel(const __gr
         // H: both edge owners are done with the y-halo rows H is about to refill (their phase A).
         if (owner) {
           await(prog + TY, ph0 + 1, P.flag);
-        } else {
+        } else if (!HALL) {
           await(prog + 0, ph0 + 1, P.flag);
           await(prog + TY - 1, ph0 + 1, P.flag);
         }
@@ -332,6 +336,16 @@ __global__ void __launch_bounds__(32 * (TY + 1), MINB) stage3d_kernel(const __gr
             R[r] = lo;
             WLz[v * ZS + tid] = hi;
           }
+          if (HALL) {
+            // face k-1/2 of the own column: C = plane k-1, D = plane k; transverse x (lanes), y (rows; halo rows at
+            // the tile's edges)
+            const int oC = sm + own_off, oD = sc + own_off;
+            const int hm = hbuf_of(k - 1) + lane + 2;
+            const int oCym = (wid == 0) ? hm + RS : oC - RS, oCyp = (wid == TY - 1) ? hm + 2 * RS : oC + RS;
+            const int oDym = (wid == 0) ? hb + RS + lane + 2 : oD - RS, oDyp = (wid == TY - 1) ? hb + 2 * RS + lane + 2 : oD + RS;
+            hall_current<2>(W, QS, oC, oD, oC + 1, oC - 1, oD + 1, oD - 1, oCyp, oCym, oDyp, oDym, P.idz, 0.25 * P.idx,
+                            0.25 * P.idy, Jr);
+          }
           flux = true;
         } else if (full) {
           if (s == 1) {
@@ -339,6 +353,17 @@ __global__ void __launch_bounds__(32 * (TY + 1), MINB) stage3d_kernel(const __gr
             for (int r = 0; r < NV; ++r) {
               L[r] = Ly[r];
               R[r] = Y[rv(r, 1) * YS + (wid + 1) * 32 + lane];
+            }
+            if (HALL) {
+              // face j+1/2: C = own cell, D = the row above (halo row TY for the top row); transverse z (planes
+              // k-1, k+1), x (lanes; the halo rows carry their x corners)
+              const bool top = (wid == TY - 1);
+              const int oC = sc + own_off, oD = top ? hb + 2 * RS + lane + 2 : oC + RS;
+              const int oCzp = sp + own_off, oCzm = sm + own_off;
+              const int oDzp = top ? hbuf_of(k + 1) + 2 * RS + lane + 2 : oCzp + RS;
+              const int oDzm = top ? hbuf_of(k - 1) + 2 * RS + lane + 2 : oCzm + RS;
+              hall_current<1>(W, QS, oC, oD, oCzp, oCzm, oDzp, oDzm, oC + 1, oC - 1, oD + 1, oD - 1, P.idy, 0.25 * P.idz,
+                              0.25 * P.idx, Jr);
             }
           } else {
             // A2 (x): own slope; the right state of face i+1/2 comes from lane i+1 (lane 31: from H)
@@ -351,6 +376,13 @@ __global__ void __launch_bounds__(32 * (TY + 1), MINB) stage3d_kernel(const __gr
               L[r] = hi;
               const double rn = __shfl_down_sync(0xffffffffu, lo, 1);
               R[r] = (lane == 31) ? XR[r * XS + wid] : rn;
+            }
+            if (HALL) {
+              // face i+1/2: C = own cell, D = the next column (x-halo column for lane 31); transverse y (rows), z
+              const int oC = c, oD = c + 1;
+              const int oCym = (wid == 0) ? hb + RS + lane + 2 : oC - RS, oCyp = (wid == TY - 1) ? hb + 2 * RS + lane + 2 : oC + RS;
+              hall_current<0>(W, QS, oC, oD, oCyp, oCym, oCyp + 1, oCym + 1, sp + own_off, sm + own_off, sp + own_off + 1,
+                              sm + own_off + 1, P.idx, 0.25 * P.idy, 0.25 * P.idz, Jr);
             }
           }
           flux = true;
@@ -391,6 +423,30 @@ __global__ void __launch_bounds__(32 * (TY + 1), MINB) stage3d_kernel(const __gr
               L[r] = hi;
               R[r] = __shfl_down_sync(0xffffffffu, lo, 16);
             }
+            if (HALL) {
+              // face x = -1/2 of row `row`: C = column -1, D = column 0.  D's cell of plane k+1 belongs to an owner
+              // that may still be converting it: its B comes straight from the stage input (the copy that brought
+              // it into shared memory has already pulled the line into L2)
+              const int oC = sc + row * RS + 1, oD = oC + 1;
+              const int oCym = (row == 0) ? hb + RS + 1 : oC - RS, oCyp = (row == TY - 1) ? hb + 2 * RS + 1 : oC + RS;
+              const int oCzm = sm + row * RS + 1;
+              // B_x, B_y of columns -1 and 0 in plane k+1 straight from the stage input (the halo copies of that plane
+              // were issued a moment ago; column 0 belongs to an owner that may still be converting it)
+              double bc[2] = {0.0, 0.0}, bd[2] = {0.0, 0.0};
+              if (y0 + row + 2 < P.nyp) {
+                const double* g = P.Uin + 5 * P.sq + (long long)(k + 3) * P.sz + (long long)(y0 + row + 2) * P.sy + (x0 + 1);
+                bc[0] = __ldg(g); bc[1] = __ldg(g + P.sq);
+                bd[0] = __ldg(g + 1); bd[1] = __ldg(g + P.sq + 1);
+              }
+              const double* Bx = W + 5 * QS; const double* By = W + 6 * QS; const double* Bz = W + 7 * QS;
+              const double q1 = 0.25 * P.idy, q2 = 0.25 * P.idz;
+              const double dnB1 = (By[oD] - By[oC]) * P.idx, dnB2 = (Bz[oD] - Bz[oC]) * P.idx;
+              const double d1Bn = ((Bx[oCyp] - Bx[oCym]) + (Bx[oCyp + 1] - Bx[oCym + 1])) * q1;
+              const double d1B2 = ((Bz[oCyp] - Bz[oCym]) + (Bz[oCyp + 1] - Bz[oCym + 1])) * q1;
+              const double d2Bn = ((bc[0] - Bx[oCzm]) + (bd[0] - Bx[oCzm + 1])) * q2;
+              const double d2B1 = ((bc[1] - By[oCzm]) + (bd[1] - By[oCzm + 1])) * q2;
+              Jr[0] = d1B2 - d2B1; Jr[1] = d2Bn - dnB2; Jr[2] = dnB1 - d1Bn;
+            }
           }
           flux = true;
         } else if (s == 1) {
@@ -404,6 +460,14 @@ __global__ void __launch_bounds__(32 * (TY + 1), MINB) stage3d_kernel(const __gr
             plm_faces(limiter, beta2, a, b, c, lo, hi);
             L[r] = hi;
             R[r] = Y[v * YS + lane];
+          }
+          if (HALL) {
+            // face y = -1/2: C = halo row -1, D = row 0; transverse z (the halo rows of planes k-1, k+1; owner 0's
+            // cells), x (the halo row carries its x corners)
+            const int oC = c0r, oD = cp;
+            const int oCzp = hbuf_of(k + 1) + RS + lane + 2, oCzm = hbuf_of(k - 1) + RS + lane + 2;
+            hall_current<1>(W, QS, oC, oD, oCzp, oCzm, sp + lane + 2, sm + lane + 2, oC + 1, oC - 1, oD + 1, oD - 1, P.idy,
+                            0.25 * P.idz, 0.25 * P.idx, Jr);
           }
           flux = true;
         }
@@ -421,7 +485,7 @@ __global__ void __launch_bounds__(32 * (TY + 1), MINB) stage3d_kernel(const __gr
         F[NV - 1] = ch * ch * bns;
       } else if (flux) {
         if (CGL) flux_hll_cgl(L, R, F);
-        else riemann_flux<RIEMANN, false>(P.ph, L, R, nullptr, F);
+        else riemann_flux<RIEMANN, HALL>(P.ph, L, R, HALL ? Jr : nullptr, F);
       }
 
       // ------------------------------------------------------------------ consume the flux of task s
@@ -476,7 +540,7 @@ __global__ void __launch_bounds__(32 * (TY + 1), MINB) stage3d_kernel(const __gr
             ACC[v * ZS + tid] = t;
           }
           if (P.vnext != nullptr && emit && cell_ok) {                    // A7 on the values just stored
-            const double sp = cell_speed_inline(P.ph, o);
+            const double sp = cell_speed_inline<HALL>(P.ph, o);
             if (sp < 0.0) bad = 1; else vmx = dmax(vmx, sp);
           }
         } else if (full) {
@@ -491,6 +555,8 @@ __global__ void __launch_bounds__(32 * (TY + 1), MINB) stage3d_kernel(const __gr
               const double fl = __shfl_up_sync(0xffffffffu, F[r], 1);
               dFx[r] = F[r] - ((lane == 0) ? XF[r * XS + wid] : fl);
             }
+            // Hall: the row below reads this row's cell of plane k-1 until the end of its phase B1 (current at its y face)
+            if (HALL) await(prog + (wid == 0 ? TY : wid - 1), ph0 + 2, P.flag);
             // own cell of plane k+2 -> the slot plane k-1 left in phase A
             if (own_in && k + 2 <= k1 + 1) copy_cell(sm + own_off, gm + 3 * P.sz);
             // second SSP stage: U0 of plane k+1 is first touched two steps from now; pull its lines into L2 (one
@@ -500,7 +566,7 @@ __global__ void __launch_bounds__(32 * (TY + 1), MINB) stage3d_kernel(const __gr
               for (int q = 0; q < NV; ++q) prefetch_l2(P.U0 + q * P.sq + gm + 2 * P.sz);
             }
             // A5 (y): Y[j+1] holds this row's own flux (phase B1), Y[j] the flux of the row below (its phase B1)
-            await(prog + (wid == 0 ? TY : wid - 1), ph0 + 2, P.flag);
+            if (!HALL) await(prog + (wid == 0 ? TY : wid - 1), ph0 + 2, P.flag);
 #pragma unroll
             for (int v = 0; v < NV; ++v) {
               constexpr int inv1[9] = {0, 3, 1, 2, 4, 7, 5, 6, 8};        // rv(inv1[v], 1) == v
@@ -516,6 +582,7 @@ __global__ void __launch_bounds__(32 * (TY + 1), MINB) stage3d_kernel(const __gr
 #pragma unroll
             for (int r = 0; r < NV; ++r) XF[r * XS + lane] = F[r];
           }
+          if (HALL) cp_async_wait_all();       // plane k+1's halo cells have landed when this phase is published
         } else if (s == 1) {
           if (full) {
 #pragma unroll
@@ -523,9 +590,9 @@ __global__ void __launch_bounds__(32 * (TY + 1), MINB) stage3d_kernel(const __gr
           }
         } else {
           // A1 for the halo cells of plane k+1 (copies issued one phase B2 ago), then the copies for plane k+2
-          cp_async_wait_all();
+          if (!HALL) cp_async_wait_all();
           if (k + 1 < k1) h_conv(k + 1, sp);
-          if (k + 2 < k1) h_copy(k + 2, sm);
+          if (!HALL && k + 2 < k1) h_copy(k + 2, sm);
         }
       }
       publish(prog + wid, ++ph, lane);   // end of phase A, B1, B2

@@ -197,6 +197,10 @@ _CONFIGS = {
     # the initial anisotropy to zero"), HLL, default relaxation dt/(dt+tau) = 0.99
     7: dict(ndim=2, n=2048, eqset=CGL, riemann=HLL, beta=1.3, cfl=0.45, d_i=0.0, n_steps=100, relax=0.99,
             name="cfg7: 2D Orszag-Tang CGL 2048^2 HLL MC"),
+    # not a BASELINE.json config: config 4's setting (Hall MHD, HLL, eq.4 at beta = 1, d_i across ~50 zones) on config
+    # 3's three-dimensional recipe, for the 3-D Hall path of the row-owner kernel
+    8: dict(ndim=3, n=256, eqset=HALL, riemann=HLL, beta=1.0, cfl=0.325, d_i=0.2, n_steps=50,
+            name="cfg8: 3D Hall 256^3 HLL minmod"),
 }
 
 
@@ -262,7 +266,7 @@ def make_workload(config_id: int, n: int | None = None, n_steps: int | None = No
         W[6] = by * s
         W[7] = 0.0
         W[4] = 1.0
-    elif config_id == 3:
+    elif config_id in (3, 8):
         W[0] = 1.0 + 0.2 * F(8, 4)
         Px, Py, Pz = F(8, 4), F(8, 4), F(8, 4)
         vx, vy, vz = curl_c(Px, Py, Pz, dx, ndim)
@@ -292,7 +296,7 @@ def make_workload(config_id: int, n: int | None = None, n_steps: int | None = No
         raise ValueError(f"unknown config {config_id}")
 
     d_i = c["d_i"]
-    if config_id == 4 and scale_d_i and n != nfull:
+    if config_id in (4, 8) and scale_d_i and n != nfull:
         d_i = d_i * nfull / n
     U = prim_to_cons_cgl(W) if c["eqset"] == CGL else prim_to_cons(W, g)
     return Workload(config_id=config_id, ndim=ndim, shape=shape, dx=dx, gamma=g, eqset=c["eqset"],
