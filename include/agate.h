@@ -63,12 +63,12 @@ typedef struct {
 enum { AGATE_IDEAL = 0, AGATE_HALL = 1, AGATE_CGL = 2, AGATE_IDEAL_GLM = 3 };
 /* AGATE_CGL (NEXT-2; eqs.14-33; R24): CGL MHD with the logarithmic state variable of
  * eq.18.  NINE variables per cell: U = (rho, m, E, B, A_log) with E = rho v^2/2 + B^2/2 + p_par/2 + p_perp.  HLL only,
- * speeds eq.29, dt eq.28, anisotropy relaxation eqs.31-33 (C1 = 0.3, C2 = 0.5) after the Runge-Kutta update.  2-D
- * and 3-D grids (a 1-D problem runs as a few identical rows). */
+ * speeds eq.29, dt eq.28, anisotropy relaxation eqs.31-33 (C1 = 0.3, C2 = 0.5) after the Runge-Kutta update.  1-D grids
+ * run through the 2-D kernel as one row that is its own periodic neighbour (exact: both y faces carry the same flux). */
 /* AGATE_IDEAL_GLM (NEXT-1; eqs.10-11, constants L142; R22): ideal MHD with GLM
  * divergence cleaning.  NINE variables per cell, the scalar psi last: every U below is U[9][nz][ny][nx].  Per step
  * c_h = 0.95 v_max(U^n), c_p^2 = 0.18 c_h; face (B_n, psi) from the 2x2 linear Riemann problem; psi is multiplied by
- * exp(-dt c_h^2/c_p^2) after the Runge-Kutta update.  2-D and 3-D grids (1-D: agate_init returns AGATE_ERR_ARG). */
+ * exp(-dt c_h^2/c_p^2) after the Runge-Kutta update.  1-D grids run through the 2-D kernel as one row (see AGATE_CGL). */
 
 enum { AGATE_HLL = 0, AGATE_HLLD = 1 };
 enum {

@@ -75,9 +75,8 @@ int check_args(const agate_grid* g, double gamma, int eqset, const agate_solver*
   if (!(g->dx > 0.0) || (g->ndim >= 2 && !(g->dy > 0.0)) || (g->ndim >= 3 && !(g->dz > 0.0))) return AGATE_ERR_ARG;
   if (!(gamma > 1.0)) return AGATE_ERR_ARG;
   if (eqset != AGATE_IDEAL && eqset != AGATE_HALL && eqset != AGATE_IDEAL_GLM && eqset != AGATE_CGL) return AGATE_ERR_ARG;
-  if (eqset == AGATE_CGL && (g->ndim < 2 || s->riemann != AGATE_HLL)) return AGATE_ERR_ARG;    // CGL: 2-D and 3-D kernels, HLL
+  if (eqset == AGATE_CGL && s->riemann != AGATE_HLL) return AGATE_ERR_ARG;    // CGL: HLL (the paper names no other solver)
   if (eqset == AGATE_CGL && !(s->relax >= 0.0 && s->relax <= 1.0)) return AGATE_ERR_ARG;
-  if (eqset == AGATE_IDEAL_GLM && g->ndim < 2) return AGATE_ERR_ARG;             // GLM: 2-D and 3-D kernels
   if (s->riemann < 0 || s->riemann > 1 || s->limiter < 0 || s->limiter > 2 || s->rk < 1 || s->rk > 5) return AGATE_ERR_ARG;
   if (s->limiter == 2 && !(s->beta >= 1.0 && s->beta <= 2.0)) return AGATE_ERR_ARG;
   for (int d = 0; d < 3; ++d) if (s->bc[d] < 0 || s->bc[d] > ((d == 1) ? 2 : 1)) return AGATE_ERR_ARG;
@@ -85,6 +84,16 @@ int check_args(const agate_grid* g, double gamma, int eqset, const agate_solver*
   if (eqset == AGATE_HALL && s->riemann == AGATE_HLLD) return AGATE_ERR_ARG;   // no Hall-HLLD in the paper
   if (eqset == AGATE_HALL && !(s->d_i >= 0.0)) return AGATE_ERR_ARG;
   return AGATE_OK;
+}
+
+// The nine-variable equation sets (GLM, CGL) have no 1-D kernel: a 1-D grid runs through the 2-D strip kernel as ONE row
+// that is its own periodic neighbour in y.  Both y faces of a zone then see identical states, their fluxes are the same
+// number and the y difference is an exact zero, so the result is that of the 1-D scheme (the oracle has no y sweep at
+// all); Courant number and dx_min are still those of the 1-D grid.
+agate_grid kernel_grid(const agate_grid& g, int eqset) {
+  agate_grid k = g;
+  if (g.ndim == 1 && (eqset == AGATE_IDEAL_GLM || eqset == AGATE_CGL)) { k.ndim = 2; k.dy = g.dx; }
+  return k;
 }
 
 typedef void (*stage_fn_t)(const StageParams);
@@ -112,6 +121,7 @@ StageKernel make_stage3d() {
   StageKernel k;
   k.fn = stage3d_kernel<TY, R, LIM, MINB, GLM, CGL, HALL>;
   using SM = Stage3dSmem<TY, (GLM || CGL) ? 9 : 8, HALL ? 3 : 2>;
+  static_assert(SM::BYTES <= 232448, "stage3d shared memory exceeds 227 KB");
   k.ty = TY; k.np = 3; k.threads = SM::NT;
   k.smem = SM::BYTES;
   k.even_split = true;
@@ -463,7 +473,7 @@ extern "C" {
 
 size_t agate_workspace_bytes(const agate_grid* grid, int eqset, const agate_solver* solver) {
   if (check_args(grid, 5.0 / 3.0, eqset, solver) != AGATE_OK) return 0;
-  return make_layout(*grid, (eqset == AGATE_IDEAL_GLM || eqset == AGATE_CGL) ? 9 : 8, solver->rk).total;
+  return make_layout(kernel_grid(*grid, eqset), (eqset == AGATE_IDEAL_GLM || eqset == AGATE_CGL) ? 9 : 8, solver->rk).total;
 }
 
 int agate_init(const agate_grid* grid, double gamma, int eqset, const agate_solver* solver, void* workspace,
@@ -473,6 +483,9 @@ int agate_init(const agate_grid* grid, double gamma, int eqset, const agate_solv
   if (rc) return rc;
   if (!workspace) return AGATE_ERR_ARG;
   const int nv = (eqset == AGATE_IDEAL_GLM || eqset == AGATE_CGL) ? 9 : 8;
+  const agate_grid user_grid = *grid;                 // Courant number and dx_min follow the caller's dimensionality
+  const agate_grid kgrid = kernel_grid(*grid, eqset);
+  grid = &kgrid;
   Layout L = make_layout(*grid, nv, solver->rk);
   if (workspace_bytes < L.total || ((uintptr_t)workspace & 255u)) return AGATE_ERR_NOMEM;
   int ndev = 0;
@@ -481,11 +494,11 @@ int agate_init(const agate_grid* grid, double gamma, int eqset, const agate_solv
   agate_ctx* c = new (std::nothrow) agate_ctx;
   if (!c) return AGATE_ERR_NOMEM;
   c->g = *grid; c->s = *solver; c->gamma = gamma; c->eqset = eqset; c->L = L; c->nv = nv;
-  c->dxmin = grid->dx;
-  if (grid->ndim >= 2) c->dxmin = fmin(c->dxmin, grid->dy);      // R5: min over ACTIVE dimensions
-  if (grid->ndim >= 3) c->dxmin = fmin(c->dxmin, grid->dz);
+  c->dxmin = user_grid.dx;
+  if (user_grid.ndim >= 2) c->dxmin = fmin(c->dxmin, user_grid.dy);      // R5: min over ACTIVE dimensions
+  if (user_grid.ndim >= 3) c->dxmin = fmin(c->dxmin, user_grid.dz);
   c->cfl = solver->cfl;
-  if (!(c->cfl > 0.0)) c->cfl = (grid->ndim == 1) ? 0.8 : (grid->ndim == 2 ? 0.45 : 0.325);
+  if (!(c->cfl > 0.0)) c->cfl = (user_grid.ndim == 1) ? 0.8 : (user_grid.ndim == 2 ? 0.45 : 0.325);
   c->ph = make_phys(gamma, (eqset == AGATE_HALL) ? solver->d_i : 0.0, c->dxmin);
   c->stream = (cudaStream_t)stream;
   c->ws = (char*)workspace;
@@ -676,7 +689,7 @@ int agate_stage_time(agate_ctx* c, double* ms_out, int64_t* launches_out, int re
 // ---- NEXT-4: slab decomposition along the last active dimension -------------------------------------
 int agate_set_slab(agate_ctx* c, int ext_lo, int ext_hi) {
   if (!c) return AGATE_ERR_ARG;
-  if (c->g.ndim < 2) return AGATE_ERR_ARG;
+  if (c->g.ndim < 2 || ((c->g.ndim == 3) ? c->g.nz : c->g.ny) < 2) return AGATE_ERR_ARG;   // two layers per cut face
   c->ext_lo = ext_lo != 0; c->ext_hi = ext_hi != 0;
   c->gpA = make_ghost(c, c->UA); c->gpB = make_ghost(c, c->UB); c->gpC = make_ghost(c, c->UC);
   if (c->graph) { cudaGraphExecDestroy(c->graph); c->graph = nullptr; }

@@ -647,9 +647,9 @@ AG_HD double cgl_relaxed_alog(double f, const double U[9]) {
   cgl_cons_to_prim(U, w);
   const double B2 = w[5] * w[5] + w[6] * w[6] + w[7] * w[7];
   const double dP = w[8] - w[4];
-  const double mirror = (w[4] / w[8]) * B2 / 2.0;
-  const double ic = 0.3 * w[4] * sqrt(B2 / (2.0 * w[4]));
-  const double dPs = fmax(-B2, fmin(dP, fmin(mirror, ic)));
+  const double mirror = (w[4] * rcp(w[8])) * (0.5 * B2);
+  const double ic = 0.3 * sqrt_pos(dmax(0.5 * B2 * w[4], kTiny));      // C1 p_par (B^2 / 2 p_par)^(1/2) = C1 (p_par B^2 / 2)^(1/2)
+  const double dPs = dmax(-B2, dmin(dP, dmin(mirror, ic)));
   const double ppar = w[4] - (2.0 / 3.0) * (dPs - dP) * f;
   const double pperp = w[8] + (1.0 / 3.0) * (dPs - dP) * f;
   return cgl_alog(w[0], B2, ppar, pperp);

@@ -130,10 +130,11 @@ def test_glm_3d_parity(ag, riemann, grid):
     ref.close(); gpu.close()
 
 
-def test_glm_rejected_where_not_built(ag):
-    with pytest.raises(ag.AgateError) as ei:
-        ag.Agate(shape=(8, 1, 1), dx=(1 / 8, 1, 1), ndim=1, eqset=ag.IDEAL_GLM)
-    assert ei.value.code == ag.ERR_ARG
+def test_glm_1d_grid_is_accepted(ag):
+    """1-D GLM runs through the strip kernel as one periodic row (parity: tests/test_gpu_next3.py)."""
+    g = ag.Agate(shape=(8, 1, 1), dx=(1 / 8, 1, 1), ndim=1, eqset=ag.IDEAL_GLM)
+    assert g.nvar == 9
+    g.close()
 
 
 @pytest.mark.parametrize("seed", range(8))

@@ -147,3 +147,43 @@ def test_device_source_is_read_in_stream_order(ag):
     assert gpu.step(0.0) == dtr or abs(gpu.compute_dt()) > 0
     assert np.all(rel_linf(gpu.get_state(), ref.get_state()) <= TOL_1)
     ref.close(); gpu.close()
+
+
+@pytest.mark.parametrize("eqset_name", ["glm", "cgl"])
+@pytest.mark.parametrize("n", [64, 75])
+def test_nine_variable_sets_on_1d_grids(ag, eqset_name, n):
+    """1-D GLM / CGL problems (the paper's CGL benchmarks are 1-D) run through the 2-D strip kernel as one
+    row that is its own periodic neighbour; the oracle runs them as genuinely 1-D (no y sweep, C = 0.8)."""
+    x = (np.arange(n) + 0.5) / n
+    if eqset_name == "glm":
+        W = np.zeros((8, 1, 1, n))
+        W[0] = 1.0 + 0.3 * np.sin(2 * np.pi * x); W[1] = 0.2; W[2] = 0.1 * np.cos(2 * np.pi * x); W[4] = 0.7
+        W[5] = 0.8 + 0.05 * np.sin(4 * np.pi * x)                  # a divergence error for the cleaning to act on
+        W[6, 0, 0], W[7, 0, 0] = 0.3 * np.cos(2 * np.pi * x), 0.3 * np.sin(4 * np.pi * x)
+        U = np.concatenate([workloads.prim_to_cons(W, 5 / 3), 0.01 * np.sin(2 * np.pi * x)[None, None, None, :]], axis=0)
+        eo, eg, rie = oracle.IDEAL_GLM, ag.IDEAL_GLM, HLLD
+    else:
+        W = np.zeros((9, n))
+        W[0] = 1.0 + 0.2 * np.sin(2 * np.pi * x); W[1] = 0.3 * np.cos(2 * np.pi * x); W[2] = 0.1
+        W[4] = 0.8 + 0.2 * np.cos(2 * np.pi * x); W[8] = 0.6 + 0.3 * np.sin(2 * np.pi * x)
+        W[5] = 0.7; W[6] = 0.3 * np.sin(2 * np.pi * x); W[7] = 0.2
+        U = np.stack([oracle.cgl_prim_to_cons(W[:, i]) for i in range(n)], axis=1).reshape(9, 1, 1, n)
+        eo, eg, rie = oracle.CGL, ag.CGL, HLL
+    kw = dict(shape=(n, 1, 1), dx=(1.0 / n, 1, 1), ndim=1, riemann=rie, beta=1.3, rk=2,
+              relax=0.99 if eqset_name == "cgl" else 0.0)
+    ref = oracle.RefSolver(eqset=eo, **kw); gpu = ag.Agate(eqset=eg, **kw)
+    ref.set_state(U); gpu.set_state(U)
+    for s in range(6):
+        dtr, dtg = ref.compute_dt(), gpu.compute_dt()
+        assert abs(dtg - dtr) <= TOL_DT * dtr
+        ref.step(dtr)
+        assert gpu.step(0.0) == dtg
+    Ug, Ur = gpu.get_state(), ref.get_state()
+    for q in range(9):
+        sc = max(np.max(np.abs(Ur[q])), np.max(np.abs(Ur[0])) if q == 8 else 0.0, 1e-300)
+        if 1 <= q <= 3: sc = np.max(np.abs(Ur[1:4]))
+        if 5 <= q <= 7: sc = np.max(np.abs(Ur[5:8]))
+        assert np.max(np.abs(Ug[q] - Ur[q])) <= TOL_N * sc, (q,)
+    tr, tg = ref.advance(3), gpu.advance(3)
+    assert abs(tg - tr) <= 1e-13 * tr
+    ref.close(); gpu.close()
