@@ -295,30 +295,66 @@ AG_HD void phys_flux(const Phys& ph, const double w[8], const Side& s, const dou
 
 // HLL, eq.5 with the Davis speeds eq.6; all 8 components through eq.5 (R9).
 // Hall (R15): c = max(c_f, c_w) per side, v_H^a = -d_i J / rho^a in phi.  J in the rotated frame.
+// Written for the FP64 pipe: the fast speed from rho c_f^2 = N = H + sqrt(H^2 - gamma p Bn^2), H = (gamma p + B^2)/2
+// (no reciprocal of rho in ideal MHD: c_f = N rsqrt(N rho)); each side's physical flux and conserved vector share their
+// kinetic and magnetic terms; eq.5 as  F = a F_L + b F_R + c (U_R - U_L)  with a = s_R/(s_R-s_L), b = -s_L/(s_R-s_L),
+// c = s_L s_R/(s_R-s_L) (three multiplies once instead of one per component).  ~150 FP64 instructions per face
+// (ideal), ~205 (Hall), from ~190 / ~235 as eq.5 is printed.
+template <bool HALL>
+AG_HD void hll_side(const Phys& ph, const double w[8], const double* dJ, double& cout, double f[8], double& E, double& rv,
+                    double& rw) {
+  const double bn2 = w[5] * w[5];
+  const double hB = 0.5 * fma(w[7], w[7], fma(w[6], w[6], bn2));           // |B|^2 / 2
+  const double pt = w[4] + hB;
+  const double g = ph.hgamma * w[4], H = g + hB;
+  const double Q = dmax(fma(H, H, -(g * (bn2 + bn2))), kTiny);
+  const double N = H + sqrt_pos(Q);                                         // rho c_f^2 (eq.12, R3)
+  double tn = w[1], t1 = w[2], t2 = w[3];
+  if (HALL) {
+    const double ir = rcp(w[0]);
+    const double B2 = hB + hB;
+    double c = sqrt_pos(N * ir);
+    const double aw = ph.cwk * sqrt_pos(dmax(B2, kTiny)) * ir;              // eq.13
+    c = dmax(c, aw + sqrt_pos(dmax(fma(aw, aw, B2 * ir), kTiny)));
+    cout = c;
+    tn = fma(-dJ[0], ir, tn); t1 = fma(-dJ[1], ir, t1); t2 = fma(-dJ[2], ir, t2);   // v_T = v - d_i J / rho
+  } else {
+    cout = N * rsq(N * w[0]);
+  }
+  const double ru = w[0] * w[1];
+  const double ke = (0.5 * w[0]) * fma(w[3], w[3], fma(w[2], w[2], w[1] * w[1]));
+  E = fma(w[4], ph.igm1, ke + hB);                                          // P:L140, R2
+  rv = w[0] * w[2]; rw = w[0] * w[3];
+  const double tB = fma(t2, w[7], fma(t1, w[6], tn * w[5]));
+  f[0] = ru;                                                                // eq.7
+  f[1] = fma(ru, w[1], pt - bn2);                                           // eq.8
+  f[2] = fma(ru, w[2], -(w[5] * w[6]));
+  f[3] = fma(ru, w[3], -(w[5] * w[7]));
+  f[4] = fma(-tB, w[5], fma(hB + hB, tn, fma(ph.gogm1, w[4], ke) * w[1]));  // eq.9
+  f[5] = 0.0;                                                               // eq.10, c == n
+  f[6] = fma(tn, w[6], -(w[5] * t1));
+  f[7] = fma(tn, w[7], -(w[5] * t2));
+}
+
 template <bool HALL>
 AG_HD void flux_hll(const Phys& ph, const double L[8], const double R[8], const double* J, double F[8]) {
-  const Side sl = side_of(ph, L), sr = side_of(ph, R);
-  double cl = sl.cf, cr = sr.cf;
-  double vhl[3], vhr[3];
-  if (HALL) {
-    cl = dmax(cl, whistler_speed(ph, L, sl));
-    cr = dmax(cr, whistler_speed(ph, R, sr));
-    for (int c = 0; c < 3; ++c) {
-      vhl[c] = -(ph.d_i * J[c]) * sl.ir;
-      vhr[c] = -(ph.d_i * J[c]) * sr.ir;
-    }
-  }
+  double dJ[3] = {0.0, 0.0, 0.0};
+  if (HALL) { dJ[0] = ph.d_i * J[0]; dJ[1] = ph.d_i * J[1]; dJ[2] = ph.d_i * J[2]; }
+  double fl[8], fr[8], cl, cr, El, Er, rvl, rwl, rvr, rwr;
+  hll_side<HALL>(ph, L, dJ, cl, fl, El, rvl, rwl);
+  hll_side<HALL>(ph, R, dJ, cr, fr, Er, rvr, rwr);
   const double sL = dmin(dmin(L[1] - cl, R[1] - cr), 0.0);       // s'_L = min(s_L, 0)
   const double sR = dmax(dmax(L[1] + cl, R[1] + cr), 0.0);       // s'_R = max(s_R, 0)
-  double fl[8], fr[8];
-  phys_flux(ph, L, sl, HALL ? vhl : nullptr, fl);
-  phys_flux(ph, R, sr, HALL ? vhr : nullptr, fr);
-  const double ul[8] = {L[0], L[0] * L[1], L[0] * L[2], L[0] * L[3], energy_of(ph, L, sl), L[5], L[6], L[7]};
-  const double ur[8] = {R[0], R[0] * R[1], R[0] * R[2], R[0] * R[3], energy_of(ph, R, sr), R[5], R[6], R[7]};
   const double iw = rcp(sR - sL);
-  const double ss = sL * sR;
-#pragma unroll
-  for (int q = 0; q < 8; ++q) F[q] = (sR * fl[q] - sL * fr[q] + ss * (ur[q] - ul[q])) * iw;
+  const double a = sR * iw, b = -(sL * iw), c = sL * a;
+  F[0] = fma(a, fl[0], fma(b, fr[0], c * (R[0] - L[0])));
+  F[1] = fma(a, fl[1], fma(b, fr[1], c * (fr[0] - fl[0])));      // U[1] = rho u = F[0] of the side
+  F[2] = fma(a, fl[2], fma(b, fr[2], c * (rvr - rvl)));
+  F[3] = fma(a, fl[3], fma(b, fr[3], c * (rwr - rwl)));
+  F[4] = fma(a, fl[4], fma(b, fr[4], c * (Er - El)));
+  F[5] = c * (R[5] - L[5]);                                      // eq.5 on Bn (R9): both physical fluxes are zero
+  F[6] = fma(a, fl[6], fma(b, fr[6], c * (R[6] - L[6])));
+  F[7] = fma(a, fl[7], fma(b, fr[7], c * (R[7] - L[7])));
 }
 
 // Star-state transverse components behind one outer wave (R10):  S = outer speed, m = rho (S - u).
