@@ -54,7 +54,7 @@ NCU_TRAFFIC_BYTES = {5: 0.5 * (11892200000 + 8929501000 + 20747918000 + 88745590
                      8: 0.5 * (1430480000 + 1094991000 + 2598487000 + 1093660000)}
 # ... and the kernels they were captured on: sha256 over csrc/*.cu* at capture time.  When the kernels have changed
 # since, the figure is stale and the line reports "traffic": null instead (profiles/ names the capture).
-NCU_TRAFFIC_CSRC_SHA = "f008dafa7a08f96c"
+NCU_TRAFFIC_CSRC_SHA = "d9964bdfc154968b"
 
 
 def csrc_sha():
