@@ -64,6 +64,33 @@ __device__ __forceinline__ void await(const int* prog_w, int value, int* flag) {
 }
 __device__ __forceinline__ void prefetch_l2(const void* p) { asm volatile("prefetch.global.L2 [%0];" ::"l"(p)); }
 
+// Bulk asynchronous copies (the TMA engine's 1-D form, cp.async.bulk) for the y-halo rows: a halo row of a tile, its x
+// halo and corners included, is 36 contiguous doubles of the padded array, so one 288-byte copy per (row, variable)
+// replaces 36 eight-byte cp.async.  Completion is counted in bytes on an mbarrier in shared memory.
+__device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ void mbar_init(unsigned long long* bar, int count) {
+  asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count) : "memory");
+}
+__device__ __forceinline__ void mbar_arrive_expect_tx(unsigned long long* bar, uint32_t bytes) {
+  asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void bulk_g2s(double* sdst, const double* gsrc, uint32_t bytes, unsigned long long* bar) {
+  asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(smem_u32(sdst)),
+               "l"(gsrc), "r"(bytes), "r"(smem_u32(bar))
+               : "memory");
+}
+__device__ __forceinline__ bool mbar_test_wait(unsigned long long* bar, uint32_t parity) {
+  uint32_t ok;
+  asm volatile(
+      "{\n\t.reg .pred p;\n\tmbarrier.test_wait.parity.shared::cta.b64 p, [%1], %2;\n\tselp.u32 %0, 1, 0, p;\n\t}"
+      : "=r"(ok)
+      : "r"(smem_u32(bar)), "r"(parity)
+      : "memory");
+  return ok != 0;
+}
+// generic-proxy accesses to a shared buffer are ordered before the async proxy (the bulk copy) overwrites it
+__device__ __forceinline__ void fence_proxy_async() { asm volatile("fence.proxy.async.shared::cta;" ::: "memory"); }
+
 // rotated slot -> fixed variable; the GLM scalar (slot 8) is not rotated
 __host__ __device__ __forceinline__ int rv(int r, int n) { return (r < 8) ? rot_var(r, n) : r; }
 
@@ -84,7 +111,8 @@ struct Stage3dSmem {
   static constexpr int OFF_XR = OFF_ACC + NV * ZS;
   static constexpr int OFF_XF = OFF_XR + NV * XS;
   static constexpr int OFF_PROG = OFF_XF + NV * XS;  // 16 ints: per-warp phase counters
-  static constexpr int TOTAL = OFF_PROG + 8;
+  static constexpr int OFF_MBAR = OFF_PROG + 8;      // one mbarrier: H's bulk copies of the y-halo rows
+  static constexpr int TOTAL = OFF_MBAR + 2;
   static constexpr size_t BYTES = sizeof(double) * (size_t)TOTAL;
 };
 
@@ -135,6 +163,7 @@ __global__ void __launch_bounds__(32 * (TY + 1), MINB) stage3d_kernel(const __gr
   double* const XR = smem + SM::OFF_XR;      // [8][XS]  right state of cell x = 32, per row
   double* const XF = smem + SM::OFF_XF;      // [8][XS]  x flux through face -1/2, per row
   int* const prog = reinterpret_cast<int*>(smem + SM::OFF_PROG);   // [TY+1] phases completed, per warp
+  unsigned long long* const hbar = reinterpret_cast<unsigned long long*>(smem + SM::OFF_MBAR);
 
   const int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5;
   const bool owner = wid < TY;
@@ -159,7 +188,17 @@ __global__ void __launch_bounds__(32 * (TY + 1), MINB) stage3d_kernel(const __gr
   int bad = 0;
   int ph = 0;                                     // phases this warp has completed (the same count in every warp)
   if (tid < 16) prog[tid] = 0;
+  if (tid == 0) mbar_init(hbar, 1);
+  asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
   __syncthreads();
+  // bulk copies need 16-byte aligned rows: an even padded row length (the arrays start 256-byte aligned and every
+  // variable, plane and tile starts at an even element); odd nx falls back to the eight-byte copies
+  // Used by the Hall variant only (its halo rows need their corners and are copied on H's critical path: 5.16 -> 5.04 ms
+  // per step at 256^3); the ideal-MHD kernel measured slower with them (31.3 -> 33.6 ms at 512^3, profiles/r2_stage3d.md).
+  constexpr bool BULK = HALL;
+  const bool bulk_ok = BULK && ((P.nxp & 1) == 0) && ((P.sq & 1) == 0);
+  uint32_t hpar = 0;                              // parity of the mbarrier phase H waits for next
+  bool hpend = false;                             // a bulk transfer is in flight
   const int ntile = P.ntx * P.nty;
   const int nround = ntile / (int)gridDim.x;
   const long long wtot = (long long)(ntile - nround * (int)gridDim.x) * P.nz;
@@ -216,14 +255,16 @@ __global__ void __launch_bounds__(32 * (TY + 1), MINB) stage3d_kernel(const __gr
   // Hall: also the x-halo corners (columns -1 and 32) of the four y-halo rows, for the transverse differences of J
   constexpr int NHC = (4 * TY + (HALL ? 8 : 0) + 31) / 32;
   auto hbuf_of = [](int p) { return 3 * PL + ((p + NHB) % NHB) * SB; };       // y-halo rows of plane p >= -2
-  auto h_cells = [&](int p, int slot, auto&& fn) {
+  auto h_cells = [&](int p, int slot, bool rows, auto&& fn) {
     const long long gp = (long long)(p + 2) * P.sz + x0;
     const bool xin = x0 + lane + 2 < P.nxp;
+    if (rows) {
 #pragma unroll
-    for (int r = 0; r < 4; ++r) {
-      const int j = (r < 2) ? r - 2 : TY + r - 2;
-      if (xin && y0 + j + 2 < P.nyp)
-        fn(hbuf_of(p) + r * RS + lane + 2, gp + (long long)(y0 + j + 2) * P.sy + lane + 2);
+      for (int r = 0; r < 4; ++r) {
+        const int j = (r < 2) ? r - 2 : TY + r - 2;
+        if (xin && y0 + j + 2 < P.nyp)
+          fn(hbuf_of(p) + r * RS + lane + 2, gp + (long long)(y0 + j + 2) * P.sy + lane + 2);
+      }
     }
 #pragma unroll
     for (int i = 0; i < NHC; ++i) {
@@ -231,14 +272,54 @@ __global__ void __launch_bounds__(32 * (TY + 1), MINB) stage3d_kernel(const __gr
       if (t < 4 * TY) {
         const int j = t >> 2, cc = t & 3, c = (cc < 2) ? cc : 32 + cc;
         if (x0 + c < P.nxp && y0 + j + 2 < P.nyp) fn(slot + j * RS + c, gp + (long long)(y0 + j + 2) * P.sy + c);
-      } else if (HALL && t < 4 * TY + 8) {
+      } else if (HALL && rows && t < 4 * TY + 8) {
         const int u = t - 4 * TY, r = u >> 1, c = (u & 1) ? 34 : 1, j = (r < 2) ? r - 2 : TY + r - 2;
         if (x0 + c < P.nxp && y0 + j + 2 < P.nyp) fn(hbuf_of(p) + r * RS + c, gp + (long long)(y0 + j + 2) * P.sy + c);
       }
     }
   };
-  auto h_copy = [&](int p, int slot) { h_cells(p, slot, [&](int off, long long g) { copy_cell(off, g); }); };
-  auto h_conv = [&](int p, int slot) { h_cells(p, slot, [&](int off, long long) { conv_in_place(off); }); };
+  // the four y-halo rows of plane p as bulk copies: lane = (row r, variable q), 4 x 8 = 32 (a ninth variable: second
+  // pass); each moves the row's 36 cells (fewer at the right end of the grid), x halo and corners included
+  auto h_rows_bulk = [&](int p) {
+    const long long gp = (long long)(p + 2) * P.sz + x0;
+    const int ncell = min(RS, P.nxp - x0) & ~1;
+    uint32_t total = 0;
+#pragma unroll
+    for (int pass = 0; pass < (NV + 7) / 8; ++pass) {
+      const int r = lane & 3, q = (lane >> 2) + 8 * pass, j = (r < 2) ? r - 2 : TY + r - 2;
+      const bool ok = q < NV && y0 + j + 2 < P.nyp && ncell > 0;
+      total += __reduce_add_sync(0xffffffffu, ok ? (uint32_t)ncell * 8u : 0u);
+    }
+    if (total == 0) return;
+    fence_proxy_async();
+    if (lane == 0) mbar_arrive_expect_tx(hbar, total);
+    __syncwarp();
+#pragma unroll
+    for (int pass = 0; pass < (NV + 7) / 8; ++pass) {
+      const int r = lane & 3, q = (lane >> 2) + 8 * pass, j = (r < 2) ? r - 2 : TY + r - 2;
+      if (q < NV && y0 + j + 2 < P.nyp && ncell > 0)
+        bulk_g2s(W + q * QS + hbuf_of(p) + r * RS, P.Uin + q * P.sq + gp + (long long)(y0 + j + 2) * P.sy, (uint32_t)ncell * 8u, hbar);
+    }
+    hpend = true;
+  };
+  // H: every copy it has issued has landed (eight-byte copies of this thread; the bulk transfer of the warp)
+  auto h_wait = [&]() {
+    cp_async_wait_all();
+    if (hpend) {
+      int spins = 0;
+      while (!mbar_test_wait(hbar, hpar)) {      // bounded like the hand-over waits: a lost transfer must not hang the GPU
+        __nanosleep(20);
+        if (++spins > (1 << 22)) { atomicOr(P.flag, 2); break; }
+      }
+      hpar ^= 1u;
+      hpend = false;
+    }
+  };
+  auto h_copy = [&](int p, int slot) {
+    if (bulk_ok) h_rows_bulk(p);
+    h_cells(p, slot, !bulk_ok, [&](int off, long long g) { copy_cell(off, g); });
+  };
+  auto h_conv = [&](int p, int slot) { h_cells(p, slot, true, [&](int off, long long) { conv_in_place(off); }); };
 
   // ---- prologue: everything step k0 needs that the steady state would have produced earlier ----
   for (int i = tid; i < NV * QS; i += NT) W[i] = 1.0;           // cells outside the padded array (ragged tiles)
@@ -266,9 +347,9 @@ __global__ void __launch_bounds__(32 * (TY + 1), MINB) stage3d_kernel(const __gr
     // plane k0+1 goes into the slot plane k0-2 just left (own cell only: no other thread touches it)
     if (own_in) copy_cell(slot_of(k0 + 1) + own_off, own_g + (long long)(k0 + 3) * P.sz);
   } else {
-    if (HALL) h_copy(k0 - 1, slot_of(k0 - 1));        // only its B is read (the current at face k0 - 1/2): no conversion
+    if (HALL) { h_copy(k0 - 1, slot_of(k0 - 1)); h_wait(); }   // only its B is read (current at face k0 - 1/2): no conversion
     h_copy(k0, slot_of(k0));
-    cp_async_wait_all();
+    h_wait();
     h_conv(k0, slot_of(k0));
     if (!HALL && k0 + 1 < k1) h_copy(k0 + 1, slot_of(k0 + 1));
   }
@@ -582,7 +663,7 @@ __global__ void __launch_bounds__(32 * (TY + 1), MINB) stage3d_kernel(const __gr
 #pragma unroll
             for (int r = 0; r < NV; ++r) XF[r * XS + lane] = F[r];
           }
-          if (HALL) cp_async_wait_all();       // plane k+1's halo cells have landed when this phase is published
+          if (HALL) h_wait();                  // plane k+1's halo cells have landed when this phase is published
         } else if (s == 1) {
           if (full) {
 #pragma unroll
@@ -590,7 +671,7 @@ __global__ void __launch_bounds__(32 * (TY + 1), MINB) stage3d_kernel(const __gr
           }
         } else {
           // A1 for the halo cells of plane k+1 (copies issued one phase B2 ago), then the copies for plane k+2
-          if (!HALL) cp_async_wait_all();
+          if (!HALL) h_wait();
           if (k + 1 < k1) h_conv(k + 1, sp);
           if (!HALL && k + 2 < k1) h_copy(k + 2, sm);
         }
@@ -599,7 +680,7 @@ __global__ void __launch_bounds__(32 * (TY + 1), MINB) stage3d_kernel(const __gr
     }
     { const int t = sm; sm = sc; sc = sp; sp = t; }
   }
-  cp_async_wait_all();
+  if (owner) cp_async_wait_all(); else h_wait();
   __syncthreads();                 // the next segment reuses the shared buffers
   }
   if (P.vnext != nullptr) {
