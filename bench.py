@@ -296,7 +296,7 @@ def run_ours(args):
     bytes_step = BYTES_PER_ZONE_STEP * (9.0 / 8.0 if cfg in (6, 7) else 1.0)
     hbm_frac = (bytes_step / 5.0 * 2.5 * zones / (stage_ms * 1e-3) / 1e9) / peaks["hbm_gbs"]
     roofline = {"bound": "alu", "achieved": achieved, "peak": fp64_peak, "unit": "TFLOP/s",
-                "frac": achieved / fp64_peak, "traffic": (NCU_TRAFFIC_BYTES.get(cfg) if (not args.n and csrc_sha() == NCU_TRAFFIC_CSRC_SHA) else None),
+                "frac": achieved / fp64_peak, "frac_of_nominal": achieved / FP64_NOMINAL_TFLOPS, "traffic": (NCU_TRAFFIC_BYTES.get(cfg) if (not args.n and csrc_sha() == NCU_TRAFFIC_CSRC_SHA) else None),
                 "traffic_source": f"ncu --set full capture of kernels with csrc sha {NCU_TRAFFIC_CSRC_SHA} (profiles/); "
                                   f"this run's csrc sha {csrc_sha()}",
                 "algorithmic_bytes": bytes_step / 2.0 * zones,
