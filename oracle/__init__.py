@@ -47,7 +47,7 @@ class Grid(C.Structure):
 class SolverCfg(C.Structure):
     _fields_ = [("riemann", C.c_int32), ("limiter", C.c_int32), ("beta", C.c_double),
                 ("rk", C.c_int32), ("cfl", C.c_double), ("d_i", C.c_double), ("relax", C.c_double),
-                ("bc", C.c_int32 * 3)]
+                ("bc", C.c_int32 * 3), ("cgl_form", C.c_int32)]
 
 
 _lib = None
@@ -76,6 +76,12 @@ def lib():
         L.agate_ref_cgl_cfast.restype = C.c_double
         L.agate_ref_cgl_face_flux.argtypes = [C.c_int, _dp, _dp, _dp]
         L.agate_ref_cgl_face_flux.restype = None
+        L.agate_ref_cgl_cons_to_prim_form.argtypes = [C.c_int, _dp, _dp]
+        L.agate_ref_cgl_cons_to_prim_form.restype = None
+        L.agate_ref_cgl_prim_to_cons_form.argtypes = [C.c_int, _dp, _dp]
+        L.agate_ref_cgl_prim_to_cons_form.restype = None
+        L.agate_ref_cgl_face_flux_form.argtypes = [C.c_int, C.c_int, _dp, _dp, _dp]
+        L.agate_ref_cgl_face_flux_form.restype = None
         L.agate_ref_cgl_relax.argtypes = [C.c_double, C.c_double, _dp, _dp]
         L.agate_ref_cgl_relax.restype = None
         L.agate_ref_nvar.argtypes = [vp]
@@ -163,23 +169,23 @@ def face_flux(riemann, d, gamma, WL, WR, eqset=IDEAL, d_i=0.0, dxmin=1.0, J=None
     return F
 
 
-def cgl_cons_to_prim(U):
+def cgl_cons_to_prim(U, form=0):
     u, pu = _vec(U, 9); W = np.empty(9)
-    lib().agate_ref_cgl_cons_to_prim(pu, W.ctypes.data_as(_dp)); return W
+    lib().agate_ref_cgl_cons_to_prim_form(int(form), pu, W.ctypes.data_as(_dp)); return W
 
 
-def cgl_prim_to_cons(W):
+def cgl_prim_to_cons(W, form=0):
     w, pw = _vec(W, 9); U = np.empty(9)
-    lib().agate_ref_cgl_prim_to_cons(pw, U.ctypes.data_as(_dp)); return U
+    lib().agate_ref_cgl_prim_to_cons_form(int(form), pw, U.ctypes.data_as(_dp)); return U
 
 
 def cgl_cfast(d, W):
     w, pw = _vec(W, 9); return float(lib().agate_ref_cgl_cfast(int(d), pw))
 
 
-def cgl_face_flux(d, WL, WR):
+def cgl_face_flux(d, WL, WR, form=0):
     wl, pl = _vec(WL, 9); wr, pr = _vec(WR, 9); F = np.empty(9)
-    lib().agate_ref_cgl_face_flux(int(d), pl, pr, F.ctypes.data_as(_dp)); return F
+    lib().agate_ref_cgl_face_flux_form(int(form), int(d), pl, pr, F.ctypes.data_as(_dp)); return F
 
 
 def cgl_relax(f, B2, ppar, pperp):
@@ -211,11 +217,12 @@ class RefSolver:
     """Host-memory solver with the same call shape as the product's C-ABI (agate_ref_* functions)."""
 
     def __init__(self, shape, dx, ndim, gamma=5.0 / 3.0, eqset=IDEAL, riemann=HLL, limiter=2, beta=1.3,
-                 rk=2, cfl=0.0, d_i=0.0, relax=0.0, bc=(0, 0, 0)):
+                 rk=2, cfl=0.0, d_i=0.0, relax=0.0, bc=(0, 0, 0), cgl_form=0):
         nx, ny, nz = (int(s) for s in shape)
         self.shape = (nx, ny, nz)
         self.grid = Grid(ndim, nx, ny, nz, dx[0], dx[1], dx[2])
-        self.cfg = SolverCfg(riemann, limiter, beta, rk, cfl, d_i, relax, (C.c_int32 * 3)(*[int(b) for b in bc]))
+        self.cfg = SolverCfg(riemann, limiter, beta, rk, cfl, d_i, relax, (C.c_int32 * 3)(*[int(b) for b in bc]),
+                             int(cgl_form))
         self.gamma, self.eqset = float(gamma), int(eqset)
         self._h = C.c_void_p()
         rc = lib().agate_ref_create(C.byref(self.grid), self.gamma, self.eqset, C.byref(self.cfg), C.byref(self._h))

@@ -281,29 +281,41 @@ int flux_hlld(int n, double gamma, const T WLin[8], const T WRin[8], T F[8]) {
 //                                     A_log = rho log[(rho^2/B^3)(p_perp/p_par)]      (eq.18)
 //   W = (rho, v, p_par, B, p_perp)    (p_par in slot 4, p_perp in slot 8)
 // ------------------------------------------------------------------------------------------------
-// eqs.26-27 (log form):  X = rho^2 exp(-A/rho);  p_par = 2 X e/(X + 2B^3),  p_perp = 2 B^3 e/(X + 2B^3)
-template <class T> void cgl_cons_to_prim(const T U[9], T W[9]) {
+// eqs.26-27 (log form, form = 0):  X = rho^2 exp(-A/rho);  p_par = 2 X e/(X + 2B^3),  p_perp = 2 B^3 e/(X + 2B^3)
+// eqs.24-25 (non-log form, form = 1; "AGATE supports both"):  p_par = 2 rho^3 e/(rho^3 + 2 A B^3),
+//                                                                    p_perp = 2 A B^3 e/(rho^3 + 2 A B^3)
+template <class T> void cgl_cons_to_prim(const T U[9], T W[9], int form = 0) {
   T rho = U[0];
   T vx = U[1] / rho, vy = U[2] / rho, vz = U[3] / rho;
   T v2 = vx * vx + vy * vy + vz * vz;
   T b2 = U[5] * U[5] + U[6] * U[6] + U[7] * U[7];
   T eint = U[4] - T(0.5) * rho * v2 - T(0.5) * b2;
   T B3 = b2 * tsqrt(b2);
+  W[0] = rho; W[1] = vx; W[2] = vy; W[3] = vz;
+  W[5] = U[5]; W[6] = U[6]; W[7] = U[7];
+  if (form == 1) {
+    T r3 = rho * rho * rho;
+    T AB = U[8] * B3;
+    T den = r3 + T(2.0) * AB;
+    W[4] = T(2.0) * r3 * eint / den;                  // eq.24
+    W[8] = T(2.0) * AB * eint / den;                  // eq.25
+    return;
+  }
   T X = rho * rho * texp(-U[8] / rho);
   T den = X + T(2.0) * B3;
-  W[0] = rho; W[1] = vx; W[2] = vy; W[3] = vz;
   W[4] = T(2.0) * X * eint / den;
-  W[5] = U[5]; W[6] = U[6]; W[7] = U[7];
   W[8] = T(2.0) * B3 * eint / den;
 }
-template <class T> void cgl_prim_to_cons(const T W[9], T U[9]) {
+// E of P:L166 and the thermodynamic variable: eq.18 (form 0) or eq.16 (form 1)
+template <class T> void cgl_prim_to_cons(const T W[9], T U[9], int form = 0) {
   T rho = W[0];
   T v2 = W[1] * W[1] + W[2] * W[2] + W[3] * W[3];
   T b2 = W[5] * W[5] + W[6] * W[6] + W[7] * W[7];
   U[0] = rho; U[1] = rho * W[1]; U[2] = rho * W[2]; U[3] = rho * W[3];
   U[4] = T(0.5) * rho * v2 + T(0.5) * b2 + T(0.5) * W[4] + W[8];
   U[5] = W[5]; U[6] = W[6]; U[7] = W[7];
-  U[8] = rho * tlog((rho * rho / (b2 * tsqrt(b2))) * (W[8] / W[4]));
+  if (form == 1) U[8] = (rho * rho * rho / (b2 * tsqrt(b2))) * (W[8] / W[4]);       // eq.16
+  else U[8] = rho * tlog((rho * rho / (b2 * tsqrt(b2))) * (W[8] / W[4]));             // eq.18
 }
 // eq.29, fast (+) branch, along direction d:  c^2 = (b1 + sqrt(b2^2 + c)) / (2 rho)
 template <class T> T cgl_cfast(int d, const T W[9]) {
@@ -330,9 +342,9 @@ template <class T> void cgl_phys_flux(int n, const T W[9], const T U[9], T F[9])
   F[8] = U[8] * vn;
 }
 // HLL eq.5 with the Davis speeds eq.6 and c = eq.29's fast speed; all nine components through eq.5
-template <class T> void cgl_flux_hll(int n, const T WL[9], const T WR[9], T F[9]) {
+template <class T> void cgl_flux_hll(int n, const T WL[9], const T WR[9], T F[9], int form = 0) {
   T UL[9], UR[9], fL[9], fR[9];
-  cgl_prim_to_cons(WL, UL); cgl_prim_to_cons(WR, UR);
+  cgl_prim_to_cons(WL, UL, form); cgl_prim_to_cons(WR, UR, form);
   cgl_phys_flux(n, WL, UL, fL); cgl_phys_flux(n, WR, UR, fR);
   T cl = cgl_cfast(n, WL), cr = cgl_cfast(n, WR);
   T sL = tmin(tmin(WL[1 + n] - cl, WR[1 + n] - cr), T(0.0));
@@ -443,7 +455,7 @@ template <class T> struct Solver {
       if (cgl) {
         T u9[9], w9[9];
         for (int q = 0; q < 9; ++q) u9[q] = U[q * ntot + c];
-        cgl_cons_to_prim(u9, w9);
+        cgl_cons_to_prim(u9, w9, s.cgl_form);
         for (int q = 0; q < 9; ++q) W[q * ntot + c] = w9[q];
         continue;
       }
@@ -499,7 +511,7 @@ template <class T> struct Solver {
           }
           if (hall) face_current(d, base + c * sd, J);
           if (cgl) {
-            cgl_flux_hll<T>(d, WL, WR, Ff);
+            cgl_flux_hll<T>(d, WL, WR, Ff, s.cgl_form);
           } else if (glm) {
             // eqs.10-11 (R22): (B_n, psi) decouple into a 2x2 linear system with speeds -+c_h; its Riemann
             // solution gives the single-valued face values, the MHD solver sees B_n* on both sides, and the two
@@ -543,7 +555,7 @@ template <class T> struct Solver {
           for (int q = 0; q < nv; ++q) u[q] = Un[q * ntot + c];
           if (cgl) {
             // eq.28: |v| + max_d c_cgl,d
-            cgl_cons_to_prim(u, w);
+            cgl_cons_to_prim(u, w, s.cgl_form);
             if (!(val(w[0]) > 0.0) || !(val(w[4]) > 0.0) || !(val(w[8]) > 0.0)) { bad = true; continue; }
             T cm = tmax(tmax(cgl_cfast(0, w), cgl_cfast(1, w)), cgl_cfast(2, w));
             T spc = tsqrt(w[1] * w[1] + w[2] * w[2] + w[3] * w[3]) + cm;
@@ -588,12 +600,13 @@ template <class T> struct Solver {
       const ptrdiff_t c = pidx(i, j, k);
       T u[9], w[9];
       for (int q = 0; q < 9; ++q) u[q] = Un[q * ntot + c];
-      cgl_cons_to_prim(u, w);
+      cgl_cons_to_prim(u, w, s.cgl_form);
       double ppar = val(w[4]), pperp = val(w[8]);
       const double B2 = val(w[5] * w[5] + w[6] * w[6] + w[7] * w[7]);
       cgl_relax(s.relax, B2, &ppar, &pperp);
       const double rho = val(w[0]);
-      Un[8 * ntot + c] = T(rho * std::log((rho * rho / (B2 * std::sqrt(B2))) * (pperp / ppar)));
+      if (s.cgl_form == 1) Un[8 * ntot + c] = T((rho * rho * rho / (B2 * std::sqrt(B2))) * (pperp / ppar));   // eq.16
+      else Un[8 * ntot + c] = T(rho * std::log((rho * rho / (B2 * std::sqrt(B2))) * (pperp / ppar)));
     }
   }
   // Uout = a0 Uref + a1 (Uin + c dt L)  on the interior, L = L(Uin) as left by rhs()
@@ -711,6 +724,7 @@ int check_args(const agate_ref_grid* g, double gamma, int eqset, const agate_ref
   if (eqset != AGATE_REF_IDEAL && eqset != AGATE_REF_HALL && eqset != AGATE_REF_IDEAL_GLM && eqset != AGATE_REF_CGL) return 1;
   if (eqset == AGATE_REF_CGL && s->riemann != 0) return 1;          // the paper's CGL runs use HLL
   if (eqset == AGATE_REF_CGL && !(s->relax >= 0.0 && s->relax <= 1.0)) return 1;
+  if (s->cgl_form < 0 || s->cgl_form > 1) return 1;
   if (s->riemann < 0 || s->riemann > 1 || s->limiter < 0 || s->limiter > 2 || s->rk < 1 || s->rk > 5) return 1;
   if (s->limiter == 2 && !(s->beta >= 1.0 && s->beta <= 2.0)) return 1;
   for (int d = 0; d < 3; ++d) if (s->bc[d] < 0 || s->bc[d] > ((d == 1) ? 2 : 1)) return 1;
@@ -802,6 +816,9 @@ int agate_ref_rhs(agate_ref_ctx* c, double* Lout) {
 }
 void agate_ref_cgl_cons_to_prim(const double U[9], double W[9]) { cgl_cons_to_prim<double>(U, W); }
 void agate_ref_cgl_prim_to_cons(const double W[9], double U[9]) { cgl_prim_to_cons<double>(W, U); }
+void agate_ref_cgl_cons_to_prim_form(int form, const double U[9], double W[9]) { cgl_cons_to_prim<double>(U, W, form); }
+void agate_ref_cgl_prim_to_cons_form(int form, const double W[9], double U[9]) { cgl_prim_to_cons<double>(W, U, form); }
+void agate_ref_cgl_face_flux_form(int form, int dir, const double WL[9], const double WR[9], double F[9]) { cgl_flux_hll<double>(dir, WL, WR, F, form); }
 double agate_ref_cgl_cfast(int dir, const double W[9]) { return cgl_cfast<double>(dir, W); }
 void agate_ref_cgl_face_flux(int dir, const double WL[9], const double WR[9], double F[9]) { cgl_flux_hll<double>(dir, WL, WR, F); }
 void agate_ref_cgl_relax(double f, double B2, double* ppar, double* pperp) { cgl_relax(f, B2, ppar, pperp); }

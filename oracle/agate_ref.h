@@ -37,6 +37,7 @@ typedef struct {
   double  relax;         /* CGL: dt/(dt+tau) of eqs.32-33 (paper default 0.99, L254); 0 = no relaxation */
   int32_t bc[3];         /* per dimension: 0 periodic, 1 zero-gradient (open end, L314: ghost = nearest interior zone);
                             bc[1] = 2: sheared zero-gradient ends in y (L314, R28), x periodic */
+  int32_t cgl_form;      /* CGL: 0 = logarithmic A of eq.18 (eqs.26-27; the paper's preferred form), 1 = A of eq.16 (eqs.24-25) */
 } agate_ref_solver;
 
 enum { AGATE_REF_IDEAL = 0, AGATE_REF_HALL = 1, AGATE_REF_CGL = 2, AGATE_REF_IDEAL_GLM = 3 };
@@ -61,6 +62,9 @@ void   agate_ref_cgl_prim_to_cons(const double W[9], double U[9]);              
 double agate_ref_cgl_cfast(int dir, const double W[9]);                                 /* eq.29 (+) */
 void   agate_ref_cgl_face_flux(int dir, const double WL[9], const double WR[9], double F[9]);
 void   agate_ref_cgl_relax(double f, double B2, double* p_par, double* p_perp);         /* eqs.31-33 */
+void   agate_ref_cgl_cons_to_prim_form(int form, const double U[9], double W[9]);       /* form 1: eqs.24-25 */
+void   agate_ref_cgl_prim_to_cons_form(int form, const double W[9], double U[9]);       /* form 1: eq.16 */
+void   agate_ref_cgl_face_flux_form(int form, int dir, const double WL[9], const double WR[9], double F[9]);
 int agate_ref_nvar(agate_ref_ctx*);                                       /* 8, or 9 with GLM          */
 int agate_ref_glm_ch(agate_ref_ctx*, double* ch_out);                     /* c_h of the last step / rhs */
 void agate_ref_glm_face(double ch, double bnL, double bnR, double psL, double psR, double* bn_star, double* psi_star);

@@ -204,3 +204,92 @@ def test_c9_uniform_state_is_fixed_and_hll_rejected_for_hlld():
     assert np.array_equal(s.get_state(), U)
     with pytest.raises(oracle.RefError):
         oracle.RefSolver(shape=(8, 1, 1), dx=(0.1, 1, 1), ndim=1, eqset=oracle.CGL, riemann=oracle.HLLD)
+
+
+# ------------------------------------------------------------------------------------------------
+# C11: the non-logarithmic thermodynamic variable (eq.16, eqs.24-25; "AGATE supports both")
+# ------------------------------------------------------------------------------------------------
+def test_c11_nonlog_variable_change_by_hand():
+    """rho = 2, |B| = 3, p_par = 1, p_perp = 3:  A = (rho/B)^3 p_perp/p_par = (8/27) 3 = 8/9  (eq.16);
+    E = rho v^2/2 + B^2/2 + p_par/2 + p_perp = 0.25 + 4.5 + 0.5 + 3 = 8.25.  Back through eqs.24-25: e_int = 3.5,
+    rho^3 + 2 A B^3 = 8 + 2 (8/9) 27 = 56, p_par = 2 * 8 * 3.5 / 56 = 1, p_perp = 2 * 24 * 3.5 / 56 = 3."""
+    W = np.array([2.0, 0.5, 0.0, 0.0, 1.0, 1.0, 2.0, 2.0, 3.0])
+    U = oracle.cgl_prim_to_cons(W, form=1)
+    assert abs(U[8] - 8.0 / 9.0) <= 1e-15 and abs(U[4] - 8.25) <= 1e-15
+    assert np.allclose(U[:4], [2.0, 1.0, 0.0, 0.0]) and np.array_equal(U[5:8], W[5:8])
+    back = oracle.cgl_cons_to_prim(U, form=1)
+    assert np.max(np.abs(back - W)) <= 4e-15
+    # the two forms describe the same state: A_log = rho ln(A / rho)  (eq.18 against eq.16)
+    Ulog = oracle.cgl_prim_to_cons(W, form=0)
+    assert abs(Ulog[8] - 2.0 * np.log((8.0 / 9.0) / 2.0)) <= 1e-15
+    rng = np.random.default_rng(5)
+    for _ in range(200):
+        W = np.concatenate([[0.5 + rng.random()], rng.uniform(-1, 1, 3), [0.2 + rng.random()], rng.uniform(-1, 1, 3),
+                            [0.2 + rng.random()]])
+        U1 = oracle.cgl_prim_to_cons(W, form=1)
+        assert np.max(np.abs(oracle.cgl_cons_to_prim(U1, form=1) - W)) <= 1e-13
+        assert np.array_equal(U1[:8], oracle.cgl_prim_to_cons(W, form=0)[:8])
+
+
+@pytest.mark.parametrize("d", [0, 1, 2])
+def test_c11_nonlog_flux_carries_A_with_the_flow(d):
+    """Identical states: the HLL flux is the physical flux, whose ninth component is A v_n with A of eq.16 (eq.17);
+    the other eight do not depend on the form."""
+    W = np.array([1.3, 0.3, -0.2, 0.4, 0.7, 0.5, -0.3, 0.6, 1.1])
+    F1 = oracle.cgl_face_flux(d, W, W, form=1)
+    F0 = oracle.cgl_face_flux(d, W, W, form=0)
+    A = (W[0] ** 3 / (W[5] ** 2 + W[6] ** 2 + W[7] ** 2) ** 1.5) * (W[8] / W[4])
+    assert abs(F1[8] - A * W[1 + d]) <= 1e-15 * max(1.0, abs(F1[8]))
+    assert np.max(np.abs(F1[:8] - F0[:8])) <= 1e-15
+
+
+@pytest.mark.parametrize("ap", [0.5, 2.0])
+def test_c11_nonlog_standing_wave_period(ap):
+    """The paper's standing wave (C4) with the variable of eq.16: the same period 1 / sqrt(B^2 + 2 p_perp)."""
+    n = 256
+    x = -1 + (np.arange(n) + 0.5) * 2 / n
+    ppar = 1.5 / (1 + 2 * ap)
+    pperp = ap * ppar
+    W = np.zeros((9, n)); W[0] = 1; W[6] = 1; W[4] = ppar; W[8] = pperp; W[1] = 0.01 * np.sin(2 * np.pi * x)
+    s = solver_1d(n, 2.0, cgl_form=1)
+    U = np.stack([oracle.cgl_prim_to_cons(W[:, i], form=1) for i in range(n)], axis=1)
+    s.set_state(U.reshape(9, 1, 1, n))
+    tau = 1.0 / np.sqrt(1 + 2 * pperp)
+    proj = lambda: float(np.sum((s.get_state()[1] / s.get_state()[0]).ravel() * np.sin(2 * np.pi * x)))
+    a0 = proj()
+    run_to(s, tau / 2); a1 = proj()
+    run_to(s, tau / 2); a2 = proj()
+    assert -1.0 <= a1 / a0 <= -0.995
+    assert 0.995 <= a2 / a0 <= 1.0
+
+
+def test_c11_nonlog_relaxation_and_conservation():
+    """Grid level, form 1: the eight flux-form sums are conserved with and without relaxation, the relaxed state sits
+    inside the three bounds, and the stored A is eq.16 of the relaxed pressures."""
+    n = 16
+    Ulog = _state2d(n, 3)
+    U = np.empty_like(Ulog)
+    for j in range(n):
+        for i in range(n):
+            U[:, 0, j, i] = oracle.cgl_prim_to_cons(oracle.cgl_cons_to_prim(Ulog[:, 0, j, i]), form=1)
+    out = {}
+    for f in (0.0, 1.0):
+        s = oracle.RefSolver(shape=(n, n, 1), dx=(1 / n, 1 / n, 1), ndim=2, eqset=oracle.CGL, riemann=oracle.HLL, beta=1.3,
+                             relax=f, cgl_form=1)
+        s.set_state(U)
+        s.advance(4)
+        out[f] = s.get_state()
+        s0, s1 = U.reshape(9, -1).sum(axis=1), out[f].reshape(9, -1).sum(axis=1)
+        scale = np.abs(out[f]).reshape(9, -1).sum(axis=1)
+        nq = 9 if f == 0.0 else 8
+        assert np.all(np.abs(s1[:nq] - s0[:nq]) <= 1e-13 * scale[:nq])
+    for j in range(n):
+        for i in range(n):
+            w = oracle.cgl_cons_to_prim(out[1.0][:, 0, j, i], form=1)
+            B2 = w[5] ** 2 + w[6] ** 2 + w[7] ** 2
+            dP = w[8] - w[4]
+            tol = 1e-12 * (w[4] + w[8])
+            assert -B2 - tol <= dP <= min((w[4] / w[8]) * B2 / 2, 0.3 * w[4] * np.sqrt(B2 / (2 * w[4]))) + tol
+            assert abs(out[1.0][8, 0, j, i] - (w[0] ** 3 / B2 ** 1.5) * (w[8] / w[4])) <= 1e-12 * out[1.0][8, 0, j, i]
+    with pytest.raises(oracle.RefError):
+        oracle.RefSolver(shape=(8, 8, 1), dx=(1, 1, 1), ndim=2, eqset=oracle.CGL, cgl_form=2)
