@@ -87,6 +87,8 @@ def parse():
                     help="NEXT-4: slab domain decomposition along the last active dimension instead of replicas: every "
                          "rank holds one full-size slab of a domain N times as long (weak scaling), halo exchange per "
                          "stage, one all-reduce(max) per step; at N = 1 the slab is its own periodic neighbour")
+    ap.add_argument("--cgl-form", type=int, default=0, choices=[0, 1],
+                    help="config 7: 0 = logarithmic A of eq.18 (the paper's preferred form), 1 = A of eq.16 (eqs.24-25)")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu", action="store_true")
     return ap.parse_args()
@@ -258,11 +260,19 @@ def run_ours(args):
     cfg = args.config
     wl = make_workload(cfg, n=args.n or None)
     zones = wl.zones
+    over = {}
+    if cfg == 7 and args.cgl_form == 1:
+        # input definition of the other thermodynamic variable (eq.16): A = (rho / |B|)^3 p_perp / p_par
+        W = wl.W
+        b2 = W[5] ** 2 + W[6] ** 2 + W[7] ** 2
+        wl.U[8] = (W[0] ** 3 / (b2 * np.sqrt(b2))) * (W[8] / W[4])
+        wl.name += " (A of eq.16)"
+        over["cgl_form"] = 1
     wl.W = None                                       # only U is needed; frees one state-sized host array
     K, Wm = args.steps, args.warmup
     if args.decomp:
         return run_decomp(args, ag, wl, world, rank, local, dev, barrier)
-    sim = ag.Agate.from_workload(wl, device=dev, set_state=False)
+    sim = ag.Agate.from_workload(wl, device=dev, set_state=False, **over)
     Uh = torch.from_numpy(wl.U).pin_memory()
     info = sim.launch_info()
     fp64_peak = ag.measure_fp64_peak(10)

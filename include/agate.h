@@ -58,6 +58,8 @@ typedef struct {
                            open end (R26: ghost = nearest interior zone); bc[1] = 2: the sheared
                            zero-gradient ends of the 2-D whistler test (R28: ghost (i,j) = zone (i-1,j+2)
                            at the down side, (i+1,j-2) at the up side, x periodic: needs bc[0] = 0, ndim >= 2) */
+  int32_t cgl_form;     /* eqset AGATE_CGL only: 0 = the logarithmic variable A_log of eq.18 (eqs.26-27; the paper's
+                           preferred form), 1 = A of eq.16 (eqs.24-25; "AGATE supports both"): U[8] is A      */
 } agate_solver;
 
 enum { AGATE_IDEAL = 0, AGATE_HALL = 1, AGATE_CGL = 2, AGATE_IDEAL_GLM = 3 };

@@ -44,7 +44,7 @@ class Grid(C.Structure):
 class SolverCfg(C.Structure):
     _fields_ = [("riemann", C.c_int32), ("limiter", C.c_int32), ("beta", C.c_double),
                 ("rk", C.c_int32), ("cfl", C.c_double), ("d_i", C.c_double), ("relax", C.c_double),
-                ("bc", C.c_int32 * 3)]
+                ("bc", C.c_int32 * 3), ("cgl_form", C.c_int32)]
 
 
 class Tuning(C.Structure):
@@ -116,14 +116,16 @@ class Agate:
     """One simulation context (agate_ctx) on a dedicated CUDA stream.  Names follow include/agate.h."""
 
     def __init__(self, shape, dx, ndim, gamma=5.0 / 3.0, eqset=IDEAL, riemann=HLL, limiter=2, beta=1.3, rk=2,
-                 cfl=0.0, d_i=0.0, relax=0.0, bc=(0, 0, 0), device="cuda:0", stream=None, stage_grid=0, no_graph=False):
+                 cfl=0.0, d_i=0.0, relax=0.0, bc=(0, 0, 0), device="cuda:0", stream=None, stage_grid=0, no_graph=False,
+                 cgl_form=0):
         torch = _torch_cuda()
         nx, ny, nz = (int(s) for s in shape)
         self.shape = (nx, ny, nz)
         self.zones = nx * ny * nz
         self.nvar = 9 if int(eqset) in (IDEAL_GLM, CGL) else 8
         self.grid = Grid(ndim, nx, ny, nz, dx[0], dx[1], dx[2])
-        self.cfg = SolverCfg(riemann, limiter, beta, rk, cfl, d_i, relax, (C.c_int32 * 3)(*[int(b) for b in bc]))
+        self.cfg = SolverCfg(riemann, limiter, beta, rk, cfl, d_i, relax, (C.c_int32 * 3)(*[int(b) for b in bc]),
+                             int(cgl_form))
         self.device = torch.device(device)
         L = lib()
         nbytes = L.agate_workspace_bytes(C.byref(self.grid), eqset, C.byref(self.cfg))

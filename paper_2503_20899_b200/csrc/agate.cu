@@ -77,6 +77,7 @@ int check_args(const agate_grid* g, double gamma, int eqset, const agate_solver*
   if (eqset != AGATE_IDEAL && eqset != AGATE_HALL && eqset != AGATE_IDEAL_GLM && eqset != AGATE_CGL) return AGATE_ERR_ARG;
   if (eqset == AGATE_CGL && s->riemann != AGATE_HLL) return AGATE_ERR_ARG;    // CGL: HLL (the paper names no other solver)
   if (eqset == AGATE_CGL && !(s->relax >= 0.0 && s->relax <= 1.0)) return AGATE_ERR_ARG;
+  if (s->cgl_form < 0 || s->cgl_form > 1) return AGATE_ERR_ARG;
   if (s->riemann < 0 || s->riemann > 1 || s->limiter < 0 || s->limiter > 2 || s->rk < 1 || s->rk > 5) return AGATE_ERR_ARG;
   if (s->limiter == 2 && !(s->beta >= 1.0 && s->beta <= 2.0)) return AGATE_ERR_ARG;
   for (int d = 0; d < 3; ++d) if (s->bc[d] < 0 || s->bc[d] > ((d == 1) ? 2 : 1)) return AGATE_ERR_ARG;
@@ -500,6 +501,7 @@ int agate_init(const agate_grid* grid, double gamma, int eqset, const agate_solv
   c->cfl = solver->cfl;
   if (!(c->cfl > 0.0)) c->cfl = (user_grid.ndim == 1) ? 0.8 : (user_grid.ndim == 2 ? 0.45 : 0.325);
   c->ph = make_phys(gamma, (eqset == AGATE_HALL) ? solver->d_i : 0.0, c->dxmin);
+  c->ph.cgl_form = (eqset == AGATE_CGL) ? solver->cgl_form : 0;
   c->stream = (cudaStream_t)stream;
   c->ws = (char*)workspace;
   c->UA = (double*)(c->ws + L.off_A);

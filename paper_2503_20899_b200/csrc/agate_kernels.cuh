@@ -434,7 +434,7 @@ __global__ void __launch_bounds__(256) dt_kernel(const __grid_constant__ DtParam
       u[8] = P.cgl ? __ldg(P.U + 8 * P.sq + base + i) : 0.0;
       // the same straight-line function the fused stage epilogue uses, so that a stand-alone reduction and the
       // fused one give the same dt bit for bit
-      const double sp = P.cgl ? cell_speed_cgl(u) : cell_speed_inline<HALL>(P.ph, u);
+      const double sp = P.cgl ? cell_speed_cgl(u, P.ph.cgl_form) : cell_speed_inline<HALL>(P.ph, u);
       if (sp < 0.0) bad = 1; else vm = fmax(vm, sp);
     }
   }

@@ -40,6 +40,7 @@ struct Phys {
   double hgamma;  // gamma / 2
   double d_i;     // Hall: normalised ion inertial length
   double cwk;     // Hall: d_i * pi / (2 dx_min)   (eq.13 with k_max = pi / dx_min, R15)
+  int cgl_form;   // CGL: 0 = logarithmic A of eq.18 (eqs.26-27), 1 = A of eq.16 (eqs.24-25)
 };
 
 AG_HD Phys make_phys(double gamma, double d_i, double dxmin) {
@@ -51,6 +52,7 @@ AG_HD Phys make_phys(double gamma, double d_i, double dxmin) {
   ph.hgamma = 0.5 * gamma;
   ph.d_i = d_i;
   ph.cwk = d_i * 3.14159265358979323846264338327950288 / (2.0 * dxmin);
+  ph.cgl_form = 0;
   return ph;
 }
 
@@ -620,21 +622,25 @@ AG_HD double cell_speed(const Phys& ph, const double U[8]) {
 //   W = (rho, v, p_par, B, p_perp): p_par in slot 4, p_perp in slot 8 (slot 8 is not rotated)
 // Reciprocals and roots as in the ideal path (MUFU seed + Newton, a few ulp); exp / log from the CUDA math library.
 // ------------------------------------------------------------------------------------------------------------
-AG_HD void cgl_cons_to_prim(const double U[9], double W[9]) {          // eqs.26-27
+AG_HD void cgl_cons_to_prim(const double U[9], double W[9], int form = 0) {   // eqs.26-27 (form 0), eqs.24-25 (form 1)
   const double ir = rcp(U[0]);
   const double vx = U[1] * ir, vy = U[2] * ir, vz = U[3] * ir;
   const double b2 = U[5] * U[5] + U[6] * U[6] + U[7] * U[7];
   const double eint = U[4] - 0.5 * U[0] * (vx * vx + vy * vy + vz * vz) - 0.5 * b2;
   const double B3 = b2 * sqrt_pos(dmax(b2, kTiny));
-  const double X = U[0] * U[0] * exp(-U[8] * ir);
-  const double iden = rcp(X + 2.0 * B3);
+  // X : Y = p_par : p_perp;  form 0: rho^2 exp(-A_log / rho) : B^3,  form 1: rho^3 : A B^3   (no exp, no log)
+  const double X = (form == 1) ? U[0] * U[0] * U[0] : U[0] * U[0] * exp(-U[8] * ir);
+  const double Y = (form == 1) ? U[8] * B3 : B3;
+  const double iden = rcp(X + 2.0 * Y);
   W[0] = U[0]; W[1] = vx; W[2] = vy; W[3] = vz;
   W[4] = 2.0 * X * eint * iden;
   W[5] = U[5]; W[6] = U[6]; W[7] = U[7];
-  W[8] = 2.0 * B3 * eint * iden;
+  W[8] = 2.0 * Y * eint * iden;
 }
-AG_HD double cgl_alog(double rho, double b2, double ppar, double pperp) {   // eq.18
-  return rho * log((rho * rho * pperp) * rcp(b2 * sqrt_pos(dmax(b2, kTiny)) * ppar));
+// the thermodynamic variable of a primitive state: eq.18 (form 0) or eq.16 (form 1)
+AG_HD double cgl_alog(double rho, double b2, double ppar, double pperp, int form = 0) {
+  const double ratio = (rho * rho * pperp) * rcp(b2 * sqrt_pos(dmax(b2, kTiny)) * ppar);     // (rho^2 / B^3) (p_perp / p_par)
+  return (form == 1) ? rho * ratio : rho * log(ratio);
 }
 // eq.29, fast branch, along the face normal of a ROTATED state (w[5] = B_n)
 AG_HD double cgl_cfast(const double w[9]) {
@@ -646,7 +652,7 @@ AG_HD double cgl_cfast(const double w[9]) {
   return sqrt_pos((b1 + sqrt_pos(dmax(b2 * b2 + c, kTiny))) * (0.5 * rcp(w[0])));
 }
 // eqs.19-22 (psi == 0) + eq.17 in the rotated frame; also returns the conserved vector of the state
-AG_HD void cgl_flux_and_cons(const double w[9], double f[9], double u[9]) {
+AG_HD void cgl_flux_and_cons(const double w[9], double f[9], double u[9], int form = 0) {
   const double B2 = w[5] * w[5] + w[6] * w[6] + w[7] * w[7];
   const double th = 1.0 - (w[4] - w[8]) * rcp(B2);
   const double v2 = w[1] * w[1] + w[2] * w[2] + w[3] * w[3];
@@ -654,7 +660,7 @@ AG_HD void cgl_flux_and_cons(const double w[9], double f[9], double u[9]) {
   u[0] = w[0]; u[1] = w[0] * w[1]; u[2] = w[0] * w[2]; u[3] = w[0] * w[3];
   u[4] = 0.5 * w[0] * v2 + 0.5 * B2 + 0.5 * w[4] + w[8];
   u[5] = w[5]; u[6] = w[6]; u[7] = w[7];
-  u[8] = cgl_alog(w[0], B2, w[4], w[8]);
+  u[8] = cgl_alog(w[0], B2, w[4], w[8], form);
   f[0] = w[0] * w[1];
   f[1] = w[0] * w[1] * w[1] - th * w[5] * w[5] + (w[8] + 0.5 * B2);
   f[2] = w[0] * w[2] * w[1] - th * w[6] * w[5];
@@ -666,10 +672,10 @@ AG_HD void cgl_flux_and_cons(const double w[9], double f[9], double u[9]) {
   f[8] = u[8] * w[1];
 }
 // HLL eq.5 with the Davis speeds eq.6 and eq.29's fast speed; all nine components through eq.5 (R9)
-AG_HD void flux_hll_cgl(const double L[9], const double R[9], double F[9]) {
+AG_HD void flux_hll_cgl(const double L[9], const double R[9], double F[9], int form = 0) {
   double fl[9], fr[9], ul[9], ur[9];
-  cgl_flux_and_cons(L, fl, ul);
-  cgl_flux_and_cons(R, fr, ur);
+  cgl_flux_and_cons(L, fl, ul, form);
+  cgl_flux_and_cons(R, fr, ur, form);
   const double cl = cgl_cfast(L), cr = cgl_cfast(R);
   const double sL = dmin(dmin(L[1] - cl, R[1] - cr), 0.0);
   const double sR = dmax(dmax(L[1] + cl, R[1] + cr), 0.0);
@@ -678,9 +684,9 @@ AG_HD void flux_hll_cgl(const double L[9], const double R[9], double F[9]) {
   for (int q = 0; q < 9; ++q) F[q] = (sR * fl[q] - sL * fr[q] + sL * sR * (ur[q] - ul[q])) * iw;
 }
 // eqs.31-33 on a conserved cell: relax the anisotropy, keep E, return the new A_log (C1 = 0.3, C2 = 0.5)
-AG_HD double cgl_relaxed_alog(double f, const double U[9]) {
+AG_HD double cgl_relaxed_alog(double f, const double U[9], int form = 0) {
   double w[9];
-  cgl_cons_to_prim(U, w);
+  cgl_cons_to_prim(U, w, form);
   const double B2 = w[5] * w[5] + w[6] * w[6] + w[7] * w[7];
   const double dP = w[8] - w[4];
   const double mirror = (w[4] * rcp(w[8])) * (0.5 * B2);
@@ -688,12 +694,12 @@ AG_HD double cgl_relaxed_alog(double f, const double U[9]) {
   const double dPs = dmax(-B2, dmin(dP, dmin(mirror, ic)));
   const double ppar = w[4] - (2.0 / 3.0) * (dPs - dP) * f;
   const double pperp = w[8] + (1.0 / 3.0) * (dPs - dP) * f;
-  return cgl_alog(w[0], B2, ppar, pperp);
+  return cgl_alog(w[0], B2, ppar, pperp, form);
 }
 // eq.28 per cell: |v| + max_d c_cgl,d; negative for an unphysical cell
-AG_HD double cell_speed_cgl(const double U[9]) {
+AG_HD double cell_speed_cgl(const double U[9], int form = 0) {
   double w[9], r[9];
-  cgl_cons_to_prim(U, w);
+  cgl_cons_to_prim(U, w, form);
   if (!(w[0] > 0.0) || !(w[4] > 0.0) || !(w[8] > 0.0)) return -1.0;
   double cm = 0.0;
   for (int d = 0; d < 3; ++d) {

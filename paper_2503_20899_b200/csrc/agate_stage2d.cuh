@@ -99,7 +99,7 @@ __global__ void __launch_bounds__(32 * Stage2dSmem<GLM || CGL>::NW, 2) stage2d_k
       double u[9], w[9];
 #pragma unroll
       for (int q = 0; q < 9; ++q) u[q] = ring[off + q * RW2];
-      cgl_cons_to_prim(u, w);
+      cgl_cons_to_prim(u, w, P.ph.cgl_form);
 #pragma unroll
       for (int q = 0; q < 9; ++q) ring[off + q * RW2] = w[q];
     } else {
@@ -232,7 +232,7 @@ __global__ void __launch_bounds__(32 * Stage2dSmem<GLM || CGL>::NW, 2) stage2d_k
         pss = 0.5 * (L[NV - 1] + R[NV - 1]) - 0.5 * ch * (R[5] - L[5]);
         L[5] = bns; R[5] = bns;
       }
-      if (CGL) flux_hll_cgl(L, R, F);
+      if (CGL) flux_hll_cgl(L, R, F, P.ph.cgl_form);
       else riemann_flux<RIEMANN, HALL>(P.ph, L, R, HALL ? Jr : nullptr, F);
       if (GLM) { F[5] = pss; F[NV - 1] = ch * ch * bns; }
       {
@@ -247,7 +247,7 @@ __global__ void __launch_bounds__(32 * Stage2dSmem<GLM || CGL>::NW, 2) stage2d_k
           o[v] = c0 * (acc[v] - cy * (F[r] - FyL[v * 32 + lane]));
           if (GLM && v == NV - 1) o[v] *= decay;                          // eq.11's source, integrated exactly
           if (CGL && v == NV - 1 && P.last_stage && P.relax > 0.0 && emit && cell_ok)
-            o[v] = cgl_relaxed_alog(P.relax, o);                          // eqs.31-33: E stays, A_log moves
+            o[v] = cgl_relaxed_alog(P.relax, o, P.ph.cgl_form);                          // eqs.31-33: E stays, A_log moves
           if (emit && cell_ok) *po = o[v];
           FyL[v * 32 + lane] = F[r];
           acc[v] = Uraw[((j & 1) * NV + v) * 32 + lane];
@@ -286,7 +286,7 @@ __global__ void __launch_bounds__(32 * Stage2dSmem<GLM || CGL>::NW, 2) stage2d_k
           pss = 0.5 * (L[NV - 1] + R[NV - 1]) - 0.5 * ch * (R[5] - L[5]);
           L[5] = bns; R[5] = bns;
         }
-        if (CGL) flux_hll_cgl(L, R, F);
+        if (CGL) flux_hll_cgl(L, R, F, P.ph.cgl_form);
         else riemann_flux<RIEMANN, HALL>(P.ph, L, R, HALL ? Jr : nullptr, F);
         if (GLM) { F[5] = pss; F[NV - 1] = ch * ch * bns; }
 #pragma unroll

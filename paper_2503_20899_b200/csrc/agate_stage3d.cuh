@@ -231,7 +231,7 @@ __global__ void __launch_bounds__(32 * (TY + 1), MINB) stage3d_kernel(const __gr
       double u[9], w[9];
 #pragma unroll
       for (int q = 0; q < 9; ++q) u[q] = W[q * QS + off];
-      cgl_cons_to_prim(u, w);
+      cgl_cons_to_prim(u, w, P.ph.cgl_form);
 #pragma unroll
       for (int q = 0; q < 9; ++q)
         if (q < 5 || q > 7) W[q * QS + off] = w[q];       // B is its own primitive: the copied value stays
@@ -565,7 +565,7 @@ __global__ void __launch_bounds__(32 * (TY + 1), MINB) stage3d_kernel(const __gr
         F[5] = pss;
         F[NV - 1] = ch * ch * bns;
       } else if (flux) {
-        if (CGL) flux_hll_cgl(L, R, F);
+        if (CGL) flux_hll_cgl(L, R, F, P.ph.cgl_form);
         else riemann_flux<RIEMANN, HALL>(P.ph, L, R, HALL ? Jr : nullptr, F);
       }
 
@@ -616,7 +616,7 @@ __global__ void __launch_bounds__(32 * (TY + 1), MINB) stage3d_kernel(const __gr
             o[v] = c0 * ((two ? fma(P.r0, ub[v], ua[v]) : ua[v]) + d);
             if (GLM && v == NV - 1) o[v] *= decay;                        // eq.11's source, integrated exactly
             if (CGL && v == NV - 1 && P.last_stage && P.relax > 0.0 && emit && cell_ok)
-              o[v] = cgl_relaxed_alog(P.relax, o);                        // eqs.31-33: E stays, A_log moves
+              o[v] = cgl_relaxed_alog(P.relax, o, P.ph.cgl_form);                        // eqs.31-33: E stays, A_log moves
             if (emit && cell_ok) *po = o[v];
             ACC[v * ZS + tid] = t;
           }

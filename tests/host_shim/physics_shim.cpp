@@ -63,6 +63,16 @@ void shim_cgl_face_flux(int dir, const double* WL, const double* WR, double* F) 
 }
 double shim_cgl_relaxed_alog(double f, const double* U) { return cgl_relaxed_alog(f, U); }
 double shim_cell_speed_cgl(const double* U) { return cell_speed_cgl(U); }
+// the same with the thermodynamic variable of eq.16 (form 1)
+void shim_cgl_cons_to_prim_form(int form, const double* U, double* W) { cgl_cons_to_prim(U, W, form); }
+void shim_cgl_face_flux_form(int form, int dir, const double* WL, const double* WR, double* F) {
+  double L[9], R[9], Fr[9];
+  for (int r = 0; r < 9; ++r) { const int v = (r < 8) ? rot_var(r, dir) : r; L[r] = WL[v]; R[r] = WR[v]; }
+  flux_hll_cgl(L, R, Fr, form);
+  for (int r = 0; r < 9; ++r) F[(r < 8) ? rot_var(r, dir) : r] = Fr[r];
+}
+double shim_cgl_relaxed_form(int form, double f, const double* U) { return cgl_relaxed_alog(f, U, form); }
+double shim_cell_speed_cgl_form(int form, const double* U) { return cell_speed_cgl(U, form); }
 
 double shim_cell_speed(int eqset, double gamma, double d_i, double dxmin, const double* U) {
   Phys ph = make_phys(gamma, eqset == 1 ? d_i : 0.0, dxmin);

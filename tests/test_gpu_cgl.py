@@ -195,3 +195,37 @@ def test_cgl_random_shapes_and_options(ag, seed):
         e = rel_linf9(gpu.get_state(), ref.get_state())
         assert np.all(e <= 1e-11), (kw, s, e)
     ref.close(); gpu.close()
+
+
+# ---- the non-logarithmic variable of eq.16 (cgl_form = 1) ---------------------------------------------------
+def to_form1(U):
+    """The same primitive state with A of eq.16 in place of A_log."""
+    V = np.empty_like(U)
+    fu, fv = U.reshape(9, -1), V.reshape(9, -1)
+    for i in range(fu.shape[1]):
+        fv[:, i] = oracle.cgl_prim_to_cons(oracle.cgl_cons_to_prim(fu[:, i]), form=1)
+    return V
+
+
+@pytest.mark.parametrize("relax", [0.0, 0.99])
+@pytest.mark.parametrize("ndim,n,grid", [(2, 100, 0), (2, 64, 30), (3, 36, 0), (1, 75, 0)])
+def test_cgl_nonlog_form_parity(ag, relax, ndim, n, grid):
+    if ndim == 2:
+        U = to_form1(smooth_state(n)); shape, dx = (n, n, 1), (1 / n, 1 / n, 1)
+    elif ndim == 3:
+        U2 = to_form1(smooth_state(n))
+        U = np.ascontiguousarray(np.repeat(U2, n, axis=1)) * 1.0
+        z = (np.arange(n) + 0.5) / n
+        U[3] = U[0] * 0.1 * np.sin(2 * np.pi * z)[:, None, None]          # a z-dependent flow so every sweep works
+        shape, dx = (n, n, n), (1 / n, 1 / n, 1 / n)
+    else:
+        U = to_form1(smooth_state(n))[:, :, :1, :].copy(); shape, dx = (n, 1, 1), (1 / n, 1, 1)
+    kw = dict(shape=shape, dx=dx, ndim=ndim, riemann=0, limiter=2, beta=1.3, rk=2, relax=relax, cgl_form=1)
+    ref = oracle.RefSolver(eqset=oracle.CGL, **kw); gpu = ag.Agate(eqset=ag.CGL, stage_grid=grid, **kw)
+    ref.set_state(U); gpu.set_state(U)
+    e1, eN = march(ref, gpu, 6)
+    assert np.all(e1 <= TOL_1), e1
+    assert np.all(eN <= TOL_N), eN
+    ref.close(); gpu.close()
+    with pytest.raises(ag.AgateError):
+        ag.Agate(eqset=ag.CGL, shape=(8, 8, 1), dx=(1, 1, 1), ndim=2, riemann=0, cgl_form=2)

@@ -53,6 +53,14 @@ def shim():
     L.shim_cgl_cons_to_prim.restype = None
     L.shim_cgl_face_flux.argtypes = [C.c_int, _dp, _dp, _dp]
     L.shim_cgl_face_flux.restype = None
+    L.shim_cgl_cons_to_prim_form.argtypes = [C.c_int, _dp, _dp]
+    L.shim_cgl_cons_to_prim_form.restype = None
+    L.shim_cgl_face_flux_form.argtypes = [C.c_int, C.c_int, _dp, _dp, _dp]
+    L.shim_cgl_face_flux_form.restype = None
+    L.shim_cgl_relaxed_form.argtypes = [C.c_int, C.c_double, _dp]
+    L.shim_cgl_relaxed_form.restype = C.c_double
+    L.shim_cell_speed_cgl_form.argtypes = [C.c_int, _dp]
+    L.shim_cell_speed_cgl_form.restype = C.c_double
     L.shim_cgl_relaxed_alog.argtypes = [C.c_double, _dp]
     L.shim_cgl_relaxed_alog.restype = C.c_double
     L.shim_cell_speed_cgl.argtypes = [_dp]
@@ -289,3 +297,31 @@ def test_cgl_point_functions(shim):
             assert abs(shim.shim_cgl_relaxed_alog(f, _p(U)) - want) <= 1e-13 * max(1.0, abs(want))
         vo = np.sqrt(np.sum(WL[1:4] ** 2)) + max(oracle.cgl_cfast(d, WL) for d in range(3))
         assert abs(shim.shim_cell_speed_cgl(_p(U)) - vo) <= 5e-15 * vo
+
+
+def test_cgl_point_functions_nonlog_form(shim):
+    """The same point functions with the variable of eq.16 (eqs.24-25; cgl_form = 1) against the oracle."""
+    rng = np.random.default_rng(16)
+    def rand9():
+        W = np.empty(9)
+        W[0] = 0.3 + 2 * rng.random(); W[4] = 0.2 + 2 * rng.random(); W[8] = 0.2 + 2 * rng.random()
+        W[1:4] = rng.normal(size=3) * 0.5
+        W[5:8] = 0.3 + rng.random(3)
+        return W
+    for _ in range(300):
+        WL, WR = rand9(), rand9()
+        U = oracle.cgl_prim_to_cons(WL, form=1)
+        Ws = np.empty(9)
+        shim.shim_cgl_cons_to_prim_form(1, _p(U), _p(Ws))
+        assert relerr(Ws, oracle.cgl_cons_to_prim(U, form=1)) < 1e-14
+        for d in range(3):
+            F = np.empty(9)
+            shim.shim_cgl_face_flux_form(1, d, _p(WL), _p(WR), _p(F))
+            assert relerr(F, oracle.cgl_face_flux(d, WL, WR, form=1)) < 5e-14
+        W2 = oracle.cgl_cons_to_prim(U, form=1)
+        B2 = float(np.sum(W2[5:8] ** 2))
+        a, b = oracle.cgl_relax(0.99, B2, W2[4], W2[8])
+        want = (W2[0] ** 3 / (B2 * np.sqrt(B2))) * (b / a)                           # eq.16 of the relaxed pressures
+        assert abs(shim.shim_cgl_relaxed_form(1, 0.99, _p(U)) - want) <= 1e-13 * max(1.0, abs(want))
+        vo = np.sqrt(np.sum(WL[1:4] ** 2)) + max(oracle.cgl_cfast(d, WL) for d in range(3))
+        assert abs(shim.shim_cell_speed_cgl_form(1, _p(U)) - vo) <= 5e-15 * vo
