@@ -23,6 +23,7 @@ _LIB = os.path.join(_HERE, "libagate_ref.so")
 IDEAL, HALL = 0, 1
 CGL = 2              # CGL MHD: 9 variables per cell, U = (rho, m, E, B, A_log), W = (rho, v, p_par, B, p_perp) (R24)
 IDEAL_GLM = 3        # ideal MHD + GLM divergence cleaning: 9 variables per cell, psi last (eqs.10-11; R22)
+HALL_GLM = 4         # Hall MHD + GLM (R29): 9 variables per cell
 HLL, HLLD = 0, 1
 
 

@@ -167,7 +167,7 @@ void flux_hll(int eqset, int n, double gamma, double d_i, double dxmin,
               const T WL[8], const T WR[8], const T* J, T F[8]) {
   T cL = cfast(n, gamma, WL), cR = cfast(n, gamma, WR);
   T vHL[3], vHR[3];
-  const bool hall = (eqset == AGATE_REF_HALL);
+  const bool hall = (eqset == AGATE_REF_HALL || eqset == AGATE_REF_HALL_GLM);
   if (hall) {
     cL = tmax(cL, cwhistler(d_i, dxmin, WL));
     cR = tmax(cR, cwhistler(d_i, dxmin, WR));
@@ -414,7 +414,7 @@ template <class T> struct Solver {
     for (int d = 1; d < g.ndim; ++d) dxmin = std::fmin(dxmin, h[d]);
     cfl = s.cfl;
     if (!(cfl > 0.0)) cfl = (g.ndim == 1) ? 0.8 : (g.ndim == 2 ? 0.45 : 0.325);
-    glm = (eqset == AGATE_REF_IDEAL_GLM);
+    glm = (eqset == AGATE_REF_IDEAL_GLM || eqset == AGATE_REF_HALL_GLM);
     cgl = (eqset == AGATE_REF_CGL);
     nv = (glm || cgl) ? 9 : 8;
     Un.assign(nv * ntot, T(0.0)); U1.assign(nv * ntot, T(0.0)); W.assign(nv * ntot, T(0.0));
@@ -488,7 +488,7 @@ template <class T> struct Solver {
   void sweep(int d) {
     const int n = nd[d], d1 = (d + 1) % 3, d2 = (d + 2) % 3;
     const ptrdiff_t sd = st[d];
-    const bool hall = (eqset == AGATE_REF_HALL);
+    const bool hall = (eqset == AGATE_REF_HALL || eqset == AGATE_REF_HALL_GLM);
 #pragma omp parallel for collapse(2) num_threads(g_threads) if (g_threads > 1)
     for (int a2 = 0; a2 < nd[d2]; ++a2)
       for (int a1 = 0; a1 < nd[d1]; ++a1) {
@@ -519,7 +519,8 @@ template <class T> struct Solver {
             T bns, pss;
             glm_face<T>(ch, WL[5 + d], WR[5 + d], WL[8], WR[8], &bns, &pss);
             WL[5 + d] = bns; WR[5 + d] = bns;
-            face_flux<T>(AGATE_REF_IDEAL, s.riemann, d, gamma, s.d_i, dxmin, WL, WR, nullptr, Ff);
+            // Hall + GLM: the Hall flux of the same face states with B_n* on both sides (R29)
+            face_flux<T>(hall ? AGATE_REF_HALL : AGATE_REF_IDEAL, s.riemann, d, gamma, s.d_i, dxmin, WL, WR, hall ? J : nullptr, Ff);
             Ff[5 + d] = pss;
             Ff[8] = T(ch) * T(ch) * bns;
           } else {
@@ -566,7 +567,7 @@ template <class T> struct Solver {
           cons_to_prim(gamma, u, w);
           if (!(val(w[0]) > 0.0) || !(val(w[4]) > 0.0)) { bad = true; continue; }
           T cmax = tmax(tmax(cfast(0, gamma, w), cfast(1, gamma, w)), cfast(2, gamma, w));
-          if (eqset == AGATE_REF_HALL) cmax = tmax(cmax, cwhistler(s.d_i, dxmin, w));
+          if (eqset == AGATE_REF_HALL || eqset == AGATE_REF_HALL_GLM) cmax = tmax(cmax, cwhistler(s.d_i, dxmin, w));
           T sp = tsqrt(w[1] * w[1] + w[2] * w[2] + w[3] * w[3]) + cmax;
           if (!std::isfinite(val(sp))) { bad = true; continue; }
           vm = tmax(vm, sp);
@@ -721,7 +722,8 @@ int check_args(const agate_ref_grid* g, double gamma, int eqset, const agate_ref
   if (g->ndim < 2 && g->ny != 1) return 1;
   if (!(g->dx > 0.0) || (g->ndim >= 2 && !(g->dy > 0.0)) || (g->ndim >= 3 && !(g->dz > 0.0))) return 1;
   if (!(gamma > 1.0)) return 1;
-  if (eqset != AGATE_REF_IDEAL && eqset != AGATE_REF_HALL && eqset != AGATE_REF_IDEAL_GLM && eqset != AGATE_REF_CGL) return 1;
+  if (eqset != AGATE_REF_IDEAL && eqset != AGATE_REF_HALL && eqset != AGATE_REF_IDEAL_GLM && eqset != AGATE_REF_CGL &&
+      eqset != AGATE_REF_HALL_GLM) return 1;
   if (eqset == AGATE_REF_CGL && s->riemann != 0) return 1;          // the paper's CGL runs use HLL
   if (eqset == AGATE_REF_CGL && !(s->relax >= 0.0 && s->relax <= 1.0)) return 1;
   if (s->cgl_form < 0 || s->cgl_form > 1) return 1;
@@ -729,8 +731,9 @@ int check_args(const agate_ref_grid* g, double gamma, int eqset, const agate_ref
   if (s->limiter == 2 && !(s->beta >= 1.0 && s->beta <= 2.0)) return 1;
   for (int d = 0; d < 3; ++d) if (s->bc[d] < 0 || s->bc[d] > ((d == 1) ? 2 : 1)) return 1;
   if (s->bc[1] == 2 && (g->ndim < 2 || s->bc[0] != 0)) return 1;   // sheared ends in y need a periodic x (R28)
-  if (eqset == AGATE_REF_HALL && s->riemann == 1) return 1;        // no Hall-HLLD in the paper
-  if (eqset == AGATE_REF_HALL && !(s->d_i >= 0.0)) return 1;
+  const bool hall_set = (eqset == AGATE_REF_HALL || eqset == AGATE_REF_HALL_GLM);
+  if (hall_set && s->riemann == 1) return 1;        // no Hall-HLLD in the paper
+  if (hall_set && !(s->d_i >= 0.0)) return 1;
   return 0;
 }
 

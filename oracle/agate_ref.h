@@ -40,7 +40,9 @@ typedef struct {
   int32_t cgl_form;      /* CGL: 0 = logarithmic A of eq.18 (eqs.26-27; the paper's preferred form), 1 = A of eq.16 (eqs.24-25) */
 } agate_ref_solver;
 
-enum { AGATE_REF_IDEAL = 0, AGATE_REF_HALL = 1, AGATE_REF_CGL = 2, AGATE_REF_IDEAL_GLM = 3 };
+enum { AGATE_REF_IDEAL = 0, AGATE_REF_HALL = 1, AGATE_REF_CGL = 2, AGATE_REF_IDEAL_GLM = 3, AGATE_REF_HALL_GLM = 4 };
+/* AGATE_REF_HALL_GLM (R29): Hall MHD with the GLM scalar: the nine variables and every GLM rule of
+ * AGATE_REF_IDEAL_GLM, the Hall flux (face current, v_H, whistler speed) of AGATE_REF_HALL; HLL only. */
 /* AGATE_REF_CGL (R24): 9 variables, U = (rho, m, E, B, A_log) with eq.18's A_log,
  * W = (rho, v, p_par, B, p_perp); fluxes eqs.19-22 + eq.17, HLL only, speeds eq.29, dt eq.28, relaxation eqs.31-33
  * after the Runge-Kutta update. */

@@ -182,3 +182,60 @@ def test_g7_transposition_symmetry():
     # a mirror-free transposition changes the handedness: v_z and B_z pick up no sign, so equality is exact up to
     # the order of the x and y flux differences (round-off)
     assert np.max(np.abs(Va - Vb)) <= 1e-13
+
+
+# ------------------------------------------------------------------------------------------------
+# G8: Hall MHD with the GLM scalar (eqset HALL_GLM, R29)
+# ------------------------------------------------------------------------------------------------
+def test_g8_hall_glm_reduces_to_its_two_parents():
+    """(i) d_i = 0: no Hall velocity and c_w = v_A <= c_f, so every bit is that of IDEAL_GLM.  (ii) psi = 0 and a
+    constant B_n on a 1-D grid (the paper's whistler setup): B_n* = B_n, psi* = 0 exactly, so the first eight
+    variables are bit for bit those of HALL (which P9 ties to Table 1) and psi stays zero."""
+    import workloads
+    wl = workloads.make_workload(6, n=24)
+    a = oracle.RefSolver.from_workload(wl)
+    b = oracle.RefSolver.from_workload(wl, eqset=oracle.HALL_GLM, d_i=0.0)
+    a.advance(5); b.advance(5)
+    assert np.array_equal(a.get_state().view(np.uint64), b.get_state().view(np.uint64))
+    n = 32
+    x = (np.arange(n) + 0.5) * 200.0 / n
+    k = 2 * np.pi / 200.0
+    W = np.zeros((8, 1, 1, n)); W[0] = 1; W[4] = 1; W[5] = 100.0
+    W[2, 0, 0], W[3, 0, 0] = -6e-4 * np.cos(k * x), 6e-4 * np.sin(k * x)
+    W[6, 0, 0], W[7, 0, 0] = 1e-3 * np.cos(k * x), -1e-3 * np.sin(k * x)
+    U8 = workloads.prim_to_cons(W, 5.0 / 3.0)
+    U9 = np.concatenate([U8, np.zeros((1, 1, 1, n))], axis=0)
+    kw = dict(shape=(n, 1, 1), dx=(200.0 / n, 1, 1), ndim=1, riemann=oracle.HLL, beta=1.3, d_i=35.1076)
+    h = oracle.RefSolver(eqset=oracle.HALL, **kw); h.set_state(U8)
+    g = oracle.RefSolver(eqset=oracle.HALL_GLM, **kw); g.set_state(U9)
+    for _ in range(20):
+        dt = h.compute_dt()
+        assert g.compute_dt() == dt
+        h.step(dt); g.step(dt)
+    V = g.get_state()
+    assert np.array_equal(V[:8].view(np.uint64), h.get_state().view(np.uint64))
+    assert np.all(V[8] == 0.0)
+
+
+def test_g8_hall_glm_conservation_uniform_and_rejections():
+    import workloads
+    wl = workloads.make_workload(4, n=24)
+    rng = np.random.default_rng(3)
+    U = np.concatenate([wl.U, 0.01 * rng.standard_normal((1,) + wl.U.shape[1:])], axis=0)
+    s = oracle.RefSolver(shape=wl.shape, dx=wl.dx, ndim=2, eqset=oracle.HALL_GLM, riemann=oracle.HLL, beta=1.0, d_i=wl.d_i,
+                         cfl=wl.cfl)
+    s.set_state(U)
+    s0 = U.reshape(9, -1).sum(axis=1)
+    s.advance(6)
+    V = s.get_state()
+    scale = np.abs(V).reshape(9, -1).sum(axis=1) + 1e-300
+    assert np.all(np.abs(V.reshape(9, -1).sum(axis=1)[:8] - s0[:8]) <= 1e-13 * scale[:8])      # psi has a source
+    assert not np.array_equal(V, U)
+    Wc = np.array([1.1, 0.1, 0.2, -0.1, 0.8, 0.3, 0.2, 1.0])
+    Uc = np.concatenate([workloads.prim_to_cons(np.tile(Wc[:, None, None, None], (1, 1, 6, 6)), 5.0 / 3.0),
+                         np.zeros((1, 1, 6, 6))], axis=0)
+    u = oracle.RefSolver(shape=(6, 6, 1), dx=(0.1, 0.1, 1), ndim=2, eqset=oracle.HALL_GLM, riemann=oracle.HLL, d_i=0.5)
+    u.set_state(Uc); u.advance(3)
+    assert np.array_equal(u.get_state().view(np.uint64), Uc.view(np.uint64))
+    with pytest.raises(oracle.RefError):
+        oracle.RefSolver(shape=(6, 6, 1), dx=(0.1, 0.1, 1), ndim=2, eqset=oracle.HALL_GLM, riemann=oracle.HLLD)
