@@ -66,6 +66,10 @@ Layout make_layout(const agate_grid& g, int nv, int rk = 2) {
   return L;
 }
 
+inline bool is_hall(int eqset) { return eqset == AGATE_HALL || eqset == AGATE_HALL_GLM; }
+inline bool is_glm(int eqset) { return eqset == AGATE_IDEAL_GLM || eqset == AGATE_HALL_GLM; }
+inline int nvar_of(int eqset) { return (is_glm(eqset) || eqset == AGATE_CGL) ? 9 : 8; }
+
 int check_args(const agate_grid* g, double gamma, int eqset, const agate_solver* s) {
   if (!g || !s) return AGATE_ERR_ARG;
   if (g->ndim < 1 || g->ndim > 3) return AGATE_ERR_ARG;
@@ -74,7 +78,9 @@ int check_args(const agate_grid* g, double gamma, int eqset, const agate_solver*
   if (g->ndim < 2 && g->ny != 1) return AGATE_ERR_ARG;
   if (!(g->dx > 0.0) || (g->ndim >= 2 && !(g->dy > 0.0)) || (g->ndim >= 3 && !(g->dz > 0.0))) return AGATE_ERR_ARG;
   if (!(gamma > 1.0)) return AGATE_ERR_ARG;
-  if (eqset != AGATE_IDEAL && eqset != AGATE_HALL && eqset != AGATE_IDEAL_GLM && eqset != AGATE_CGL) return AGATE_ERR_ARG;
+  if (eqset != AGATE_IDEAL && eqset != AGATE_HALL && eqset != AGATE_IDEAL_GLM && eqset != AGATE_CGL && eqset != AGATE_HALL_GLM)
+    return AGATE_ERR_ARG;
+  if (eqset == AGATE_HALL_GLM && g->ndim == 3) return AGATE_ERR_ARG;            // Hall + GLM: strip kernel (1-D, 2-D grids)
   if (eqset == AGATE_CGL && s->riemann != AGATE_HLL) return AGATE_ERR_ARG;    // CGL: HLL (the paper names no other solver)
   if (eqset == AGATE_CGL && !(s->relax >= 0.0 && s->relax <= 1.0)) return AGATE_ERR_ARG;
   if (s->cgl_form < 0 || s->cgl_form > 1) return AGATE_ERR_ARG;
@@ -82,8 +88,8 @@ int check_args(const agate_grid* g, double gamma, int eqset, const agate_solver*
   if (s->limiter == 2 && !(s->beta >= 1.0 && s->beta <= 2.0)) return AGATE_ERR_ARG;
   for (int d = 0; d < 3; ++d) if (s->bc[d] < 0 || s->bc[d] > ((d == 1) ? 2 : 1)) return AGATE_ERR_ARG;
   if (s->bc[1] == 2 && (g->ndim < 2 || s->bc[0] != 0)) return AGATE_ERR_ARG;   // sheared ends in y need a periodic x (R28)
-  if (eqset == AGATE_HALL && s->riemann == AGATE_HLLD) return AGATE_ERR_ARG;   // no Hall-HLLD in the paper
-  if (eqset == AGATE_HALL && !(s->d_i >= 0.0)) return AGATE_ERR_ARG;
+  if (is_hall(eqset) && s->riemann == AGATE_HLLD) return AGATE_ERR_ARG;   // no Hall-HLLD in the paper
+  if (is_hall(eqset) && !(s->d_i >= 0.0)) return AGATE_ERR_ARG;
   return AGATE_OK;
 }
 
@@ -93,7 +99,7 @@ int check_args(const agate_grid* g, double gamma, int eqset, const agate_solver*
 // all); Courant number and dx_min are still those of the 1-D grid.
 agate_grid kernel_grid(const agate_grid& g, int eqset) {
   agate_grid k = g;
-  if (g.ndim == 1 && (eqset == AGATE_IDEAL_GLM || eqset == AGATE_CGL)) { k.ndim = 2; k.dy = g.dx; }
+  if (g.ndim == 1 && nvar_of(eqset) == 9) { k.ndim = 2; k.dy = g.dx; }
   return k;
 }
 
@@ -160,6 +166,7 @@ StageKernel pick_stage(int ndim, int eqset, int riemann, int limiter) {
     return make_stage3d<TY3, 0, -1, AGATE_MINB3>();
   }
   if (ndim == 2) {   // warp-autonomous strips
+    if (eqset == AGATE_HALL_GLM) return (limiter == 2) ? make_stage2d<0, 2, true, true>() : make_stage2d<0, -1, true, true>();
     if (eqset == AGATE_HALL)
       return (limiter == 3) ? make_stage2d<0, 3, true>() : ((limiter == 2) ? make_stage2d<0, 2, true>() : make_stage2d<0, -1, true>());
     if (eqset == AGATE_CGL) return (limiter == 2) ? make_stage2d<0, 2, false, false, true>() : make_stage2d<0, -1, false, false, true>();
@@ -290,7 +297,7 @@ int launch_dt(agate_ctx* c, int add_t) {
   p.scal = c->scal; p.flag = c->flag; p.ticket = c->ticket; p.partial = c->partial;
   p.add_t = add_t;
   p.cgl = (c->eqset == AGATE_CGL) ? 1 : 0;
-  if (c->eqset == AGATE_HALL) dt_kernel<true><<<c->dt_blocks, 256, 0, c->stream>>>(p);
+  if (is_hall(c->eqset)) dt_kernel<true><<<c->dt_blocks, 256, 0, c->stream>>>(p);
   else dt_kernel<false><<<c->dt_blocks, 256, 0, c->stream>>>(p);
   CU_TRY(cudaGetLastError());
   return AGATE_OK;
@@ -474,7 +481,7 @@ extern "C" {
 
 size_t agate_workspace_bytes(const agate_grid* grid, int eqset, const agate_solver* solver) {
   if (check_args(grid, 5.0 / 3.0, eqset, solver) != AGATE_OK) return 0;
-  return make_layout(kernel_grid(*grid, eqset), (eqset == AGATE_IDEAL_GLM || eqset == AGATE_CGL) ? 9 : 8, solver->rk).total;
+  return make_layout(kernel_grid(*grid, eqset), nvar_of(eqset), solver->rk).total;
 }
 
 int agate_init(const agate_grid* grid, double gamma, int eqset, const agate_solver* solver, void* workspace,
@@ -483,7 +490,7 @@ int agate_init(const agate_grid* grid, double gamma, int eqset, const agate_solv
   int rc = check_args(grid, gamma, eqset, solver);
   if (rc) return rc;
   if (!workspace) return AGATE_ERR_ARG;
-  const int nv = (eqset == AGATE_IDEAL_GLM || eqset == AGATE_CGL) ? 9 : 8;
+  const int nv = nvar_of(eqset);
   const agate_grid user_grid = *grid;                 // Courant number and dx_min follow the caller's dimensionality
   const agate_grid kgrid = kernel_grid(*grid, eqset);
   grid = &kgrid;
@@ -500,7 +507,7 @@ int agate_init(const agate_grid* grid, double gamma, int eqset, const agate_solv
   if (user_grid.ndim >= 3) c->dxmin = fmin(c->dxmin, user_grid.dz);
   c->cfl = solver->cfl;
   if (!(c->cfl > 0.0)) c->cfl = (user_grid.ndim == 1) ? 0.8 : (user_grid.ndim == 2 ? 0.45 : 0.325);
-  c->ph = make_phys(gamma, (eqset == AGATE_HALL) ? solver->d_i : 0.0, c->dxmin);
+  c->ph = make_phys(gamma, is_hall(eqset) ? solver->d_i : 0.0, c->dxmin);
   c->ph.cgl_form = (eqset == AGATE_CGL) ? solver->cgl_form : 0;
   c->stream = (cudaStream_t)stream;
   c->ws = (char*)workspace;
@@ -576,7 +583,7 @@ int agate_step(agate_ctx* c, double dt, double* dt_used) {
   if (!c->have_state || c->ext_lo || c->ext_hi) return AGATE_ERR_STATE;   // a slab steps through agate_stage_pre / _post
   int rc;
   if (dt > 0.0) {
-    if (c->eqset == AGATE_IDEAL_GLM && (rc = ensure_vmax(c))) return rc;      // c_h = 0.95 v_max(U^n) whoever chose dt
+    if (is_glm(c->eqset) && (rc = ensure_vmax(c))) return rc;      // c_h = 0.95 v_max(U^n) whoever chose dt
     set_dt_kernel<<<1, 1, 0, c->stream>>>(c->scal, dt, c->sk.fused_dt ? c->vnext : nullptr);
     CU_TRY(cudaGetLastError());
   } else {
@@ -743,7 +750,7 @@ int agate_step_begin(agate_ctx* c, double dt) {
   int rc;
   const bool have_v = c->vmax_given || (c->sk.fused_dt && c->vmax_valid);
   if (dt > 0.0) {
-    if (c->eqset == AGATE_IDEAL_GLM && !have_v && (rc = ensure_vmax(c))) return rc;
+    if (is_glm(c->eqset) && !have_v && (rc = ensure_vmax(c))) return rc;
     set_dt_kernel<<<1, 1, 0, c->stream>>>(c->scal, dt, (c->sk.fused_dt || c->vmax_given) ? c->vnext : nullptr);
     CU_TRY(cudaGetLastError());
   } else {

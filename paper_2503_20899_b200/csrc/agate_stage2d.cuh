@@ -47,7 +47,7 @@ struct Stage2dSmem {
 // CGL = true: CGL MHD (NEXT-2; R24): nine variables, W = (rho, v, p_par, B, p_perp), HLL only
 template <int RIEMANN, int LIM, bool HALL, bool GLM, bool CGL = false>
 __global__ void __launch_bounds__(32 * Stage2dSmem<GLM || CGL>::NW, 2) stage2d_kernel(const __grid_constant__ StageParams P) {
-  static_assert(!(HALL && GLM) && !(CGL && (HALL || GLM || RIEMANN != 0)), "combination not built");
+  static_assert(!(HALL && RIEMANN != 0) && !(CGL && (HALL || GLM || RIEMANN != 0)), "combination not built");
   using SM = Stage2dSmem<GLM || CGL>;
   constexpr int NV = SM::NV, NW2 = SM::NW;
   extern __shared__ __align__(16) double smem[];

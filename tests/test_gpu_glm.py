@@ -164,3 +164,56 @@ def test_glm_random_shapes_and_options(ag, seed):
         e = rel_linf9(gpu.get_state(), ref.get_state(), ref.glm_ch())
         assert np.all(e <= 1e-11), (kw, s, e)
     ref.close(); gpu.close()
+
+
+# ---- Hall MHD with the GLM scalar (eqset HALL_GLM, R29): strip kernel, 1-D and 2-D grids ------------------------------
+@pytest.mark.parametrize("n,grid,rk", [(64, 0, 2), (100, 0, 2), (100, 37, 3), (64, 5, 5)])
+def test_hall_glm_2d_parity(ag, n, grid, rk):
+    """Config 4's recipe (2-D Hall, d_i across 51 zones, whistler-limited dt) with a live cleaning field."""
+    wl = make_workload(4, n=n)
+    x = (np.arange(n) + 0.5) / n
+    U = np.concatenate([wl.U, (0.01 * np.sin(2 * np.pi * x)[None, :] * np.cos(4 * np.pi * x)[:, None])[None, None]], axis=0)
+    U[5] += 0.02 * np.exp(-((x[None, None, :] - 0.5) ** 2 + (x[None, :, None] - 0.4) ** 2) / 0.01)   # a divergence error
+    U[4] = wl.U[4] + 0.5 * (U[5] ** 2 - wl.U[5] ** 2)
+    kw = dict(shape=wl.shape, dx=wl.dx, ndim=2, gamma=wl.gamma, riemann=oracle.HLL, limiter=2, beta=1.3, rk=rk, cfl=wl.cfl,
+              d_i=wl.d_i)
+    ref = oracle.RefSolver(eqset=oracle.HALL_GLM, **kw); ref.set_state(U)
+    gpu = ag.Agate(eqset=ag.HALL_GLM, stage_grid=grid, **kw); gpu.set_state(U)
+    e1 = None
+    for s in range(6):
+        dtr, dtg = ref.compute_dt(), gpu.compute_dt()
+        assert abs(dtg - dtr) <= TOL_DT * dtr
+        ref.step(dtr)
+        assert gpu.step(0.0) == dtg
+        if s == 0:
+            e1 = rel_linf9(gpu.get_state(), ref.get_state(), ref.glm_ch())
+    eN = rel_linf9(gpu.get_state(), ref.get_state(), ref.glm_ch())
+    assert np.all(e1 <= TOL_1), e1
+    assert np.all(eN <= TOL_N), eN
+    tr, tg = ref.advance(3), gpu.advance(3)
+    assert abs(tg - tr) <= 1e-13 * tr
+    assert np.all(rel_linf9(gpu.get_state(), ref.get_state(), ref.glm_ch()) <= TOL_N)
+    ref.close(); gpu.close()
+
+
+def test_hall_glm_1d_and_rejections(ag):
+    import workloads
+    n = 80
+    x = (np.arange(n) + 0.5) / n
+    W = np.zeros((8, 1, 1, n))
+    W[0] = 1.0 + 0.3 * np.sin(2 * np.pi * x); W[1] = 0.2; W[4] = 0.7
+    W[5] = 0.8 + 0.05 * np.sin(4 * np.pi * x)
+    W[6, 0, 0], W[7, 0, 0] = 0.3 * np.cos(2 * np.pi * x), 0.3 * np.sin(4 * np.pi * x)
+    U = np.concatenate([workloads.prim_to_cons(W, 5 / 3), 0.01 * np.sin(2 * np.pi * x)[None, None, None, :]], axis=0)
+    kw = dict(shape=(n, 1, 1), dx=(1.0 / n, 1, 1), ndim=1, riemann=oracle.HLL, beta=1.3, d_i=0.05)
+    ref = oracle.RefSolver(eqset=oracle.HALL_GLM, **kw); gpu = ag.Agate(eqset=ag.HALL_GLM, **kw)
+    ref.set_state(U); gpu.set_state(U)
+    for s in range(6):
+        dtr, dtg = ref.compute_dt(), gpu.compute_dt()
+        assert abs(dtg - dtr) <= TOL_DT * dtr
+        ref.step(dtr); gpu.step(0.0)
+    assert np.all(rel_linf9(gpu.get_state(), ref.get_state(), ref.glm_ch()) <= TOL_N)
+    ref.close(); gpu.close()
+    for bad in (dict(shape=(8, 8, 8), dx=(1, 1, 1), ndim=3), dict(shape=(8, 8, 1), dx=(1, 1, 1), ndim=2, riemann=1)):
+        with pytest.raises(ag.AgateError):
+            ag.Agate(eqset=ag.HALL_GLM, **bad)
