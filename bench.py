@@ -47,14 +47,16 @@ FLOP_PER_ZONE_STEP = {1: 1430.0, 2: 1890.0, 3: 2770.0, 4: 1760.0, 5: 2770.0, 6: 
 FLOP_DT_PER_ZONE = {1: 45.0, 2: 45.0, 3: 45.0, 4: 60.0, 5: 45.0, 6: 45.0, 7: 90.0, 8: 60.0}
 BYTES_PER_ZONE_STEP = 320.0            # 5 x 8 variables x 8 B; 360 with the GLM scalar (config 6)
 # DRAM bytes per launch of the dominant kernel (dram__bytes_read.sum + dram__bytes_write.sum, mean of the two stage
-# launches of one step) from the committed `ncu` capture of the same command: profiles/r2_stage3d.md, r2_metrics.csv
-NCU_TRAFFIC_BYTES = {5: 0.5 * (11892200000 + 8929501000 + 20747918000 + 8874559000),
-                     2: 0.5 * (283633664 + 225516544 + 558816768 + 230311424),
-                     4: 0.5 * (79128064 + 24174336 + 152972544 + 28391680),
-                     8: 0.5 * (1430480000 + 1094991000 + 2598487000 + 1093660000)}
+# launches of one step) from `ncu --metrics dram__bytes_read.sum,dram__bytes_write.sum -k regex:stage -s 2 -c 2` on the
+# same bench command with the final kernels (profiles/r2_stage3d.md "final traffic"; the full captures in r2_metrics.csv
+# were taken a few commits earlier and agree within 1.5 %)
+NCU_TRAFFIC_BYTES = {5: 0.5 * (11739362560 + 8909190656 + 20846405888 + 8877627904),
+                     2: 0.5 * (283597056 + 225877248 + 558534656 + 226669824),
+                     4: 0.5 * (79398144 + 23402752 + 153257984 + 24535808),
+                     8: 0.5 * (1410853120 + 1090140416 + 2536635648 + 1086547712)}
 # ... and the kernels they were captured on: sha256 over csrc/*.cu* at capture time.  When the kernels have changed
 # since, the figure is stale and the line reports "traffic": null instead (profiles/ names the capture).
-NCU_TRAFFIC_CSRC_SHA = "d9964bdfc154968b"
+NCU_TRAFFIC_CSRC_SHA = "80187edfa4f09e49"
 
 
 def csrc_sha():
