@@ -64,8 +64,7 @@ typedef struct {
 
 enum { AGATE_IDEAL = 0, AGATE_HALL = 1, AGATE_CGL = 2, AGATE_IDEAL_GLM = 3, AGATE_HALL_GLM = 4 };
 /* AGATE_HALL_GLM (R29): Hall MHD with GLM divergence cleaning: the nine variables and every GLM rule of
- * AGATE_IDEAL_GLM with the Hall flux (face current, v_H, whistler speed) of AGATE_HALL; HLL only; 1-D and 2-D grids
- * (3-D: agate_init returns AGATE_ERR_ARG). */
+ * AGATE_IDEAL_GLM with the Hall flux (face current, v_H, whistler speed) of AGATE_HALL; HLL only. */
 /* AGATE_CGL (NEXT-2; eqs.14-33; R24): CGL MHD with the logarithmic state variable of
  * eq.18.  NINE variables per cell: U = (rho, m, E, B, A_log) with E = rho v^2/2 + B^2/2 + p_par/2 + p_perp.  HLL only,
  * speeds eq.29, dt eq.28, anisotropy relaxation eqs.31-33 (C1 = 0.3, C2 = 0.5) after the Runge-Kutta update.  1-D grids

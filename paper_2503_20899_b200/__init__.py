@@ -24,7 +24,7 @@ from . import build as _build
 IDEAL, HALL = 0, 1
 CGL = 2              # CGL MHD: 9 variables per cell, U = (rho, m, E, B, A_log); see include/agate.h
 IDEAL_GLM = 3        # 9 variables per cell (psi last); see include/agate.h
-HALL_GLM = 4         # Hall MHD + GLM: 9 variables per cell; 1-D and 2-D grids
+HALL_GLM = 4         # Hall MHD + GLM: 9 variables per cell
 HLL, HLLD = 0, 1
 OK, ERR_ARG, ERR_STATE, ERR_UNPHYSICAL, ERR_CUDA, ERR_NOMEM = range(6)
 

@@ -80,7 +80,6 @@ int check_args(const agate_grid* g, double gamma, int eqset, const agate_solver*
   if (!(gamma > 1.0)) return AGATE_ERR_ARG;
   if (eqset != AGATE_IDEAL && eqset != AGATE_HALL && eqset != AGATE_IDEAL_GLM && eqset != AGATE_CGL && eqset != AGATE_HALL_GLM)
     return AGATE_ERR_ARG;
-  if (eqset == AGATE_HALL_GLM && g->ndim == 3) return AGATE_ERR_ARG;            // Hall + GLM: strip kernel (1-D, 2-D grids)
   if (eqset == AGATE_CGL && s->riemann != AGATE_HLL) return AGATE_ERR_ARG;    // CGL: HLL (the paper names no other solver)
   if (eqset == AGATE_CGL && !(s->relax >= 0.0 && s->relax <= 1.0)) return AGATE_ERR_ARG;
   if (s->cgl_form < 0 || s->cgl_form > 1) return AGATE_ERR_ARG;
@@ -149,6 +148,9 @@ StageKernel make_stage2d() {
 
 StageKernel pick_stage(int ndim, int eqset, int riemann, int limiter) {
   if (ndim == 3) {
+    if (eqset == AGATE_HALL_GLM)
+      return (limiter == 2) ? make_stage3d<TY3N, 0, 2, AGATE_MINB3, true, false, true>()
+                            : make_stage3d<TY3N, 0, -1, AGATE_MINB3, true, false, true>();
     if (eqset == AGATE_HALL)
       return (limiter == 2) ? make_stage3d<TY3, 0, 2, AGATE_MINB3, false, false, true>()
                             : make_stage3d<TY3, 0, -1, AGATE_MINB3, false, false, true>();

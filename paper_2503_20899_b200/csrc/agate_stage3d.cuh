@@ -147,7 +147,7 @@ __device__ __forceinline__ void hall_current(const double* W, int QS, int oC, in
 // three planes, carry their x-halo corners, and a few more hand-overs guard the planes k-1 and k+1.
 template <int TY, int RIEMANN, int LIM, int MINB, bool GLM = false, bool CGL = false, bool HALL = false>
 __global__ void __launch_bounds__(32 * (TY + 1), MINB) stage3d_kernel(const __grid_constant__ StageParams P) {
-  static_assert(!(CGL && (GLM || RIEMANN != 0)) && !(HALL && (GLM || CGL || RIEMANN != 0)), "combination not built");
+  static_assert(!(CGL && (GLM || RIEMANN != 0)) && !(HALL && (CGL || RIEMANN != 0)), "combination not built");
   constexpr int NV = (GLM || CGL) ? 9 : 8;
   constexpr int NHB = HALL ? 3 : 2;
   using SM = Stage3dSmem<TY, NV, NHB>;
@@ -561,7 +561,7 @@ __global__ void __launch_bounds__(32 * (TY + 1), MINB) stage3d_kernel(const __gr
         const double bns = 0.5 * (L[5] + R[5]) - 0.5 * (R[NV - 1] - L[NV - 1]) * ich;
         const double pss = 0.5 * (L[NV - 1] + R[NV - 1]) - 0.5 * ch * (R[5] - L[5]);
         L[5] = bns; R[5] = bns;
-        riemann_flux<RIEMANN, false>(P.ph, L, R, nullptr, F);
+        riemann_flux<RIEMANN, HALL>(P.ph, L, R, HALL ? Jr : nullptr, F);      // Hall + GLM (R29): Hall flux with B_n*
         F[5] = pss;
         F[NV - 1] = ch * ch * bns;
       } else if (flux) {

@@ -214,6 +214,35 @@ def test_hall_glm_1d_and_rejections(ag):
         ref.step(dtr); gpu.step(0.0)
     assert np.all(rel_linf9(gpu.get_state(), ref.get_state(), ref.glm_ch()) <= TOL_N)
     ref.close(); gpu.close()
-    for bad in (dict(shape=(8, 8, 8), dx=(1, 1, 1), ndim=3), dict(shape=(8, 8, 1), dx=(1, 1, 1), ndim=2, riemann=1)):
-        with pytest.raises(ag.AgateError):
-            ag.Agate(eqset=ag.HALL_GLM, **bad)
+    with pytest.raises(ag.AgateError):
+        ag.Agate(eqset=ag.HALL_GLM, shape=(8, 8, 1), dx=(1, 1, 1), ndim=2, riemann=1)          # Hall + HLLD
+
+
+@pytest.mark.parametrize("grid,rk", [(0, 2), (23, 3)])
+def test_hall_glm_3d_parity(ag, grid, rk):
+    """Hall + GLM through the 3-D row-owner kernel (nine variables, three halo-row planes, bulk row copies): config 8's
+    recipe at 40^3 (ragged tiles) with a smooth psi and a divergence error in B_x."""
+    wl = make_workload(8, n=40)
+    n = 40
+    x = (np.arange(n) + 0.5) / n
+    U = np.empty((9, n, n, n))
+    U[:8] = wl.U
+    U[5] += 0.02 * np.exp(-((x[None, None, :] - 0.5) ** 2 + (x[None, :, None] - 0.4) ** 2 + (x[:, None, None] - 0.6) ** 2) / 0.02)
+    U[4] = wl.U[4] + 0.5 * (U[5] ** 2 - wl.U[5] ** 2)
+    U[8] = 0.01 * np.sin(2 * np.pi * x)[None, None, :] * np.cos(2 * np.pi * x)[:, None, None]
+    kw = dict(shape=wl.shape, dx=wl.dx, ndim=3, gamma=wl.gamma, riemann=oracle.HLL, limiter=2, beta=1.3, rk=rk, cfl=wl.cfl,
+              d_i=wl.d_i)
+    ref = oracle.RefSolver(eqset=oracle.HALL_GLM, **kw); ref.set_state(U)
+    gpu = ag.Agate(eqset=ag.HALL_GLM, stage_grid=grid, **kw); gpu.set_state(U)
+    e1 = None
+    for s in range(4):
+        dtr, dtg = ref.compute_dt(), gpu.compute_dt()
+        assert abs(dtg - dtr) <= TOL_DT * dtr
+        ref.step(dtr)
+        assert gpu.step(0.0) == dtg
+        if s == 0:
+            e1 = rel_linf9(gpu.get_state(), ref.get_state(), ref.glm_ch())
+    eN = rel_linf9(gpu.get_state(), ref.get_state(), ref.glm_ch())
+    assert np.all(e1 <= TOL_1), e1
+    assert np.all(eN <= TOL_N), eN
+    ref.close(); gpu.close()
