@@ -651,37 +651,51 @@ AG_HD double cgl_cfast(const double w[9]) {
   const double c = 4.0 * w[8] * w[8] * cos2 * (1.0 - cos2);
   return sqrt_pos((b1 + sqrt_pos(dmax(b2 * b2 + c, kTiny))) * (0.5 * rcp(w[0])));
 }
-// eqs.19-22 (psi == 0) + eq.17 in the rotated frame; also returns the conserved vector of the state
-AG_HD void cgl_flux_and_cons(const double w[9], double f[9], double u[9], int form = 0) {
-  const double B2 = w[5] * w[5] + w[6] * w[6] + w[7] * w[7];
-  const double th = 1.0 - (w[4] - w[8]) * rcp(B2);
-  const double v2 = w[1] * w[1] + w[2] * w[2] + w[3] * w[3];
-  const double vB = w[1] * w[5] + w[2] * w[6] + w[3] * w[7];
-  u[0] = w[0]; u[1] = w[0] * w[1]; u[2] = w[0] * w[2]; u[3] = w[0] * w[3];
-  u[4] = 0.5 * w[0] * v2 + 0.5 * B2 + 0.5 * w[4] + w[8];
+// One side of the CGL face problem in the rotated frame: eqs.19-22 (psi == 0) + eq.17, the conserved vector, and the
+// fast speed eq.29 -- |B|^2 and its reciprocal are formed once for Theta, cos^2 and the thermodynamic variable.
+AG_HD void cgl_side(const double w[9], double f[9], double u[9], double& cfast, int form) {
+  const double bn2 = w[5] * w[5];
+  const double B2 = fma(w[7], w[7], fma(w[6], w[6], bn2));
+  const double iB2 = rcp(B2);
+  const double th = fma(-(w[4] - w[8]), iB2, 1.0);                       // Theta = 1 - (p_par - p_perp)/B^2
+  const double v2 = fma(w[3], w[3], fma(w[2], w[2], w[1] * w[1]));
+  const double vB = fma(w[3], w[7], fma(w[2], w[6], w[1] * w[5]));
+  const double ru = w[0] * w[1];
+  const double ke = (0.5 * w[0]) * v2;
+  u[0] = w[0]; u[1] = ru; u[2] = w[0] * w[2]; u[3] = w[0] * w[3];
+  u[4] = fma(0.5, B2 + w[4], ke) + w[8];
   u[5] = w[5]; u[6] = w[6]; u[7] = w[7];
-  u[8] = cgl_alog(w[0], B2, w[4], w[8], form);
-  f[0] = w[0] * w[1];
-  f[1] = w[0] * w[1] * w[1] - th * w[5] * w[5] + (w[8] + 0.5 * B2);
-  f[2] = w[0] * w[2] * w[1] - th * w[6] * w[5];
-  f[3] = w[0] * w[3] * w[1] - th * w[7] * w[5];
-  f[4] = (0.5 * w[0] * v2 + 0.5 * w[4] + 2.0 * w[8] + B2) * w[1] - th * vB * w[5];
+  // (rho^2 / B^3) (p_perp / p_par):  1/B^3 = (1/B^2) rsqrt(B^2)
+  const double ratio = (w[0] * w[0] * w[8]) * (iB2 * rsq(dmax(B2, kTiny))) * rcp(w[4]);
+  u[8] = (form == 1) ? w[0] * ratio : w[0] * log(ratio);                   // eq.16 / eq.18
+  const double tb = th * w[5];
+  f[0] = ru;
+  f[1] = fma(ru, w[1], fma(-tb, w[5], fma(0.5, B2, w[8])));
+  f[2] = fma(ru, w[2], -(tb * w[6]));
+  f[3] = fma(ru, w[3], -(tb * w[7]));
+  f[4] = fma(-tb, vB, (fma(0.5, w[4], ke) + fma(2.0, w[8], B2)) * w[1]);
   f[5] = 0.0;
-  f[6] = w[1] * w[6] - w[5] * w[2];
-  f[7] = w[1] * w[7] - w[5] * w[3];
+  f[6] = fma(w[1], w[6], -(w[5] * w[2]));
+  f[7] = fma(w[1], w[7], -(w[5] * w[3]));
   f[8] = u[8] * w[1];
+  const double cos2 = bn2 * iB2;
+  const double b1 = fma(cos2, fma(2.0, w[4], -w[8]), fma(2.0, w[8], B2));
+  const double b2 = fma(-6.0 * cos2, w[4], b1);
+  const double c = (4.0 * w[8] * w[8]) * (cos2 * (1.0 - cos2));
+  cfast = sqrt_pos((b1 + sqrt_pos(dmax(fma(b2, b2, c), kTiny))) * (0.5 * rcp(w[0])));
 }
-// HLL eq.5 with the Davis speeds eq.6 and eq.29's fast speed; all nine components through eq.5 (R9)
+// HLL eq.5 with the Davis speeds eq.6 and eq.29's fast speed; all nine components through eq.5 (R9), written as
+// a F_L + b F_R + c (U_R - U_L)  with a = s_R/(s_R-s_L), b = -s_L/(s_R-s_L), c = s_L s_R/(s_R-s_L)
 AG_HD void flux_hll_cgl(const double L[9], const double R[9], double F[9], int form = 0) {
-  double fl[9], fr[9], ul[9], ur[9];
-  cgl_flux_and_cons(L, fl, ul, form);
-  cgl_flux_and_cons(R, fr, ur, form);
-  const double cl = cgl_cfast(L), cr = cgl_cfast(R);
+  double fl[9], fr[9], ul[9], ur[9], cl, cr;
+  cgl_side(L, fl, ul, cl, form);
+  cgl_side(R, fr, ur, cr, form);
   const double sL = dmin(dmin(L[1] - cl, R[1] - cr), 0.0);
   const double sR = dmax(dmax(L[1] + cl, R[1] + cr), 0.0);
   const double iw = rcp(sR - sL);
+  const double a = sR * iw, b = -(sL * iw), c = sL * a;
 #pragma unroll
-  for (int q = 0; q < 9; ++q) F[q] = (sR * fl[q] - sL * fr[q] + sL * sR * (ur[q] - ul[q])) * iw;
+  for (int q = 0; q < 9; ++q) F[q] = fma(a, fl[q], fma(b, fr[q], c * (ur[q] - ul[q])));
 }
 // eqs.31-33 on a conserved cell: relax the anisotropy, keep E, return the new A_log (C1 = 0.3, C2 = 0.5)
 AG_HD double cgl_relaxed_alog(double f, const double U[9], int form = 0) {
