@@ -24,6 +24,7 @@ IDEAL, HALL = 0, 1
 CGL = 2              # CGL MHD: 9 variables per cell, U = (rho, m, E, B, A_log), W = (rho, v, p_par, B, p_perp) (R24)
 IDEAL_GLM = 3        # ideal MHD + GLM divergence cleaning: 9 variables per cell, psi last (eqs.10-11; R22)
 HALL_GLM = 4         # Hall MHD + GLM (R29): 9 variables per cell
+CGL_GLM = 5          # CGL MHD + GLM (eqs.19-23; R30): 10 variables per cell, U = (rho, m, E, B, A, psi)
 HLL, HLLD = 0, 1
 
 

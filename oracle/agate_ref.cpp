@@ -394,7 +394,7 @@ template <class T> struct Solver {
   size_t ntot, nint;    // padded / interior cell counts
   double h[3];          // spacings
   double dxmin, cfl;
-  int nv;               // variables per cell: 8, or 9 with the GLM scalar psi (index 8) behind the MHD ones
+  int nv;               // variables per cell: 8, + CGL's A (index 8), + the GLM scalar psi (the last index, nv-1)
   bool glm;
   bool cgl = false;
   double ch = 0.0;      // GLM: c_h of the step being taken (R22: 0.95 v_max(U^n))
@@ -414,9 +414,9 @@ template <class T> struct Solver {
     for (int d = 1; d < g.ndim; ++d) dxmin = std::fmin(dxmin, h[d]);
     cfl = s.cfl;
     if (!(cfl > 0.0)) cfl = (g.ndim == 1) ? 0.8 : (g.ndim == 2 ? 0.45 : 0.325);
-    glm = (eqset == AGATE_REF_IDEAL_GLM || eqset == AGATE_REF_HALL_GLM);
-    cgl = (eqset == AGATE_REF_CGL);
-    nv = (glm || cgl) ? 9 : 8;
+    glm = (eqset == AGATE_REF_IDEAL_GLM || eqset == AGATE_REF_HALL_GLM || eqset == AGATE_REF_CGL_GLM);
+    cgl = (eqset == AGATE_REF_CGL || eqset == AGATE_REF_CGL_GLM);
+    nv = 8 + (glm ? 1 : 0) + (cgl ? 1 : 0);          // psi is always the last variable; CGL's A is index 8
     Un.assign(nv * ntot, T(0.0)); U1.assign(nv * ntot, T(0.0)); W.assign(nv * ntot, T(0.0));
     L.assign(nv * nint, T(0.0));
   }
@@ -457,6 +457,7 @@ template <class T> struct Solver {
         for (int q = 0; q < 9; ++q) u9[q] = U[q * ntot + c];
         cgl_cons_to_prim(u9, w9, s.cgl_form);
         for (int q = 0; q < 9; ++q) W[q * ntot + c] = w9[q];
+        if (glm) W[9 * ntot + c] = U[9 * ntot + c];               // psi is its own primitive
         continue;
       }
       T u[8], w[8];
@@ -503,14 +504,22 @@ template <class T> struct Solver {
             dW[q * (n + 2) + (c + 1)] = slope<T>(s.limiter, s.beta, dp, dm);
           }
         for (int c = -1; c < n; ++c) {                                   // face c+1/2, between cells c and c+1
-          T WL[9], WR[9], Ff[9], J[3];
+          T WL[10], WR[10], Ff[10], J[3];
           for (int q = 0; q < nv; ++q) {
             const T* Wq = &W[q * ntot + base];
             WL[q] = Wq[c * sd] + T(0.5) * dW[q * (n + 2) + (c + 1)];             // eq.2
             WR[q] = Wq[(c + 1) * sd] - T(0.5) * dW[q * (n + 2) + (c + 2)];       // eq.3
           }
           if (hall) face_current(d, base + c * sd, J);
-          if (cgl) {
+          if (cgl && glm) {
+            // eqs.22-23 (R30): the same (B_n, psi) subsystem as eqs.10-11; CGL's flux sees B_n* on both sides
+            T bns, pss;
+            glm_face<T>(ch, WL[5 + d], WR[5 + d], WL[9], WR[9], &bns, &pss);
+            WL[5 + d] = bns; WR[5 + d] = bns;
+            cgl_flux_hll<T>(d, WL, WR, Ff, s.cgl_form);
+            Ff[5 + d] = pss;
+            Ff[9] = T(ch) * T(ch) * bns;
+          } else if (cgl) {
             cgl_flux_hll<T>(d, WL, WR, Ff, s.cgl_form);
           } else if (glm) {
             // eqs.10-11 (R22): (B_n, psi) decouple into a 2x2 linear system with speeds -+c_h; its Riemann
@@ -551,7 +560,7 @@ template <class T> struct Solver {
     for (int k = 0; k < nd[2]; ++k)
       for (int j = 0; j < nd[1]; ++j)
         for (int i = 0; i < nd[0]; ++i) {
-          T u[9], w[9];
+          T u[10], w[10];
           const ptrdiff_t c = pidx(i, j, k);
           for (int q = 0; q < nv; ++q) u[q] = Un[q * ntot + c];
           if (cgl) {
@@ -589,7 +598,7 @@ template <class T> struct Solver {
   void glm_source(double dt) {
     const T decay = T(std::exp(-dt * ch / 0.18));
     for (int k = 0; k < nd[2]; ++k) for (int j = 0; j < nd[1]; ++j) for (int i = 0; i < nd[0]; ++i) {
-      const size_t p = 8 * ntot + pidx(i, j, k);
+      const size_t p = (size_t)(nv - 1) * ntot + pidx(i, j, k);
       Un[p] = Un[p] * decay;
     }
   }
@@ -723,9 +732,10 @@ int check_args(const agate_ref_grid* g, double gamma, int eqset, const agate_ref
   if (!(g->dx > 0.0) || (g->ndim >= 2 && !(g->dy > 0.0)) || (g->ndim >= 3 && !(g->dz > 0.0))) return 1;
   if (!(gamma > 1.0)) return 1;
   if (eqset != AGATE_REF_IDEAL && eqset != AGATE_REF_HALL && eqset != AGATE_REF_IDEAL_GLM && eqset != AGATE_REF_CGL &&
-      eqset != AGATE_REF_HALL_GLM) return 1;
-  if (eqset == AGATE_REF_CGL && s->riemann != 0) return 1;          // the paper's CGL runs use HLL
-  if (eqset == AGATE_REF_CGL && !(s->relax >= 0.0 && s->relax <= 1.0)) return 1;
+      eqset != AGATE_REF_HALL_GLM && eqset != AGATE_REF_CGL_GLM) return 1;
+  const bool cgl_set = (eqset == AGATE_REF_CGL || eqset == AGATE_REF_CGL_GLM);
+  if (cgl_set && s->riemann != 0) return 1;          // the paper's CGL runs use HLL
+  if (cgl_set && !(s->relax >= 0.0 && s->relax <= 1.0)) return 1;
   if (s->cgl_form < 0 || s->cgl_form > 1) return 1;
   if (s->riemann < 0 || s->riemann > 1 || s->limiter < 0 || s->limiter > 2 || s->rk < 1 || s->rk > 5) return 1;
   if (s->limiter == 2 && !(s->beta >= 1.0 && s->beta <= 2.0)) return 1;

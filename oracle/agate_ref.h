@@ -40,7 +40,10 @@ typedef struct {
   int32_t cgl_form;      /* CGL: 0 = logarithmic A of eq.18 (eqs.26-27; the paper's preferred form), 1 = A of eq.16 (eqs.24-25) */
 } agate_ref_solver;
 
-enum { AGATE_REF_IDEAL = 0, AGATE_REF_HALL = 1, AGATE_REF_CGL = 2, AGATE_REF_IDEAL_GLM = 3, AGATE_REF_HALL_GLM = 4 };
+enum { AGATE_REF_IDEAL = 0, AGATE_REF_HALL = 1, AGATE_REF_CGL = 2, AGATE_REF_IDEAL_GLM = 3, AGATE_REF_HALL_GLM = 4, AGATE_REF_CGL_GLM = 5 };
+/* AGATE_REF_CGL_GLM (eqs.19-23; R30): CGL MHD with the GLM scalar: ten variables,
+ * U = (rho, m, E, B, A, psi); CGL's rules for the first nine, IDEAL_GLM's (B_n*, psi*) face rule, fluxes and source
+ * for B_n and psi (index 9), c_h = 0.95 v_max with eq.28's CGL speeds. */
 /* AGATE_REF_HALL_GLM (R29): Hall MHD with the GLM scalar: the nine variables and every GLM rule of
  * AGATE_REF_IDEAL_GLM, the Hall flux (face current, v_H, whistler speed) of AGATE_REF_HALL; HLL only. */
 /* AGATE_REF_CGL (R24): 9 variables, U = (rho, m, E, B, A_log) with eq.18's A_log,
