@@ -43,8 +43,9 @@ UNIT = "zone-updates/s"
 # 1's lean / as-written ratio (1430 / 1774)
 # config 8 (3-D Hall, not a BASELINE.json config): the oracle's as-written count (3202) scaled by config 4's lean /
 # as-written ratio (1760 / 2072)
-FLOP_PER_ZONE_STEP = {1: 1430.0, 2: 1890.0, 3: 2770.0, 4: 1760.0, 5: 2770.0, 6: 1550.0, 7: 1690.0, 8: 2720.0}
-FLOP_DT_PER_ZONE = {1: 45.0, 2: 45.0, 3: 45.0, 4: 60.0, 5: 45.0, 6: 45.0, 7: 90.0, 8: 60.0}
+# config 9 (CGL + GLM): config 7's count + config 6's 120 for the GLM scalar
+FLOP_PER_ZONE_STEP = {1: 1430.0, 2: 1890.0, 3: 2770.0, 4: 1760.0, 5: 2770.0, 6: 1550.0, 7: 1690.0, 8: 2720.0, 9: 1810.0}
+FLOP_DT_PER_ZONE = {1: 45.0, 2: 45.0, 3: 45.0, 4: 60.0, 5: 45.0, 6: 45.0, 7: 90.0, 8: 60.0, 9: 90.0}
 BYTES_PER_ZONE_STEP = 320.0            # 5 x 8 variables x 8 B; 360 with the GLM scalar (config 6)
 # DRAM bytes per launch of the dominant kernel (dram__bytes_read.sum + dram__bytes_write.sum, mean of the two stage
 # launches of one step) from `ncu --metrics dram__bytes_read.sum,dram__bytes_write.sum -k regex:stage -s 2 -c 2` on the
@@ -69,7 +70,7 @@ def csrc_sha():
 FP64_NOMINAL_TFLOPS = 148 * 64 * 2 * 1.965e9 / 1e12     # 148 SMs x 64 DFMA lanes x 2 x max SM clock = 37.2
 
 # reduced size of the bounded CPU sample per config (same recipe and seed), and its step count
-CPU_SAMPLE = {1: (128, 10), 2: (512, 8), 3: (96, 4), 4: (512, 8), 5: (96, 4), 6: (512, 8), 7: (512, 8), 8: (96, 4)}
+CPU_SAMPLE = {1: (128, 10), 2: (512, 8), 3: (96, 4), 4: (512, 8), 5: (96, 4), 6: (512, 8), 7: (512, 8), 8: (96, 4), 9: (512, 8)}
 
 
 def parse():
@@ -77,7 +78,7 @@ def parse():
     ap.add_argument("--gpus", type=int, default=1)
     ap.add_argument("--steps", type=int, default=20)
     ap.add_argument("--warmup", type=int, default=3)
-    ap.add_argument("--config", type=int, default=5, choices=[1, 2, 3, 4, 5, 6, 7, 8],
+    ap.add_argument("--config", type=int, default=5, choices=[1, 2, 3, 4, 5, 6, 7, 8, 9],
                     help="1-5: BASELINE.json configs; 6: Orszag-Tang + GLM, the workload of the paper's Table 2; "
                          "7: Orszag-Tang in CGL MHD; 8: Hall MHD on config 3's 3-D recipe")
     ap.add_argument("--to-time", type=float, default=0.0,
@@ -263,7 +264,7 @@ def run_ours(args):
     wl = make_workload(cfg, n=args.n or None)
     zones = wl.zones
     over = {}
-    if cfg == 7 and args.cgl_form == 1:
+    if cfg in (7, 9) and args.cgl_form == 1:
         # input definition of the other thermodynamic variable (eq.16): A = (rho / |B|)^3 p_perp / p_par
         W = wl.W
         b2 = W[5] ** 2 + W[6] ** 2 + W[7] ** 2
@@ -305,7 +306,7 @@ def run_ours(args):
     flop_stage = (FLOP_PER_ZONE_STEP[cfg] - FLOP_DT_PER_ZONE[cfg]) / 2.0 * zones
     achieved = flop_stage / (stage_ms * 1e-3) / 1e12
     peaks, peak_src = measured_peaks()
-    bytes_step = BYTES_PER_ZONE_STEP * (9.0 / 8.0 if cfg in (6, 7) else 1.0)
+    bytes_step = BYTES_PER_ZONE_STEP * {6: 9.0 / 8.0, 7: 9.0 / 8.0, 9: 10.0 / 8.0}.get(cfg, 1.0)
     hbm_frac = (bytes_step / 5.0 * 2.5 * zones / (stage_ms * 1e-3) / 1e9) / peaks["hbm_gbs"]
     roofline = {"bound": "alu", "achieved": achieved, "peak": fp64_peak, "unit": "TFLOP/s",
                 "frac": achieved / fp64_peak, "frac_of_nominal": achieved / FP64_NOMINAL_TFLOPS, "traffic": (NCU_TRAFFIC_BYTES.get(cfg) if (not args.n and csrc_sha() == NCU_TRAFFIC_CSRC_SHA) else None),

@@ -52,17 +52,22 @@ typedef struct {
                            rk >= 3 needs a third state copy in the workspace                             */
   double  cfl;          /* Courant number C; <= 0 selects the paper default 0.8/0.45/0.325   */
   double  d_i;          /* normalised ion inertial length (eqset AGATE_HALL only)            */
-  double  relax;        /* eqset AGATE_CGL only: dt/(dt+tau) of eqs.32-33 in [0,1]; the paper's default is
+  double  relax;        /* eqsets AGATE_CGL, AGATE_CGL_GLM: dt/(dt+tau) of eqs.32-33 in [0,1]; the paper's default is
                            0.99; 0 = no relaxation                                            */
   int32_t bc[3];        /* ghost rule per dimension (x, y, z): 0 = periodic, 1 = zero-gradient /
                            open end (R26: ghost = nearest interior zone); bc[1] = 2: the sheared
                            zero-gradient ends of the 2-D whistler test (R28: ghost (i,j) = zone (i-1,j+2)
                            at the down side, (i+1,j-2) at the up side, x periodic: needs bc[0] = 0, ndim >= 2) */
-  int32_t cgl_form;     /* eqset AGATE_CGL only: 0 = the logarithmic variable A_log of eq.18 (eqs.26-27; the paper's
+  int32_t cgl_form;     /* eqsets AGATE_CGL, AGATE_CGL_GLM: 0 = the logarithmic variable A_log of eq.18 (eqs.26-27; the paper's
                            preferred form), 1 = A of eq.16 (eqs.24-25; "AGATE supports both"): U[8] is A      */
 } agate_solver;
 
-enum { AGATE_IDEAL = 0, AGATE_HALL = 1, AGATE_CGL = 2, AGATE_IDEAL_GLM = 3, AGATE_HALL_GLM = 4 };
+enum { AGATE_IDEAL = 0, AGATE_HALL = 1, AGATE_CGL = 2, AGATE_IDEAL_GLM = 3, AGATE_HALL_GLM = 4, AGATE_CGL_GLM = 5 };
+/* AGATE_CGL_GLM (eqs.19-23; R30): CGL MHD with GLM divergence cleaning: TEN variables per
+ * cell, U = (rho, m, E, B, A, psi); AGATE_CGL's rules (relax, cgl_form, HLL only) for the first nine and
+ * AGATE_IDEAL_GLM's for B_n and psi -- face values (B_n*, psi*) from the 2x2 linear Riemann problem, CGL's flux of the
+ * two face states with B_n* on both sides, F[B_n] = psi*, F[psi] = c_h^2 B_n*, psi *= exp(-dt c_h^2/c_p^2) after the
+ * Runge-Kutta update; c_h = 0.95 v_max with eq.28's CGL speeds. */
 /* AGATE_HALL_GLM (R29): Hall MHD with GLM divergence cleaning: the nine variables and every GLM rule of
  * AGATE_IDEAL_GLM with the Hall flux (face current, v_H, whistler speed) of AGATE_HALL; HLL only. */
 /* AGATE_CGL (NEXT-2; eqs.14-33; R24): CGL MHD with the logarithmic state variable of
@@ -95,7 +100,7 @@ size_t agate_workspace_bytes(const agate_grid* grid, int eqset, const agate_solv
 int agate_init(const agate_grid* grid, double gamma, int eqset, const agate_solver* solver,
                void* workspace, size_t workspace_bytes, void* stream, agate_ctx** out);
 
-/* Copy an interior-only SoA state U[8][nz][ny][nx] (U[9]... for AGATE_IDEAL_GLM / AGATE_CGL) into the context and set
+/* Copy an interior-only SoA state U[8][nz][ny][nx] (U[9]... for AGATE_IDEAL_GLM / AGATE_HALL_GLM / AGATE_CGL, U[10]... for AGATE_CGL_GLM) into the context and set
  * the time to t0.
  * `U` is a HOST pointer when src_is_device == 0 (borrowed for the call only: the call synchronises the stream), else
  * a DEVICE pointer, read in stream order without any synchronisation: whatever produced it must be ordered before

@@ -25,6 +25,7 @@ IDEAL, HALL = 0, 1
 CGL = 2              # CGL MHD: 9 variables per cell, U = (rho, m, E, B, A_log); see include/agate.h
 IDEAL_GLM = 3        # 9 variables per cell (psi last); see include/agate.h
 HALL_GLM = 4         # Hall MHD + GLM: 9 variables per cell
+CGL_GLM = 5          # CGL MHD + GLM (eqs.19-23): 10 variables per cell, U = (rho, m, E, B, A, psi)
 HLL, HLLD = 0, 1
 OK, ERR_ARG, ERR_STATE, ERR_UNPHYSICAL, ERR_CUDA, ERR_NOMEM = range(6)
 
@@ -123,7 +124,7 @@ class Agate:
         nx, ny, nz = (int(s) for s in shape)
         self.shape = (nx, ny, nz)
         self.zones = nx * ny * nz
-        self.nvar = 9 if int(eqset) in (IDEAL_GLM, CGL, HALL_GLM) else 8
+        self.nvar = {IDEAL_GLM: 9, CGL: 9, HALL_GLM: 9, CGL_GLM: 10}.get(int(eqset), 8)
         self.grid = Grid(ndim, nx, ny, nz, dx[0], dx[1], dx[2])
         self.cfg = SolverCfg(riemann, limiter, beta, rk, cfl, d_i, relax, (C.c_int32 * 3)(*[int(b) for b in bc]),
                              int(cgl_form))

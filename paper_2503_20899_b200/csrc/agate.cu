@@ -25,6 +25,9 @@ using namespace agate;
 #ifndef AGATE_TY3N
 #define AGATE_TY3N 11   // ... with nine variables (GLM, CGL): 182 KB
 #endif
+#ifndef AGATE_TY3X
+#define AGATE_TY3X 11   // ... with ten variables (CGL + GLM): 202 KB
+#endif
 #ifndef AGATE_MINB3
 #define AGATE_MINB3 1
 #endif
@@ -33,6 +36,7 @@ namespace {
 
 constexpr int TY3 = AGATE_TY3;   // 3-D tile height (rows); CTA = 32 x (TY3+1) threads (agate_stage3d.cuh)
 constexpr int TY3N = AGATE_TY3N;
+constexpr int TY3X = AGATE_TY3X;
 constexpr int TY2 = 6;    // 1-D / 2-D: 32x6 tile, 8 warps, 2 CTAs / SM
 constexpr int kDtBlocksMax = 148 * 8;
 
@@ -67,8 +71,9 @@ Layout make_layout(const agate_grid& g, int nv, int rk = 2) {
 }
 
 inline bool is_hall(int eqset) { return eqset == AGATE_HALL || eqset == AGATE_HALL_GLM; }
-inline bool is_glm(int eqset) { return eqset == AGATE_IDEAL_GLM || eqset == AGATE_HALL_GLM; }
-inline int nvar_of(int eqset) { return (is_glm(eqset) || eqset == AGATE_CGL) ? 9 : 8; }
+inline bool is_glm(int eqset) { return eqset == AGATE_IDEAL_GLM || eqset == AGATE_HALL_GLM || eqset == AGATE_CGL_GLM; }
+inline bool is_cgl(int eqset) { return eqset == AGATE_CGL || eqset == AGATE_CGL_GLM; }
+inline int nvar_of(int eqset) { return 8 + (is_glm(eqset) ? 1 : 0) + (is_cgl(eqset) ? 1 : 0); }
 
 int check_args(const agate_grid* g, double gamma, int eqset, const agate_solver* s) {
   if (!g || !s) return AGATE_ERR_ARG;
@@ -78,10 +83,11 @@ int check_args(const agate_grid* g, double gamma, int eqset, const agate_solver*
   if (g->ndim < 2 && g->ny != 1) return AGATE_ERR_ARG;
   if (!(g->dx > 0.0) || (g->ndim >= 2 && !(g->dy > 0.0)) || (g->ndim >= 3 && !(g->dz > 0.0))) return AGATE_ERR_ARG;
   if (!(gamma > 1.0)) return AGATE_ERR_ARG;
-  if (eqset != AGATE_IDEAL && eqset != AGATE_HALL && eqset != AGATE_IDEAL_GLM && eqset != AGATE_CGL && eqset != AGATE_HALL_GLM)
+  if (eqset != AGATE_IDEAL && eqset != AGATE_HALL && eqset != AGATE_IDEAL_GLM && eqset != AGATE_CGL && eqset != AGATE_HALL_GLM &&
+      eqset != AGATE_CGL_GLM)
     return AGATE_ERR_ARG;
-  if (eqset == AGATE_CGL && s->riemann != AGATE_HLL) return AGATE_ERR_ARG;    // CGL: HLL (the paper names no other solver)
-  if (eqset == AGATE_CGL && !(s->relax >= 0.0 && s->relax <= 1.0)) return AGATE_ERR_ARG;
+  if (is_cgl(eqset) && s->riemann != AGATE_HLL) return AGATE_ERR_ARG;    // CGL: HLL (the paper names no other solver)
+  if (is_cgl(eqset) && !(s->relax >= 0.0 && s->relax <= 1.0)) return AGATE_ERR_ARG;
   if (s->cgl_form < 0 || s->cgl_form > 1) return AGATE_ERR_ARG;
   if (s->riemann < 0 || s->riemann > 1 || s->limiter < 0 || s->limiter > 2 || s->rk < 1 || s->rk > 5) return AGATE_ERR_ARG;
   if (s->limiter == 2 && !(s->beta >= 1.0 && s->beta <= 2.0)) return AGATE_ERR_ARG;
@@ -92,13 +98,13 @@ int check_args(const agate_grid* g, double gamma, int eqset, const agate_solver*
   return AGATE_OK;
 }
 
-// The nine-variable equation sets (GLM, CGL) have no 1-D kernel: a 1-D grid runs through the 2-D strip kernel as ONE row
+// The equation sets with extra variables (GLM, CGL) have no 1-D kernel: a 1-D grid runs through the 2-D strip kernel as ONE row
 // that is its own periodic neighbour in y.  Both y faces of a zone then see identical states, their fluxes are the same
 // number and the y difference is an exact zero, so the result is that of the 1-D scheme (the oracle has no y sweep at
 // all); Courant number and dx_min are still those of the 1-D grid.
 agate_grid kernel_grid(const agate_grid& g, int eqset) {
   agate_grid k = g;
-  if (g.ndim == 1 && nvar_of(eqset) == 9) { k.ndim = 2; k.dy = g.dx; }
+  if (g.ndim == 1 && nvar_of(eqset) > 8) { k.ndim = 2; k.dy = g.dx; }
   return k;
 }
 
@@ -126,7 +132,7 @@ template <int TY, int R, int LIM, int MINB, bool GLM = false, bool CGL = false, 
 StageKernel make_stage3d() {
   StageKernel k;
   k.fn = stage3d_kernel<TY, R, LIM, MINB, GLM, CGL, HALL>;
-  using SM = Stage3dSmem<TY, (GLM || CGL) ? 9 : 8, HALL ? 3 : 2>;
+  using SM = Stage3dSmem<TY, 8 + (GLM ? 1 : 0) + (CGL ? 1 : 0), HALL ? 3 : 2>;
   static_assert(SM::BYTES <= 232448, "stage3d shared memory exceeds 227 KB");
   k.ty = TY; k.np = 3; k.threads = SM::NT;
   k.smem = SM::BYTES;
@@ -139,8 +145,9 @@ template <int R, int LIM, bool H, bool GLM = false, bool CGL = false>
 StageKernel make_stage2d() {
   StageKernel k;
   k.fn = stage2d_kernel<R, LIM, H, GLM, CGL>;
-  k.ty = 1; k.np = 1; k.threads = 32 * Stage2dSmem<GLM || CGL>::NW; k.smem = Stage2dSmem<GLM || CGL>::BYTES;
-  k.warps2d = Stage2dSmem<GLM || CGL>::NW;
+  using SM = Stage2dSmem<8 + (GLM ? 1 : 0) + (CGL ? 1 : 0)>;
+  k.ty = 1; k.np = 1; k.threads = 32 * SM::NW; k.smem = SM::BYTES;
+  k.warps2d = SM::NW;
   k.strips2d = true;
   k.fused_dt = !CGL;         // the fused reduction evaluates the ideal / Hall speed; CGL keeps the dt_kernel pass
   return k;
@@ -154,6 +161,8 @@ StageKernel pick_stage(int ndim, int eqset, int riemann, int limiter) {
     if (eqset == AGATE_HALL)
       return (limiter == 2) ? make_stage3d<TY3, 0, 2, AGATE_MINB3, false, false, true>()
                             : make_stage3d<TY3, 0, -1, AGATE_MINB3, false, false, true>();
+    if (eqset == AGATE_CGL_GLM)
+      return (limiter == 2) ? make_stage3d<TY3X, 0, 2, AGATE_MINB3, true, true>() : make_stage3d<TY3X, 0, -1, AGATE_MINB3, true, true>();
     if (eqset == AGATE_CGL)
       return (limiter == 2) ? make_stage3d<TY3N, 0, 2, AGATE_MINB3, false, true>() : make_stage3d<TY3N, 0, -1, AGATE_MINB3, false, true>();
     if (eqset == AGATE_IDEAL_GLM) {
@@ -171,6 +180,7 @@ StageKernel pick_stage(int ndim, int eqset, int riemann, int limiter) {
     if (eqset == AGATE_HALL_GLM) return (limiter == 2) ? make_stage2d<0, 2, true, true>() : make_stage2d<0, -1, true, true>();
     if (eqset == AGATE_HALL)
       return (limiter == 3) ? make_stage2d<0, 3, true>() : ((limiter == 2) ? make_stage2d<0, 2, true>() : make_stage2d<0, -1, true>());
+    if (eqset == AGATE_CGL_GLM) return (limiter == 2) ? make_stage2d<0, 2, false, true, true>() : make_stage2d<0, -1, false, true, true>();
     if (eqset == AGATE_CGL) return (limiter == 2) ? make_stage2d<0, 2, false, false, true>() : make_stage2d<0, -1, false, false, true>();
     if (eqset == AGATE_IDEAL_GLM) {
       if (riemann == AGATE_HLLD) return (limiter == 2) ? make_stage2d<1, 2, false, true>() : make_stage2d<1, -1, false, true>();
@@ -196,7 +206,7 @@ struct agate_ctx {
   agate_solver s;
   double gamma;
   int eqset;
-  int nv;                          // variables per cell: 8, or 9 with the GLM scalar
+  int nv;                          // variables per cell: 8, +1 with CGL's A, +1 with the GLM scalar
   Layout L;
   Phys ph;
   double dxmin, cfl;
@@ -274,7 +284,7 @@ StageParams make_stage_params(const agate_ctx* c, const double* Uin, const doubl
   p.flag = c->flag;
   p.ch_ptr = c->scal + 3;
   p.last_stage = last_stage ? 1 : 0;
-  p.relax = (c->eqset == AGATE_CGL) ? c->s.relax : 0.0;
+  p.relax = is_cgl(c->eqset) ? c->s.relax : 0.0;
   p.lz = c->lz;
   p.ntx = (c->g.nx + TX - 1) / TX;
   p.nty = (c->g.ny + c->sk.ty - 1) / c->sk.ty;
@@ -298,7 +308,7 @@ int launch_dt(agate_ctx* c, int add_t) {
   p.ph = c->ph;
   p.scal = c->scal; p.flag = c->flag; p.ticket = c->ticket; p.partial = c->partial;
   p.add_t = add_t;
-  p.cgl = (c->eqset == AGATE_CGL) ? 1 : 0;
+  p.cgl = is_cgl(c->eqset) ? 1 : 0;
   if (is_hall(c->eqset)) dt_kernel<true><<<c->dt_blocks, 256, 0, c->stream>>>(p);
   else dt_kernel<false><<<c->dt_blocks, 256, 0, c->stream>>>(p);
   CU_TRY(cudaGetLastError());
@@ -420,6 +430,13 @@ int ensure_vmax(agate_ctx* c) {
   return AGATE_OK;
 }
 
+// GLM with a host-chosen dt: c_h = 0.95 v_max(U^n) must still be on the device.  The fused path hands v_max to
+// set_dt_kernel; a kernel without the fused reduction (CGL + GLM) runs the reduction pass, which writes c_h itself.
+int ensure_ch(agate_ctx* c) {
+  if (c->sk.fused_dt) return ensure_vmax(c);
+  return launch_dt(c, 0);
+}
+
 int collect_status(agate_ctx* c) {
   CU_TRY(cudaStreamSynchronize(c->stream));
   int flag = 0;
@@ -510,7 +527,7 @@ int agate_init(const agate_grid* grid, double gamma, int eqset, const agate_solv
   c->cfl = solver->cfl;
   if (!(c->cfl > 0.0)) c->cfl = (user_grid.ndim == 1) ? 0.8 : (user_grid.ndim == 2 ? 0.45 : 0.325);
   c->ph = make_phys(gamma, is_hall(eqset) ? solver->d_i : 0.0, c->dxmin);
-  c->ph.cgl_form = (eqset == AGATE_CGL) ? solver->cgl_form : 0;
+  c->ph.cgl_form = is_cgl(eqset) ? solver->cgl_form : 0;
   c->stream = (cudaStream_t)stream;
   c->ws = (char*)workspace;
   c->UA = (double*)(c->ws + L.off_A);
@@ -585,7 +602,7 @@ int agate_step(agate_ctx* c, double dt, double* dt_used) {
   if (!c->have_state || c->ext_lo || c->ext_hi) return AGATE_ERR_STATE;   // a slab steps through agate_stage_pre / _post
   int rc;
   if (dt > 0.0) {
-    if (is_glm(c->eqset) && (rc = ensure_vmax(c))) return rc;      // c_h = 0.95 v_max(U^n) whoever chose dt
+    if (is_glm(c->eqset) && (rc = ensure_ch(c))) return rc;        // c_h = 0.95 v_max(U^n) whoever chose dt
     set_dt_kernel<<<1, 1, 0, c->stream>>>(c->scal, dt, c->sk.fused_dt ? c->vnext : nullptr);
     CU_TRY(cudaGetLastError());
   } else {
@@ -752,7 +769,7 @@ int agate_step_begin(agate_ctx* c, double dt) {
   int rc;
   const bool have_v = c->vmax_given || (c->sk.fused_dt && c->vmax_valid);
   if (dt > 0.0) {
-    if (is_glm(c->eqset) && !have_v && (rc = ensure_vmax(c))) return rc;
+    if (is_glm(c->eqset) && !have_v && (rc = ensure_ch(c))) return rc;
     set_dt_kernel<<<1, 1, 0, c->stream>>>(c->scal, dt, (c->sk.fused_dt || c->vmax_given) ? c->vnext : nullptr);
     CU_TRY(cudaGetLastError());
   } else {

@@ -32,10 +32,10 @@ constexpr int RW2 = 34;        // cells per ring row: x = xs-2 .. xs+31
 constexpr int NW2 = 6;         // warps per CTA of the 8-variable kernels
 
 // GLM = true: nine variables per cell, the scalar psi (index 8) behind the MHD ones (NEXT-1; eqs.10-11; R22)
-template <bool NINE>
+template <int NVAR>
 struct Stage2dSmem {
-  static constexpr int NV = NINE ? 9 : 8;
-  static constexpr int NW = NINE ? 5 : 6;            // warps per CTA (two CTAs per SM must fit 227 KB)
+  static constexpr int NV = NVAR;                   // 8; 9 with GLM or CGL; 10 with both (A at 8, psi at 9)
+  static constexpr int NW = (NVAR > 8) ? 5 : 6;     // warps per CTA (two CTAs per SM must fit 227 KB)
   static constexpr int RING = 4 * NV * RW2;         // [slot][q][c]
   static constexpr int OFF_WLY = RING;              // [q][lane]
   static constexpr int OFF_FYL = OFF_WLY + NV * 32;
@@ -46,9 +46,10 @@ struct Stage2dSmem {
 
 // CGL = true: CGL MHD (NEXT-2; R24): nine variables, W = (rho, v, p_par, B, p_perp), HLL only
 template <int RIEMANN, int LIM, bool HALL, bool GLM, bool CGL = false>
-__global__ void __launch_bounds__(32 * Stage2dSmem<GLM || CGL>::NW, 2) stage2d_kernel(const __grid_constant__ StageParams P) {
-  static_assert(!(HALL && RIEMANN != 0) && !(CGL && (HALL || GLM || RIEMANN != 0)), "combination not built");
-  using SM = Stage2dSmem<GLM || CGL>;
+__global__ void __launch_bounds__(32 * Stage2dSmem<8 + (GLM ? 1 : 0) + (CGL ? 1 : 0)>::NW, 2) stage2d_kernel(const __grid_constant__ StageParams P) {
+  static_assert(!(HALL && RIEMANN != 0) && !(CGL && (HALL || RIEMANN != 0)), "combination not built");
+  using SM = Stage2dSmem<8 + (GLM ? 1 : 0) + (CGL ? 1 : 0)>;
+  static_assert(2 * (SM::BYTES + 1024) <= 233472, "two CTAs per SM");
   constexpr int NV = SM::NV, NW2 = SM::NW;
   extern __shared__ __align__(16) double smem[];
   const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
@@ -241,12 +242,12 @@ __global__ void __launch_bounds__(32 * Stage2dSmem<GLM || CGL>::NW, 2) stage2d_k
         double o[NV];
 #pragma unroll
         for (int v = 0; v < NV; ++v, po += P.sq) {
-          constexpr int inv1[9] = {0, 3, 1, 2, 4, 7, 5, 6, 8};            // rot_var(inv1[v], 1) == v
+          constexpr int inv1[10] = {0, 3, 1, 2, 4, 7, 5, 6, 8, 9};          // rot_var(inv1[v], 1) == v
           const int r = inv1[v];
           // the difference is formed before it meets U, so that a uniform state stays bitwise fixed (pin P1)
           o[v] = c0 * (acc[v] - cy * (F[r] - FyL[v * 32 + lane]));
           if (GLM && v == NV - 1) o[v] *= decay;                          // eq.11's source, integrated exactly
-          if (CGL && v == NV - 1 && P.last_stage && P.relax > 0.0 && emit && cell_ok)
+          if (CGL && v == 8 && P.last_stage && P.relax > 0.0 && emit && cell_ok)
             o[v] = cgl_relaxed_alog(P.relax, o, P.ph.cgl_form);                          // eqs.31-33: E stays, A_log moves
           if (emit && cell_ok) *po = o[v];
           FyL[v * 32 + lane] = F[r];

@@ -26,7 +26,7 @@
 //   * the three tasks of a warp per plane run through one loop that is unrolled: three inlined copies of the solver,
 //     each with its direction's variable permutation resolved at compile time.
 //
-// Shared memory per CTA (NV = 8 variables; 9 with GLM or CGL): ring 3 planes x NV x TY x 36, y-halo rows
+// Shared memory per CTA (NV = 8 variables; 9 with GLM or CGL, 10 with both): ring 3 planes x NV x TY x 36, y-halo rows
 // 2 x NV x 4 x 36, Y NV x (TY+1) x 32, z carry and accumulator NV x TY x 32 each, XR / XF NV x TY each, 16 counters:
 // TY = 11 -> 162 KB (182 KB with 9 variables), one CTA of 12 warps per SM, <= 168 registers.  (TY = 15, 16 warps at
 // 128 registers without spills, fits in 213 KB and was measured slower: profiles/r2_stage3d.md.)
@@ -91,7 +91,7 @@ __device__ __forceinline__ bool mbar_test_wait(unsigned long long* bar, uint32_t
 // generic-proxy accesses to a shared buffer are ordered before the async proxy (the bulk copy) overwrites it
 __device__ __forceinline__ void fence_proxy_async() { asm volatile("fence.proxy.async.shared::cta;" ::: "memory"); }
 
-// rotated slot -> fixed variable; the GLM scalar (slot 8) is not rotated
+// rotated slot -> fixed variable; the scalars behind the MHD variables (CGL's A, the GLM psi) are not rotated
 __host__ __device__ __forceinline__ int rv(int r, int n) { return (r < 8) ? rot_var(r, n) : r; }
 
 template <int TY, int NV = 8, int NHB = 2>
@@ -142,13 +142,14 @@ __device__ __forceinline__ void hall_current(const double* W, int QS, int oC, in
 // LIM < 0 reads it from the parameters.
 // GLM = true: nine variables per cell, the scalar psi (index 8) behind the MHD ones (NEXT-1; eqs.10-11; R22).
 // CGL = true: CGL MHD (NEXT-2; R24): nine variables, W = (rho, v, p_par, B, p_perp), HLL only.
+// GLM and CGL (eqs.19-23; R30): ten variables, A at index 8, psi at index 9.
 // HALL = true: Hall MHD (A8; R15): HLL with the Hall velocity in the induction and energy fluxes and
 // max(c_f, c_w) in the Davis speeds; the face current needs B one zone around every face, so the y-halo rows keep
 // three planes, carry their x-halo corners, and a few more hand-overs guard the planes k-1 and k+1.
 template <int TY, int RIEMANN, int LIM, int MINB, bool GLM = false, bool CGL = false, bool HALL = false>
 __global__ void __launch_bounds__(32 * (TY + 1), MINB) stage3d_kernel(const __grid_constant__ StageParams P) {
-  static_assert(!(CGL && (GLM || RIEMANN != 0)) && !(HALL && (CGL || RIEMANN != 0)), "combination not built");
-  constexpr int NV = (GLM || CGL) ? 9 : 8;
+  static_assert(!(CGL && RIEMANN != 0) && !(HALL && (CGL || RIEMANN != 0)), "combination not built");
+  constexpr int NV = 8 + (GLM ? 1 : 0) + (CGL ? 1 : 0);      // CGL's A is index 8; psi is always the last variable
   constexpr int NHB = HALL ? 3 : 2;
   using SM = Stage3dSmem<TY, NV, NHB>;
   constexpr int NT = SM::NT, PL = SM::PL, SB = SM::SB, QS = SM::QS, YS = SM::YS, ZS = SM::ZS, XS = SM::XS;
@@ -561,7 +562,8 @@ __global__ void __launch_bounds__(32 * (TY + 1), MINB) stage3d_kernel(const __gr
         const double bns = 0.5 * (L[5] + R[5]) - 0.5 * (R[NV - 1] - L[NV - 1]) * ich;
         const double pss = 0.5 * (L[NV - 1] + R[NV - 1]) - 0.5 * ch * (R[5] - L[5]);
         L[5] = bns; R[5] = bns;
-        riemann_flux<RIEMANN, HALL>(P.ph, L, R, HALL ? Jr : nullptr, F);      // Hall + GLM (R29): Hall flux with B_n*
+        if (CGL) flux_hll_cgl(L, R, F, P.ph.cgl_form);                         // CGL + GLM (R30): CGL's flux with B_n*
+        else riemann_flux<RIEMANN, HALL>(P.ph, L, R, HALL ? Jr : nullptr, F);  // Hall + GLM (R29): Hall flux with B_n*
         F[5] = pss;
         F[NV - 1] = ch * ch * bns;
       } else if (flux) {
@@ -610,12 +612,12 @@ __global__ void __launch_bounds__(32 * (TY + 1), MINB) stage3d_kernel(const __gr
           double o[NV];
 #pragma unroll
           for (int v = 0; v < NV; ++v, po += P.sq) {
-            constexpr int inv2[9] = {0, 2, 3, 1, 4, 6, 7, 5, 8};          // rv(inv2[v], 2) == v
+            constexpr int inv2[10] = {0, 2, 3, 1, 4, 6, 7, 5, 8, 9};         // rv(inv2[v], 2) == v
             const double t = cz * F[inv2[v]];
             const double d = ACC[v * ZS + tid] - t;
             o[v] = c0 * ((two ? fma(P.r0, ub[v], ua[v]) : ua[v]) + d);
             if (GLM && v == NV - 1) o[v] *= decay;                        // eq.11's source, integrated exactly
-            if (CGL && v == NV - 1 && P.last_stage && P.relax > 0.0 && emit && cell_ok)
+            if (CGL && v == 8 && P.last_stage && P.relax > 0.0 && emit && cell_ok)
               o[v] = cgl_relaxed_alog(P.relax, o, P.ph.cgl_form);                        // eqs.31-33: E stays, A_log moves
             if (emit && cell_ok) *po = o[v];
             ACC[v * ZS + tid] = t;
@@ -650,7 +652,7 @@ __global__ void __launch_bounds__(32 * (TY + 1), MINB) stage3d_kernel(const __gr
             if (!HALL) await(prog + (wid == 0 ? TY : wid - 1), ph0 + 2, P.flag);
 #pragma unroll
             for (int v = 0; v < NV; ++v) {
-              constexpr int inv1[9] = {0, 3, 1, 2, 4, 7, 5, 6, 8};        // rv(inv1[v], 1) == v
+              constexpr int inv1[10] = {0, 3, 1, 2, 4, 7, 5, 6, 8, 9};       // rv(inv1[v], 1) == v
               const int r = inv1[v];
               const double dFy = Y[r * YS + (wid + 1) * 32 + lane] - Y[r * YS + wid * 32 + lane];
               ACC[v * ZS + tid] = fma(-cx, dFx[v], fma(-cy, dFy, ACC[v * ZS + tid]));

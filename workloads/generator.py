@@ -32,6 +32,7 @@ NVAR = 8
 IDEAL, HALL = 0, 1
 IDEAL_GLM = 3          # 9 variables per cell: the GLM scalar psi behind the 8 MHD ones
 CGL = 2                # 9 variables per cell: U = (rho, m, E, B, A_log), W = (rho, v, p_par, B, p_perp)
+CGL_GLM = 5            # 10 variables per cell: CGL's nine, then the GLM scalar psi (eqs.19-23)
 HLL, HLLD = 0, 1
 GAMMA = 5.0 / 3.0
 SEED_BASE = 2503208990
@@ -168,9 +169,11 @@ def prim_to_cons(W: np.ndarray, gamma: float) -> np.ndarray:
 def prim_to_cons_cgl(W: np.ndarray) -> np.ndarray:
     """Definition of the CGL conserved vector from W = (rho, v, p_par, B, p_perp): E = rho v^2/2 + B^2/2 + p_par/2 +
     p_perp, A_log = rho log[(rho^2/B^3)(p_perp/p_par)] (eq.18)."""
-    rho, vx, vy, vz, ppar, bx, by, bz, pperp = W
+    rho, vx, vy, vz, ppar, bx, by, bz, pperp = W[:9]
     b2 = bx * bx + by * by + bz * bz
     U = np.empty_like(W)
+    if W.shape[0] > 9:
+        U[9:] = W[9:]                 # the GLM scalar is its own conserved variable
     U[0] = rho; U[1] = rho * vx; U[2] = rho * vy; U[3] = rho * vz
     U[4] = 0.5 * rho * (vx * vx + vy * vy + vz * vz) + 0.5 * b2 + 0.5 * ppar + pperp
     U[5] = bx; U[6] = by; U[7] = bz
@@ -201,6 +204,9 @@ _CONFIGS = {
     # 3's three-dimensional recipe, for the 3-D Hall path of the row-owner kernel
     8: dict(ndim=3, n=256, eqset=HALL, riemann=HLL, beta=1.0, cfl=0.325, d_i=0.2, n_steps=50,
             name="cfg8: 3D Hall 256^3 HLL minmod"),
+    # not a BASELINE.json config: config 7 with the GLM scalar, i.e. the whole of eqs.19-23 on the Orszag-Tang vortex
+    9: dict(ndim=2, n=2048, eqset=CGL_GLM, riemann=HLL, beta=1.3, cfl=0.45, d_i=0.0, n_steps=100, relax=0.99,
+            name="cfg9: 2D Orszag-Tang CGL + GLM 2048^2 HLL MC"),
 }
 
 
@@ -222,10 +228,10 @@ def make_workload(config_id: int, n: int | None = None, n_steps: int | None = No
     rng = SplitMix64(SEED_BASE + config_id)
     g = GAMMA
     nx, ny, nz = shape
-    W = np.empty((NVAR + (1 if c["eqset"] in (IDEAL_GLM, CGL) else 0), nz, ny, nx))
+    W = np.empty((NVAR + {IDEAL_GLM: 1, CGL: 1, CGL_GLM: 2}.get(c["eqset"], 0), nz, ny, nx))
     F = lambda M, K: _field(rng, M, K, ndim, shape)
 
-    if config_id in (6, 7):
+    if config_id in (6, 7, 9):
         # rho = 25/(36 pi), p = 5/(12 pi), v = (-sin 2 pi y, sin 2 pi x, 0), B = B0 (-sin 2 pi y, sin 4 pi x, 0),
         # B0 = 1/sqrt(4 pi), unit box, cell centres; psi = 0
         xc = ((np.arange(nx) + 0.5) / nx)[None, None, :]
@@ -240,6 +246,8 @@ def make_workload(config_id: int, n: int | None = None, n_steps: int | None = No
         W[6] = B0 * np.sin(4.0 * math.pi * xc) + 0.0 * yc
         W[7] = 0.0
         W[8] = 0.0 if config_id == 6 else W[4]      # GLM: psi = 0;  CGL: p_perp = p_par = p
+        if config_id == 9:
+            W[9] = 0.0
     elif config_id in (1, 4):
         W[0] = 1.0 + 0.1 * F(4, 4)
         W[1] = 0.1 * F(4, 4)
@@ -298,7 +306,7 @@ def make_workload(config_id: int, n: int | None = None, n_steps: int | None = No
     d_i = c["d_i"]
     if config_id in (4, 8) and scale_d_i and n != nfull:
         d_i = d_i * nfull / n
-    U = prim_to_cons_cgl(W) if c["eqset"] == CGL else prim_to_cons(W, g)
+    U = prim_to_cons_cgl(W) if c["eqset"] in (CGL, CGL_GLM) else prim_to_cons(W, g)
     return Workload(config_id=config_id, ndim=ndim, shape=shape, dx=dx, gamma=g, eqset=c["eqset"],
                     riemann=c["riemann"], limiter=2, beta=c["beta"], rk=2, cfl=c["cfl"], d_i=d_i,
                     n_steps=c["n_steps"] if n_steps is None else n_steps, W=W, U=U, relax=c.get("relax", 0.0),
