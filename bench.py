@@ -264,7 +264,10 @@ def run_ours(args):
     wl = make_workload(cfg, n=args.n or None)
     zones = wl.zones
     over = {}
-    if cfg in (7, 9) and args.cgl_form == 1:
+    if cfg == 9 and args.cgl_form == 1:
+        raise SystemExit("--cgl-form 1 is offered for config 7 only: with the GLM scalar on, eq.16's A runs out of the "
+                         "physical range at the vortex's field nulls, in the oracle as on the GPU (DESIGN.md section 11)")
+    if cfg == 7 and args.cgl_form == 1:
         # input definition of the other thermodynamic variable (eq.16): A = (rho / |B|)^3 p_perp / p_par
         W = wl.W
         b2 = W[5] ** 2 + W[6] ** 2 + W[7] ** 2
