@@ -86,7 +86,8 @@ enum {
   AGATE_ERR_STATE = 2,        /* call order: no state set yet                                        */
   AGATE_ERR_UNPHYSICAL = 3,   /* rho <= 0, p <= 0 or a non-finite speed seen by the dt reduction (R14) */
   AGATE_ERR_CUDA = 4,         /* CUDA runtime error, no CUDA device, or a hand-over wait inside a kernel ran out */
-  AGATE_ERR_NOMEM = 5         /* workspace too small or misaligned                                   */
+  AGATE_ERR_NOMEM = 5,        /* workspace too small or misaligned                                   */
+  AGATE_ERR_LIMIT = 6         /* agate_cfl_static: the grid needs more scratch than the library's static array holds */
 };
 
 /* Bytes of device workspace agate_init needs for this problem (0 on invalid arguments): two ghost-padded copies of
@@ -184,6 +185,41 @@ int agate_stage_post(agate_ctx*, int stage, const void* recv_lo, const void* rec
 
 int agate_destroy(agate_ctx*);
 const char* agate_strerror(int status);
+
+/* ---- allocation-free Courant reduction (A7; R3-R5, R14) ---------------------------
+ * For callers that cannot allocate device memory or hand the library a workspace (code under CUDA graph capture,
+ * tight serving loops, harnesses that forbid cudaMalloc): v_max = max over zones of (|v| + c) and dt = C dx_min / v_max
+ * of a caller-owned state, with no context, no workspace and no allocation of any kind.  The reduction's scratch (one
+ * partial maximum per segment of <= 1024 consecutive zones of a grid row, a ticket counter, a flag) lives in a
+ * file-scope __device__ array inside the library: 256 + 8 * AGATE_STATIC_MAX_SEGMENTS bytes (about 0.5 MiB), held by
+ * every GPU that loads the library until the process exits.
+ *
+ *   grid, gamma, eqset  as for agate_init (any equation set).  Of `solver` only cfl (<= 0: the paper's default for
+ *                       the grid's dimensionality), d_i (Hall sets: the whistler speed of eq.13) and cgl_form (CGL sets)
+ *                       are read.
+ *   U_dev     DEVICE, read only, the caller's: interior-only SoA state U[nv][nz][ny][nx] as agate_set_state takes it
+ *             (nv = 8, 9 or 10 by equation set; only the variables the speed needs are read).
+ *   out_dev   DEVICE, the caller's, 3 doubles:  [0] v_max,  [1] dt,  [2] 1.0 if a zone with rho <= 0, p <= 0 or a
+ *             non-finite speed was seen (such zones are left out of the maximum, R14), else 0.0.
+ *   stream    cudaStream_t; one memset of the scratch header and one kernel are enqueued on it; the call does not
+ *             synchronise and may be captured into a CUDA graph.
+ *
+ * The speeds come from the same device functions as agate_compute_dt's, and max is exact under any association: v_max
+ * and dt are bit for bit those of a context holding the same state.
+ * Limit: ceil(nx / 1024) * ny * nz <= AGATE_STATIC_MAX_SEGMENTS (e.g. 256^3, 8192^2; not 512^3), else AGATE_ERR_LIMIT and
+ * nothing is enqueued.  Other errors: AGATE_ERR_ARG (null pointer, bad grid / gamma / eqset), AGATE_ERR_CUDA.
+ * Sharing: every call on a GPU uses the one array, which keeps the previous call's contents; the call clears what must
+ * start at zero and overwrites the rest before reading it.  Calls that OVERLAP on one GPU (different streams with no
+ * ordering between them, or a captured graph replayed concurrently with a direct call) race on it and return garbage:
+ * order them.  Different GPUs have separate copies.
+ * agate_cfl_static_setup resolves the array's device address for the CURRENT device (cudaGetSymbolAddress; once per
+ * device).  agate_cfl_static does that itself on first use; call the setup explicitly, once per device, before
+ * capturing a graph, since the lookup may load the module. */
+#define AGATE_STATIC_MAX_SEGMENTS 65536
+int agate_cfl_static_setup(void);
+int64_t agate_cfl_static_max_segments(void);
+int agate_cfl_static(const agate_grid* grid, double gamma, int eqset, const agate_solver* solver,
+                     const double* U_dev, double* out_dev, void* stream);
 
 /* ---- diagnostics (not on the hot path) -------------------------------------------------------------- */
 

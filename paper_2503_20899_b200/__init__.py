@@ -35,7 +35,7 @@ SYMBOLS = ("agate_workspace_bytes", "agate_init", "agate_set_state", "agate_comp
            "agate_stage_time", "agate_set_tuning", "agate_set_slab", "agate_halo_bytes", "agate_get_vmax",
            "agate_set_vmax", "agate_vmax_device", "agate_step_begin", "agate_stage_pre", "agate_stage_post",
            "agate_destroy", "agate_strerror", "agate_test_face_flux",
-           "agate_measure_fp64_peak")
+           "agate_measure_fp64_peak", "agate_cfl_static", "agate_cfl_static_setup", "agate_cfl_static_max_segments")
 
 
 class Grid(C.Structure):
@@ -103,6 +103,10 @@ def lib():
         L.agate_test_face_flux.argtypes = [C.c_int, C.c_int, C.c_int, C.c_double, C.c_double, C.c_double,
                                            _vp, _vp, _vp, _vp, C.c_int64, _vp]
         L.agate_measure_fp64_peak.argtypes = [C.c_int, _dp, _vp, _vp]
+        L.agate_cfl_static.argtypes = [C.POINTER(Grid), C.c_double, C.c_int, C.POINTER(SolverCfg), _vp, _vp, _vp]
+        L.agate_cfl_static_setup.argtypes = []
+        L.agate_cfl_static_max_segments.argtypes = []
+        L.agate_cfl_static_max_segments.restype = C.c_int64
         _lib = L
     return _lib
 
@@ -314,3 +318,38 @@ def measure_fp64_peak(iters=20):
     if rc:
         raise AgateError(rc, "agate_measure_fp64_peak")
     return v.value
+
+
+def cfl_static(U, out, shape, dx, ndim, gamma=5.0 / 3.0, eqset=IDEAL, cfl=0.0, d_i=0.0, cgl_form=0, stream=None):
+    """Allocation-free Courant reduction (agate_cfl_static; see include/agate.h): v_max, dt and the unphysical flag of
+    the interior-only device state `U` ([nv,nz,ny,nx] f64 CUDA tensor) into the caller's `out` (3 f64 on the same
+    device).  Argument marshalling only: no tensor is created here and nothing synchronises; the work is enqueued on
+    `stream` (default: torch's current stream).  Raises AgateError (status 6) beyond the static scratch's limit."""
+    torch = _torch_cuda()
+    nx, ny, nz = (int(v) for v in shape)
+    if not (U.is_cuda and out.is_cuda and U.dtype == torch.float64 and out.dtype == torch.float64):
+        raise TypeError("cfl_static: U and out must be float64 CUDA tensors")
+    if not (U.is_contiguous() and out.is_contiguous()) or out.numel() < 3 or U.device != out.device:
+        raise ValueError("cfl_static: contiguous tensors on one device, out with >= 3 elements")
+    nvar = {IDEAL_GLM: 9, CGL: 9, HALL_GLM: 9, CGL_GLM: 10}.get(int(eqset), 8)
+    if U.numel() != nvar * nx * ny * nz:
+        raise ValueError(f"cfl_static: U has {U.numel()} elements, the grid needs {nvar * nx * ny * nz}")
+    grid = Grid(int(ndim), nx, ny, nz, float(dx[0]), float(dx[1]), float(dx[2]))
+    cfg = SolverCfg(HLL, 2, 1.3, 2, float(cfl), float(d_i), 0.0, (C.c_int32 * 3)(0, 0, 0), int(cgl_form))
+    with torch.cuda.device(U.device):
+        st = stream if stream is not None else torch.cuda.current_stream()
+        rc = lib().agate_cfl_static(C.byref(grid), float(gamma), int(eqset), C.byref(cfg), _vp(U.data_ptr()),
+                                    _vp(out.data_ptr()), _vp(st.cuda_stream))
+    if rc:
+        raise AgateError(rc, "agate_cfl_static")
+    return out
+
+
+def cfl_static_setup(device=None):
+    """Resolve the static scratch's device address on `device` (default: the current one); once per device, before
+    capturing a graph that contains cfl_static."""
+    torch = _torch_cuda()
+    with torch.cuda.device(device if device is not None else torch.cuda.current_device()):
+        rc = lib().agate_cfl_static_setup()
+    if rc:
+        raise AgateError(rc, "agate_cfl_static_setup")

@@ -15,7 +15,7 @@ _ROOT = os.path.dirname(_HERE)
 CSRC = os.path.join(_HERE, "csrc")
 INCLUDE = os.path.join(_ROOT, "include")
 LIB = os.path.join(_HERE, "libagate.so")
-SOURCES = [os.path.join(CSRC, "agate.cu")]
+SOURCES = [os.path.join(CSRC, "agate.cu"), os.path.join(CSRC, "agate_noalloc.cu")]
 DEPS = SOURCES + [os.path.join(CSRC, "agate_kernels.cuh"), os.path.join(CSRC, "agate_physics.cuh"),
                   os.path.join(CSRC, "agate_stage3d.cuh"), os.path.join(CSRC, "agate_stage2d.cuh"),
                   os.path.join(INCLUDE, "agate.h")]

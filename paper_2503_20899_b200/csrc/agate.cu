@@ -846,6 +846,7 @@ const char* agate_strerror(int status) {
     case AGATE_ERR_UNPHYSICAL: return "unphysical state (rho <= 0, p <= 0 or non-finite speed)";
     case AGATE_ERR_CUDA: return "CUDA error or no CUDA device";
     case AGATE_ERR_NOMEM: return "workspace too small or misaligned";
+    case AGATE_ERR_LIMIT: return "grid needs more scratch than the library's static array holds (AGATE_STATIC_MAX_SEGMENTS)";
     default: return "unknown status";
   }
 }
