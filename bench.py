@@ -51,13 +51,13 @@ BYTES_PER_ZONE_STEP = 320.0            # 5 x 8 variables x 8 B; 
 # launches of one step) from `ncu --metrics dram__bytes_read.sum,dram__bytes_write.sum -k regex:stage -s 2 -c 2` on the
 # same bench command with the final kernels (profiles/r2_stage3d.md "final traffic"; the full captures in r2_metrics.csv
 # were taken a few commits earlier and agree within 1.5 %)
-NCU_TRAFFIC_BYTES = {5: 0.5 * (11752420096 + 8916774912 + 20709065216 + 8867503360),
-                     2: 0.5 * (283619072 + 226279424 + 558610688 + 226200576),
-                     4: 0.5 * (79377920 + 23228672 + 153306368 + 24793856),
-                     8: 0.5 * (1410646784 + 1089779200 + 2518610432 + 1086041856)}
+NCU_TRAFFIC_BYTES = {5: 0.5 * (11793633024 + 8912302080 + 20819086592 + 8866547200),
+                     2: 0.5 * (283740928 + 225785088 + 558584576 + 226272256),
+                     4: 0.5 * (79430400 + 23967488 + 153255680 + 24544000),
+                     8: 0.5 * (1412550400 + 1090506496 + 2525984000 + 1086049280)}
 # ... and the kernels they were captured on: sha256 over csrc/*.cu* at capture time.  When the kernels have changed
 # since, the figure is stale and the line reports "traffic": null instead (profiles/ names the capture).
-NCU_TRAFFIC_CSRC_SHA = "b836b146f8831573"
+NCU_TRAFFIC_CSRC_SHA = "80e84362947e08fa"
 
 
 def csrc_sha():
