@@ -18,7 +18,7 @@
 //   * Hall (A8): the face current comes from the cell-centred B of the three ring rows around the face.
 //
 // Shared memory per warp: ring 4 x 8 x 34, two y carries 8 x 32, raw U 2 x 8 x 32  =  16.5 KB;  6 warps per CTA,
-// 2 CTAs per SM (12 warps, <= 168 registers).
+// 2 CTAs per SM (12 warps, <= 168 registers).  Nine / ten variables: one CTA of 12 / 11 warps per SM.
 #pragma once
 #include <cuda_runtime.h>
 #include <stdint.h>
@@ -35,7 +35,11 @@ constexpr int NW2 = 6;         // warps per CTA of the 8-variable kernels
 template <int NVAR>
 struct Stage2dSmem {
   static constexpr int NV = NVAR;                   // 8; 9 with GLM or CGL; 10 with both (A at 8, psi at 9)
-  static constexpr int NW = (NVAR > 8) ? 5 : 6;     // warps per CTA (two CTAs per SM must fit 227 KB)
+  // warps per CTA.  The warps are autonomous, so only their number per SM matters: 8 variables 2 CTAs x 6 warps; with
+  // 9 (10) variables a warp's buffers take 18.6 (20.6) KB and two CTAs would hold 2 x 5 warps, so ONE CTA of 12 (11) warps
+  // fills the 227 KB instead
+  static constexpr int NW = (NVAR == 8) ? 6 : ((NVAR == 9) ? 12 : 11);
+  static constexpr int MINB = (NVAR == 8) ? 2 : 1;  // CTAs per SM
   static constexpr int RING = 4 * NV * RW2;         // [slot][q][c]
   static constexpr int OFF_WLY = RING;              // [q][lane]
   static constexpr int OFF_FYL = OFF_WLY + NV * 32;
@@ -46,10 +50,11 @@ struct Stage2dSmem {
 
 // CGL = true: CGL MHD (NEXT-2; R24): nine variables, W = (rho, v, p_par, B, p_perp), HLL only
 template <int RIEMANN, int LIM, bool HALL, bool GLM, bool CGL = false>
-__global__ void __launch_bounds__(32 * Stage2dSmem<8 + (GLM ? 1 : 0) + (CGL ? 1 : 0)>::NW, 2) stage2d_kernel(const __grid_constant__ StageParams P) {
+__global__ void __launch_bounds__(32 * Stage2dSmem<8 + (GLM ? 1 : 0) + (CGL ? 1 : 0)>::NW,
+                                  Stage2dSmem<8 + (GLM ? 1 : 0) + (CGL ? 1 : 0)>::MINB) stage2d_kernel(const __grid_constant__ StageParams P) {
   static_assert(!(HALL && RIEMANN != 0) && !(CGL && (HALL || RIEMANN != 0)), "combination not built");
   using SM = Stage2dSmem<8 + (GLM ? 1 : 0) + (CGL ? 1 : 0)>;
-  static_assert(2 * (SM::BYTES + 1024) <= 233472, "two CTAs per SM");
+  static_assert(SM::MINB * (SM::BYTES + 1024) <= 233472 && SM::BYTES <= 232448, "shared memory per SM / per CTA");
   constexpr int NV = SM::NV, NW2 = SM::NW;
   extern __shared__ __align__(16) double smem[];
   const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
