@@ -364,11 +364,13 @@ __global__ void __launch_bounds__(32 * (TY + 1), MINB) stage3d_kernel(const __gr
     const bool emit = k > k0;       // plane k-1 is completed in this step
     const int hb = hbuf_of(k);                            // y-halo rows of plane k
     const int ph0 = ph;                                   // sub-phases completed when this plane starts
-    double Ly[NV], ua[NV], ub[NV];
+    double ua[NV], ub[NV];
+    // face states and flux of the task in hand.  L outlives a sub-phase once: the y slope formed in phase A leaves the
+    // left state of face j+1/2 in it for phase B1 (no copy at the hand-over between the two)
+    double L[NV], R[NV], F[NV], Jr[3];
 
 #pragma unroll
     for (int s = 0; s < 3; ++s) {
-      double L[NV], R[NV], F[NV], Jr[3];
       bool flux = false;
       // ---- hand-over: what this sub-phase reads must be published, what it overwrites must have been read.  Every
       //      wait is on a sub-phase EARLIER than the one about to start, so the waits cannot form a cycle.
@@ -433,8 +435,7 @@ __global__ void __launch_bounds__(32 * (TY + 1), MINB) stage3d_kernel(const __gr
           if (s == 1) {
 #pragma unroll
             for (int r = 0; r < NV; ++r) {
-              L[r] = Ly[r];
-              R[r] = Y[rv(r, 1) * YS + (wid + 1) * 32 + lane];
+              R[r] = Y[rv(r, 1) * YS + (wid + 1) * 32 + lane];      // L: left there by phase A
             }
             if (HALL) {
               // face j+1/2: C = own cell, D = the row above (halo row TY for the top row); transverse z (planes
@@ -602,7 +603,7 @@ __global__ void __launch_bounds__(32 * (TY + 1), MINB) stage3d_kernel(const __gr
               double lo, hi;
               plm_faces(limiter, beta2, a, b, cc, lo, hi);
               Y[v * YS + wid * 32 + lane] = lo;
-              Ly[r] = hi;
+              L[r] = hi;
             }
           }
           // A5 (z) + A6: plane k-1 is complete:  Uout = a1 ((a0/a1) U0 + Uin + [-dt (flux differences)]);  the
