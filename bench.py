@@ -51,16 +51,16 @@ BYTES_PER_ZONE_STEP = 320.0            # 5 x 8 variables x 8 B; 
 # launches of one step) from `ncu --metrics dram__bytes_read.sum,dram__bytes_write.sum -k regex:stage -s 2 -c 2` on the
 # same bench command with the final kernels (profiles/r2_stage3d.md "final traffic"; the full captures in r2_metrics.csv
 # were taken a few commits earlier and agree within 1.5 %)
-NCU_TRAFFIC_BYTES = {5: 0.5 * (11708311808 + 8911286016 + 20953554176 + 8879029760),
-                     2: 0.5 * (283820544 + 225776896 + 558598912 + 226664192),
-                     4: 0.5 * (79426816 + 23955968 + 153204992 + 25742848),
-                     8: 0.5 * (1411074816 + 1090209792 + 2522631936 + 1086123264),
-                     6: 0.5 * (318538752 + 258601472 + 627715072 + 259940608),
-                     7: 0.5 * (318523136 + 258355712 + 627545856 + 260858624),
-                     9: 0.5 * (373766400 + 297001472 + 738395392 + 299035136)}
+NCU_TRAFFIC_BYTES = {5: 0.5 * (11525812736 + 8910902016 + 20068614912 + 8812694528),
+                     2: 0.5 * (283653632 + 225981952 + 558576640 + 226220800),
+                     4: 0.5 * (79418368 + 23350016 + 153315328 + 24589824),
+                     8: 0.5 * (1412547840 + 1090191616 + 2523881728 + 1086261504),
+                     6: 0.5 * (318541568 + 258995200 + 627718400 + 260007936),
+                     7: 0.5 * (318549760 + 258905088 + 627584768 + 260304128),
+                     9: 0.5 * (374100480 + 297494528 + 739145984 + 299099648)}
 # ... and the kernels they were captured on: sha256 over csrc/*.cu* at capture time.  When the kernels have changed
 # since, the figure is stale and the line reports "traffic": null instead (profiles/ names the capture).
-NCU_TRAFFIC_CSRC_SHA = "2d7f768665add46c"
+NCU_TRAFFIC_CSRC_SHA = "2877b02b7181cef3"
 
 
 def csrc_sha():
