@@ -1,6 +1,7 @@
 """NEXT-4 on ONE GPU (-m gpu): two (or three) contexts hold the slabs of one problem, exchange their halos by device
 copies every stage and take the maximum of their v_max every step; they must reproduce the undivided run bit for bit
-(dt included), on 3-D grids (z slabs) and 2-D grids (y slabs), for ideal, Hall and GLM, periodic and open ends."""
+(dt included), on 3-D grids (z slabs) and 2-D grids (y slabs), for ideal, Hall, GLM, CGL and CGL + GLM, periodic and open
+ends."""
 import numpy as np
 import pytest
 
@@ -105,6 +106,32 @@ def test_glm_slabs_share_ch(ag):
     U2, ts = run_slabs(ag, kw, wl.U, 2, 4, periodic=True, eqset=ag.IDEAL_GLM)
     assert all(t == t1 for t in ts)
     assert np.array_equal(U1.view(np.uint64), U2.view(np.uint64))
+
+
+@pytest.mark.parametrize("cfg,ndim,n,nslab", [(7, 2, 64, 2), (9, 2, 66, 3), (9, 3, 24, 2)])
+def test_cgl_and_cgl_glm_slabs(ag, cfg, ndim, n, nslab):
+    """CGL and CGL + GLM: kernels without the fused reduction, so every step's v_max (and with it c_h) goes through
+    agate_get_vmax / agate_set_vmax; relaxation and the psi source act in the last stage of every slab alike."""
+    wl = make_workload(cfg, n=n)
+    U = wl.U
+    shape, dx = wl.shape, wl.dx
+    if ndim == 3:                         # the Orszag-Tang rows stacked along z with a z-dependent flow on top
+        z = (np.arange(n) + 0.5) / n
+        U = np.ascontiguousarray(np.repeat(U, n, axis=1))
+        U[3] = U[0] * 0.2 * np.sin(2 * np.pi * z)[:, None, None]
+        U[4] = U[4] + 0.5 * U[3] ** 2 / U[0]
+        shape, dx = (n, n, n), (1.0 / n,) * 3
+    kw = dict(shape=shape, dx=dx, ndim=ndim, gamma=wl.gamma, riemann=wl.riemann, limiter=2, beta=wl.beta, rk=2,
+              cfl=wl.cfl if ndim == 2 else 0.325, relax=wl.relax)
+    one = ag.Agate(eqset=wl.eqset, **kw)
+    one.set_state(U)
+    t1 = one.advance(4)
+    U1 = one.get_state()
+    one.close()
+    U2, ts = run_slabs(ag, kw, U, nslab, 4, periodic=True, eqset=wl.eqset)
+    assert all(t == t1 for t in ts)
+    assert np.array_equal(U1.view(np.uint64), U2.view(np.uint64))
+    assert not np.array_equal(U1, U)
 
 
 def test_single_rank_stepper_periodic_self_exchange(ag):
